@@ -1,0 +1,179 @@
+/*
+ * shuntstage.h — C-ABI of libshuntstage.so: the forward pass of ONE pipeline stage of ShuntServe
+ * (arxiv/paper_2606_18600), hand-written CUDA for sm_100a.
+ *
+ * What a "stage" is: the contiguous range of decoder layers [l0,l1) that the paper's placement optimizer
+ * assigns to one node (§2.3 "uneven layer partitioning"; Algorithm 1 line 9 `add_stage(i,
+ * l_new)`).  Its input and output is the hidden-state tensor [tokens, H] of E-byte elements that
+ * crosses stage boundaries (Eq. 2; E = 2, bf16).  The operations inside a layer
+ * are the ones Table 2 costs: QKV projection, attention (prefill / decode), output
+ * projection, up-and-gate projection, down projection, logits — "the de-facto standard of transformer-based
+ * generative LLMs", i.e. the public Llama-3 / Qwen3 pre-norm decoder layer.  The two calls are
+ *   - ss_stage_decode : one batched decode iteration over a paged GQA KV cache ("memory-bound decode",
+ *                       PAPER.md:21, 96, 222);
+ *   - ss_stage_prefill: causal prefill; this is also the compute of the paper's output-preserving request
+ *                       migration, which re-runs "input sequence and already-generated output sequence" to
+ *                       reconstruct the KV cache (§5.1).
+ *
+ * All pointers named "dev" are CUDA device pointers, all others are host pointers.  Nothing in this header is
+ * a torch type.  The library never allocates or frees device memory: weights, KV pool, workspace, inputs and
+ * outputs are BORROWED from the caller (this mirrors the paper's engine, which attaches to tensors owned by the
+ * Shared Tensor Store).  Borrowed pointers must stay valid and unchanged until ss_stage_destroy.
+ *
+ * Calls enqueue work on the stage's CUDA stream and return; results are valid after the caller synchronises
+ * that stream.  Errors that the host can detect are returned synchronously and nothing is enqueued.  A stage
+ * is not thread-safe; distinct stages are independent.
+ *
+ * Readings of points the paper leaves open are listed in DESIGN.md ("Readings"), numbered A1..A22 after
+ * SURVEY.md §8(c).
+ */
+#ifndef SHUNTSTAGE_H
+#define SHUNTSTAGE_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* ---- error codes (0 = OK, negative = error) ------------------------------------------------------------ */
+#define SS_OK                 0
+#define SS_ERR_INVALID_ARG   -1  /* null / contradictory pointers, l0>=l1, both or neither of hidden/token_ids */
+#define SS_ERR_UNSUPPORTED   -2  /* head_dim not in {64,128}, page_size != 16, n_q % n_kv != 0, G > 16,
+                                    hidden/ffn/n_q*d not multiples of 8, misaligned pointers */
+#define SS_ERR_CAPACITY      -3  /* tokens / seqs / max_blocks over the dims' maxima; pool or workspace too small */
+#define SS_ERR_NO_PAGES      -4  /* ss_kv_alloc: fewer than n pages free — nothing was allocated */
+#define SS_ERR_BAD_PAGE      -5  /* ss_kv_free: id out of range or already free — nothing was freed */
+#define SS_ERR_CUDA          -6  /* a CUDA runtime/driver call failed; see ss_last_cuda_error */
+
+typedef struct ss_stage ss_stage; /* opaque */
+
+/* Model dimensions (Table 3 notation: H = hidden, H_kv = n_kv_heads*head_dim (reading A2),
+ * H_ffn = ffn, V = vocab) and the capacity of one call. */
+typedef struct {
+  int32_t hidden;            /* H */
+  int32_t n_q_heads;         /* query heads; Hq = n_q_heads*head_dim (may differ from H: Qwen3-32B, A4) */
+  int32_t n_kv_heads;        /* KV heads; q heads [h*G,(h+1)*G) share kv head h, G = n_q/n_kv (A16) */
+  int32_t head_dim;          /* d: 64 or 128 */
+  int32_t ffn;               /* H_ffn */
+  int32_t n_layers_total;    /* layers of the whole model; l1 <= n_layers_total */
+  int32_t vocab;             /* V; used only when edge weights are given */
+  float   rms_eps;           /* RMSNorm epsilon (also the per-head QK-norm epsilon) (A8) */
+  float   rope_theta;        /* RoPE base; inv_freq[c] = theta^(-2c/d), rotate-half pairing (A10) */
+  int32_t qk_norm;           /* 0 Llama; 1 Qwen3: per-head RMSNorm on q and k before RoPE, gain [d] (A11) */
+  int32_t page_size;         /* tokens per KV page; must be 16 */
+  int32_t max_pos;           /* RoPE table length: positions 0..max_pos-1 are legal */
+  int32_t max_tokens;        /* capacity T of one prefill call (a decode call needs batch <= max_seqs) */
+  int32_t max_seqs;          /* capacity: sequences per call */
+  int32_t max_blocks_per_seq;/* capacity: block-table row length */
+} ss_model_dims;
+
+/* Per-layer weights: dev pointers, bf16, row-major [out_features, in_features] ("K-major": row n is the weight
+ * vector of output feature n), no biases (A7).  Every pointer 16-byte aligned.  Borrowed. */
+typedef struct {
+  const void *ln1;     /* [H]        RMSNorm gain before attention                           (step S1) */
+  const void *wq;      /* [Hq, H]    Table 2 "QKV Projection", PAPER.md:141-142              (S2) */
+  const void *wk;      /* [Hkv, H] */
+  const void *wv;      /* [Hkv, H] */
+  const void *q_norm;  /* [d] or NULL when qk_norm == 0                                      (S3) */
+  const void *k_norm;  /* [d] or NULL */
+  const void *wo;      /* [H, Hq]    Table 2 "Output Projection", PAPER.md:145-146           (S7) */
+  const void *ln2;     /* [H]        RMSNorm gain before the FFN                             (S8) */
+  const void *w_gate;  /* [F, H]     Table 2 "Up and Gate Projection", PAPER.md:147-148      (S9) */
+  const void *w_up;    /* [F, H] */
+  const void *w_down;  /* [H, F]     Table 2 "Down Projection", PAPER.md:149-150             (S10) */
+} ss_layer_weights;
+
+/* Optional first-/last-stage weights (dev, bf16, borrowed).  Any member may be NULL. */
+typedef struct {
+  const void  *embed;       /* [V, H]: needed for token_ids input (stage 0 takes tokens)  (S0) */
+  const void  *final_norm;  /* [H]                                                                     (S11) */
+  const void  *lm_head;     /* [V, H]: Table 2 "Logits Calculation", PAPER.md:151-152                   (S11) */
+  const float *inv_freq;    /* HOST pointer, [d/2] fp32, or NULL -> theta^(-2c/d); read at create only */
+} ss_edge_weights;
+
+/* Bytes of caller-allocated device workspace a stage with these dims and layer range needs. 0 on bad dims. */
+size_t ss_stage_workspace_bytes(const ss_model_dims *dims, int l0, int l1);
+
+/* Bytes of one KV page over all layers of the stage: (l1-l0) * 2 * n_kv_heads * 16 * head_dim * 2. */
+size_t ss_kv_page_bytes(const ss_model_dims *dims, int l0, int l1);
+
+/*
+ * Create a stage for layers [l0,l1).  `layers` is a HOST array of l1-l0 structs (copied).  `edge` may be NULL.
+ * kv_pool: dev, 1024-byte aligned, layout (bf16, contiguous; part of the contract because page contents are
+ * compared bit for bit):
+ *     pool[layer - l0][kv in {0:K,1:V}][page][h_kv][slot 0..15][c 0..d-1]
+ * with num_pages = kv_pool_bytes / ss_kv_page_bytes(); the token at position p of a sequence whose block-table
+ * row is bt lives in page bt[p >> 4], slot p & 15 (paged KV cache: PAPER.md:265, 271; [31] PAPER.md:540).
+ * workspace: dev, 1024-byte aligned, >= ss_stage_workspace_bytes().  cuda_stream: a cudaStream_t (may be 0).
+ * The call uploads the RoPE table and builds TMA descriptors; it synchronises the stream once.
+ */
+int ss_stage_create(ss_stage **out, const ss_model_dims *dims, int l0, int l1,
+                    const ss_layer_weights *layers, const ss_edge_weights *edge,
+                    void *kv_pool, size_t kv_pool_bytes,
+                    void *workspace, size_t workspace_bytes,
+                    void *cuda_stream);
+int ss_stage_destroy(ss_stage *st);
+
+/* Page pool (host-side free list over page ids 0..num_pages-1; no device work). */
+int ss_kv_num_pages(const ss_stage *st);
+int ss_kv_num_free(const ss_stage *st);
+int ss_kv_alloc(ss_stage *st, int n, int32_t *out_page_ids /* host, [n] */);   /* all-or-nothing */
+int ss_kv_free(ss_stage *st, int n, const int32_t *page_ids /* host, [n] */);  /* all-or-nothing */
+
+/*
+ * Causal prefill of n_seqs packed sequences (steps S0-S11 of DESIGN.md; migration recompute).
+ * Token i of sequence s sits in packed row cu_q[s]+i and at global position ctx_before[s]+i; it attends keys
+ * 0..ctx_before[s]+i, which are read from the pages (including those this call appends).  Rows with q_len = 1
+ * are legal, so a mixed decode+prefill iteration is one call (A19: decode rows first).
+ *   hidden_bf16 XOR token_ids: dev [T,H] bf16, or dev [T] int32 (needs edge->embed and l0 == 0).
+ *   cu_q: dev int32 [n_seqs+1], cu_q[0] = 0, cu_q[n_seqs] = total_tokens.  ctx_before: dev int32 [n_seqs].
+ *   block_tables: dev int32 [n_seqs, max_blocks]; pages for positions [0, ctx_before+q_len) must be listed.
+ *   out_hidden_bf16: dev [T,H] or NULL (every token: the next stage needs all of them to build its KV).
+ *   out_logits: dev fp32 [n_seqs,V] or NULL; out_argmax: dev int32 [n_seqs] or NULL — for the LAST token of
+ *   each sequence; need edge->final_norm and edge->lm_head.  argmax ties resolve to the lowest index.
+ */
+int ss_stage_prefill(ss_stage *st, int n_seqs,
+                     const void *hidden_bf16, const int32_t *token_ids,
+                     const int32_t *cu_q, const int32_t *ctx_before,
+                     const int32_t *block_tables, int max_blocks, int total_tokens,
+                     void *out_hidden_bf16, float *out_logits, int32_t *out_argmax);
+
+/*
+ * One decode iteration for `batch` sequences, one new token each (Table 2 "Decode" rows).
+ * context_lens[b] = tokens already cached (A20); the new token's K/V are appended at that position by the
+ * attention kernel itself and attended to.  The page bt[b][context_lens[b] >> 4] must exist.
+ *   hidden_bf16 XOR token_ids: dev [B,H] bf16 / dev [B] int32.   block_tables: dev int32 [B, max_blocks].
+ *   out_hidden_bf16 dev [B,H] or NULL; out_logits dev fp32 [B,V] or NULL; out_argmax dev int32 [B] or NULL.
+ * The kernel sequence of a decode call is captured into a CUDA graph per (batch, max_blocks, output kind) and
+ * replayed; user pointers are passed through a small device-side argument block, so they may change per call.
+ */
+int ss_stage_decode(ss_stage *st, int batch,
+                    const void *hidden_bf16, const int32_t *token_ids,
+                    const int32_t *block_tables, int max_blocks, const int32_t *context_lens,
+                    void *out_hidden_bf16, float *out_logits, int32_t *out_argmax);
+
+/* Number of kernels the stage launched (directly or inside replayed graphs) since creation. */
+int64_t ss_stage_launch_count(const ss_stage *st);
+
+/* ---- op-level entry points (the same kernels the stage uses; for per-kernel parity tests and profiling) -- */
+
+/* C[T, N] (fp32, row-major, ld = N) = X[T, K] (bf16, row-major) * W[N, K]^T (bf16) through the tcgen05/TMEM
+ * GEMM.  `splits` >= 1 K-splits are reduced in fixed order.  scratch: dev, >= splits*T*N*4 bytes when
+ * splits > 1 (may be NULL when splits == 1).  K % 8 == 0.  Synchronous w.r.t. the host only via the stream. */
+int ss_op_gemm_bf16(const void *x_dev, const void *w_dev, float *c_dev, int T, int N, int K,
+                    int splits, void *scratch_dev, void *cuda_stream);
+
+/* Fused gate/up GEMM + SwiGLU: A[T, F] (bf16) = silu(X Wg^T) * (X Wu^T). */
+int ss_op_gemm_swiglu_bf16(const void *x_dev, const void *wg_dev, const void *wu_dev, void *a_dev,
+                           int T, int F, int K, void *cuda_stream);
+
+const char *ss_strerror(int code);
+const char *ss_last_cuda_error(void); /* text of the last CUDA error seen by this thread ("" if none) */
+const char *ss_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SHUNTSTAGE_H */
