@@ -1,0 +1,347 @@
+// attn_decode.cu — step S6a (+S5): paged GQA decode attention with split-K over the context and a fused KV append
+// (Table 2 "Attention / Decode"; "memory-bound decode"; paged KV cache,
+// PAPER.md:265, 271).  HBM-bound: every cached K/V byte is read exactly once per step.
+//
+// Work partition.  The (sequence b, kv head h, page) triples of the batch are flattened in that order into
+// P_total = n_kv * sum_b pages_b items of one 16-token page (K 16xd + V 16xd bf16, each a contiguous block of the
+// pool).  Each worker WARP takes a contiguous range of ceil(P_total / n_workers) items, so the load is balanced
+// to one page whatever the length mix (the paper's workloads have lognormal lengths).  A range is cut
+// at (b,h) boundaries into segments; each segment yields one partial (m, l, O[G x d]) in slot `worker + pair`,
+// which is unique and monotone along the flattened order.  decode_merge combines the segments of a pair.
+//
+// A warp is an independent pipeline: cp.async 16-byte copies of whole pages into its private XOR-swizzled smem
+// ring (no block barrier anywhere), ldmatrix + mma.sync m16n8k16 with the G query heads of the group as the M rows
+// (each K/V byte feeds all G heads), online softmax in fp32 with quad shuffles.  The warp that owns a sequence's
+// last page writes the new token's K/V (bf16, post-RoPE, from qkv_post) into that page — in smem for its own use
+// and in the pool — which is the fused append of step S5.
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdlib.h>
+
+#include "common.cuh"
+#include "internal.h"
+
+namespace ss {
+
+constexpr int DA_WARPS = 4;
+constexpr int DA_STAGES = 3;
+
+// ---- plan: prefix sum of pages per sequence --------------------------------------------------------------------
+__global__ void decode_plan_kernel(const CallArgs *__restrict__ args, int batch, int n_kv, int n_workers,
+                                   DecodePlan plan) {
+  if (threadIdx.x == 0 && blockIdx.x == 0) {
+    int acc = 0;
+    plan.cum_pages[0] = 0;
+    for (int b = 0; b < batch; ++b) {
+      acc += (args->ctx[b] + 1 + 15) >> 4;
+      plan.cum_pages[b + 1] = acc;
+    }
+    const int total = acc * n_kv;
+    plan.meta[0] = total;
+    plan.meta[1] = (total + n_workers - 1) / n_workers;
+  }
+}
+
+cudaError_t launch_decode_plan(const CallArgs *args, int batch, int n_kv, int n_workers, DecodePlan plan,
+                               cudaStream_t s) {
+  decode_plan_kernel<<<1, 32, 0, s>>>(args, batch, n_kv, n_workers, plan);
+  count_launch();
+  return cudaGetLastError();
+}
+
+struct Cursor {
+  int b, h, pg, pages_b;
+};
+
+template <int D>
+__global__ void __launch_bounds__(DA_WARPS * 32) decode_attn_kernel(const DecodeAttnParams p) {
+  constexpr int ROW_BYTES = D * 2;
+  constexpr int CHUNKS = ROW_BYTES / 16;       // 16-byte chunks per row: 16 (d=128) or 8 (d=64)
+  constexpr int PAGE_BYTES = 16 * ROW_BYTES;   // one K (or V) page of one head
+  constexpr int KSTEPS = D / 16;
+  constexpr int NT = D / 8;                    // output n-tiles
+  extern __shared__ __align__(128) uint8_t smem[];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int w = blockIdx.x * DA_WARPS + warp;
+  uint8_t *ring = smem + (size_t)warp * DA_STAGES * 2 * PAGE_BYTES;
+
+  const int total = p.plan.meta[0], quota = p.plan.meta[1];
+  const int g0 = w * quota;
+  const int g1 = min(g0 + quota, total);
+  if (g0 >= g1) return;
+  const int n_kv = p.n_kv, G = p.n_q / p.n_kv;
+  const int32_t *cum = p.plan.cum_pages;
+  const CallArgs *args = p.args;
+  const int32_t *bt = args->block_tables;
+  const int max_blocks = args->max_blocks;
+  const __nv_bfloat16 *kpool = (const __nv_bfloat16 *)p.kpool;
+  const __nv_bfloat16 *vpool = (const __nv_bfloat16 *)p.vpool;
+
+  // locate g0: largest b with cum[b]*n_kv <= g0
+  Cursor lc;
+  {
+    int lo = 0, hi = p.batch;  // invariant: cum[lo]*n_kv <= g0 < cum[hi]*n_kv
+    while (hi - lo > 1) {
+      const int mid = (lo + hi) >> 1;
+      if (cum[mid] * n_kv <= g0) lo = mid; else hi = mid;
+    }
+    lc.b = lo;
+    lc.pages_b = cum[lo + 1] - cum[lo];
+    const int r = g0 - cum[lo] * n_kv;
+    lc.h = r / lc.pages_b;
+    lc.pg = r - lc.h * lc.pages_b;
+  }
+  Cursor cc = lc;
+
+  auto advance = [&](Cursor &c) {
+    if (++c.pg == c.pages_b) {
+      c.pg = 0;
+      if (++c.h == n_kv) {
+        c.h = 0;
+        ++c.b;
+        c.pages_b = (c.b < p.batch) ? cum[c.b + 1] - cum[c.b] : 1;
+      }
+    }
+  };
+  auto issue_load = [&](const Cursor &c, int slot) {
+    const int page = bt[(size_t)c.b * max_blocks + c.pg];
+    const size_t off = ((size_t)page * n_kv + c.h) * 16 * D;
+    const uint8_t *ks = (const uint8_t *)(kpool + off);
+    const uint8_t *vs = (const uint8_t *)(vpool + off);
+    uint8_t *kd = ring + (size_t)slot * 2 * PAGE_BYTES;
+    uint8_t *vd = kd + PAGE_BYTES;
+#pragma unroll
+    for (int i = 0; i < PAGE_BYTES / 16 / 32; ++i) {
+      const int idx = i * 32 + lane;
+      const int r = idx / CHUNKS, ch = idx % CHUNKS;
+      const int dst = r * ROW_BYTES + ((ch ^ (r & 7)) << 4);
+      cp_async16(kd + dst, ks + (size_t)idx * 16);
+      cp_async16(vd + dst, vs + (size_t)idx * 16);
+    }
+  };
+
+  const int n = g1 - g0;
+#pragma unroll
+  for (int i = 0; i < DA_STAGES - 1; ++i) {
+    if (i < n) {
+      issue_load(lc, i);
+      advance(lc);
+    }
+    cp_async_commit();
+  }
+
+  const float sl2 = 1.4426950408889634f / sqrtf((float)D);  // log2(e) / sqrt(d)
+  uint32_t qf[KSTEPS][4];
+  float o[NT][4];
+  float m_run[2], l_run[2];
+  bool seg_open = false;
+  const int qrow = lane >> 2, qcol = (lane & 3) * 2;
+
+  for (int i = 0; i < n; ++i) {
+    if (i + DA_STAGES - 1 < n) {
+      issue_load(lc, (i + DA_STAGES - 1) % DA_STAGES);
+      advance(lc);
+    }
+    cp_async_commit();
+    cp_async_wait<DA_STAGES - 1>();
+    __syncwarp();
+
+    const int ctx = args->ctx[cc.b];
+    if (!seg_open) {
+      // new (b,h) segment: query fragments of the G heads of kv head h (rows >= G are zero)
+      const __nv_bfloat16 *qb = (const __nv_bfloat16 *)p.q + (size_t)cc.b * p.n_q * D + (size_t)cc.h * G * D;
+#pragma unroll
+      for (int ks = 0; ks < KSTEPS; ++ks) {
+        const int c = ks * 16 + qcol;
+        qf[ks][0] = (qrow < G) ? *reinterpret_cast<const uint32_t *>(qb + (size_t)qrow * D + c) : 0u;
+        qf[ks][2] = (qrow < G) ? *reinterpret_cast<const uint32_t *>(qb + (size_t)qrow * D + c + 8) : 0u;
+        qf[ks][1] = (qrow + 8 < G) ? *reinterpret_cast<const uint32_t *>(qb + (size_t)(qrow + 8) * D + c) : 0u;
+        qf[ks][3] = (qrow + 8 < G) ? *reinterpret_cast<const uint32_t *>(qb + (size_t)(qrow + 8) * D + c + 8) : 0u;
+      }
+#pragma unroll
+      for (int t = 0; t < NT; ++t) o[t][0] = o[t][1] = o[t][2] = o[t][3] = 0.f;
+      m_run[0] = m_run[1] = -INFINITY;
+      l_run[0] = l_run[1] = 0.f;
+      seg_open = true;
+    }
+
+    uint8_t *ksm = ring + (size_t)(i % DA_STAGES) * 2 * PAGE_BYTES;
+    uint8_t *vsm = ksm + PAGE_BYTES;
+    const int last_pg = ctx >> 4;
+    int n_valid = 16;
+    if (cc.pg == last_pg) {
+      // fused KV append (step S5): slot ctx & 15 of the sequence's last page <- bf16 k', v' of the new token
+      n_valid = (ctx & 15) + 1;
+      const int r = ctx & 15;
+      const int page = bt[(size_t)cc.b * max_blocks + cc.pg];
+      const uint8_t *src = (const uint8_t *)p.kv_new + ((size_t)cc.b * 2 * n_kv * D + (size_t)cc.h * D) * 2;
+      const size_t goff = (((size_t)page * n_kv + cc.h) * 16 + r) * ROW_BYTES;
+      for (int idx = lane; idx < 2 * CHUNKS; idx += 32) {
+        const int isv = idx / CHUNKS, ch = idx % CHUNKS;
+        const uint4 val = *reinterpret_cast<const uint4 *>(src + (size_t)isv * n_kv * D * 2 + ch * 16);
+        uint8_t *sdst = (isv ? vsm : ksm) + r * ROW_BYTES + ((ch ^ (r & 7)) << 4);
+        *reinterpret_cast<uint4 *>(sdst) = val;
+        uint8_t *gdst = (uint8_t *)(isv ? p.vpool : p.kpool) + goff + ch * 16;
+        *reinterpret_cast<uint4 *>(gdst) = val;
+      }
+      // slots past the sequence end hold whatever the pool held: zero their V rows so that 0 * garbage (possibly
+      // NaN) cannot reach the output; their scores are overwritten with -inf below
+      for (int idx = lane; idx < (15 - r) * CHUNKS; idx += 32) {
+        const int rr2 = r + 1 + idx / CHUNKS, ch = idx % CHUNKS;
+        *reinterpret_cast<uint4 *>(vsm + rr2 * ROW_BYTES + (ch << 4)) = make_uint4(0u, 0u, 0u, 0u);
+      }
+      __syncwarp();
+    }
+
+    // ---- S = Q K^T for the 16 tokens of the page: two n-tiles of 8 tokens
+    float s0[4] = {0.f, 0.f, 0.f, 0.f}, s1[4] = {0.f, 0.f, 0.f, 0.f};
+    {
+      const int mtx = lane >> 3, rr = lane & 7;
+      const int tok = (mtx >> 1) * 8 + rr;
+      const uint32_t kbase = smem_u32(ksm) + tok * ROW_BYTES;
+#pragma unroll
+      for (int ks = 0; ks < KSTEPS; ++ks) {
+        const int ch = ks * 2 + (mtx & 1);
+        uint32_t kb[4];
+        ldmatrix_x4(kb, kbase + ((ch ^ (tok & 7)) << 4));
+        mma_bf16_16816(s0, qf[ks], kb[0], kb[1]);
+        mma_bf16_16816(s1, qf[ks], kb[2], kb[3]);
+      }
+    }
+    // mask tokens past the sequence end (only on the last page)
+    if (n_valid < 16) {
+      if (qcol >= n_valid) s0[0] = s0[2] = -INFINITY;
+      if (qcol + 1 >= n_valid) s0[1] = s0[3] = -INFINITY;
+      if (qcol + 8 >= n_valid) s1[0] = s1[2] = -INFINITY;
+      if (qcol + 9 >= n_valid) s1[1] = s1[3] = -INFINITY;
+    }
+    // ---- online softmax (rows qrow and qrow+8), statistics across the quad
+    float mx0 = fmaxf(fmaxf(s0[0], s0[1]), fmaxf(s1[0], s1[1]));
+    float mx1 = fmaxf(fmaxf(s0[2], s0[3]), fmaxf(s1[2], s1[3]));
+    mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 1));
+    mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 2));
+    mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 1));
+    mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 2));
+    const float mn0 = fmaxf(m_run[0], mx0), mn1 = fmaxf(m_run[1], mx1);
+    const float a0 = exp2f((m_run[0] - mn0) * sl2), a1 = exp2f((m_run[1] - mn1) * sl2);
+    m_run[0] = mn0;
+    m_run[1] = mn1;
+    float pr0[4], pr1[4];
+    pr0[0] = exp2f((s0[0] - mn0) * sl2); pr0[1] = exp2f((s0[1] - mn0) * sl2);
+    pr0[2] = exp2f((s0[2] - mn1) * sl2); pr0[3] = exp2f((s0[3] - mn1) * sl2);
+    pr1[0] = exp2f((s1[0] - mn0) * sl2); pr1[1] = exp2f((s1[1] - mn0) * sl2);
+    pr1[2] = exp2f((s1[2] - mn1) * sl2); pr1[3] = exp2f((s1[3] - mn1) * sl2);
+    float rs0 = pr0[0] + pr0[1] + pr1[0] + pr1[1];
+    float rs1 = pr0[2] + pr0[3] + pr1[2] + pr1[3];
+    rs0 += __shfl_xor_sync(0xffffffffu, rs0, 1);
+    rs0 += __shfl_xor_sync(0xffffffffu, rs0, 2);
+    rs1 += __shfl_xor_sync(0xffffffffu, rs1, 1);
+    rs1 += __shfl_xor_sync(0xffffffffu, rs1, 2);
+    l_run[0] = l_run[0] * a0 + rs0;
+    l_run[1] = l_run[1] * a1 + rs1;
+    uint32_t pa[4];
+    pa[0] = pack_bf16x2(pr0[0], pr0[1]);
+    pa[1] = pack_bf16x2(pr0[2], pr0[3]);
+    pa[2] = pack_bf16x2(pr1[0], pr1[1]);
+    pa[3] = pack_bf16x2(pr1[2], pr1[3]);
+    // ---- O = O * alpha + P V
+    {
+      const int mtx = lane >> 3, rr = lane & 7;
+      const int tok = (mtx & 1) * 8 + rr;
+      const uint32_t vbase = smem_u32(vsm) + tok * ROW_BYTES;
+#pragma unroll
+      for (int t2 = 0; t2 < NT / 2; ++t2) {
+        const int ch = t2 * 2 + (mtx >> 1);
+        uint32_t vb[4];
+        ldmatrix_x4_trans(vb, vbase + ((ch ^ (tok & 7)) << 4));
+        float *oa = o[2 * t2], *ob = o[2 * t2 + 1];
+        oa[0] *= a0; oa[1] *= a0; oa[2] *= a1; oa[3] *= a1;
+        ob[0] *= a0; ob[1] *= a0; ob[2] *= a1; ob[3] *= a1;
+        mma_bf16_16816(o[2 * t2], pa, vb[0], vb[1]);
+        mma_bf16_16816(o[2 * t2 + 1], pa, vb[2], vb[3]);
+      }
+    }
+
+    // ---- segment end?  (next item belongs to another (b,h), or this was the warp's last item)
+    const bool seg_end = (i == n - 1) || (cc.pg + 1 == cc.pages_b);
+    if (seg_end) {
+      const int slot = w + cc.b * n_kv + cc.h;
+      float *po = p.part_o + (size_t)slot * 16 * D;
+      float *pml = p.part_ml + (size_t)slot * 32;
+      if (qrow < G) {
+#pragma unroll
+        for (int t = 0; t < NT; ++t)
+          *reinterpret_cast<float2 *>(po + (size_t)qrow * D + t * 8 + qcol) = make_float2(o[t][0], o[t][1]);
+        if ((lane & 3) == 0) *reinterpret_cast<float2 *>(pml + qrow * 2) = make_float2(m_run[0], l_run[0]);
+      }
+      if (qrow + 8 < G) {
+#pragma unroll
+        for (int t = 0; t < NT; ++t)
+          *reinterpret_cast<float2 *>(po + (size_t)(qrow + 8) * D + t * 8 + qcol) = make_float2(o[t][2], o[t][3]);
+        if ((lane & 3) == 0) *reinterpret_cast<float2 *>(pml + (qrow + 8) * 2) = make_float2(m_run[1], l_run[1]);
+      }
+      seg_open = false;
+    }
+    advance(cc);
+    __syncwarp();
+  }
+}
+
+// ---- merge the segments of each (b, kv head): out[b][hq][:] = sum_i w_i O_i / sum_i w_i l_i, w_i = 2^((m_i-M) sl2)
+template <int D>
+__global__ void __launch_bounds__(D) decode_merge_kernel(const DecodeAttnParams p) {
+  const int pair = blockIdx.x;
+  const int b = pair / p.n_kv, h = pair % p.n_kv;
+  const int G = p.n_q / p.n_kv;
+  const int32_t *cum = p.plan.cum_pages;
+  const int quota = p.plan.meta[1];
+  const int pages_b = cum[b + 1] - cum[b];
+  const int start = cum[b] * p.n_kv + h * pages_b;
+  const int w_first = start / quota, w_last = (start + pages_b - 1) / quota;
+  const float sl2 = 1.4426950408889634f / sqrtf((float)D);
+  const int c = threadIdx.x;
+  for (int g = 0; g < G; ++g) {
+    float M = -INFINITY;
+    for (int w = w_first; w <= w_last; ++w) M = fmaxf(M, p.part_ml[(size_t)(w + pair) * 32 + g * 2]);
+    float num = 0.f, den = 0.f;
+    for (int w = w_first; w <= w_last; ++w) {
+      const size_t slot = (size_t)(w + pair);
+      const float2 ml = *reinterpret_cast<const float2 *>(p.part_ml + slot * 32 + g * 2);
+      const float wt = exp2f((ml.x - M) * sl2);
+      num += wt * p.part_o[slot * 16 * D + (size_t)g * D + c];
+      den += wt * ml.y;
+    }
+    ((__nv_bfloat16 *)p.out)[(size_t)b * p.n_q * D + (size_t)(h * G + g) * D + c] = __float2bfloat16_rn(num / den);
+  }
+}
+
+static size_t decode_smem(int d) { return (size_t)DA_WARPS * DA_STAGES * 2 * 16 * d * 2; }
+
+cudaError_t attn_init() {
+  cudaError_t e =
+      cudaFuncSetAttribute(decode_attn_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)decode_smem(128));
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(decode_attn_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              (int)decode_smem(64));
+}
+
+cudaError_t launch_decode_attn(const DecodeAttnParams &p, cudaStream_t s) {
+  const int ctas = p.n_workers / DA_WARPS;
+  if (p.d == 128)
+    decode_attn_kernel<128><<<ctas, DA_WARPS * 32, decode_smem(128), s>>>(p);
+  else
+    decode_attn_kernel<64><<<ctas, DA_WARPS * 32, decode_smem(64), s>>>(p);
+  count_launch();
+  return cudaGetLastError();
+}
+
+cudaError_t launch_decode_merge(const DecodeAttnParams &p, cudaStream_t s) {
+  if (p.d == 128)
+    decode_merge_kernel<128><<<p.batch * p.n_kv, 128, 0, s>>>(p);
+  else
+    decode_merge_kernel<64><<<p.batch * p.n_kv, 64, 0, s>>>(p);
+  count_launch();
+  return cudaGetLastError();
+}
+
+}  // namespace ss

@@ -1,0 +1,304 @@
+// elementwise.cu — the HBM-bound glue steps of a decoder layer, fused around the GEMMs' fp32 split-K partials:
+//   S0/S1  input_rmsnorm      : widen the stage input (or gather embeddings) into the fp32 residual + RMSNorm-1
+//   S3/S4  qkv_post           : split-K reduce + per-head QK RMSNorm (Qwen3) + RoPE; q -> bf16; k,v -> bf16 to the
+//                               decode staging buffer (appended by the attention kernel) or, in prefill, to pages (S5)
+//   S7/S8, S10/S1' residual_rmsnorm : residual += sum of split-K partials (fixed order), then the next RMSNorm
+//   S11    final_norm_rows, logits_argmax
+// The paper costs none of these (Table 2 has no norm / RoPE row); their math is readings A1,
+// A8, A10, A11 of DESIGN.md.  All statistics and the residual stream are fp32.
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+
+#include "common.cuh"
+#include "internal.h"
+
+namespace ss {
+
+constexpr int EW_THREADS = 256;
+
+__device__ __forceinline__ float block_sum(float v, float *red /* [32] */) {
+  v = warp_sum(v);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (lane == 0) red[warp] = v;
+  __syncthreads();
+  const int nw = (blockDim.x + 31) >> 5;
+  float r = (lane < nw) ? red[lane] : 0.f;
+  r = warp_sum(r);
+  __syncthreads();
+  return r;
+}
+
+// ---- S0 + S1 -------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(EW_THREADS)
+input_rmsnorm_kernel(const CallArgs *__restrict__ args, const __nv_bfloat16 *__restrict__ embed,
+                     const __nv_bfloat16 *__restrict__ w, float eps, int H, float *__restrict__ x,
+                     __nv_bfloat16 *__restrict__ h) {
+  __shared__ float red[32];
+  const int t = blockIdx.x;
+  const __nv_bfloat16 *src;
+  if (args->hidden_in)
+    src = (const __nv_bfloat16 *)args->hidden_in + (size_t)t * H;
+  else
+    src = embed + (size_t)args->token_ids[t] * H;
+  float *xr = x + (size_t)t * H;
+  float ss = 0.f;
+  for (int j = threadIdx.x * 8; j < H; j += EW_THREADS * 8) {
+    const uint4 v = *reinterpret_cast<const uint4 *>(src + j);
+    float f[8] = {bf16_lo(v.x), bf16_hi(v.x), bf16_lo(v.y), bf16_hi(v.y),
+                  bf16_lo(v.z), bf16_hi(v.z), bf16_lo(v.w), bf16_hi(v.w)};
+#pragma unroll
+    for (int i = 0; i < 8; ++i) ss += f[i] * f[i];
+    *reinterpret_cast<float4 *>(xr + j) = make_float4(f[0], f[1], f[2], f[3]);
+    *reinterpret_cast<float4 *>(xr + j + 4) = make_float4(f[4], f[5], f[6], f[7]);
+  }
+  ss = block_sum(ss, red);
+  const float inv = 1.0f / sqrtf(ss / (float)H + eps);
+  for (int j = threadIdx.x * 8; j < H; j += EW_THREADS * 8) {
+    const uint4 v = *reinterpret_cast<const uint4 *>(src + j);
+    const uint4 g = *reinterpret_cast<const uint4 *>(w + j);
+    uint4 o;
+    o.x = pack_bf16x2(bf16_lo(v.x) * inv * bf16_lo(g.x), bf16_hi(v.x) * inv * bf16_hi(g.x));
+    o.y = pack_bf16x2(bf16_lo(v.y) * inv * bf16_lo(g.y), bf16_hi(v.y) * inv * bf16_hi(g.y));
+    o.z = pack_bf16x2(bf16_lo(v.z) * inv * bf16_lo(g.z), bf16_hi(v.z) * inv * bf16_hi(g.z));
+    o.w = pack_bf16x2(bf16_lo(v.w) * inv * bf16_lo(g.w), bf16_hi(v.w) * inv * bf16_hi(g.w));
+    *reinterpret_cast<uint4 *>(h + (size_t)t * H + j) = o;
+  }
+}
+
+cudaError_t launch_input_rmsnorm(const CallArgs *args, const void *embed, const void *ln_w, float eps, int H,
+                                 int T, float *x, void *h, cudaStream_t s) {
+  input_rmsnorm_kernel<<<T, EW_THREADS, 0, s>>>(args, (const __nv_bfloat16 *)embed, (const __nv_bfloat16 *)ln_w,
+                                                eps, H, x, (__nv_bfloat16 *)h);
+  count_launch();
+  return cudaGetLastError();
+}
+
+// ---- residual += sum_s part[s]; optional RMSNorm -> h; optional bf16 stage output -----------------------------
+__global__ void __launch_bounds__(EW_THREADS)
+residual_rmsnorm_kernel(float *__restrict__ x, const float *__restrict__ part, int splits, long long split_stride,
+                        const __nv_bfloat16 *__restrict__ w, float eps, int H, __nv_bfloat16 *__restrict__ h,
+                        const CallArgs *__restrict__ args, int write_out) {
+  __shared__ float red[32];
+  const int t = blockIdx.x;
+  float *xr = x + (size_t)t * H;
+  const float *pr = part + (size_t)t * H;
+  __nv_bfloat16 *outp = nullptr;
+  if (write_out && args->out_hidden) outp = (__nv_bfloat16 *)args->out_hidden + (size_t)t * H;
+  float ss = 0.f;
+  for (int j = threadIdx.x * 4; j < H; j += EW_THREADS * 4) {
+    float4 y = *reinterpret_cast<const float4 *>(pr + j);
+    for (int s = 1; s < splits; ++s) {
+      const float4 q = *reinterpret_cast<const float4 *>(pr + (size_t)s * split_stride + j);
+      y.x += q.x; y.y += q.y; y.z += q.z; y.w += q.w;
+    }
+    float4 v = *reinterpret_cast<const float4 *>(xr + j);
+    v.x += y.x; v.y += y.y; v.z += y.z; v.w += y.w;
+    *reinterpret_cast<float4 *>(xr + j) = v;
+    ss += v.x * v.x + v.y * v.y + v.z * v.z + v.w * v.w;
+    if (outp) {
+      uint2 o;
+      o.x = pack_bf16x2(v.x, v.y);
+      o.y = pack_bf16x2(v.z, v.w);
+      *reinterpret_cast<uint2 *>(outp + j) = o;
+    }
+  }
+  if (w == nullptr) return;
+  ss = block_sum(ss, red);
+  const float inv = 1.0f / sqrtf(ss / (float)H + eps);
+  for (int j = threadIdx.x * 4; j < H; j += EW_THREADS * 4) {
+    const float4 v = *reinterpret_cast<const float4 *>(xr + j);  // written by this thread above
+    const uint2 g = *reinterpret_cast<const uint2 *>(w + j);
+    uint2 o;
+    o.x = pack_bf16x2(v.x * inv * bf16_lo(g.x), v.y * inv * bf16_hi(g.x));
+    o.y = pack_bf16x2(v.z * inv * bf16_lo(g.y), v.w * inv * bf16_hi(g.y));
+    *reinterpret_cast<uint2 *>(h + (size_t)t * H + j) = o;
+  }
+}
+
+cudaError_t launch_residual_rmsnorm(float *x, const float *part, int splits, long long split_stride,
+                                    const void *ln_w, float eps, int H, int T, void *h, const CallArgs *args,
+                                    bool write_out_hidden, cudaStream_t s) {
+  residual_rmsnorm_kernel<<<T, EW_THREADS, 0, s>>>(x, part, splits, split_stride, (const __nv_bfloat16 *)ln_w, eps,
+                                                   H, (__nv_bfloat16 *)h, args, write_out_hidden ? 1 : 0);
+  count_launch();
+  return cudaGetLastError();
+}
+
+// ---- S11a: final RMSNorm of the last row of each sequence -----------------------------------------------------
+__global__ void __launch_bounds__(EW_THREADS)
+final_norm_rows_kernel(const float *__restrict__ x, const CallArgs *__restrict__ args, int decode,
+                       const __nv_bfloat16 *__restrict__ wf, float eps, int H, __nv_bfloat16 *__restrict__ hl) {
+  __shared__ float red[32];
+  const int s = blockIdx.x;
+  const int row = decode ? s : (args->cu_q[s + 1] - 1);
+  const float *xr = x + (size_t)row * H;
+  float ss = 0.f;
+  for (int j = threadIdx.x; j < H; j += EW_THREADS) ss += xr[j] * xr[j];
+  ss = block_sum(ss, red);
+  const float inv = 1.0f / sqrtf(ss / (float)H + eps);
+  for (int j = threadIdx.x; j < H; j += EW_THREADS)
+    hl[(size_t)s * H + j] = __float2bfloat16_rn(xr[j] * inv * __bfloat162float(wf[j]));
+}
+
+cudaError_t launch_final_norm_rows(const float *x, const CallArgs *args, bool decode, const void *wf, float eps,
+                                   int H, int n_seqs, void *hl, cudaStream_t s) {
+  final_norm_rows_kernel<<<n_seqs, EW_THREADS, 0, s>>>(x, args, decode ? 1 : 0, (const __nv_bfloat16 *)wf, eps, H,
+                                                       (__nv_bfloat16 *)hl);
+  count_launch();
+  return cudaGetLastError();
+}
+
+// ---- S11b: reduce logits splits, copy out, argmax (lowest index among maxima) ---------------------------------
+__global__ void __launch_bounds__(1024)
+logits_argmax_kernel(const float *__restrict__ part, int splits, long long split_stride, int V,
+                     float *__restrict__ logits_ws, const CallArgs *__restrict__ args) {
+  __shared__ float smax[32];
+  __shared__ int sidx[32];
+  const int r = blockIdx.x;
+  float *outl = args->out_logits ? args->out_logits + (size_t)r * V : nullptr;
+  float best = -INFINITY;
+  int bi = 0x7fffffff;
+  for (int j = threadIdx.x; j < V; j += blockDim.x) {
+    float v = part[(size_t)r * V + j];
+    for (int s = 1; s < splits; ++s) v += part[(size_t)s * split_stride + (size_t)r * V + j];
+    if (splits > 1) logits_ws[(size_t)r * V + j] = v;
+    if (outl) outl[j] = v;
+    if (v > best) {  // j ascending per thread: strict > keeps the lowest index
+      best = v;
+      bi = j;
+    }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    const float ob = __shfl_xor_sync(0xffffffffu, best, o);
+    const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+    if (ob > best || (ob == best && oi < bi)) {
+      best = ob;
+      bi = oi;
+    }
+  }
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (lane == 0) {
+    smax[warp] = best;
+    sidx[warp] = bi;
+  }
+  __syncthreads();
+  if (warp == 0) {
+    const int nw = blockDim.x >> 5;
+    best = lane < nw ? smax[lane] : -INFINITY;
+    bi = lane < nw ? sidx[lane] : 0x7fffffff;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      const float ob = __shfl_xor_sync(0xffffffffu, best, o);
+      const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+      if (ob > best || (ob == best && oi < bi)) {
+        best = ob;
+        bi = oi;
+      }
+    }
+    if (lane == 0 && args->out_argmax) args->out_argmax[r] = bi;
+  }
+}
+
+cudaError_t launch_logits_argmax(const float *part, int splits, long long split_stride, int V, int n_rows,
+                                 float *logits_ws, const CallArgs *args, cudaStream_t s) {
+  logits_argmax_kernel<<<n_rows, 1024, 0, s>>>(part, splits, split_stride, V, logits_ws, args);
+  count_launch();
+  return cudaGetLastError();
+}
+
+// ---- S3 + S4 (+ S5 in prefill): one warp per (token, head) ----------------------------------------------------
+__global__ void __launch_bounds__(EW_THREADS) qkv_post_kernel(const QkvPostParams p) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int n_heads = p.n_q + 2 * p.n_kv;
+  const int head = blockIdx.y * (EW_THREADS / 32) + warp;
+  const int t = blockIdx.x;
+  if (head >= n_heads) return;
+  const int d = p.d, half = d >> 1;
+  const int ldq = n_heads * d;
+  const float *src = p.qkv_part + (size_t)t * ldq + (size_t)head * d;
+  // lane owns pairs (c, c+half) for c = lane, lane+32 (d = 128) or c = lane (d = 64)
+  float lo[2], hi[2];
+  const int npair = half >> 5;  // 1 or 2
+#pragma unroll
+  for (int i = 0; i < 2; ++i) {
+    lo[i] = hi[i] = 0.f;
+    if (i < npair) {
+      const int c = lane + 32 * i;
+      float a = src[c], b = src[c + half];
+      for (int s = 1; s < p.splits; ++s) {
+        a += src[(size_t)s * p.split_stride + c];
+        b += src[(size_t)s * p.split_stride + c + half];
+      }
+      lo[i] = a;
+      hi[i] = b;
+    }
+  }
+  const bool is_q = head < p.n_q;
+  const bool is_k = !is_q && head < p.n_q + p.n_kv;
+  int pos, seq;
+  if (p.decode) {
+    seq = t;
+    pos = p.args->ctx[t];
+  } else {
+    seq = p.tok_seq[t];
+    pos = p.tok_pos[t];
+  }
+  if (is_q || is_k) {
+    if (p.qk_norm) {
+      float ss = 0.f;
+#pragma unroll
+      for (int i = 0; i < 2; ++i) ss += lo[i] * lo[i] + hi[i] * hi[i];
+      ss = warp_sum(ss);
+      const float inv = 1.0f / sqrtf(ss / (float)d + p.eps);
+      const __nv_bfloat16 *g = (const __nv_bfloat16 *)(is_q ? p.q_norm : p.k_norm);
+#pragma unroll
+      for (int i = 0; i < 2; ++i)
+        if (i < npair) {
+          const int c = lane + 32 * i;
+          lo[i] = lo[i] * inv * __bfloat162float(g[c]);
+          hi[i] = hi[i] * inv * __bfloat162float(g[c + half]);
+        }
+    }
+    const float2 *rt = reinterpret_cast<const float2 *>(p.rope) + (size_t)pos * half;
+#pragma unroll
+    for (int i = 0; i < 2; ++i)
+      if (i < npair) {
+        const float2 cs = rt[lane + 32 * i];
+        const float a = lo[i], b = hi[i];
+        lo[i] = a * cs.x - b * cs.y;
+        hi[i] = b * cs.x + a * cs.y;
+      }
+  }
+  __nv_bfloat16 *dst;
+  if (is_q) {
+    dst = (__nv_bfloat16 *)p.q_out + (size_t)t * p.n_q * d + (size_t)head * d;
+  } else {
+    const int hk = is_k ? head - p.n_q : head - p.n_q - p.n_kv;
+    if (p.decode) {
+      dst = (__nv_bfloat16 *)p.kv_new + (size_t)t * 2 * p.n_kv * d + (size_t)(is_k ? 0 : p.n_kv * d) +
+            (size_t)hk * d;
+    } else {
+      const int page = p.args->block_tables[(size_t)seq * p.args->max_blocks + (pos >> 4)];
+      __nv_bfloat16 *pool = (__nv_bfloat16 *)(is_k ? p.kpool : p.vpool);
+      dst = pool + (((size_t)page * p.n_kv + hk) * 16 + (size_t)(pos & 15)) * d;
+    }
+  }
+#pragma unroll
+  for (int i = 0; i < 2; ++i)
+    if (i < npair) {
+      const int c = lane + 32 * i;
+      dst[c] = __float2bfloat16_rn(lo[i]);
+      dst[c + half] = __float2bfloat16_rn(hi[i]);
+    }
+}
+
+cudaError_t launch_qkv_post(const QkvPostParams &p, cudaStream_t s) {
+  const int n_heads = p.n_q + 2 * p.n_kv;
+  dim3 grid(p.T, (n_heads + EW_THREADS / 32 - 1) / (EW_THREADS / 32));
+  qkv_post_kernel<<<grid, EW_THREADS, 0, s>>>(p);
+  count_launch();
+  return cudaGetLastError();
+}
+
+}  // namespace ss

@@ -1,0 +1,150 @@
+// internal.h — host-side declarations shared by the translation units of libshuntstage.so (not installed).
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+namespace ss {
+
+// ---------------------------------------------------------------------------------------------------------------
+// tcgen05 GEMM (gemm_tcgen05.cu).  Orientation ("swap-AB", used for every shape): the UMMA M dimension (128 TMEM
+// lanes) runs over OUTPUT FEATURES, i.e. rows of the weight matrix W[N,K]; the UMMA N dimension (TMEM columns,
+// bn in {16,32,64,128,256}) runs over TOKENS, rows of X[T,K].  out[t][n] = sum_k X[t,k] W[n,k].
+// ---------------------------------------------------------------------------------------------------------------
+constexpr int GEMM_BM = 128;  // weight rows per tile
+constexpr int GEMM_BK = 64;   // K elements per stage (= one 128-byte swizzle row of bf16)
+
+enum GemmEpilogue { EPI_F32 = 0, EPI_SWIGLU_BF16 = 1, EPI_BF16 = 2 };
+
+struct GemmParams {
+  int n_seg;            // 1..3 weight segments laid side by side in the output (q | k | v)
+  int seg_rows[3];      // rows (output features) of each segment
+  int seg_tile0[3];     // first tile index of each segment
+  int seg_col[3];       // output column of each segment's row 0
+  int T, K;             // tokens, reduction length
+  int bn;               // tokens per tile (UMMA N)
+  int stages;           // smem pipeline depth
+  int kb_per_split;     // k-blocks (of 64) per split; gridDim.z = splits
+  int epi;              // GemmEpilogue
+  int ld_out;           // leading dimension (elements) of the output
+  long long split_stride;  // elements between consecutive splits' partial outputs (EPI_F32)
+  float *out_f32;
+  void *out_bf16;
+};
+
+struct GemmLaunch {
+  const CUtensorMap *a[3];  // weight maps, box {64, 128}; dual (SwiGLU): a[0] = gate, a[1] = up, n_seg = 1
+  const CUtensorMap *b;     // activation map, box {64, bn}
+  bool dual;
+  int splits;
+  GemmParams p;
+  cudaStream_t stream;
+};
+
+// Encode a 2-D bf16 row-major [rows, cols] tensor map with box {64 cols, box_rows}, SWIZZLE_128B.
+int make_tmap_bf16_2d(CUtensorMap *out, const void *base, uint64_t rows, uint64_t cols, uint32_t box_rows,
+                      bool weight_like);
+cudaError_t gemm_launch(const GemmLaunch &g);
+cudaError_t gemm_init();  // sets max dynamic smem attributes once
+int gemm_pick_bn(int T);  // smallest of {16,32,64,128,256} >= min(T,256)
+int gemm_pick_stages(int bn, bool dual);
+size_t gemm_smem_bytes(int bn, bool dual, int stages);
+
+// ---------------------------------------------------------------------------------------------------------------
+// element-wise / reduction kernels (elementwise.cu)
+// ---------------------------------------------------------------------------------------------------------------
+struct CallArgs {  // device-resident block of user pointers, rewritten before every call (graph-replay safe)
+  const void *hidden_in;       // bf16 [T,H] or null
+  const int32_t *token_ids;    // [T] or null
+  const int32_t *block_tables; // [n_seqs,max_blocks]
+  const int32_t *ctx;          // decode: context_lens[B]; prefill: ctx_before[n_seqs]
+  const int32_t *cu_q;         // prefill only
+  void *out_hidden;            // bf16 [T,H] or null
+  float *out_logits;           // [n_seqs,V] or null
+  int32_t *out_argmax;         // [n_seqs] or null
+  int32_t n_seqs, T, max_blocks, pad;
+};
+
+// x[t,:] = widen(input row t) (bf16 hidden or embedding gather); h[t,:] = bf16(rmsnorm(x[t,:]) * w)
+cudaError_t launch_input_rmsnorm(const CallArgs *args, const void *embed, const void *ln_w, float eps, int H,
+                                 int T, float *x, void *h, cudaStream_t s);
+// x[t,:] += sum_{s<splits} part[s][t,:]; then (w != null) h = bf16(rmsnorm(x) * w); (out_from_args) the bf16 of
+// x goes to args->out_hidden when that is non-null.
+cudaError_t launch_residual_rmsnorm(float *x, const float *part, int splits, long long split_stride,
+                                    const void *ln_w, float eps, int H, int T, void *h, const CallArgs *args,
+                                    bool write_out_hidden, cudaStream_t s);
+// gather the last row of each sequence: hl[s,:] = bf16(rmsnorm(x[last(s),:]) * wf)
+cudaError_t launch_final_norm_rows(const float *x, const CallArgs *args, bool decode, const void *wf, float eps,
+                                   int H, int n_seqs, void *hl, cudaStream_t s);
+// logits = sum of splits -> out (args->out_logits or internal), argmax (lowest index among maxima)
+cudaError_t launch_logits_argmax(const float *part, int splits, long long split_stride, int V, int n_rows,
+                                 float *logits_ws, const CallArgs *args, cudaStream_t s);
+
+struct QkvPostParams {
+  const float *qkv_part;   // [splits][T][Hq+2Hkv]
+  int splits;
+  long long split_stride;
+  int T, n_q, n_kv, d;
+  int qk_norm;
+  float eps;
+  const void *q_norm, *k_norm;  // bf16 [d]
+  const float *rope;            // [max_pos][d/2][2] (cos, sin)
+  void *q_out;                  // bf16 [T,Hq]
+  void *kv_new;                 // decode: bf16 [T,2*Hkv] (k | v), appended by the attention kernel
+  void *kpool, *vpool;          // prefill: this layer's pools, appended here
+  int n_pages;
+  const int32_t *tok_seq;       // prefill: [T] sequence of each token
+  const int32_t *tok_pos;       // prefill: [T] global position of each token
+  const CallArgs *args;
+  int decode;
+};
+cudaError_t launch_qkv_post(const QkvPostParams &p, cudaStream_t s);
+
+// ---------------------------------------------------------------------------------------------------------------
+// attention (attn_decode.cu, attn_prefill.cu)
+// ---------------------------------------------------------------------------------------------------------------
+struct DecodePlan {          // device buffers in the workspace
+  int32_t *cum_pages;        // [max_seqs+1] prefix sum of pages per sequence (pages = (ctx+1+15)/16)
+  int32_t *meta;             // [4]: total flattened pages (x n_kv), pages per worker warp, n_workers
+};
+cudaError_t launch_decode_plan(const CallArgs *args, int batch, int n_kv, int n_workers, DecodePlan plan,
+                               cudaStream_t s);
+struct DecodeAttnParams {
+  const void *q;             // bf16 [B,Hq]
+  const void *kv_new;        // bf16 [B,2*Hkv]
+  void *kpool, *vpool;       // this layer
+  int n_pages;
+  int batch, n_q, n_kv, d;
+  DecodePlan plan;
+  float *part_o;             // [n_slots][16][d]  (rows >= G unused)
+  float *part_ml;            // [n_slots][16][2]
+  void *out;                 // bf16 [B,Hq]
+  const CallArgs *args;
+  int n_workers;             // worker warps in the grid
+  int warps_per_cta;
+};
+cudaError_t launch_decode_attn(const DecodeAttnParams &p, cudaStream_t s);
+cudaError_t launch_decode_merge(const DecodeAttnParams &p, cudaStream_t s);
+cudaError_t attn_init();
+
+struct PrefillPlan {
+  int32_t *tok_seq;          // [max_tokens]
+  int32_t *tok_pos;          // [max_tokens]
+  int32_t *tile_cum;         // [max_seqs+1] prefix sum of 64-row query tiles per sequence
+};
+cudaError_t launch_prefill_plan(const CallArgs *args, int n_seqs, PrefillPlan plan, cudaStream_t s);
+struct PrefillAttnParams {
+  const void *q;             // bf16 [T,Hq]
+  const void *kpool, *vpool;
+  int n_seqs, T, n_q, n_kv, d;
+  PrefillPlan plan;
+  void *out;                 // bf16 [T,Hq]
+  const CallArgs *args;
+  int max_tiles;             // upper bound on query tiles = ceil(T/64) + n_seqs
+};
+cudaError_t launch_prefill_attn(const PrefillAttnParams &p, cudaStream_t s);
+
+void count_launch(int n = 1);  // stage.cu: per-thread launch counter hook
+
+}  // namespace ss

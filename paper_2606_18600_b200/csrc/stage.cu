@@ -1,0 +1,727 @@
+// stage.cu — host runtime and C-ABI of libshuntstage.so (include/shuntstage.h): argument validation, workspace
+// carving, TMA descriptors, the per-layer kernel sequence of ss_stage_decode / ss_stage_prefill (steps S0-S11 of
+// DESIGN.md; Table 2 of the paper), CUDA-graph capture of the decode step, and the host-side
+// page allocator.  The library never allocates device memory (the paper's engine attaches to tensors owned by
+// the Shared Tensor Store).
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <map>
+#include <string>
+#include <vector>
+
+#include "../../include/shuntstage.h"
+#include "internal.h"
+
+namespace ss {
+
+static thread_local int64_t g_launches = 0;
+static thread_local std::string g_cuda_err;
+void count_launch(int n) { g_launches += n; }
+
+static int cuda_fail(cudaError_t e, const char *where) {
+  g_cuda_err = std::string(where) + ": " + cudaGetErrorString(e);
+  return SS_ERR_CUDA;
+}
+#define CK(call)                                          \
+  do {                                                    \
+    cudaError_t e__ = (call);                             \
+    if (e__ != cudaSuccess) return cuda_fail(e__, #call); \
+  } while (0)
+
+constexpr int S_MAX = 8;           // max K-splits of a projection
+constexpr int SPLIT_ROWS = 256;    // split-K is only used when T <= SPLIT_ROWS
+constexpr int MAX_WORKERS = 4096;  // upper bound on decode-attention worker warps (sizes the partial buffers)
+
+static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+struct Carve {  // byte offsets into the workspace
+  size_t args, rope, x, h, qkv_part, q, kv_new, attn_out, proj_part, a, part_o, part_ml, cum_pages, meta, tok_seq,
+      tok_pos, tile_cum, hl, logits, total;
+};
+
+static bool dims_ok(const ss_model_dims *d, int l0, int l1, int *why) {
+  *why = SS_ERR_INVALID_ARG;
+  if (!d || l0 < 0 || l0 >= l1 || l1 > d->n_layers_total) return false;
+  if (d->hidden <= 0 || d->n_q_heads <= 0 || d->n_kv_heads <= 0 || d->ffn <= 0 || d->max_tokens <= 0 ||
+      d->max_seqs <= 0 || d->max_blocks_per_seq <= 0 || d->max_pos <= 0)
+    return false;
+  *why = SS_ERR_UNSUPPORTED;
+  if (d->head_dim != 64 && d->head_dim != 128) return false;
+  if (d->page_size != 16) return false;
+  if (d->n_q_heads % d->n_kv_heads != 0 || d->n_q_heads / d->n_kv_heads > 16) return false;
+  if (d->hidden % 8 != 0 || d->ffn % 8 != 0) return false;
+  return true;
+}
+
+static Carve carve(const ss_model_dims *d) {
+  Carve c;
+  const size_t Tm = (size_t)(d->max_tokens > d->max_seqs ? d->max_tokens : d->max_seqs);
+  const size_t H = d->hidden, Hq = (size_t)d->n_q_heads * d->head_dim, Hkv = (size_t)d->n_kv_heads * d->head_dim;
+  const size_t F = d->ffn, Nqkv = Hq + 2 * Hkv;
+  const size_t split_rows = (size_t)S_MAX * (Tm < (size_t)SPLIT_ROWS ? Tm : (size_t)SPLIT_ROWS);
+  const size_t part_rows = split_rows > Tm ? split_rows : Tm;
+  const size_t n_slots = (size_t)MAX_WORKERS + (size_t)d->max_seqs * d->n_kv_heads;
+  size_t o = 0;
+  auto take = [&](size_t bytes) {
+    size_t at = o;
+    o = align_up(o + bytes, 1024);
+    return at;
+  };
+  c.args = take(sizeof(CallArgs));
+  c.rope = take((size_t)d->max_pos * (d->head_dim / 2) * 2 * sizeof(float));
+  c.x = take(Tm * H * 4);
+  c.h = take(Tm * H * 2);
+  c.qkv_part = take(part_rows * Nqkv * 4);
+  c.q = take(Tm * Hq * 2);
+  c.kv_new = take((size_t)d->max_seqs * 2 * Hkv * 2);
+  c.attn_out = take(Tm * Hq * 2);
+  c.proj_part = take(part_rows * H * 4);
+  c.a = take(Tm * F * 2);
+  c.part_o = take(n_slots * 16 * d->head_dim * 4);
+  c.part_ml = take(n_slots * 32 * 4);
+  c.cum_pages = take(((size_t)d->max_seqs + 1) * 4);
+  c.meta = take(16);
+  c.tok_seq = take(Tm * 4);
+  c.tok_pos = take(Tm * 4);
+  c.tile_cum = take(((size_t)d->max_seqs + 1) * 4);
+  c.hl = take((size_t)d->max_seqs * H * 2);
+  c.logits = take(d->vocab > 0 ? (size_t)d->max_seqs * d->vocab * 4 : 0);
+  c.total = o;
+  return c;
+}
+
+struct LayerMaps {
+  CUtensorMap wq, wk, wv, wo, wg, wu, wd;
+};
+
+struct Graph {
+  cudaGraphExec_t exec = nullptr;
+  int64_t kernels = 0;
+};
+
+}  // namespace ss
+
+using namespace ss;
+
+struct ss_stage {
+  ss_model_dims d;
+  int l0, l1, L;
+  std::vector<ss_layer_weights> lw;
+  ss_edge_weights edge;
+  bool has_edge;
+  uint8_t *pool;
+  size_t pool_bytes;
+  int num_pages;
+  uint8_t *ws;
+  Carve c;
+  cudaStream_t stream;
+  int n_sm;
+  int n_workers;
+  std::vector<LayerMaps> maps;
+  CUtensorMap lm_map;
+  CUtensorMap b_h[5], b_attn[5], b_a[5], b_hl[5];  // activation maps for bn = 16,32,64,128,256
+  std::vector<int32_t> free_list;
+  std::vector<uint8_t> is_free;
+  int64_t launches;
+  std::map<int, Graph> graphs;  // key = batch*2 + tail
+  bool use_graph;
+  int force_split[3];  // qkv, o, down (0 = heuristic)
+  CallArgs *h_args;    // pinned host staging for the argument block
+
+  size_t layer_kv_elems() const { return (size_t)num_pages * d.n_kv_heads * 16 * d.head_dim; }
+  __nv_bfloat16 *kpool(int l) const { return (__nv_bfloat16 *)pool + (size_t)l * 2 * layer_kv_elems(); }
+  __nv_bfloat16 *vpool(int l) const { return kpool(l) + layer_kv_elems(); }
+  template <typename T>
+  T *at(size_t off) const { return (T *)(ws + off); }
+};
+
+
+static int env_int(const char *name, int dflt) {
+  const char *e = getenv(name);
+  return e ? atoi(e) : dflt;
+}
+
+extern "C" {
+
+const char *ss_strerror(int code) {
+  switch (code) {
+    case SS_OK: return "ok";
+    case SS_ERR_INVALID_ARG: return "invalid argument";
+    case SS_ERR_UNSUPPORTED: return "unsupported configuration";
+    case SS_ERR_CAPACITY: return "capacity exceeded";
+    case SS_ERR_NO_PAGES: return "not enough free KV pages";
+    case SS_ERR_BAD_PAGE: return "bad KV page id";
+    case SS_ERR_CUDA: return "CUDA error";
+    default: return "unknown error";
+  }
+}
+const char *ss_last_cuda_error(void) { return g_cuda_err.c_str(); }
+const char *ss_version(void) { return "shuntstage 0.1 (sm_100a)"; }
+
+size_t ss_stage_workspace_bytes(const ss_model_dims *dims, int l0, int l1) {
+  int why;
+  if (!dims_ok(dims, l0, l1, &why)) return 0;
+  return carve(dims).total;
+}
+
+size_t ss_kv_page_bytes(const ss_model_dims *dims, int l0, int l1) {
+  int why;
+  if (!dims_ok(dims, l0, l1, &why)) return 0;
+  return (size_t)(l1 - l0) * 2 * dims->n_kv_heads * 16 * dims->head_dim * 2;
+}
+
+int ss_stage_create(ss_stage **out, const ss_model_dims *dims, int l0, int l1, const ss_layer_weights *layers,
+                    const ss_edge_weights *edge, void *kv_pool, size_t kv_pool_bytes, void *workspace,
+                    size_t workspace_bytes, void *cuda_stream) {
+  int why;
+  if (!out) return SS_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (!dims_ok(dims, l0, l1, &why)) return why;
+  if (!layers || !kv_pool || !workspace) return SS_ERR_INVALID_ARG;
+  if (((uintptr_t)kv_pool & 1023) || ((uintptr_t)workspace & 1023)) return SS_ERR_UNSUPPORTED;
+  const int L = l1 - l0;
+  for (int l = 0; l < L; ++l) {
+    const ss_layer_weights &w = layers[l];
+    const void *req[] = {w.ln1, w.wq, w.wk, w.wv, w.wo, w.ln2, w.w_gate, w.w_up, w.w_down};
+    for (const void *p : req) {
+      if (!p) return SS_ERR_INVALID_ARG;
+      if ((uintptr_t)p & 15) return SS_ERR_UNSUPPORTED;
+    }
+    if (dims->qk_norm && (!w.q_norm || !w.k_norm)) return SS_ERR_INVALID_ARG;
+  }
+  if (edge && edge->lm_head && (!edge->final_norm || dims->vocab <= 0)) return SS_ERR_INVALID_ARG;
+  Carve c = carve(dims);
+  if (workspace_bytes < c.total) return SS_ERR_CAPACITY;
+  const size_t page_bytes = ss_kv_page_bytes(dims, l0, l1);
+  if (kv_pool_bytes < page_bytes) return SS_ERR_CAPACITY;
+
+  ss_stage *st = new ss_stage();
+  st->d = *dims;
+  st->l0 = l0; st->l1 = l1; st->L = L;
+  st->lw.assign(layers, layers + L);
+  st->has_edge = edge != nullptr;
+  if (edge) st->edge = *edge; else memset(&st->edge, 0, sizeof(st->edge));
+  st->pool = (uint8_t *)kv_pool;
+  st->pool_bytes = kv_pool_bytes;
+  st->num_pages = (int)(kv_pool_bytes / page_bytes);
+  st->ws = (uint8_t *)workspace;
+  st->c = c;
+  st->stream = (cudaStream_t)cuda_stream;
+  st->launches = 0;
+  st->use_graph = (cuda_stream != nullptr) && env_int("SS_NO_GRAPH", 0) == 0;
+  st->force_split[0] = env_int("SS_SPLIT_QKV", 0);
+  st->force_split[1] = env_int("SS_SPLIT_O", 0);
+  st->force_split[2] = env_int("SS_SPLIT_DOWN", 0);
+  st->h_args = nullptr;
+
+  auto fail = [&](int code) {
+    if (st->h_args) cudaFreeHost(st->h_args);
+    delete st;
+    return code;
+  };
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return fail(cuda_fail(e, "cudaGetDevice"));
+  e = cudaDeviceGetAttribute(&st->n_sm, cudaDevAttrMultiProcessorCount, dev);
+  if (e != cudaSuccess) return fail(cuda_fail(e, "cudaDeviceGetAttribute"));
+  int ctas_per_sm = env_int("SS_ATTN_CTAS_PER_SM", 2);
+  st->n_workers = st->n_sm * ctas_per_sm * 4;
+  if (st->n_workers > MAX_WORKERS) st->n_workers = MAX_WORKERS / 4 * 4;
+  if ((e = gemm_init()) != cudaSuccess) return fail(cuda_fail(e, "gemm_init"));
+  if ((e = attn_init()) != cudaSuccess) return fail(cuda_fail(e, "attn_init"));
+  if ((e = cudaMallocHost((void **)&st->h_args, sizeof(CallArgs))) != cudaSuccess)
+    return fail(cuda_fail(e, "cudaMallocHost"));
+
+  // RoPE table: cos/sin in double, stored fp32 (reading A10)
+  {
+    const int half = dims->head_dim / 2;
+    std::vector<float> tab((size_t)dims->max_pos * half * 2);
+    for (int c2 = 0; c2 < half; ++c2) {
+      const double f = (edge && edge->inv_freq) ? (double)edge->inv_freq[c2]
+                                                : pow((double)dims->rope_theta, -2.0 * (double)c2 / dims->head_dim);
+      for (int p = 0; p < dims->max_pos; ++p) {
+        const double ang = (double)p * f;
+        tab[((size_t)p * half + c2) * 2 + 0] = (float)cos(ang);
+        tab[((size_t)p * half + c2) * 2 + 1] = (float)sin(ang);
+      }
+    }
+    e = cudaMemcpyAsync(st->ws + c.rope, tab.data(), tab.size() * sizeof(float), cudaMemcpyHostToDevice, st->stream);
+    if (e != cudaSuccess) return fail(cuda_fail(e, "rope upload"));
+    e = cudaStreamSynchronize(st->stream);
+    if (e != cudaSuccess) return fail(cuda_fail(e, "rope upload sync"));
+  }
+
+  // TMA descriptors
+  const uint64_t H = dims->hidden, Hq = (uint64_t)dims->n_q_heads * dims->head_dim,
+                 Hkv = (uint64_t)dims->n_kv_heads * dims->head_dim, F = dims->ffn;
+  const uint64_t Tm = (uint64_t)(dims->max_tokens > dims->max_seqs ? dims->max_tokens : dims->max_seqs);
+  int rc = 0;
+  st->maps.resize(L);
+  for (int l = 0; l < L && rc == 0; ++l) {
+    const ss_layer_weights &w = layers[l];
+    LayerMaps &m = st->maps[l];
+    rc |= make_tmap_bf16_2d(&m.wq, w.wq, Hq, H, GEMM_BM, true);
+    rc |= make_tmap_bf16_2d(&m.wk, w.wk, Hkv, H, GEMM_BM, true);
+    rc |= make_tmap_bf16_2d(&m.wv, w.wv, Hkv, H, GEMM_BM, true);
+    rc |= make_tmap_bf16_2d(&m.wo, w.wo, H, Hq, GEMM_BM, true);
+    rc |= make_tmap_bf16_2d(&m.wg, w.w_gate, F, H, GEMM_BM, true);
+    rc |= make_tmap_bf16_2d(&m.wu, w.w_up, F, H, GEMM_BM, true);
+    rc |= make_tmap_bf16_2d(&m.wd, w.w_down, H, F, GEMM_BM, true);
+  }
+  if (rc == 0 && edge && edge->lm_head)
+    rc |= make_tmap_bf16_2d(&st->lm_map, edge->lm_head, (uint64_t)dims->vocab, H, GEMM_BM, true);
+  const int bns[5] = {16, 32, 64, 128, 256};
+  for (int i = 0; i < 5 && rc == 0; ++i) {
+    rc |= make_tmap_bf16_2d(&st->b_h[i], st->ws + c.h, Tm, H, bns[i], false);
+    rc |= make_tmap_bf16_2d(&st->b_attn[i], st->ws + c.attn_out, Tm, Hq, bns[i], false);
+    rc |= make_tmap_bf16_2d(&st->b_a[i], st->ws + c.a, Tm, F, bns[i], false);
+    rc |= make_tmap_bf16_2d(&st->b_hl[i], st->ws + c.hl, (uint64_t)dims->max_seqs, H, bns[i], false);
+  }
+  if (rc != 0) {
+    g_cuda_err = "cuTensorMapEncodeTiled failed (code " + std::to_string(rc) + ")";
+    return fail(SS_ERR_CUDA);
+  }
+
+  st->free_list.resize(st->num_pages);
+  for (int i = 0; i < st->num_pages; ++i) st->free_list[i] = st->num_pages - 1 - i;  // pop gives 0,1,2,...
+  st->is_free.assign(st->num_pages, 1);
+  *out = st;
+  return SS_OK;
+}
+
+int ss_stage_destroy(ss_stage *st) {
+  if (!st) return SS_ERR_INVALID_ARG;
+  for (auto &g : st->graphs)
+    if (g.second.exec) cudaGraphExecDestroy(g.second.exec);
+  if (st->h_args) cudaFreeHost(st->h_args);
+  delete st;
+  return SS_OK;
+}
+
+// ---- page pool --------------------------------------------------------------------------------------------------
+int ss_kv_num_pages(const ss_stage *st) { return st ? st->num_pages : SS_ERR_INVALID_ARG; }
+int ss_kv_num_free(const ss_stage *st) { return st ? (int)st->free_list.size() : SS_ERR_INVALID_ARG; }
+
+int ss_kv_alloc(ss_stage *st, int n, int32_t *out_page_ids) {
+  if (!st || n < 0 || (n > 0 && !out_page_ids)) return SS_ERR_INVALID_ARG;
+  if ((size_t)n > st->free_list.size()) return SS_ERR_NO_PAGES;
+  for (int i = 0; i < n; ++i) {
+    const int32_t id = st->free_list.back();
+    st->free_list.pop_back();
+    st->is_free[id] = 0;
+    out_page_ids[i] = id;
+  }
+  return SS_OK;
+}
+
+int ss_kv_free(ss_stage *st, int n, const int32_t *page_ids) {
+  if (!st || n < 0 || (n > 0 && !page_ids)) return SS_ERR_INVALID_ARG;
+  int bad = -1;  // validate first (all-or-nothing); 2 marks "seen in this call" so duplicates are caught in O(n)
+  for (int i = 0; i < n; ++i) {
+    const int32_t id = page_ids[i];
+    if (id < 0 || id >= st->num_pages || st->is_free[id] != 0) {
+      bad = i;
+      break;
+    }
+    st->is_free[id] = 2;
+  }
+  if (bad >= 0) {
+    for (int i = 0; i < bad; ++i) st->is_free[page_ids[i]] = 0;
+    return SS_ERR_BAD_PAGE;
+  }
+  for (int i = 0; i < n; ++i) {
+    st->is_free[page_ids[i]] = 1;
+    st->free_list.push_back(page_ids[i]);
+  }
+  return SS_OK;
+}
+
+int64_t ss_stage_launch_count(const ss_stage *st) { return st ? st->launches : 0; }
+
+}  // extern "C"
+
+// ===================================================================================================================
+// the forward pass
+// ===================================================================================================================
+namespace ss {
+
+// K-split heuristic for the HBM-bound small-T case: enough CTAs to cover the SMs, each with a long enough K loop.
+static int pick_splits(const ss_stage *st, int tiles, int t_tiles, int nkb, int T, int forced) {
+  if (T > SPLIT_ROWS) return 1;
+  int s = 1;
+  if (forced > 0) {
+    s = forced;
+  } else if (tiles * t_tiles < st->n_sm) {
+    s = (st->n_sm + tiles * t_tiles - 1) / (tiles * t_tiles);
+    while (s > 1 && nkb / s < 16) --s;  // keep >= 16 k-blocks (1024 K elements) per CTA
+  }
+  if (s > S_MAX) s = S_MAX;
+  if (s > nkb) s = nkb;
+  if (s < 1) s = 1;
+  return s;
+}
+
+struct GemmOut {
+  int splits;
+  long long split_stride;
+};
+
+// one projection: out_f32 partials [splits][T][ld] (EPI_F32) or fused SwiGLU bf16 (dual)
+static cudaError_t run_gemm(const ss_stage *st, const CUtensorMap *const a[3], int n_seg, const int rows[3],
+                            bool dual, const CUtensorMap bmaps[5], int T, int K, float *out_f32, void *out_bf16,
+                            int ld_out, int forced_split, GemmOut *res) {
+  GemmLaunch g;
+  memset(&g, 0, sizeof(g));
+  GemmParams &p = g.p;
+  p.n_seg = n_seg;
+  int tiles = 0, col = 0;
+  for (int i = 0; i < 3; ++i) {
+    g.a[i] = a[i];
+    p.seg_rows[i] = i < n_seg ? rows[i] : 0;
+    p.seg_tile0[i] = tiles;
+    p.seg_col[i] = col;
+    if (i < n_seg) {
+      tiles += (rows[i] + GEMM_BM - 1) / GEMM_BM;
+      col += rows[i];
+    }
+  }
+  p.T = T;
+  p.K = K;
+  p.bn = gemm_pick_bn(T);
+  p.stages = gemm_pick_stages(p.bn, dual);
+  const int nkb = (K + GEMM_BK - 1) / GEMM_BK;
+  const int t_tiles = (T + p.bn - 1) / p.bn;
+  int splits = dual ? 1 : pick_splits(st, tiles, t_tiles, nkb, T, forced_split);
+  p.kb_per_split = (nkb + splits - 1) / splits;
+  splits = (nkb + p.kb_per_split - 1) / p.kb_per_split;
+  p.epi = dual ? EPI_SWIGLU_BF16 : EPI_F32;
+  p.ld_out = ld_out;
+  p.split_stride = (long long)T * ld_out;
+  p.out_f32 = out_f32;
+  p.out_bf16 = out_bf16;
+  g.b = &bmaps[p.bn == 16 ? 0 : p.bn == 32 ? 1 : p.bn == 64 ? 2 : p.bn == 128 ? 3 : 4];
+  g.dual = dual;
+  g.splits = splits;
+  g.stream = st->stream;
+  if (res) {
+    res->splits = splits;
+    res->split_stride = p.split_stride;
+  }
+  return gemm_launch(g);
+}
+
+#define CKE(call)                      \
+  do {                                 \
+    cudaError_t e__ = (call);          \
+    if (e__ != cudaSuccess) return e__; \
+  } while (0)
+
+// enqueue every kernel of one call; `decode` selects the q_len == 1 fast path
+static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T, bool tail) {
+  const ss_model_dims &d = st->d;
+  const int H = d.hidden, dh = d.head_dim, Hq = d.n_q_heads * dh, Hkv = d.n_kv_heads * dh, F = d.ffn;
+  const int Nqkv = Hq + 2 * Hkv;
+  const Carve &c = st->c;
+  const CallArgs *args = st->at<CallArgs>(c.args);
+  float *x = st->at<float>(c.x);
+  void *h = st->at<void>(c.h);
+  float *qkv_part = st->at<float>(c.qkv_part);
+  float *proj_part = st->at<float>(c.proj_part);
+  cudaStream_t s = st->stream;
+
+  DecodePlan dplan{st->at<int32_t>(c.cum_pages), st->at<int32_t>(c.meta)};
+  PrefillPlan pplan{st->at<int32_t>(c.tok_seq), st->at<int32_t>(c.tok_pos), st->at<int32_t>(c.tile_cum)};
+  if (decode)
+    CKE(launch_decode_plan(args, n_seqs, d.n_kv_heads, st->n_workers, dplan, s));
+  else
+    CKE(launch_prefill_plan(args, n_seqs, pplan, s));
+  CKE(launch_input_rmsnorm(args, st->edge.embed, st->lw[0].ln1, d.rms_eps, H, T, x, h, s));
+
+  for (int l = 0; l < st->L; ++l) {
+    const ss_layer_weights &w = st->lw[l];
+    const LayerMaps &m = st->maps[l];
+    GemmOut go;
+    {  // S2: QKV projection -> fp32 partials [splits][T][Hq+2Hkv]
+      const CUtensorMap *a[3] = {&m.wq, &m.wk, &m.wv};
+      const int rows[3] = {Hq, Hkv, Hkv};
+      CKE(run_gemm(st, a, 3, rows, false, st->b_h, T, H, qkv_part, nullptr, Nqkv, st->force_split[0], &go));
+    }
+    QkvPostParams qp;
+    memset(&qp, 0, sizeof(qp));
+    qp.qkv_part = qkv_part;
+    qp.splits = go.splits;
+    qp.split_stride = go.split_stride;
+    qp.T = T; qp.n_q = d.n_q_heads; qp.n_kv = d.n_kv_heads; qp.d = dh;
+    qp.qk_norm = d.qk_norm;
+    qp.eps = d.rms_eps;
+    qp.q_norm = w.q_norm; qp.k_norm = w.k_norm;
+    qp.rope = st->at<float>(c.rope);
+    qp.q_out = st->at<void>(c.q);
+    qp.kv_new = st->at<void>(c.kv_new);
+    qp.kpool = st->kpool(l); qp.vpool = st->vpool(l);
+    qp.n_pages = st->num_pages;
+    qp.tok_seq = pplan.tok_seq; qp.tok_pos = pplan.tok_pos;
+    qp.args = args;
+    qp.decode = decode ? 1 : 0;
+    CKE(launch_qkv_post(qp, s));  // S3, S4 (+S5 in prefill)
+
+    if (decode) {  // S5 + S6a
+      DecodeAttnParams ap;
+      memset(&ap, 0, sizeof(ap));
+      ap.q = st->at<void>(c.q);
+      ap.kv_new = st->at<void>(c.kv_new);
+      ap.kpool = st->kpool(l); ap.vpool = st->vpool(l);
+      ap.n_pages = st->num_pages;
+      ap.batch = n_seqs; ap.n_q = d.n_q_heads; ap.n_kv = d.n_kv_heads; ap.d = dh;
+      ap.plan = dplan;
+      ap.part_o = st->at<float>(c.part_o);
+      ap.part_ml = st->at<float>(c.part_ml);
+      ap.out = st->at<void>(c.attn_out);
+      ap.args = args;
+      ap.n_workers = st->n_workers;
+      ap.warps_per_cta = 4;
+      CKE(launch_decode_attn(ap, s));
+      CKE(launch_decode_merge(ap, s));
+    } else {  // S6b
+      PrefillAttnParams ap;
+      memset(&ap, 0, sizeof(ap));
+      ap.q = st->at<void>(c.q);
+      ap.kpool = st->kpool(l); ap.vpool = st->vpool(l);
+      ap.n_seqs = n_seqs; ap.T = T; ap.n_q = d.n_q_heads; ap.n_kv = d.n_kv_heads; ap.d = dh;
+      ap.plan = pplan;
+      ap.out = st->at<void>(c.attn_out);
+      ap.args = args;
+      ap.max_tiles = (T + 63) / 64 + n_seqs;
+      CKE(launch_prefill_attn(ap, s));
+    }
+    {  // S7: output projection, then S8: x1 = x + o Wo^T ; h2 = rmsnorm(x1; ln2)
+      const CUtensorMap *a[3] = {&m.wo, nullptr, nullptr};
+      const int rows[3] = {H, 0, 0};
+      CKE(run_gemm(st, a, 1, rows, false, st->b_attn, T, Hq, proj_part, nullptr, H, st->force_split[1], &go));
+      CKE(launch_residual_rmsnorm(x, proj_part, go.splits, go.split_stride, w.ln2, d.rms_eps, H, T, h, args, false,
+                                  s));
+    }
+    {  // S9: gate/up + SwiGLU fused -> a bf16 [T,F]
+      const CUtensorMap *a[3] = {&m.wg, &m.wu, nullptr};
+      const int rows[3] = {F, 0, 0};
+      CKE(run_gemm(st, a, 1, rows, true, st->b_h, T, H, nullptr, st->at<void>(c.a), F, 0, &go));
+    }
+    {  // S10: down projection + residual, then the next layer's RMSNorm-1 (or the stage output)
+      const CUtensorMap *a[3] = {&m.wd, nullptr, nullptr};
+      const int rows[3] = {H, 0, 0};
+      CKE(run_gemm(st, a, 1, rows, false, st->b_a, T, F, proj_part, nullptr, H, st->force_split[2], &go));
+      const bool last = (l == st->L - 1);
+      const void *next_ln = last ? nullptr : st->lw[l + 1].ln1;
+      CKE(launch_residual_rmsnorm(x, proj_part, go.splits, go.split_stride, next_ln, d.rms_eps, H, T, h, args, last,
+                                  s));
+    }
+  }
+  if (tail) {  // S11: final norm of each sequence's last row, lm_head, argmax
+    GemmOut go;
+    CKE(launch_final_norm_rows(x, args, decode, st->edge.final_norm, d.rms_eps, H, n_seqs, st->at<void>(c.hl), s));
+    const CUtensorMap *a[3] = {&st->lm_map, nullptr, nullptr};
+    const int rows[3] = {d.vocab, 0, 0};
+    // the partial buffer of the logits is the logits workspace itself (never split: V/128 tiles cover the SMs)
+    CKE(run_gemm(st, a, 1, rows, false, st->b_hl, n_seqs, H, st->at<float>(c.logits), nullptr, d.vocab, 1, &go));
+    CKE(launch_logits_argmax(st->at<float>(c.logits), 1, 0, d.vocab, n_seqs, st->at<float>(c.logits), args, s));
+  }
+  return cudaSuccess;
+}
+
+static int common_checks(ss_stage *st, int n_seqs, int T, const void *hidden, const int32_t *ids,
+                         const int32_t *bt, int max_blocks, const int32_t *ctx, float *out_logits,
+                         int32_t *out_argmax) {
+  if (!st || n_seqs <= 0 || T <= 0 || !bt || !ctx || max_blocks <= 0) return SS_ERR_INVALID_ARG;
+  if ((hidden == nullptr) == (ids == nullptr)) return SS_ERR_INVALID_ARG;
+  if (ids && (!st->edge.embed || st->l0 != 0)) return SS_ERR_INVALID_ARG;
+  if ((out_logits || out_argmax) && !st->edge.lm_head) return SS_ERR_INVALID_ARG;
+  if (n_seqs > st->d.max_seqs || max_blocks > st->d.max_blocks_per_seq) return SS_ERR_CAPACITY;
+  if (hidden && ((uintptr_t)hidden & 15)) return SS_ERR_UNSUPPORTED;
+  return SS_OK;
+}
+
+static int upload_args(ss_stage *st, const CallArgs &a) {
+  // the previous call's copy may still be in flight from the same pinned block: the stream orders the copies,
+  // but the host must not overwrite the block before the previous copy has read it
+  static thread_local cudaEvent_t ev = nullptr;
+  if (!ev) CK(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+  CK(cudaEventSynchronize(ev));
+  *st->h_args = a;
+  CK(cudaMemcpyAsync(st->ws + st->c.args, st->h_args, sizeof(CallArgs), cudaMemcpyHostToDevice, st->stream));
+  CK(cudaEventRecord(ev, st->stream));
+  return SS_OK;
+}
+
+}  // namespace ss
+
+extern "C" {
+
+int ss_stage_prefill(ss_stage *st, int n_seqs, const void *hidden_bf16, const int32_t *token_ids,
+                     const int32_t *cu_q, const int32_t *ctx_before, const int32_t *block_tables, int max_blocks,
+                     int total_tokens, void *out_hidden_bf16, float *out_logits, int32_t *out_argmax) {
+  int rc = common_checks(st, n_seqs, total_tokens, hidden_bf16, token_ids, block_tables, max_blocks, ctx_before,
+                         out_logits, out_argmax);
+  if (rc != SS_OK) return rc;
+  if (!cu_q) return SS_ERR_INVALID_ARG;
+  if (total_tokens > st->d.max_tokens) return SS_ERR_CAPACITY;
+  CallArgs a;
+  memset(&a, 0, sizeof(a));
+  a.hidden_in = hidden_bf16; a.token_ids = token_ids; a.block_tables = block_tables; a.ctx = ctx_before;
+  a.cu_q = cu_q; a.out_hidden = out_hidden_bf16; a.out_logits = out_logits; a.out_argmax = out_argmax;
+  a.n_seqs = n_seqs; a.T = total_tokens; a.max_blocks = max_blocks;
+  if ((rc = upload_args(st, a)) != SS_OK) return rc;
+  const int64_t before = g_launches;
+  cudaError_t e = enqueue_forward(st, false, n_seqs, total_tokens, out_logits || out_argmax);
+  st->launches += g_launches - before;
+  if (e != cudaSuccess) return cuda_fail(e, "ss_stage_prefill");
+  return SS_OK;
+}
+
+int ss_stage_decode(ss_stage *st, int batch, const void *hidden_bf16, const int32_t *token_ids,
+                    const int32_t *block_tables, int max_blocks, const int32_t *context_lens,
+                    void *out_hidden_bf16, float *out_logits, int32_t *out_argmax) {
+  int rc = common_checks(st, batch, batch, hidden_bf16, token_ids, block_tables, max_blocks, context_lens,
+                         out_logits, out_argmax);
+  if (rc != SS_OK) return rc;
+  CallArgs a;
+  memset(&a, 0, sizeof(a));
+  a.hidden_in = hidden_bf16; a.token_ids = token_ids; a.block_tables = block_tables; a.ctx = context_lens;
+  a.out_hidden = out_hidden_bf16; a.out_logits = out_logits; a.out_argmax = out_argmax;
+  a.n_seqs = batch; a.T = batch; a.max_blocks = max_blocks;
+  if ((rc = upload_args(st, a)) != SS_OK) return rc;
+  const bool tail = out_logits || out_argmax;
+  if (!st->use_graph) {
+    const int64_t before = g_launches;
+    cudaError_t e = enqueue_forward(st, true, batch, batch, tail);
+    st->launches += g_launches - before;
+    if (e != cudaSuccess) return cuda_fail(e, "ss_stage_decode");
+    return SS_OK;
+  }
+  const int key = batch * 2 + (tail ? 1 : 0);
+  auto it = st->graphs.find(key);
+  if (it == st->graphs.end()) {
+    // capture the kernel sequence once; user pointers are reached through the device-side CallArgs block
+    cudaGraph_t graph = nullptr;
+    const int64_t before = g_launches;
+    CK(cudaStreamBeginCapture(st->stream, cudaStreamCaptureModeThreadLocal));
+    cudaError_t e = enqueue_forward(st, true, batch, batch, tail);
+    cudaError_t e2 = cudaStreamEndCapture(st->stream, &graph);
+    const int64_t n_kernels = g_launches - before;
+    if (e != cudaSuccess || e2 != cudaSuccess) {
+      if (graph) cudaGraphDestroy(graph);
+      return cuda_fail(e != cudaSuccess ? e : e2, "decode graph capture");
+    }
+    Graph gr;
+    e = cudaGraphInstantiate(&gr.exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGraphInstantiate");
+    gr.kernels = n_kernels;
+    it = st->graphs.emplace(key, gr).first;
+  }
+  CK(cudaGraphLaunch(it->second.exec, st->stream));
+  st->launches += it->second.kernels;
+  return SS_OK;
+}
+
+}  // extern "C"
+
+// ===================================================================================================================
+// op-level entry points: the same GEMM kernel, stand-alone (per-kernel parity tests, profiling)
+// ===================================================================================================================
+namespace ss {
+__global__ void reduce_splits_kernel(const float *__restrict__ part, int splits, long long stride, long long n,
+                                     float *__restrict__ out) {
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+    float v = part[i];
+    for (int s = 1; s < splits; ++s) v += part[(long long)s * stride + i];
+    out[i] = v;
+  }
+}
+}  // namespace ss
+
+extern "C" {
+
+int ss_op_gemm_bf16(const void *x_dev, const void *w_dev, float *c_dev, int T, int N, int K, int splits,
+                    void *scratch_dev, void *cuda_stream) {
+  if (!x_dev || !w_dev || !c_dev || T <= 0 || N <= 0 || K <= 0 || splits < 1) return SS_ERR_INVALID_ARG;
+  if (K % 8 != 0 || ((uintptr_t)x_dev & 15) || ((uintptr_t)w_dev & 15)) return SS_ERR_UNSUPPORTED;
+  if (splits > 1 && !scratch_dev) return SS_ERR_INVALID_ARG;
+  cudaError_t e = gemm_init();
+  if (e != cudaSuccess) return cuda_fail(e, "gemm_init");
+  CUtensorMap ta, tb;
+  GemmLaunch g;
+  memset(&g, 0, sizeof(g));
+  GemmParams &p = g.p;
+  p.bn = gemm_pick_bn(T);
+  if (make_tmap_bf16_2d(&ta, w_dev, (uint64_t)N, (uint64_t)K, GEMM_BM, true) != 0 ||
+      make_tmap_bf16_2d(&tb, x_dev, (uint64_t)T, (uint64_t)K, (uint32_t)p.bn, false) != 0) {
+    g_cuda_err = "cuTensorMapEncodeTiled failed";
+    return SS_ERR_CUDA;
+  }
+  const int nkb = (K + GEMM_BK - 1) / GEMM_BK;
+  if (splits > nkb) splits = nkb;
+  p.n_seg = 1;
+  p.seg_rows[0] = N;
+  p.T = T; p.K = K;
+  p.stages = gemm_pick_stages(p.bn, false);
+  p.kb_per_split = (nkb + splits - 1) / splits;
+  splits = (nkb + p.kb_per_split - 1) / p.kb_per_split;
+  p.epi = EPI_F32;
+  p.ld_out = N;
+  p.split_stride = (long long)T * N;
+  p.out_f32 = splits > 1 ? (float *)scratch_dev : c_dev;
+  g.a[0] = &ta; g.b = &tb; g.dual = false; g.splits = splits; g.stream = (cudaStream_t)cuda_stream;
+  e = gemm_launch(g);
+  if (e != cudaSuccess) return cuda_fail(e, "gemm_launch");
+  if (splits > 1) {
+    const long long n = (long long)T * N;
+    int blocks = (int)((n + 255) / 256 > 4096 ? 4096 : (n + 255) / 256);
+    reduce_splits_kernel<<<blocks, 256, 0, (cudaStream_t)cuda_stream>>>((const float *)scratch_dev, splits, n, n,
+                                                                         c_dev);
+    count_launch();
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "reduce_splits");
+  }
+  return SS_OK;
+}
+
+int ss_op_gemm_swiglu_bf16(const void *x_dev, const void *wg_dev, const void *wu_dev, void *a_dev, int T, int F,
+                           int K, void *cuda_stream) {
+  if (!x_dev || !wg_dev || !wu_dev || !a_dev || T <= 0 || F <= 0 || K <= 0) return SS_ERR_INVALID_ARG;
+  if (K % 8 != 0 || ((uintptr_t)x_dev & 15) || ((uintptr_t)wg_dev & 15) || ((uintptr_t)wu_dev & 15))
+    return SS_ERR_UNSUPPORTED;
+  cudaError_t e = gemm_init();
+  if (e != cudaSuccess) return cuda_fail(e, "gemm_init");
+  CUtensorMap tg, tu, tb;
+  GemmLaunch g;
+  memset(&g, 0, sizeof(g));
+  GemmParams &p = g.p;
+  p.bn = gemm_pick_bn(T);
+  if (make_tmap_bf16_2d(&tg, wg_dev, (uint64_t)F, (uint64_t)K, GEMM_BM, true) != 0 ||
+      make_tmap_bf16_2d(&tu, wu_dev, (uint64_t)F, (uint64_t)K, GEMM_BM, true) != 0 ||
+      make_tmap_bf16_2d(&tb, x_dev, (uint64_t)T, (uint64_t)K, (uint32_t)p.bn, false) != 0) {
+    g_cuda_err = "cuTensorMapEncodeTiled failed";
+    return SS_ERR_CUDA;
+  }
+  const int nkb = (K + GEMM_BK - 1) / GEMM_BK;
+  p.n_seg = 1;
+  p.seg_rows[0] = F;
+  p.T = T; p.K = K;
+  p.stages = gemm_pick_stages(p.bn, true);
+  p.kb_per_split = nkb;
+  p.epi = EPI_SWIGLU_BF16;
+  p.ld_out = F;
+  p.out_bf16 = a_dev;
+  g.a[0] = &tg; g.a[1] = &tu; g.b = &tb; g.dual = true; g.splits = 1; g.stream = (cudaStream_t)cuda_stream;
+  e = gemm_launch(g);
+  if (e != cudaSuccess) return cuda_fail(e, "gemm_launch");
+  return SS_OK;
+}
+
+}  // extern "C"
