@@ -101,12 +101,12 @@ size_t ss_kv_page_bytes(const ss_model_dims *dims, int l0, int l1);
 
 /*
  * Create a stage for layers [l0,l1).  `layers` is a HOST array of l1-l0 structs (copied).  `edge` may be NULL.
- * kv_pool: dev, 1024-byte aligned, layout (bf16, contiguous; part of the contract because page contents are
+ * kv_pool: dev, 256-byte aligned, layout (bf16, contiguous; part of the contract because page contents are
  * compared bit for bit):
  *     pool[layer - l0][kv in {0:K,1:V}][page][h_kv][slot 0..15][c 0..d-1]
  * with num_pages = kv_pool_bytes / ss_kv_page_bytes(); the token at position p of a sequence whose block-table
  * row is bt lives in page bt[p >> 4], slot p & 15 (paged KV cache: PAPER.md:265, 271; [31] PAPER.md:540).
- * workspace: dev, 1024-byte aligned, >= ss_stage_workspace_bytes().  cuda_stream: a cudaStream_t (may be 0).
+ * workspace: dev, 256-byte aligned, >= ss_stage_workspace_bytes().  cuda_stream: a cudaStream_t (may be 0).
  * The call uploads the RoPE table and builds TMA descriptors; it synchronises the stream once.
  */
 int ss_stage_create(ss_stage **out, const ss_model_dims *dims, int l0, int l1,

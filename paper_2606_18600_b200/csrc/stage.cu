@@ -184,7 +184,7 @@ int ss_stage_create(ss_stage **out, const ss_model_dims *dims, int l0, int l1, c
   *out = nullptr;
   if (!dims_ok(dims, l0, l1, &why)) return why;
   if (!layers || !kv_pool || !workspace) return SS_ERR_INVALID_ARG;
-  if (((uintptr_t)kv_pool & 1023) || ((uintptr_t)workspace & 1023)) return SS_ERR_UNSUPPORTED;
+  if (((uintptr_t)kv_pool & 255) || ((uintptr_t)workspace & 255)) return SS_ERR_UNSUPPORTED;
   const int L = l1 - l0;
   for (int l = 0; l < L; ++l) {
     const ss_layer_weights &w = layers[l];

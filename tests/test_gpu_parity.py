@@ -1,0 +1,405 @@
+"""Parity of the CUDA path (through the C-ABI) with the CPU oracle on the same seeded inputs.  All -m gpu.
+
+Tolerances (north_star): stage-output hidden max relative error 2e-2 (reading A15: per row ||g-r||inf / ||r||inf),
+per layer 1e-2, bit-exact KV indexing / page bytes outside written slots / argmax kernel; KV values vs the R1
+oracle per reading A13(iii).
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import Oracle
+from paper_2606_18600_b200 import synth
+from tests import helpers as hp
+
+pytestmark = pytest.mark.gpu
+
+F32 = Oracle("f32")
+STAGE_TOL = 2e-2
+LAYER_TOL = 1e-2
+
+
+def _gh():
+    from tests import gpu_helpers
+    return gpu_helpers
+
+
+def f32b(b):
+    return synth.bf16_bits_to_f32(np.asarray(b))
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# op level: the tcgen05 GEMM against the oracle's projection (Table 2 GEMM rows)
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("T,N,K,splits", [
+    (64, 256, 256, 1), (4, 512, 256, 1), (7, 688, 256, 1), (5, 256, 688, 1), (64, 1024, 2048, 4),
+    (130, 384, 512, 2), (300, 200, 1000, 1), (16, 128, 64, 1), (1, 8, 64, 1), (33, 3000, 4096, 3),
+])
+def test_op_gemm_vs_oracle(T, N, K, splits):
+    from paper_2606_18600_b200 import binding
+    g = torch.Generator().manual_seed(T * 7 + N + K)
+    x = synth.randn_bf16((T, K), 1.0, g)
+    w = synth.randn_bf16((N, K), 0.05, g)
+    want = F32.matmul(f32b(synth.bits(x)), synth.bits(w))
+    got = binding.op_gemm_bf16(x.cuda(), w.cuda(), splits=splits)
+    torch.cuda.synchronize()
+    got = got.cpu().numpy()
+    scale = np.abs(want).max()
+    assert np.abs(got - want).max() <= 2e-5 * scale * np.sqrt(K / 64) + 1e-6
+
+
+@pytest.mark.parametrize("T,F,K", [(64, 256, 256), (4, 688, 256), (130, 1376, 512), (300, 200, 1000), (16, 128, 64)])
+def test_op_gemm_swiglu_vs_oracle(T, F, K):
+    from paper_2606_18600_b200 import binding
+    g = torch.Generator().manual_seed(T + F + K)
+    x = synth.randn_bf16((T, K), 1.0, g)
+    wg = synth.randn_bf16((F, K), 0.08, g)
+    wu = synth.randn_bf16((F, K), 0.08, g)
+    xf = f32b(synth.bits(x))
+    want = F32.swiglu(F32.matmul(xf, synth.bits(wg)), F32.matmul(xf, synth.bits(wu)))
+    got = binding.op_gemm_swiglu_bf16(x.cuda(), wg.cuda(), wu.cuda())
+    torch.cuda.synchronize()
+    got = f32b(got.cpu().view(torch.int16).numpy().view(np.uint16))
+    # output is bf16: half an ulp (2^-9 relative) plus accumulation noise
+    assert np.abs(got - want).max() <= 2.0 ** -8 * np.abs(want).max() + 1e-6
+    assert np.abs(got - want).mean() <= 2.0 ** -9 * np.abs(want).mean() + 1e-7
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# whole stage on the tiny configs (cfg-1 of BASELINE.json and variants)
+# ---------------------------------------------------------------------------------------------------------------
+def _problem(shape, seed=0, proj_std=0.02, lens=None, with_edge=False, extra=4):
+    gh = _gh()
+    rng = np.random.default_rng(seed)
+    lens = synth.cfg1_contexts(seed) if lens is None else np.asarray(lens)
+    pb = synth.paged_batch(rng, lens, extra_tokens=extra, pool_factor=2.0)
+    P = gh.Problem(shape, seed, proj_std, n_pages=pb.n_pages_pool, max_tokens=int(lens.sum()) + 64,
+                   max_seqs=max(16, len(lens)), max_blocks=pb.max_blocks, with_edge=with_edge)
+    x = synth.bits(synth.hidden_rows(int(lens.sum()) + 64, shape.hidden, seed))
+    return P, lens.astype(np.int32), pb, x
+
+
+def _written_mask(pool_shape, bt, lens):
+    written = np.zeros((pool_shape[2], 16), dtype=bool)
+    for s in range(len(lens)):
+        for p in range(lens[s]):
+            written[bt[s, p >> 4], p & 15] = True
+    return np.broadcast_to(written[None, None, :, None, :, None], pool_shape)
+
+
+def _check_kv(pool_gpu, pool_r1, mask, first_layer_only_ulp=True):
+    # A13(i): indexing strict — bytes outside the written slots are untouched, written slots are all written
+    assert (pool_gpu[~mask] == 0x7FC1).all(), "a byte outside the written KV slots changed"
+    assert (pool_gpu[mask] != 0x7FC1).all(), "a KV slot that must be written still holds the sentinel"
+    # A13(iii): values vs the R1 oracle: first layer equal or adjacent bf16 values; deeper layers close
+    gh = _gh()
+    ulp = gh.bf16_ulp_distance(pool_gpu[0][mask[0]], pool_r1[0][mask[0]])
+    a, b = f32b(pool_gpu[0][mask[0]]), f32b(pool_r1[0][mask[0]])
+    # near zero (cancellation in RoPE / projections) an absolute bound replaces the ulp bound
+    ok = (ulp <= 1) | (np.abs(a - b) <= 2e-3 * np.abs(b).max())
+    assert ok.all(), f"first-layer KV differs by more than 1 bf16 ulp in {np.count_nonzero(~ok)} elements"
+    assert (ulp == 0).mean() > 0.97
+    for l in range(1, pool_gpu.shape[0]):
+        a, b = f32b(pool_gpu[l][mask[l]]).astype(np.float64), f32b(pool_r1[l][mask[l]]).astype(np.float64)
+        assert np.abs(a - b).max() <= 1e-2 * np.abs(b).max()
+
+
+@pytest.mark.parametrize("shape,proj_std", [(synth.TINY, 0.02), (synth.TINY, 0.16), (synth.TINY_QWEN, 0.02),
+                                            (synth.TINY128, 0.05)])
+def test_stage_prefill_then_decode_vs_oracle(shape, proj_std):
+    P, lens, pb, x = _problem(shape, proj_std=proj_std)
+    try:
+        T = int(lens.sum())
+        bt = pb.block_tables
+        # ---- prefill (migration recompute path)
+        pool0 = hp.new_pool(shape, pb.n_pages_pool, P.L)
+        want, _, cu = hp.run_oracle_prefill(F32, shape, P.wb, pool0, lens, bt, x[:T])
+        pool1 = hp.new_pool(shape, pb.n_pages_pool, P.L)
+        hp.run_oracle_prefill(F32, shape, P.wb, pool1, lens, bt, x[:T], rounding=1)
+        got = P.prefill(lens, bt, x[:T])
+        err = hp.rel_err_rows(got, want)
+        print(f"{shape.name} std={proj_std} prefill stage rel err {err:.3e}")
+        assert err < STAGE_TOL
+        mask = _written_mask(pool0.shape, bt, lens)
+        _check_kv(P.pool_bits(), pool1, mask)
+        # ---- two decode steps on top (both sides continue from their own pools)
+        for step in range(2):
+            xs = x[T + step * len(lens): T + (step + 1) * len(lens)]
+            want_d, _ = hp.run_oracle_decode(F32, shape, P.wb, pool0, lens + step, bt, xs)
+            hp.run_oracle_decode(F32, shape, P.wb, pool1, lens + step, bt, xs, rounding=1)
+            got_d = P.decode(lens + step, bt, xs)
+            err = hp.rel_err_rows(got_d, want_d)
+            print(f"{shape.name} decode step {step} stage rel err {err:.3e}")
+            assert err < STAGE_TOL
+        mask = _written_mask(pool0.shape, bt, lens + 2)
+        _check_kv(P.pool_bits(), pool1, mask)
+    finally:
+        P.close()
+
+
+def test_per_layer_teacher_forced_decode_vs_oracle():
+    """Reading A15 'per layer': a 1-layer stage run from the oracle's bf16-rounded layer input and the oracle's KV."""
+    shape = synth.TINY
+    gh = _gh()
+    rng = np.random.default_rng(3)
+    lens = synth.cfg1_contexts(3).astype(np.int32)
+    pb = synth.paged_batch(rng, lens, extra_tokens=2, pool_factor=1.5)
+    _, wb_all = hp.weights_bits(shape, 3)
+    T = int(lens.sum())
+    x = synth.bits(synth.hidden_rows(T + 8, shape.hidden, 3))
+    pool = hp.new_pool(shape, pb.n_pages_pool)
+    _, taps, _ = hp.run_oracle_prefill(F32, shape, wb_all, pool, lens, pb.block_tables, x[:T], taps=True)
+    xs = x[T:T + len(lens)]
+    pool_before = pool.copy()
+    _, dtaps = hp.run_oracle_decode(F32, shape, wb_all, pool, lens, pb.block_tables, xs, taps=True)
+    for l in range(shape.n_layers):
+        # oracle input of layer l at the decode step, rounded to bf16 (the stage boundary dtype)
+        x_in = f32b(xs) if l == 0 else dtaps[l - 1]["out"]
+        x_in_bits = synth.bits(torch.from_numpy(np.ascontiguousarray(x_in, dtype=np.float32)).to(torch.bfloat16))
+        pool_l = pool_before[l:l + 1].copy()
+        want = f32b(x_in_bits).copy()
+        w_l = [wb_all[l]]
+        F32.layer(hp.odims(shape), w_l[0], pool_l[0, 0], pool_l[0, 1], np.arange(len(lens) + 1, dtype=np.int32), lens,
+                  pb.block_tables, want)
+        # GPU: 1-layer stage holding layer l's weights and the oracle's KV for that layer
+        sub = synth.ModelShape(shape.name, shape.hidden, shape.n_q, shape.n_kv, shape.d, shape.ffn, 1, shape.eps,
+                               shape.theta, shape.qk_norm, shape.vocab)
+        P = gh.Problem(sub, 3, n_pages=pb.n_pages_pool, max_tokens=64, max_seqs=16, max_blocks=pb.max_blocks)
+        try:
+            tw = synth.layer_weights(shape, l, 3)
+            for k, v in tw.items():
+                if v is not None:
+                    P.dw[0][k].copy_(v.to("cuda:0"))
+            P.stage.pool_view().copy_(torch.from_numpy(pool_before[l:l + 1].view(np.int16).copy())
+                                      .view(torch.bfloat16).to("cuda:0"))
+            got = P.decode(lens, pb.block_tables, x_in_bits)
+        finally:
+            P.close()
+        err = hp.rel_err_rows(got, want)
+        print(f"layer {l} teacher-forced decode rel err {err:.3e}")
+        assert err < LAYER_TOL
+
+
+def test_migration_invariant_on_gpu():
+    """recompute (one prefill over prompt + generated tokens) must reproduce incremental decode:
+    same next-token hidden state within tolerance, KV pages equal or adjacent bf16 values."""
+    shape = synth.TINY
+    gh = _gh()
+    P, lens, pb, x = _problem(shape, seed=1)
+    Q, _, _, _ = _problem(shape, seed=1)
+    try:
+        bt = pb.block_tables
+        T = int(lens.sum())
+        cu = np.concatenate([[0], np.cumsum(lens)]).astype(np.int32)
+        gen = 3
+        prompt = lens - gen
+        # (a) recompute
+        P.prefill(lens, bt, x[:T])
+        # (b) incremental
+        rows = np.concatenate([np.arange(cu[s], cu[s] + prompt[s]) for s in range(len(lens))])
+        Q.prefill(prompt, bt, x[rows])
+        for g in range(gen):
+            rows = np.array([cu[s] + prompt[s] + g for s in range(len(lens))])
+            Q.decode(prompt + g, bt, x[rows])
+        pa, pq = P.pool_bits(), Q.pool_bits()
+        mask = _written_mask(pa.shape, bt, lens)
+        assert (pa[~mask] == 0x7FC1).all() and (pq[~mask] == 0x7FC1).all()
+        ulp = gh.bf16_ulp_distance(pa[mask], pq[mask])
+        a, b = f32b(pa[mask]), f32b(pq[mask])
+        assert ((ulp <= 2) | (np.abs(a - b) <= 4e-3 * np.abs(b).max())).all()
+        assert (ulp == 0).mean() > 0.9
+        # next decode step from both states
+        xs = x[T:T + len(lens)]
+        ya = P.decode(lens, bt, xs)
+        yq = Q.decode(lens, bt, xs)
+        assert hp.rel_err_rows(ya, yq) < STAGE_TOL
+        # and both match the oracle's (bitwise-invariant) answer
+        pool0 = hp.new_pool(shape, pb.n_pages_pool, P.L)
+        hp.run_oracle_prefill(F32, shape, P.wb, pool0, lens, bt, x[:T])
+        want, _ = hp.run_oracle_decode(F32, shape, P.wb, pool0, lens, bt, xs)
+        assert hp.rel_err_rows(ya, want) < STAGE_TOL and hp.rel_err_rows(yq, want) < STAGE_TOL
+    finally:
+        P.close()
+        Q.close()
+
+
+def test_chunked_prefill_and_mixed_batch_on_gpu():
+    """Prior context (ctx_before > 0) and q_len = 1 rows in a prefill call (mixed iteration, reading A19)."""
+    shape = synth.TINY_QWEN
+    P, lens, pb, x = _problem(shape, seed=2, lens=[70, 33, 150, 16])
+    try:
+        bt = pb.block_tables
+        first = np.array([40, 33 - 1, 100, 15], dtype=np.int32)      # chunk 1
+        cu_full = np.concatenate([[0], np.cumsum(lens)]).astype(np.int32)
+        rows1 = np.concatenate([np.arange(cu_full[s], cu_full[s] + first[s]) for s in range(4)])
+        rows2 = np.concatenate([np.arange(cu_full[s] + first[s], cu_full[s + 1]) for s in range(4)])
+        pool0 = hp.new_pool(shape, pb.n_pages_pool, P.L)
+        w1, _, _ = hp.run_oracle_prefill(F32, shape, P.wb, pool0, first, bt, x[rows1])
+        w2, _, _ = hp.run_oracle_prefill(F32, shape, P.wb, pool0, lens, bt, x[rows2], ctx_before=first)
+        g1 = P.prefill(first, bt, x[rows1])
+        g2 = P.prefill(lens, bt, x[rows2], ctx_before=first)    # seqs 1 and 3 have q_len = 1
+        assert hp.rel_err_rows(g1, w1) < STAGE_TOL
+        assert hp.rel_err_rows(g2, w2) < STAGE_TOL
+        mask = _written_mask(pool0.shape, bt, lens)
+        pg = P.pool_bits()
+        assert (pg[~mask] == 0x7FC1).all() and (pg[mask] != 0x7FC1).all()
+    finally:
+        P.close()
+
+
+def test_token_ids_logits_and_argmax():
+    """S0 embedding gather and S11 logits/argmax (Table 2 'Logits Calculation'; reading A14)."""
+    shape = synth.TINY
+    gh = _gh()
+    P, lens, pb, _ = _problem(shape, seed=4, with_edge=True)
+    try:
+        bt = pb.block_tables
+        T = int(lens.sum())
+        rng = np.random.default_rng(4)
+        ids = rng.integers(0, shape.vocab, T + len(lens)).astype(np.int32)
+        eb = {k: synth.bits(v) for k, v in P.edge_cpu.items()}
+        cu = np.concatenate([[0], np.cumsum(lens)]).astype(np.int32)
+        pool0 = hp.new_pool(shape, pb.n_pages_pool, P.L)
+        y, _ = F32.stage(hp.odims(shape), P.wb, pool0, cu, np.zeros_like(lens), bt, token_ids=ids[:T],
+                         embed=eb["embed"])
+        wl, wa, wm = F32.logits(hp.odims(shape), y[cu[1:] - 1], eb["final_norm"], eb["lm_head"])
+        out = torch.empty((T, shape.hidden), dtype=torch.bfloat16, device="cuda:0")
+        lg = torch.empty((len(lens), shape.vocab), dtype=torch.float32, device="cuda:0")
+        am = torch.empty((len(lens),), dtype=torch.int32, device="cuda:0")
+        a = (P.i32(cu), P.i32(np.zeros_like(lens)), P.i32(bt), P.i32(ids[:T]))
+        torch.cuda.synchronize()
+        P.stage.prefill(len(lens), a[0], a[1], a[2], T, token_ids=a[3], out_hidden=out, out_logits=lg,
+                        out_argmax=am)
+        P.stage.synchronize()
+        got = f32b(out.cpu().view(torch.int16).numpy().view(np.uint16))
+        assert hp.rel_err_rows(got, y) < STAGE_TOL
+        lg, am = lg.cpu().numpy(), am.cpu().numpy()
+        # (i) the argmax kernel is bit-exact on the GPU's own logits, ties -> lowest index
+        assert np.array_equal(am, np.argmax(lg, axis=1).astype(np.int32))
+        # (ii) ids equal the oracle's wherever the oracle's top-2 margin exceeds 8x the measured logit error
+        lerr = np.abs(lg - wl).max()
+        safe = wm > 8 * lerr
+        print(f"logit max err {lerr:.3e}; rows over margin {safe.sum()}/{len(safe)}")
+        assert np.array_equal(am[safe], wa[safe])
+        assert hp.rel_err_rows(lg, wl) < STAGE_TOL
+        # decode with token ids + logits
+        ids_d = ids[T:]
+        yd, _ = F32.stage(hp.odims(shape), P.wb, pool0, np.arange(len(lens) + 1, dtype=np.int32), lens, bt,
+                          token_ids=ids_d, embed=eb["embed"])
+        wl2, wa2, wm2 = F32.logits(hp.odims(shape), yd, eb["final_norm"], eb["lm_head"])
+        lg2 = torch.empty((len(lens), shape.vocab), dtype=torch.float32, device="cuda:0")
+        am2 = torch.empty((len(lens),), dtype=torch.int32, device="cuda:0")
+        a2 = (P.i32(bt), P.i32(lens), P.i32(ids_d))
+        torch.cuda.synchronize()
+        P.stage.decode(len(lens), a2[0], a2[1], token_ids=a2[2], out_logits=lg2, out_argmax=am2)
+        P.stage.synchronize()
+        lg2, am2 = lg2.cpu().numpy(), am2.cpu().numpy()
+        assert np.array_equal(am2, np.argmax(lg2, axis=1).astype(np.int32))
+        assert hp.rel_err_rows(lg2, wl2) < STAGE_TOL
+        safe2 = wm2 > 8 * np.abs(lg2 - wl2).max()
+        assert np.array_equal(am2[safe2], wa2[safe2])
+    finally:
+        P.close()
+
+
+def test_decode_graph_replay_is_deterministic_and_pointer_safe():
+    """The decode step is replayed from a CUDA graph; user pointers change between calls (device-side arg block)."""
+    shape = synth.TINY
+    P, lens, pb, x = _problem(shape, seed=5)
+    try:
+        bt = pb.block_tables
+        T = int(lens.sum())
+        P.prefill(lens, bt, x[:T])
+        xs = x[T:T + len(lens)]
+        snap = P.stage.pool_view().clone()
+        y1 = P.decode(lens, bt, xs)
+        n1 = P.stage.launch_count()
+        P.stage.pool_view().copy_(snap)
+        torch.cuda.synchronize()
+        y2 = P.decode(lens, bt, xs)            # new tensors -> new pointers, same values
+        n2 = P.stage.launch_count()
+        assert np.array_equal(y1, y2)
+        assert n2 - n1 > 0 and (n2 - n1) == 2 + shape.n_layers * 9
+    finally:
+        P.close()
+
+
+def test_edge_cases_and_error_codes():
+    shape = synth.TINY
+    gh = _gh()
+    from paper_2606_18600_b200 import binding
+    # single sequence, single token prompt (ctx = 0), then decode across a page boundary
+    P, lens, pb, x = _problem(shape, seed=6, lens=[1], extra=40)
+    try:
+        bt = pb.block_tables
+        pool0 = hp.new_pool(shape, pb.n_pages_pool, P.L)
+        want, _, _ = hp.run_oracle_prefill(F32, shape, P.wb, pool0, lens, bt, x[:1])
+        got = P.prefill(lens, bt, x[:1])
+        assert hp.rel_err_rows(got, want) < STAGE_TOL
+        for step in range(18):
+            xs = x[1 + step: 2 + step]
+            want, _ = hp.run_oracle_decode(F32, shape, P.wb, pool0, lens + step, bt, xs)
+            got = P.decode(lens + step, bt, xs)
+            assert hp.rel_err_rows(got, want) < STAGE_TOL, step
+        # error codes
+        st = P.stage
+        out = torch.empty((1, shape.hidden), dtype=torch.bfloat16, device="cuda:0")
+        btd, cx, hx = P.i32(bt), P.i32(lens), P.bf16(x[:1])
+        assert st.decode(1, btd, cx, hidden=None, token_ids=None, out_hidden=out, check=False) == -1
+        assert st.decode(1, btd, cx, hidden=hx, token_ids=cx, out_hidden=out, check=False) == -1
+        assert st.decode(1, btd, cx, token_ids=cx, out_hidden=out, check=False) == -1      # no embed
+        assert st.decode(1, btd, cx, hidden=hx, out_argmax=cx, check=False) == -1           # no lm_head
+        assert st.decode(10 ** 6, btd, cx, hidden=hx, out_hidden=out, check=False) == -3
+        assert st.prefill(1, cx, cx, btd, 10 ** 7, hidden=hx, out_hidden=out, check=False) == -3
+    finally:
+        P.close()
+    # unsupported dims
+    bad = binding.make_dims(synth.TINY, 64, 4, 8)
+    bad.head_dim = 96
+    lib = binding.load_library()
+    import ctypes as C
+    assert lib.ss_stage_workspace_bytes(C.byref(bad), 0, 2) == 0
+
+
+def test_kv_allocator_invariants():
+    """P15: alloc/free conserve the page multiset; double free / over-allocation return the documented errors."""
+    shape = synth.TINY
+    P, lens, pb, x = _problem(shape, seed=7)
+    try:
+        st = P.stage
+        n = st.num_pages()
+        assert st.num_free() == n
+        a = st.kv_alloc(5)
+        b = st.kv_alloc(n - 5)
+        assert sorted(a + b) == list(range(n)) and st.num_free() == 0
+        import ctypes as C
+        one = (C.c_int32 * 1)()
+        assert st.lib.ss_kv_alloc(st.h, 1, one) == -4
+        st.kv_free(a)
+        assert st.num_free() == 5
+        arr = (C.c_int32 * 2)(a[0], a[1])
+        assert st.lib.ss_kv_free(st.h, 2, arr) == -5 and st.num_free() == 5          # already free
+        arr = (C.c_int32 * 2)(b[0], b[0])
+        assert st.lib.ss_kv_free(st.h, 2, arr) == -5 and st.num_free() == 5          # duplicate in one call
+        arr = (C.c_int32 * 1)(n)
+        assert st.lib.ss_kv_free(st.h, 1, arr) == -5                                  # out of range
+        c = st.kv_alloc(5)
+        assert sorted(c) == sorted(a)
+        st.kv_free(b + c)
+        assert st.num_free() == n
+        rng = np.random.default_rng(0)
+        held = []
+        for _ in range(200):
+            if held and rng.random() < 0.5:
+                k = int(rng.integers(1, len(held) + 1))
+                idx = rng.permutation(len(held))[:k]
+                st.kv_free([held[i] for i in idx])
+                held = [h for i, h in enumerate(held) if i not in set(idx.tolist())]
+            else:
+                k = int(rng.integers(0, st.num_free() + 1))
+                got = st.kv_alloc(k)
+                assert not set(got) & set(held)
+                held += got
+            assert st.num_free() + len(held) == n and len(set(held)) == len(held)
+    finally:
+        P.close()
