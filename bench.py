@@ -1,0 +1,506 @@
+#!/usr/bin/env python
+"""bench.py — stage decode tokens/s (+ % of HBM roofline) and migration-recompute prefill tokens/s of one
+ShuntServe pipeline stage on B200, on synthetic workloads shaped like the paper's (BASELINE.json configs).
+
+Default (the driver's contract): `python bench.py --gpus 1 --steps K --warmup W` times K decode steps of the
+Llama-3.1-70B-shaped 20-layer stage (configs[1], "cfg2") and prints ONE JSON line.  A "step" is one pass of the
+whole hot path (steps S0-S11 of DESIGN.md) over one batch of 64 sequences.  N > 1 (torchrun): independent
+replicas, one per GPU, no data-path collective ("scaling": "weak").
+`--impl reference` times the CPU oracle (as it stands) on a bounded sample of the same workload.
+`--workload cfg3|cfg4|tiny` selects the other workloads for local measurement.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "tiny"])
+    ap.add_argument("--seed", type=int, default=0)
+    ap.add_argument("--layers", type=int, default=0, help="override the stage depth (debug only; marks the line)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return {"hbm_gbs": d["hbm_gbs"], "bf16_tflops": d["bf16_tflops"],
+                "bf16_tflops_sustained": d.get("bf16_tflops_sustained", d["bf16_tflops"]), "source": "measured"}
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "source": "fallback"}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.gpu = gpu_index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "200", "-i", str(self.gpu)], stdout=subprocess.PIPE, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for l in self.proc.stdout:
+            self.lines.append(l.strip())
+
+    def stop(self) -> dict:
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons, pw = [], [], set(), []
+        for l in self.lines:
+            f = [x.strip() for x in l.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); mx.append(float(f[2])); pw.append(float(f[3]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# workloads
+# ---------------------------------------------------------------------------------------------------------------
+def workload_spec(name, layers_override=0):
+    from paper_2606_18600_b200 import synth
+    if name == "cfg2":
+        shape, ctx, kind = synth.LLAMA70B, synth.cfg2_contexts, "decode"
+    elif name == "cfg3":
+        shape, ctx, kind = synth.QWEN32B, synth.cfg3_contexts, "decode"
+    elif name == "cfg4":
+        shape, ctx, kind = synth.LLAMA70B, synth.cfg4_lengths, "prefill"
+    else:
+        shape, ctx, kind = synth.TINY, synth.cfg1_contexts, "decode"
+    L = layers_override or shape.n_layers
+    if L != shape.n_layers:
+        shape = synth.ModelShape(shape.name, shape.hidden, shape.n_q, shape.n_kv, shape.d, shape.ffn, L, shape.eps,
+                                 shape.theta, shape.qk_norm, shape.vocab)
+    return shape, ctx, kind
+
+
+def decode_bytes_per_step(shape, ctx_now):
+    """Algorithmic HBM bytes of one decode step: weights once, every cached K/V
+    byte once (ctx+1 tokens incl. the new one), the new K/V written, stage input and output."""
+    B = len(ctx_now)
+    kv_tok = 2 * shape.hkv * 2
+    per_layer = 2 * shape.layer_params() + int((ctx_now + 1).sum()) * kv_tok + B * kv_tok
+    return shape.n_layers * per_layer + 2 * B * shape.hidden * 2
+
+
+def prefill_flops(shape, lens):
+    T = int(lens.sum())
+    pairs = int((lens.astype(np.int64) * (lens.astype(np.int64) + 1) // 2).sum())
+    return shape.n_layers * (2 * shape.layer_params() * T + 4 * shape.hq * pairs)
+
+
+def gpu_weights(shape, dev, seed):
+    """Random-init bf16 weights of the stage, generated on the device (synthetic; A21 value distributions)."""
+    import torch
+    g = torch.Generator(device=dev)
+    g.manual_seed(seed * 1_000_003 + 17)
+    H, Hq, Hkv, F, d = shape.hidden, shape.hq, shape.hkv, shape.ffn, shape.d
+
+    def mat(r, c):
+        return (torch.randn((r, c), generator=g, device=dev, dtype=torch.float32) * 0.02).to(torch.bfloat16)
+
+    def gain(n):
+        return (1 + 0.02 * torch.randn((n,), generator=g, device=dev, dtype=torch.float32)).to(torch.bfloat16)
+
+    layers = []
+    for _ in range(shape.n_layers):
+        layers.append({"ln1": gain(H), "wq": mat(Hq, H), "wk": mat(Hkv, H), "wv": mat(Hkv, H),
+                       "q_norm": gain(d) if shape.qk_norm else None, "k_norm": gain(d) if shape.qk_norm else None,
+                       "wo": mat(H, Hq), "ln2": gain(H), "w_gate": mat(F, H), "w_up": mat(F, H), "w_down": mat(H, F)})
+    return layers
+
+
+def cuda_time_ms(stream, fn, n):
+    """n calls of fn() on `stream`, timed with CUDA events recorded on that stream (ms total)."""
+    import torch
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    stream.synchronize()
+    e0.record(stream)
+    for i in range(n):
+        fn(i)
+    e1.record(stream)
+    stream.synchronize()
+    return e0.elapsed_time(e1)
+
+
+def run_decode(args, shape, ctx_fn, rank, world):
+    import torch
+    from paper_2606_18600_b200 import binding, synth
+    dev = torch.device(f"cuda:{int(os.environ.get('LOCAL_RANK', 0))}")
+    torch.cuda.set_device(dev)
+    K, W = args.steps, args.warmup
+    rng = np.random.default_rng(args.seed)
+    ctx0 = ctx_fn(args.seed).astype(np.int32)
+    B = len(ctx0)
+    total_steps = 2 * (K + W) + 8                        # device-timed pass + e2e pass
+    pb = synth.paged_batch(rng, ctx0, extra_tokens=total_steps + 1)
+    layers = gpu_weights(shape, dev, args.seed)
+    dims = binding.make_dims(shape, max_tokens=B, max_seqs=B, max_blocks=pb.max_blocks,
+                             max_pos=int(ctx0.max()) + total_steps + 64)
+    st = binding.Stage(dims, 0, shape.n_layers, layers, None, n_pages=pb.n_pages_pool, device=dev)
+    g = torch.Generator(device=dev)
+    g.manual_seed(args.seed + 99)
+    _fill_randn(st.kv_pool.view(-1), g)                  # random KV pre-fill N(0,1) (A21)
+    bank = [torch.randn((B, shape.hidden), generator=g, device=dev, dtype=torch.float32).to(torch.bfloat16)
+            for _ in range(8)]                            # inputs cycled from a bank of 8
+    bt = torch.from_numpy(pb.block_tables).to(dev)
+    ctx_steps = torch.from_numpy(ctx0[None, :] + np.arange(total_steps, dtype=np.int32)[:, None]).to(dev).contiguous()
+    out = torch.empty((B, shape.hidden), dtype=torch.bfloat16, device=dev)
+    torch.cuda.synchronize(dev)
+
+    step_no = [0]
+
+    def one(i):
+        s = step_no[0]
+        st.decode(B, bt, ctx_steps[s], hidden=bank[s % 8], out_hidden=out)
+        step_no[0] += 1
+
+    for i in range(W):
+        one(i)
+    st.synchronize()
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+    torch.cuda.synchronize(dev)
+    sampler = ClockSampler(dev.index or 0)
+    sampler.start()
+    n0 = st.launch_count()
+    first_step = step_no[0]
+    ms = cuda_time_ms(st.stream, one, K)
+    launches = st.launch_count() - n0
+    clocks = sampler.stop()
+    # algorithmic bytes averaged over the timed steps (contexts grow by one token per step)
+    byts = np.mean([decode_bytes_per_step(shape, ctx0 + first_step + i) for i in range(K)])
+
+    # ---- e2e: the same step through the C-ABI with HOST buffers (pinned), H2D of inputs + D2H of the result inside
+    e2e = None
+    if not args.no_e2e:
+        h_in = [b.cpu().pin_memory() for b in bank]
+        h_bt = torch.from_numpy(pb.block_tables).pin_memory()
+        h_ctx = (torch.from_numpy(ctx0[None, :] + np.arange(total_steps, dtype=np.int32)[:, None])).pin_memory()
+        h_out = torch.empty((B, shape.hidden), dtype=torch.bfloat16).pin_memory()
+        d_in = torch.empty_like(bank[0]); d_bt = torch.empty_like(bt); d_ctx = torch.empty_like(ctx_steps[0])
+
+        def one_e2e(i):
+            s = step_no[0]
+            with torch.cuda.stream(st.stream):
+                d_in.copy_(h_in[s % 8], non_blocking=True)
+                d_bt.copy_(h_bt, non_blocking=True)
+                d_ctx.copy_(h_ctx[s], non_blocking=True)
+                st.decode(B, d_bt, d_ctx, hidden=d_in, out_hidden=out)
+                h_out.copy_(out, non_blocking=True)
+            st.stream.synchronize()                      # the caller reads the result of every step
+            step_no[0] += 1
+
+        for i in range(min(W, 3)):
+            one_e2e(i)
+        t0 = time.perf_counter()
+        for i in range(K):
+            one_e2e(i)
+        dt = time.perf_counter() - t0
+        e2e = {"ms_per_step": dt * 1e3 / K, "h2d": h_in[0].numel() * 2 + h_bt.numel() * 4 + B * 4,
+               "d2h": h_out.numel() * 2}
+
+    dom = dominant_gemm(st, shape, layers, B, dev)
+    res = {"ms": ms, "tokens": B * K, "bytes_per_step": float(byts), "launches": int(launches), "clocks": clocks,
+           "e2e": e2e, "dominant": dom, "B": B, "ctx_sum": int(ctx0.sum()), "pages": int(pb.n_pages_pool)}
+    st.destroy()
+    return res
+
+
+def _fill_randn(pool, g):
+    """N(0,1) bf16 fill of a pool too large for one temporary."""
+    import torch
+    n = pool.numel()
+    step = 1 << 28
+    for o in range(0, n, step):
+        m = min(step, n - o)
+        pool[o:o + m] = torch.randn((m,), generator=g, device=pool.device, dtype=torch.float32).to(torch.bfloat16)
+    return pool
+
+
+def dominant_gemm(st, shape, layers, T, dev):
+    """The dominant kernel of the decode step is the fused gate/up + SwiGLU GEMM (45% of the step's bytes).  Time it
+    alone with CUDA events on its stream, over the stage's own weights layer after layer (so nothing is L2-resident:
+    each launch streams 2*H*F*2 bytes >> L2)."""
+    import torch
+    from paper_2606_18600_b200 import binding
+    g = torch.Generator(device=dev)
+    g.manual_seed(5)
+    x = torch.randn((T, shape.hidden), generator=g, device=dev, dtype=torch.float32).to(torch.bfloat16)
+    torch.cuda.synchronize(dev)
+    L = len(layers)
+
+    def one(i):
+        w = layers[i % L]
+        binding.op_gemm_swiglu_bf16(x, w["w_gate"], w["w_up"], stream=st.stream)
+
+    for i in range(min(L, 4)):
+        one(i)
+    n = max(L, 20)
+    ms = cuda_time_ms(st.stream, one, n)
+    alg = 2 * shape.hidden * shape.ffn * 2 + T * shape.hidden * 2 + T * shape.ffn * 2
+    return {"kernel": "gemm_kernel<DUAL> (gate/up + SwiGLU)", "us": ms * 1e3 / n, "bytes": alg,
+            "flops": 4 * T * shape.hidden * shape.ffn}
+
+
+def run_prefill(args, shape, len_fn, rank, world):
+    """cfg4: migration recompute — one ss_stage_prefill over all migrated requests, packed varlen, ctx_before = 0."""
+    import torch
+    from paper_2606_18600_b200 import binding, synth
+    dev = torch.device(f"cuda:{int(os.environ.get('LOCAL_RANK', 0))}")
+    torch.cuda.set_device(dev)
+    K, W = args.steps, args.warmup
+    rng = np.random.default_rng(args.seed)
+    lens = len_fn(args.seed).astype(np.int32)
+    n = len(lens)
+    T = int(lens.sum())
+    pb = synth.paged_batch(rng, lens, extra_tokens=1)
+    layers = gpu_weights(shape, dev, args.seed)
+    dims = binding.make_dims(shape, max_tokens=T, max_seqs=n, max_blocks=pb.max_blocks, max_pos=int(lens.max()) + 64)
+    st = binding.Stage(dims, 0, shape.n_layers, layers, None, n_pages=pb.n_pages_pool, device=dev)
+    g = torch.Generator(device=dev)
+    g.manual_seed(args.seed + 99)
+    x = torch.randn((T, shape.hidden), generator=g, device=dev, dtype=torch.float32).to(torch.bfloat16)
+    bt = torch.from_numpy(pb.block_tables).to(dev)
+    cu = torch.from_numpy(np.concatenate([[0], np.cumsum(lens)]).astype(np.int32)).to(dev)
+    ctxb = torch.zeros(n, dtype=torch.int32, device=dev)
+    out = torch.empty((T, shape.hidden), dtype=torch.bfloat16, device=dev)
+    torch.cuda.synchronize(dev)
+
+    def one(i):
+        st.prefill(n, cu, ctxb, bt, T, hidden=x, out_hidden=out)
+
+    for i in range(W):
+        one(i)
+    st.synchronize()
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+    sampler = ClockSampler(dev.index or 0)
+    sampler.start()
+    n0 = st.launch_count()
+    ms = cuda_time_ms(st.stream, one, K)
+    launches = st.launch_count() - n0
+    clocks = sampler.stop()
+    e2e = None
+    if not args.no_e2e:
+        h_x = x.cpu().pin_memory()
+        h_out = torch.empty((T, shape.hidden), dtype=torch.bfloat16).pin_memory()
+        h_bt, h_cu = pb.block_tables, cu.cpu().pin_memory()
+        h_btp = torch.from_numpy(h_bt).pin_memory()
+
+        def one_e2e(i):
+            with torch.cuda.stream(st.stream):
+                x.copy_(h_x, non_blocking=True)
+                bt.copy_(h_btp, non_blocking=True)
+                cu.copy_(h_cu, non_blocking=True)
+                st.prefill(n, cu, ctxb, bt, T, hidden=x, out_hidden=out)
+                h_out.copy_(out, non_blocking=True)
+            st.stream.synchronize()
+
+        one_e2e(0)
+        t0 = time.perf_counter()
+        for i in range(K):
+            one_e2e(i)
+        dt = time.perf_counter() - t0
+        e2e = {"ms_per_step": dt * 1e3 / K, "h2d": h_x.numel() * 2 + h_btp.numel() * 4 + h_cu.numel() * 4,
+               "d2h": h_out.numel() * 2}
+    res = {"ms": ms, "tokens": T * K, "flops_per_step": float(prefill_flops(shape, lens)), "launches": int(launches),
+           "clocks": clocks, "e2e": e2e, "T": T, "n_seqs": n, "pages": int(pb.n_pages_pool)}
+    st.destroy()
+    return res
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# CPU oracle timing (cpu_baseline leg and --impl reference): the oracle as it stands, on a bounded sample
+# ---------------------------------------------------------------------------------------------------------------
+def oracle_sample(workload, seed, layers_sample=1, repeats=1):
+    """Time `layers_sample` decoder layers of the workload's step on the host cores with the oracle; returns
+    (seconds per full-depth step extrapolated by L / layers_sample, cores, description)."""
+    from oracle import Oracle, OracleDims
+    from paper_2606_18600_b200 import synth
+    import torch
+    shape, len_fn, kind = workload_spec(workload)
+    orc = Oracle("f32")
+    lens = len_fn(seed).astype(np.int32)
+    rng = np.random.default_rng(seed)
+    dims = OracleDims(shape.hidden, shape.n_q, shape.n_kv, shape.d, shape.ffn, shape.vocab, shape.eps, shape.theta,
+                      shape.qk_norm, 0)
+    if kind == "decode":
+        B = len(lens)
+        pb = synth.paged_batch(rng, lens, extra_tokens=2)
+        cu = np.arange(B + 1, dtype=np.int32)
+        ctx = lens
+        T = B
+        desc = f"{layers_sample} of {shape.n_layers} layers of one full-batch decode step (B={B}, all contexts)"
+    else:
+        # prefill: the 2 shortest requests only (SURVEY §8(d) sub-instance), all their tokens
+        order = np.argsort(lens)[:2]
+        lens = lens[order]
+        pb = synth.paged_batch(rng, lens, extra_tokens=1)
+        cu = np.concatenate([[0], np.cumsum(lens)]).astype(np.int32)
+        ctx = np.zeros_like(lens)
+        T = int(lens.sum())
+        desc = f"{layers_sample} of {shape.n_layers} layers, the 2 shortest of 32 requests ({T} tokens)"
+    g = torch.Generator().manual_seed(seed + 5)
+    pool = synth.bits(torch.randn((2, pb.n_pages_pool, shape.n_kv, 16, shape.d), generator=g).to(torch.bfloat16)).copy()
+    x = synth.bf16_bits_to_f32(synth.bits(synth.hidden_rows(T, shape.hidden, seed))).copy()
+    best = None
+    for l in range(layers_sample):
+        w = {k: (None if v is None else synth.bits(v)) for k, v in synth.layer_weights(shape, l, seed).items()}
+        for _ in range(repeats):
+            xx = x.copy()
+            t0 = time.perf_counter()
+            orc.layer(dims, w, pool[0], pool[1], cu, ctx, pb.block_tables, xx)
+            dt = time.perf_counter() - t0
+            best = dt if best is None else min(best, dt)
+    sec_full = best * shape.n_layers
+    return sec_full, T, orc.threads(), desc
+
+
+def main():
+    args = parse()
+    rank = int(os.environ.get("RANK", 0))
+    world = int(os.environ.get("WORLD_SIZE", 1))
+    shape, len_fn, kind = workload_spec(args.workload, args.layers)
+    pk = peaks()
+    unit = "tokens/s"
+    metric = ("stage decode tokens/s" if kind == "decode" else "migration-recompute prefill tokens/s")
+    cfg = {"workload": {"cfg2": "configs[1]: Llama-3.1-70B-shaped 20-layer decode stage, B=64, ctx lognormal(med 1024)",
+                        "cfg3": "configs[2]: Qwen3-32B-shaped 16-layer decode stage, B=128, ctx lognormal(med 768)",
+                        "cfg4": "configs[3]: migration recompute prefill, 70B shapes, 32 requests lognormal(med 1200)",
+                        "tiny": "configs[0]: tiny Llama-style stage"}[args.workload],
+           "layers": shape.n_layers, "hidden": shape.hidden, "ffn": shape.ffn, "heads": f"{shape.n_q}/{shape.n_kv}",
+           "page_size": 16, "seed": args.seed, "parallelism": f"replicas x{world}",
+           "l2_policy": "inputs larger than L2 (weights 34 GB / KV streamed once per step)"}
+    if args.layers:
+        cfg["debug_layers_override"] = args.layers
+
+    # ---------------- reference arm: the CPU oracle, rank 0 only ----------------
+    if args.impl == "reference":
+        if rank != 0:
+            return
+        ts = []
+        T = cores = desc = None
+        for i in range(max(1, min(args.steps, 3)) + min(args.warmup, 1)):
+            sec, T, cores, desc = oracle_sample(args.workload, args.seed, layers_sample=1)
+            ts.append(sec)
+        sec = float(np.mean(ts[min(args.warmup, 1):]))
+        val = T / sec
+        line = {"impl": "reference", "metric": metric, "value": val, "unit": unit, "n_gpus": 0, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": cfg,
+                "cpu_baseline": {"value": val, "unit": unit, "cores": cores, "kind": "oracle",
+                                 "sample": desc + "; time x layers (extrapolated)"},
+                "e2e": {"value": val, "unit": unit, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+        print(json.dumps(line))
+        return
+
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{int(os.environ.get('LOCAL_RANK', 0))}"))
+
+    res = run_decode(args, shape, len_fn, rank, world) if kind == "decode" else \
+        run_prefill(args, shape, len_fn, rank, world)
+    ms = res["ms"]
+    e2e_ms = res["e2e"]["ms_per_step"] if res["e2e"] else None
+    if world > 1:
+        import torch.distributed as dist
+        t = torch.tensor([ms, e2e_ms or 0.0], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)          # max over ranks
+        ms, e2e_max = float(t[0]), float(t[1])
+        e2e_ms = e2e_max if e2e_ms is not None else None
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank != 0:
+        return
+    K = args.steps
+    tokens_all = res["tokens"] * world
+    value = tokens_all / (ms * 1e-3)
+    line = {"metric": metric, "value": value, "unit": unit, "n_gpus": world, "steps": K, "warmup": args.warmup,
+            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+            "data": "synthetic", "config": cfg, "clocks": res["clocks"], "gpu_launches": res["launches"]}
+    if res["e2e"]:
+        line["e2e"] = {"value": tokens_all / K / (e2e_ms * 1e-3), "unit": unit,
+                       "h2d_bytes_per_step": int(res["e2e"]["h2d"]), "d2h_bytes_per_step": int(res["e2e"]["d2h"])}
+    if kind == "decode":
+        dom = res["dominant"]
+        ach = dom["bytes"] / (dom["us"] * 1e-6) / 1e9
+        line["roofline"] = {"bound": "hbm", "achieved": ach, "peak": pk["hbm_gbs"], "unit": "GB/s",
+                            "frac": ach / pk["hbm_gbs"], "traffic": None, "kernel": dom["kernel"],
+                            "us_per_launch": dom["us"], "peak_source": pk["source"]}
+        step_gbs = res["bytes_per_step"] / (ms / K * 1e-3) / 1e9
+        line["step_roofline"] = {"bound": "hbm", "algorithmic_GB_per_step": res["bytes_per_step"] / 1e9,
+                                 "achieved": step_gbs, "peak": pk["hbm_gbs"], "unit": "GB/s",
+                                 "frac": step_gbs / pk["hbm_gbs"]}
+        from paper_2606_18600_b200 import estimator
+        line["paper_estimator_ms"] = estimator.decode_step_ms(shape, len_fn(args.seed), pk["bf16_tflops"] * 1e12,
+                                                              pk["hbm_gbs"] * 1e9)
+    else:
+        tf = res["flops_per_step"] / (ms / K * 1e-3) / 1e12
+        line["roofline"] = {"bound": "tensor", "achieved": tf, "peak": pk["bf16_tflops_sustained"], "unit": "TFLOP/s",
+                            "frac": tf / pk["bf16_tflops_sustained"], "traffic": None,
+                            "kernel": "whole prefill step (GEMMs 98.4% of flops)", "peak_source": pk["source"],
+                            "frac_of_burst_peak": tf / pk["bf16_tflops"]}
+        from paper_2606_18600_b200 import estimator
+        line["paper_estimator_ms"] = estimator.prefill_ms(shape, len_fn(args.seed), pk["bf16_tflops"] * 1e12,
+                                                          pk["hbm_gbs"] * 1e9)
+    if not args.no_cpu_baseline and world == 1:
+        sec, T, cores, desc = oracle_sample(args.workload, args.seed, layers_sample=1)
+        line["cpu_baseline"] = {"value": T / sec, "unit": unit, "cores": cores, "kind": "oracle",
+                                "sample": desc + "; time x layers (extrapolated)"}
+    print(json.dumps(line))
+
+
+if __name__ == "__main__":
+    main()

@@ -104,9 +104,12 @@ def _check_kv(pool_gpu, pool_r1, mask, first_layer_only_ulp=True):
         assert np.abs(a - b).max() <= 1e-2 * np.abs(b).max()
 
 
-@pytest.mark.parametrize("shape,proj_std", [(synth.TINY, 0.02), (synth.TINY, 0.16), (synth.TINY_QWEN, 0.02),
-                                            (synth.TINY128, 0.05)])
-def test_stage_prefill_then_decode_vs_oracle(shape, proj_std):
+@pytest.mark.parametrize("shape,proj_std,ref", [(synth.TINY, 0.02, 0), (synth.TINY, 0.08, 0), (synth.TINY, 0.16, 1),
+                                                (synth.TINY_QWEN, 0.02, 0), (synth.TINY128, 0.05, 0)])
+def test_stage_prefill_then_decode_vs_oracle(shape, proj_std, ref):
+    """ref = 0: judged against the plain fp32 oracle (R0).  ref = 1: the 'sharp' variant of reading A21 (weights x8,
+    peaked softmax): there the oracle's own R1-vs-R0 distance is 6e-2 (any engine that materialises bf16
+    activations is that far from R0), so the GPU is judged against R1 — see DESIGN.md 'Tolerances'."""
     P, lens, pb, x = _problem(shape, proj_std=proj_std)
     try:
         T = int(lens.sum())
@@ -115,7 +118,9 @@ def test_stage_prefill_then_decode_vs_oracle(shape, proj_std):
         pool0 = hp.new_pool(shape, pb.n_pages_pool, P.L)
         want, _, cu = hp.run_oracle_prefill(F32, shape, P.wb, pool0, lens, bt, x[:T])
         pool1 = hp.new_pool(shape, pb.n_pages_pool, P.L)
-        hp.run_oracle_prefill(F32, shape, P.wb, pool1, lens, bt, x[:T], rounding=1)
+        want1, _, _ = hp.run_oracle_prefill(F32, shape, P.wb, pool1, lens, bt, x[:T], rounding=1)
+        if ref == 1:
+            want = want1
         got = P.prefill(lens, bt, x[:T])
         err = hp.rel_err_rows(got, want)
         print(f"{shape.name} std={proj_std} prefill stage rel err {err:.3e}")
@@ -126,7 +131,9 @@ def test_stage_prefill_then_decode_vs_oracle(shape, proj_std):
         for step in range(2):
             xs = x[T + step * len(lens): T + (step + 1) * len(lens)]
             want_d, _ = hp.run_oracle_decode(F32, shape, P.wb, pool0, lens + step, bt, xs)
-            hp.run_oracle_decode(F32, shape, P.wb, pool1, lens + step, bt, xs, rounding=1)
+            want_d1, _ = hp.run_oracle_decode(F32, shape, P.wb, pool1, lens + step, bt, xs, rounding=1)
+            if ref == 1:
+                want_d = want_d1
             got_d = P.decode(lens + step, bt, xs)
             err = hp.rel_err_rows(got_d, want_d)
             print(f"{shape.name} decode step {step} stage rel err {err:.3e}")
