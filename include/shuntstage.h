@@ -41,7 +41,7 @@ extern "C" {
 #define SS_OK                 0
 #define SS_ERR_INVALID_ARG   -1  /* null / contradictory pointers, l0>=l1, both or neither of hidden/token_ids */
 #define SS_ERR_UNSUPPORTED   -2  /* head_dim not in {64,128}, page_size != 16, n_q % n_kv != 0, G > 16,
-                                    hidden/ffn/n_q*d not multiples of 8, misaligned pointers */
+                                    hidden/ffn/n_q*d not multiples of 8, hidden > 16384, misaligned pointers */
 #define SS_ERR_CAPACITY      -3  /* tokens / seqs / max_blocks over the dims' maxima; pool or workspace too small */
 #define SS_ERR_NO_PAGES      -4  /* ss_kv_alloc: fewer than n pages free — nothing was allocated */
 #define SS_ERR_BAD_PAGE      -5  /* ss_kv_free: id out of range or already free — nothing was freed */

@@ -288,8 +288,13 @@ __global__ void __launch_bounds__(DA_WARPS * 32) decode_attn_kernel(const Decode
 }
 
 // ---- merge the segments of each (b, kv head): out[b][hq][:] = sum_i w_i O_i / sum_i w_i l_i, w_i = 2^((m_i-M) sl2)
+// One CTA per (b, kv head); D/4 threads per q head, each owning 4 output columns, so all segment loads of a thread
+// are independent 16-byte reads (no serial chain over heads).
+constexpr int MERGE_THREADS = 256;
 template <int D>
-__global__ void __launch_bounds__(D) decode_merge_kernel(const DecodeAttnParams p) {
+__global__ void __launch_bounds__(MERGE_THREADS) decode_merge_kernel(const DecodeAttnParams p) {
+  constexpr int LANES = D / 4;                  // threads per q head
+  constexpr int HEADS_PER_PASS = MERGE_THREADS / LANES;
   const int pair = blockIdx.x;
   const int b = pair / p.n_kv, h = pair % p.n_kv;
   const int G = p.n_q / p.n_kv;
@@ -299,19 +304,27 @@ __global__ void __launch_bounds__(D) decode_merge_kernel(const DecodeAttnParams 
   const int start = cum[b] * p.n_kv + h * pages_b;
   const int w_first = start / quota, w_last = (start + pages_b - 1) / quota;
   const float sl2 = 1.4426950408889634f / sqrtf((float)D);
-  const int c = threadIdx.x;
-  for (int g = 0; g < G; ++g) {
+  const int c = (threadIdx.x % LANES) * 4;
+  for (int g = threadIdx.x / LANES; g < G; g += HEADS_PER_PASS) {
     float M = -INFINITY;
+#pragma unroll 4
     for (int w = w_first; w <= w_last; ++w) M = fmaxf(M, p.part_ml[(size_t)(w + pair) * 32 + g * 2]);
-    float num = 0.f, den = 0.f;
+    float4 num = make_float4(0.f, 0.f, 0.f, 0.f);
+    float den = 0.f;
+#pragma unroll 4
     for (int w = w_first; w <= w_last; ++w) {
       const size_t slot = (size_t)(w + pair);
       const float2 ml = *reinterpret_cast<const float2 *>(p.part_ml + slot * 32 + g * 2);
+      const float4 o = *reinterpret_cast<const float4 *>(p.part_o + slot * 16 * D + (size_t)g * D + c);
       const float wt = exp2f((ml.x - M) * sl2);
-      num += wt * p.part_o[slot * 16 * D + (size_t)g * D + c];
+      num.x += wt * o.x; num.y += wt * o.y; num.z += wt * o.z; num.w += wt * o.w;
       den += wt * ml.y;
     }
-    ((__nv_bfloat16 *)p.out)[(size_t)b * p.n_q * D + (size_t)(h * G + g) * D + c] = __float2bfloat16_rn(num / den);
+    const float inv = 1.0f / den;
+    uint2 r;
+    r.x = pack_bf16x2(num.x * inv, num.y * inv);
+    r.y = pack_bf16x2(num.z * inv, num.w * inv);
+    *reinterpret_cast<uint2 *>((__nv_bfloat16 *)p.out + (size_t)b * p.n_q * D + (size_t)(h * G + g) * D + c) = r;
   }
 }
 
@@ -337,9 +350,9 @@ cudaError_t launch_decode_attn(const DecodeAttnParams &p, cudaStream_t s) {
 
 cudaError_t launch_decode_merge(const DecodeAttnParams &p, cudaStream_t s) {
   if (p.d == 128)
-    decode_merge_kernel<128><<<p.batch * p.n_kv, 128, 0, s>>>(p);
+    decode_merge_kernel<128><<<p.batch * p.n_kv, MERGE_THREADS, 0, s>>>(p);
   else
-    decode_merge_kernel<64><<<p.batch * p.n_kv, 64, 0, s>>>(p);
+    decode_merge_kernel<64><<<p.batch * p.n_kv, MERGE_THREADS, 0, s>>>(p);
   count_launch();
   return cudaGetLastError();
 }

@@ -74,7 +74,11 @@ cudaError_t launch_input_rmsnorm(const CallArgs *args, const void *embed, const 
 }
 
 // ---- residual += sum_s part[s]; optional RMSNorm -> h; optional bf16 stage output -----------------------------
-__global__ void __launch_bounds__(EW_THREADS)
+// One CTA of 1024 threads per token row; the whole row lives in registers (IT float4 per thread, H <= IT*4096), all
+// loads are issued before any use, and x is read and written exactly once.
+constexpr int RN_THREADS = 1024;
+template <int IT>
+__global__ void __launch_bounds__(RN_THREADS)
 residual_rmsnorm_kernel(float *__restrict__ x, const float *__restrict__ part, int splits, long long split_stride,
                         const __nv_bfloat16 *__restrict__ w, float eps, int H, __nv_bfloat16 *__restrict__ h,
                         const CallArgs *__restrict__ args, int write_out) {
@@ -84,42 +88,73 @@ residual_rmsnorm_kernel(float *__restrict__ x, const float *__restrict__ part, i
   const float *pr = part + (size_t)t * H;
   __nv_bfloat16 *outp = nullptr;
   if (write_out && args->out_hidden) outp = (__nv_bfloat16 *)args->out_hidden + (size_t)t * H;
-  float ss = 0.f;
-  for (int j = threadIdx.x * 4; j < H; j += EW_THREADS * 4) {
-    float4 y = *reinterpret_cast<const float4 *>(pr + j);
-    for (int s = 1; s < splits; ++s) {
-      const float4 q = *reinterpret_cast<const float4 *>(pr + (size_t)s * split_stride + j);
-      y.x += q.x; y.y += q.y; y.z += q.z; y.w += q.w;
+  float4 v[IT], y[IT];
+#pragma unroll
+  for (int i = 0; i < IT; ++i) {
+    const int j = (i * RN_THREADS + threadIdx.x) * 4;
+    v[i] = y[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (j < H) {
+      v[i] = *reinterpret_cast<const float4 *>(xr + j);
+      y[i] = *reinterpret_cast<const float4 *>(pr + j);
     }
-    float4 v = *reinterpret_cast<const float4 *>(xr + j);
-    v.x += y.x; v.y += y.y; v.z += y.z; v.w += y.w;
-    *reinterpret_cast<float4 *>(xr + j) = v;
-    ss += v.x * v.x + v.y * v.y + v.z * v.z + v.w * v.w;
-    if (outp) {
-      uint2 o;
-      o.x = pack_bf16x2(v.x, v.y);
-      o.y = pack_bf16x2(v.z, v.w);
-      *reinterpret_cast<uint2 *>(outp + j) = o;
+  }
+  for (int s = 1; s < splits; ++s) {
+#pragma unroll
+    for (int i = 0; i < IT; ++i) {
+      const int j = (i * RN_THREADS + threadIdx.x) * 4;
+      if (j < H) {
+        const float4 q = *reinterpret_cast<const float4 *>(pr + (size_t)s * split_stride + j);
+        y[i].x += q.x; y[i].y += q.y; y[i].z += q.z; y[i].w += q.w;
+      }
+    }
+  }
+  float ss = 0.f;
+#pragma unroll
+  for (int i = 0; i < IT; ++i) {
+    const int j = (i * RN_THREADS + threadIdx.x) * 4;
+    v[i].x += y[i].x; v[i].y += y[i].y; v[i].z += y[i].z; v[i].w += y[i].w;
+    if (j < H) {
+      *reinterpret_cast<float4 *>(xr + j) = v[i];
+      ss += v[i].x * v[i].x + v[i].y * v[i].y + v[i].z * v[i].z + v[i].w * v[i].w;
+      if (outp) {
+        uint2 o;
+        o.x = pack_bf16x2(v[i].x, v[i].y);
+        o.y = pack_bf16x2(v[i].z, v[i].w);
+        *reinterpret_cast<uint2 *>(outp + j) = o;
+      }
     }
   }
   if (w == nullptr) return;
   ss = block_sum(ss, red);
   const float inv = 1.0f / sqrtf(ss / (float)H + eps);
-  for (int j = threadIdx.x * 4; j < H; j += EW_THREADS * 4) {
-    const float4 v = *reinterpret_cast<const float4 *>(xr + j);  // written by this thread above
-    const uint2 g = *reinterpret_cast<const uint2 *>(w + j);
-    uint2 o;
-    o.x = pack_bf16x2(v.x * inv * bf16_lo(g.x), v.y * inv * bf16_hi(g.x));
-    o.y = pack_bf16x2(v.z * inv * bf16_lo(g.y), v.w * inv * bf16_hi(g.y));
-    *reinterpret_cast<uint2 *>(h + (size_t)t * H + j) = o;
+#pragma unroll
+  for (int i = 0; i < IT; ++i) {
+    const int j = (i * RN_THREADS + threadIdx.x) * 4;
+    if (j < H) {
+      const uint2 g = *reinterpret_cast<const uint2 *>(w + j);
+      uint2 o;
+      o.x = pack_bf16x2(v[i].x * inv * bf16_lo(g.x), v[i].y * inv * bf16_hi(g.x));
+      o.y = pack_bf16x2(v[i].z * inv * bf16_lo(g.y), v[i].w * inv * bf16_hi(g.y));
+      *reinterpret_cast<uint2 *>(h + (size_t)t * H + j) = o;
+    }
   }
 }
 
 cudaError_t launch_residual_rmsnorm(float *x, const float *part, int splits, long long split_stride,
                                     const void *ln_w, float eps, int H, int T, void *h, const CallArgs *args,
                                     bool write_out_hidden, cudaStream_t s) {
-  residual_rmsnorm_kernel<<<T, EW_THREADS, 0, s>>>(x, part, splits, split_stride, (const __nv_bfloat16 *)ln_w, eps,
-                                                   H, (__nv_bfloat16 *)h, args, write_out_hidden ? 1 : 0);
+  const __nv_bfloat16 *w = (const __nv_bfloat16 *)ln_w;
+  __nv_bfloat16 *hh = (__nv_bfloat16 *)h;
+  const int wo = write_out_hidden ? 1 : 0;
+  const int it = (H + RN_THREADS * 4 - 1) / (RN_THREADS * 4);
+  if (it <= 1)
+    residual_rmsnorm_kernel<1><<<T, RN_THREADS, 0, s>>>(x, part, splits, split_stride, w, eps, H, hh, args, wo);
+  else if (it <= 2)
+    residual_rmsnorm_kernel<2><<<T, RN_THREADS, 0, s>>>(x, part, splits, split_stride, w, eps, H, hh, args, wo);
+  else if (it <= 4)
+    residual_rmsnorm_kernel<4><<<T, RN_THREADS, 0, s>>>(x, part, splits, split_stride, w, eps, H, hh, args, wo);
+  else
+    return cudaErrorInvalidValue;  // hidden > 16384 is rejected at create
   count_launch();
   return cudaGetLastError();
 }

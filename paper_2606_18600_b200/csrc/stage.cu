@@ -55,7 +55,7 @@ static bool dims_ok(const ss_model_dims *d, int l0, int l1, int *why) {
   if (d->head_dim != 64 && d->head_dim != 128) return false;
   if (d->page_size != 16) return false;
   if (d->n_q_heads % d->n_kv_heads != 0 || d->n_q_heads / d->n_kv_heads > 16) return false;
-  if (d->hidden % 8 != 0 || d->ffn % 8 != 0) return false;
+  if (d->hidden % 8 != 0 || d->ffn % 8 != 0 || d->hidden > 16384) return false;
   return true;
 }
 
