@@ -159,15 +159,18 @@ int64_t ss_stage_launch_count(const ss_stage *st);
 
 /* ---- op-level entry points (the same kernels the stage uses; for per-kernel parity tests and profiling) -- */
 
-/* C[T, N] (fp32, row-major, ld = N) = X[T, K] (bf16, row-major) * W[N, K]^T (bf16) through the tcgen05/TMEM
- * GEMM.  `splits` >= 1 K-splits are reduced in fixed order.  scratch: dev, >= splits*T*N*4 bytes when
- * splits > 1 (may be NULL when splits == 1).  K % 8 == 0.  Synchronous w.r.t. the host only via the stream. */
+/* Scratch (dev, 256-byte aligned) the op-level GEMMs need for the stream-K fix-up: >= this many bytes, whose first
+ * 1024 bytes must be ZERO before the first call (the kernel leaves them zero). */
+size_t ss_op_gemm_scratch_bytes(void);
+
+/* C[T, N] (fp32, row-major, ld = N) = X[T, K] (bf16, row-major) * W[N, K]^T (bf16) through the persistent
+ * tcgen05/TMEM GEMM.  K % 8 == 0.  Asynchronous on cuda_stream. */
 int ss_op_gemm_bf16(const void *x_dev, const void *w_dev, float *c_dev, int T, int N, int K,
-                    int splits, void *scratch_dev, void *cuda_stream);
+                    void *scratch_dev, size_t scratch_bytes, void *cuda_stream);
 
 /* Fused gate/up GEMM + SwiGLU: A[T, F] (bf16) = silu(X Wg^T) * (X Wu^T). */
 int ss_op_gemm_swiglu_bf16(const void *x_dev, const void *wg_dev, const void *wu_dev, void *a_dev,
-                           int T, int F, int K, void *cuda_stream);
+                           int T, int F, int K, void *scratch_dev, size_t scratch_bytes, void *cuda_stream);
 
 const char *ss_strerror(int code);
 const char *ss_last_cuda_error(void); /* text of the last CUDA error seen by this thread ("" if none) */

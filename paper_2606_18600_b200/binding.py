@@ -21,7 +21,7 @@ ERRORS = {0: "SS_OK", -1: "SS_ERR_INVALID_ARG", -2: "SS_ERR_UNSUPPORTED", -3: "S
 
 EXPORTS = ["ss_stage_workspace_bytes", "ss_kv_page_bytes", "ss_stage_create", "ss_stage_destroy",
            "ss_kv_num_pages", "ss_kv_num_free", "ss_kv_alloc", "ss_kv_free", "ss_stage_prefill", "ss_stage_decode",
-           "ss_stage_launch_count", "ss_op_gemm_bf16", "ss_op_gemm_swiglu_bf16", "ss_strerror",
+           "ss_stage_launch_count", "ss_op_gemm_scratch_bytes", "ss_op_gemm_bf16", "ss_op_gemm_swiglu_bf16", "ss_strerror",
            "ss_last_cuda_error", "ss_version"]
 
 
@@ -85,10 +85,11 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
                                     C.c_void_p, C.c_void_p, C.c_void_p]
     lib.ss_stage_launch_count.restype = C.c_int64
     lib.ss_stage_launch_count.argtypes = [C.c_void_p]
-    lib.ss_op_gemm_bf16.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int,
-                                    C.c_void_p, C.c_void_p]
+    lib.ss_op_gemm_scratch_bytes.restype = C.c_size_t
+    lib.ss_op_gemm_bf16.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p,
+                                    C.c_size_t, C.c_void_p]
     lib.ss_op_gemm_swiglu_bf16.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int,
-                                           C.c_int, C.c_void_p]
+                                           C.c_int, C.c_void_p, C.c_size_t, C.c_void_p]
     lib.ss_strerror.restype = C.c_char_p
     lib.ss_strerror.argtypes = [C.c_int]
     lib.ss_last_cuda_error.restype = C.c_char_p
@@ -224,15 +225,28 @@ class Stage:
             pass
 
 
-def op_gemm_bf16(x: torch.Tensor, w: torch.Tensor, splits: int = 1, stream=None) -> torch.Tensor:
+_SCRATCH = {}
+
+
+def _op_scratch(device) -> torch.Tensor:
+    """Zero-initialised stream-K fix-up scratch for the op-level GEMMs (one per device, torch memory)."""
+    key = str(device)
+    if key not in _SCRATCH:
+        n = load_library().ss_op_gemm_scratch_bytes()
+        _SCRATCH[key] = torch.zeros(n, dtype=torch.uint8, device=device)
+        torch.cuda.synchronize(device)
+    return _SCRATCH[key]
+
+
+def op_gemm_bf16(x: torch.Tensor, w: torch.Tensor, stream=None) -> torch.Tensor:
     """C[T,N] fp32 = x[T,K] bf16 @ w[N,K]^T bf16 through the tcgen05 GEMM kernel."""
     lib = load_library()
     T, K = x.shape
     N = w.shape[0]
     c = torch.empty((T, N), dtype=torch.float32, device=x.device)
-    scratch = torch.empty((splits, T, N), dtype=torch.float32, device=x.device) if splits > 1 else None
+    sc = _op_scratch(x.device)
     s = stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream
-    rc = lib.ss_op_gemm_bf16(_ptr(x), _ptr(w), _ptr(c), T, N, K, splits, _ptr(scratch), s)
+    rc = lib.ss_op_gemm_bf16(_ptr(x), _ptr(w), _ptr(c), T, N, K, _ptr(sc), sc.numel(), s)
     if rc != SS_OK:
         raise ShuntStageError(rc, "ss_op_gemm_bf16")
     return c
@@ -243,8 +257,9 @@ def op_gemm_swiglu_bf16(x: torch.Tensor, wg: torch.Tensor, wu: torch.Tensor, str
     T, K = x.shape
     F = wg.shape[0]
     a = torch.empty((T, F), dtype=torch.bfloat16, device=x.device)
+    sc = _op_scratch(x.device)
     s = stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream
-    rc = lib.ss_op_gemm_swiglu_bf16(_ptr(x), _ptr(wg), _ptr(wu), _ptr(a), T, F, K, s)
+    rc = lib.ss_op_gemm_swiglu_bf16(_ptr(x), _ptr(wg), _ptr(wu), _ptr(a), T, F, K, _ptr(sc), sc.numel(), s)
     if rc != SS_OK:
         raise ShuntStageError(rc, "ss_op_gemm_swiglu_bf16")
     return a

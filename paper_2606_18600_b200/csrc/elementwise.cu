@@ -95,7 +95,7 @@ residual_rmsnorm_kernel(float *__restrict__ x, const float *__restrict__ part, i
     v[i] = y[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     if (j < H) {
       v[i] = *reinterpret_cast<const float4 *>(xr + j);
-      y[i] = *reinterpret_cast<const float4 *>(pr + j);
+      if (splits > 0) y[i] = *reinterpret_cast<const float4 *>(pr + j);
     }
   }
   for (int s = 1; s < splits; ++s) {
@@ -114,7 +114,7 @@ residual_rmsnorm_kernel(float *__restrict__ x, const float *__restrict__ part, i
     const int j = (i * RN_THREADS + threadIdx.x) * 4;
     v[i].x += y[i].x; v[i].y += y[i].y; v[i].z += y[i].z; v[i].w += y[i].w;
     if (j < H) {
-      *reinterpret_cast<float4 *>(xr + j) = v[i];
+      if (splits > 0) *reinterpret_cast<float4 *>(xr + j) = v[i];  // splits == 0: x already holds the sum
       ss += v[i].x * v[i].x + v[i].y * v[i].y + v[i].z * v[i].z + v[i].w * v[i].w;
       if (outp) {
         uint2 o;

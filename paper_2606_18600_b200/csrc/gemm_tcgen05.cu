@@ -1,6 +1,6 @@
 // gemm_tcgen05.cu — the bf16 projections of a decoder layer (Table 2 rows "QKV Projection", "Output Projection",
-// "Up and Gate Projection", "Down Projection", "Logits Calculation") as ONE tcgen05/TMEM GEMM
-// kernel fed by TMA, for sm_100a.
+// "Up and Gate Projection", "Down Projection", "Logits Calculation") as ONE persistent
+// tcgen05/TMEM GEMM kernel fed by TMA, for sm_100a.
 //
 // out[t][n] = sum_k X[t,k] * W[n,k]     X: activations [T,K] bf16 row-major, W: weights [N,K] bf16 row-major.
 //
@@ -10,9 +10,11 @@
 //
 // CTA = 6 warps: warp 0 = TMA producer (one lane), warp 1 = TMEM allocator + MMA issuer (one lane), warps 2-5 =
 // epilogue (one TMEM lane quadrant each).  smem ring of `stages` x {A tile 128x64 (x2 when DUAL), B tile bn x 64},
-// SWIZZLE_128B, full/empty mbarriers; accumulator(s) in TMEM; K-split over gridDim.z with fp32 partial outputs
-// reduced in fixed order by the consumer kernel.  DUAL = gate and up tiles share the B tile and the epilogue
-// writes silu(g)*u as bf16 (step S9), so [T,2F] never reaches HBM.
+// SWIZZLE_128B, full/empty mbarriers; accumulators in TMEM, double-buffered when they fit so the epilogue of one
+// work item overlaps the MMAs of the next; the producer runs ahead across work items.  Schedules: see internal.h
+// (stream-K with in-kernel fix-up for the decode shapes, band-rasterised whole tiles for the prefill shapes).
+// DUAL = gate and up tiles share the B tile and the epilogue writes silu(g)*u as bf16 (step S9), so [T,2F] never
+// reaches HBM.  EPI_RESID_F32 adds the projection straight into the fp32 residual stream (steps S7, S10).
 #include <cuda.h>
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
@@ -25,9 +27,69 @@
 namespace ss {
 
 constexpr int A_TILE_BYTES = GEMM_BM * GEMM_BK * 2;  // 16 KB
+constexpr int EPI_THREADS = 128;
+
+struct WorkItem {
+  int row_tile, t_tile, kb0, kb1;
+};
+
+// Per-CTA work list.  All roles of a CTA construct the same iterator and see the same items in the same order.
+struct WorkIter {
+  int sched, nkb, n_row_tiles, n_t_tiles, band, G, c;
+  long long u, u_end;  // stream-K: unit cursor / end of this CTA's range
+  int idx, n_tiles;    // tiles: next tile index
+
+  __device__ WorkIter(const GemmParams &p, int cta, int grid) {
+    sched = p.sched;
+    nkb = (p.K + GEMM_BK - 1) / GEMM_BK;
+    n_row_tiles = p.n_row_tiles;
+    n_t_tiles = p.n_t_tiles;
+    band = p.band;
+    G = grid;
+    c = cta;
+    n_tiles = n_row_tiles * n_t_tiles;
+    const long long U = (long long)n_tiles * nkb;
+    u = (long long)c * U / G;
+    u_end = (long long)(c + 1) * U / G;
+    idx = c;
+  }
+  // first unit of CTA cc's stream-K range
+  __device__ long long range_start(int cc) const { return (long long)cc * ((long long)n_tiles * nkb) / G; }
+
+  __device__ bool next(WorkItem &w) {
+    if (sched == SCHED_STREAMK) {
+      if (u >= u_end) return false;
+      const int tile = (int)(u / nkb);
+      w.kb0 = (int)(u - (long long)tile * nkb);
+      const long long left = u_end - u;
+      w.kb1 = (int)((long long)w.kb0 + left < (long long)nkb ? (long long)w.kb0 + left : (long long)nkb);
+      w.t_tile = tile / n_row_tiles;
+      w.row_tile = tile - w.t_tile * n_row_tiles;
+      u += w.kb1 - w.kb0;
+      return true;
+    }
+    if (idx >= n_tiles) return false;
+    const int per_band = band * n_t_tiles;
+    const int b = idx / per_band, rem = idx - b * per_band;
+    const int rb = min(band, n_row_tiles - b * band);
+    w.t_tile = rem / rb;
+    w.row_tile = b * band + (rem - w.t_tile * rb);
+    w.kb0 = 0;
+    w.kb1 = nkb;
+    idx += G;
+    return true;
+  }
+};
+
+__device__ __forceinline__ int ld_acquire(const int *p) {
+  int v;
+  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void epi_bar() { asm volatile("bar.sync 1, 128;" ::: "memory"); }
 
 template <bool DUAL>
-__global__ void __launch_bounds__(192)
+__global__ void __launch_bounds__(192, 1)
 gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUtensorMap ta1,
             const __grid_constant__ CUtensorMap ta2, const __grid_constant__ CUtensorMap tb, const GemmParams p) {
   extern __shared__ uint8_t smem_raw[];
@@ -38,35 +100,31 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
   const int stages = p.stages;
   uint64_t *full = (uint64_t *)(base + (size_t)stages * stage_bytes);
   uint64_t *empty = full + stages;
-  uint64_t *acc_full = empty + stages;
-  uint32_t *tmem_slot = (uint32_t *)(acc_full + 1);
+  uint64_t *tfull = empty + stages;   // [2]
+  uint64_t *tempty = tfull + 2;       // [2]
+  uint32_t *tmem_slot = (uint32_t *)(tempty + 2);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int cta = blockIdx.x, grid = gridDim.x;
 
-  // tile -> (segment, first row)
-  int seg = 0;
-#pragma unroll
-  for (int i = 1; i < 3; ++i)
-    if (i < p.n_seg && (int)blockIdx.x >= p.seg_tile0[i]) seg = i;
-  const int row0 = ((int)blockIdx.x - p.seg_tile0[seg]) * GEMM_BM;
-  const int t0 = blockIdx.y * bn;
-  const int nkb = (p.K + GEMM_BK - 1) / GEMM_BK;
-  const int kb0 = blockIdx.z * p.kb_per_split;
-  const int kb1 = min(nkb, kb0 + p.kb_per_split);
-
-  const uint32_t tmem_cols_needed = (uint32_t)bn * (DUAL ? 2u : 1u);
+  const uint32_t acc_cols = (uint32_t)bn * (DUAL ? 2u : 1u);
+  const int nbuf = (2 * acc_cols <= 512) ? 2 : 1;
   uint32_t tmem_cols = 32;
-  while (tmem_cols < tmem_cols_needed) tmem_cols <<= 1;
+  while (tmem_cols < acc_cols * nbuf) tmem_cols <<= 1;
 
   if (warp == 0 && lane == 0) {
-    tma_prefetch_desc(seg == 0 ? &ta0 : (seg == 1 ? &ta1 : &ta2));
-    if (DUAL) tma_prefetch_desc(&ta1);
+    tma_prefetch_desc(&ta0);
+    if (DUAL || p.n_seg > 1) tma_prefetch_desc(&ta1);
+    if (p.n_seg > 2) tma_prefetch_desc(&ta2);
     tma_prefetch_desc(&tb);
     for (int i = 0; i < stages; ++i) {
       mbar_init(&full[i], 1);
       mbar_init(&empty[i], 1);
     }
-    mbar_init(acc_full, 1);
+    for (int i = 0; i < 2; ++i) {
+      mbar_init(&tfull[i], 1);
+      mbar_init(&tempty[i], 4);  // one arrival per epilogue warp
+    }
     mbar_fence_init();
   }
   if (warp == 1) tmem_alloc_dyn(tmem_slot, tmem_cols);
@@ -78,115 +136,176 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
   if (warp == 0) {
     if (lane == 0) {
       // ---------------- TMA producer ----------------
-      const uint64_t pol_w = l2_policy_evict_first();  // weights are streamed once
+      const uint64_t pol_w = l2_policy_evict_first();  // weights are streamed
       const uint64_t pol_x = l2_policy_evict_last();   // activations are re-read by every CTA
-      const CUtensorMap *ta = DUAL ? &ta0 : (seg == 0 ? &ta0 : (seg == 1 ? &ta1 : &ta2));
-      int i = 0;
-      for (int kb = kb0; kb < kb1; ++kb, ++i) {
-        const int s = i % stages;
-        const uint32_t ph = (uint32_t)(i / stages) & 1u;
-        mbar_wait(&empty[s], ph ^ 1u);
-        uint8_t *st = base + (size_t)s * stage_bytes;
-        mbar_expect_tx(&full[s], stage_bytes);
-        tma_load_2d(st, ta, &full[s], kb * GEMM_BK, row0, pol_w);
-        if (DUAL) tma_load_2d(st + A_TILE_BYTES, &ta1, &full[s], kb * GEMM_BK, row0, pol_w);
-        tma_load_2d(st + A_TILE_BYTES * (DUAL ? 2 : 1), &tb, &full[s], kb * GEMM_BK, t0, pol_x);
+      WorkIter it(p, cta, grid);
+      WorkItem w;
+      uint32_t n = 0;  // running k-block counter across items
+      while (it.next(w)) {
+        int seg = 0;
+#pragma unroll
+        for (int i = 1; i < 3; ++i)
+          if (i < p.n_seg && w.row_tile >= p.seg_tile0[i]) seg = i;
+        const int row0 = (w.row_tile - p.seg_tile0[seg]) * GEMM_BM;
+        const int t0 = w.t_tile * bn;
+        const CUtensorMap *ta = DUAL ? &ta0 : (seg == 0 ? &ta0 : (seg == 1 ? &ta1 : &ta2));
+        for (int kb = w.kb0; kb < w.kb1; ++kb, ++n) {
+          const int s = n % stages;
+          const uint32_t ph = (n / stages) & 1u;
+          mbar_wait(&empty[s], ph ^ 1u);
+          uint8_t *st = base + (size_t)s * stage_bytes;
+          mbar_expect_tx(&full[s], stage_bytes);
+          tma_load_2d(st, ta, &full[s], kb * GEMM_BK, row0, pol_w);
+          if (DUAL) tma_load_2d(st + A_TILE_BYTES, &ta1, &full[s], kb * GEMM_BK, row0, pol_w);
+          tma_load_2d(st + A_TILE_BYTES * (DUAL ? 2 : 1), &tb, &full[s], kb * GEMM_BK, t0, pol_x);
+        }
       }
     }
   } else if (warp == 1) {
     if (lane == 0) {
       // ---------------- MMA issuer ----------------
       const uint32_t idesc = umma_idesc_bf16(GEMM_BM, (uint32_t)bn);
-      int i = 0;
-      for (int kb = kb0; kb < kb1; ++kb, ++i) {
-        const int s = i % stages;
-        const uint32_t ph = (uint32_t)(i / stages) & 1u;
-        mbar_wait(&full[s], ph);
+      WorkIter it(p, cta, grid);
+      WorkItem w;
+      uint32_t n = 0, item = 0;
+      while (it.next(w)) {
+        const uint32_t buf = item % nbuf, tph = (item / nbuf) & 1u;
+        mbar_wait(&tempty[buf], tph ^ 1u);  // epilogue has drained this accumulator
         tc_fence_after();
-        const uint32_t st = smem_u32(base + (size_t)s * stage_bytes);
-        const uint64_t da = umma_desc_k_sw128(st);
-        const uint64_t db = umma_desc_k_sw128(st + A_TILE_BYTES * (DUAL ? 2 : 1));
+        const uint32_t acc_addr = tmem_base + buf * acc_cols;
+        for (int kb = w.kb0; kb < w.kb1; ++kb, ++n) {
+          const int s = n % stages;
+          const uint32_t ph = (n / stages) & 1u;
+          mbar_wait(&full[s], ph);
+          tc_fence_after();
+          const uint32_t st = smem_u32(base + (size_t)s * stage_bytes);
+          const uint64_t da = umma_desc_k_sw128(st);
+          const uint64_t da1 = umma_desc_k_sw128(st + A_TILE_BYTES);
+          const uint64_t db = umma_desc_k_sw128(st + A_TILE_BYTES * (DUAL ? 2 : 1));
 #pragma unroll
-        for (int k = 0; k < GEMM_BK / 16; ++k) {
-          const uint32_t acc = (kb > kb0 || k > 0) ? 1u : 0u;
-          umma_bf16(tmem_base, da + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc, acc);
-          if (DUAL) {
-            const uint64_t da1 = umma_desc_k_sw128(st + A_TILE_BYTES);
-            umma_bf16(tmem_base + (uint32_t)bn, da1 + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc, acc);
+          for (int k = 0; k < GEMM_BK / 16; ++k) {
+            const uint32_t acc = (kb > w.kb0 || k > 0) ? 1u : 0u;
+            umma_bf16(acc_addr, da + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc, acc);
+            if (DUAL) umma_bf16(acc_addr + (uint32_t)bn, da1 + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc, acc);
           }
+          umma_commit(&empty[s]);  // frees the smem slot when these MMAs have read it
         }
-        umma_commit(&empty[s]);  // frees the smem slot when these MMAs have read it
+        umma_commit(&tfull[buf]);
+        ++item;
       }
-      umma_commit(acc_full);
     }
   } else {
-    // ---------------- epilogue: TMEM -> registers -> global ----------------
+    // ---------------- epilogue: TMEM -> registers -> (fix-up) -> global ----------------
     const int quad = warp & 3;
     const int r = quad * 32 + lane;  // row of the tile = TMEM lane
-    const int row_in_seg = row0 + r;
-    const bool row_ok = row_in_seg < p.seg_rows[seg];
-    const int col = p.seg_col[seg] + row_in_seg;
-    mbar_wait(acc_full, 0);
-    tc_fence_after();
-    const uint32_t tq = tmem_base + ((uint32_t)(quad * 32) << 16);
-    if (p.epi == EPI_F32) {
-      float *o = p.out_f32 + (long long)blockIdx.z * p.split_stride + col;
-      if (bn >= 32) {
-        for (int c = 0; c < bn; c += 32) {
-          uint32_t v[32];
-          tmem_ld_32x32(tq + (uint32_t)c, v);
-          tmem_ld_wait();
-          if (row_ok) {
+    const int et = threadIdx.x - 64; // 0..127
+    WorkIter it(p, cta, grid);
+    WorkItem w;
+    uint32_t item = 0;
+    const int nkb = it.nkb;
+    while (it.next(w)) {
+      const uint32_t buf = item % nbuf, tph = (item / nbuf) & 1u;
+      int seg = 0;
 #pragma unroll
-            for (int j = 0; j < 32; ++j) {
-              const int t = t0 + c + j;
-              if (t < p.T) o[(size_t)t * p.ld_out] = __uint_as_float(v[j]);
-            }
+      for (int i = 1; i < 3; ++i)
+        if (i < p.n_seg && w.row_tile >= p.seg_tile0[i]) seg = i;
+      const int row_in_seg = (w.row_tile - p.seg_tile0[seg]) * GEMM_BM + r;
+      const bool row_ok = row_in_seg < p.seg_rows[seg];
+      const int col = p.seg_col[seg] + row_in_seg;
+      const int t0 = w.t_tile * bn;
+      const bool is_first = w.kb0 == 0, is_last = w.kb1 == nkb;
+
+      // stream-K fix-up bookkeeping
+      int c_lo = 0, c_hi = -1;  // contributors [c_lo, c_hi] of a tile this CTA owns
+      if (is_first && !is_last) {
+        const long long tile_end = ((long long)(w.t_tile * p.n_row_tiles + w.row_tile) + 1) * nkb;
+        c_lo = cta + 1;
+        c_hi = cta;
+        while (c_hi + 1 < grid && it.range_start(c_hi + 1) < tile_end) ++c_hi;
+        for (int cc = c_lo; cc <= c_hi; ++cc) {
+          uint32_t spins = 0;
+          while (ld_acquire(p.fix_flags + cc) == 0) {
+            if (++spins > (1u << 28)) __trap();
           }
+        }
+      }
+
+      mbar_wait(&tfull[buf], tph);
+      tc_fence_after();
+      const uint32_t tq = tmem_base + buf * acc_cols + ((uint32_t)(quad * 32) << 16);
+
+      if (!is_first) {
+        // contributor: dump the raw fp32 accumulator(s) to this CTA's slot, [acc][col][row]
+        float *slot = p.fix_slots + (size_t)cta * (DUAL ? 2 : 1) * bn * GEMM_BM;
+        for (int c0 = 0; c0 < (int)acc_cols; c0 += 32) {
+          uint32_t v[32];
+          tmem_ld_32x32(tq + (uint32_t)c0, v);
+          tmem_ld_wait();
+#pragma unroll
+          for (int j = 0; j < 32; ++j) slot[(size_t)(c0 + j) * GEMM_BM + r] = __uint_as_float(v[j]);
+        }
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&tempty[buf]);
+        __threadfence();
+        epi_bar();
+        if (et == 0) {
+          __threadfence();
+          atomicExch(p.fix_flags + cta, 1);
         }
       } else {
-        uint32_t v[16];
-        tmem_ld_32x16(tq, v);
-        tmem_ld_wait();
-        if (row_ok) {
+        for (int c0 = 0; c0 < bn; c0 += 32) {
+          uint32_t v[32], u[32];
+          tmem_ld_32x32(tq + (uint32_t)c0, v);
+          if (DUAL) tmem_ld_32x32(tq + (uint32_t)(bn + c0), u);
+          tmem_ld_wait();
+          for (int cc = c_lo; cc <= c_hi; ++cc) {  // fixed order: deterministic sums
+            const float *slot = p.fix_slots + (size_t)cc * (DUAL ? 2 : 1) * bn * GEMM_BM;
 #pragma unroll
-          for (int j = 0; j < 16; ++j) {
-            const int t = t0 + j;
-            if (t < p.T) o[(size_t)t * p.ld_out] = __uint_as_float(v[j]);
+            for (int j = 0; j < 32; ++j) {
+              v[j] = __float_as_uint(__uint_as_float(v[j]) + __ldcg(slot + (size_t)(c0 + j) * GEMM_BM + r));
+              if (DUAL)
+                u[j] = __float_as_uint(__uint_as_float(u[j]) + __ldcg(slot + (size_t)(bn + c0 + j) * GEMM_BM + r));
+            }
           }
-        }
-      }
-    } else if (DUAL) {  // EPI_SWIGLU_BF16: a = g / (1 + exp(-g)) * u
-      __nv_bfloat16 *o = (__nv_bfloat16 *)p.out_bf16 + col;
-      const int step = bn >= 32 ? 32 : 16;
-      for (int c = 0; c < bn; c += step) {
-        uint32_t g[32], u[32];
-        if (step == 32) {
-          tmem_ld_32x32(tq + (uint32_t)c, g);
-          tmem_ld_32x32(tq + (uint32_t)(bn + c), u);
-        } else {
-          uint32_t g16[16], u16[16];
-          tmem_ld_32x16(tq, g16);
-          tmem_ld_32x16(tq + (uint32_t)bn, u16);
+          if (row_ok) {
+            if (DUAL) {  // EPI_SWIGLU_BF16: a = g / (1 + exp(-g)) * u
+              __nv_bfloat16 *o = (__nv_bfloat16 *)p.out_bf16 + col;
 #pragma unroll
-          for (int j = 0; j < 16; ++j) {
-            g[j] = g16[j];
-            u[j] = u16[j];
-          }
-        }
-        tmem_ld_wait();
-        if (row_ok) {
+              for (int j = 0; j < 32; ++j) {
+                const int t = t0 + c0 + j;
+                if (t < p.T) {
+                  const float gv = __uint_as_float(v[j]), uv = __uint_as_float(u[j]);
+                  o[(size_t)t * p.ld_out] = __float2bfloat16_rn(gv / (1.0f + __expf(-gv)) * uv);
+                }
+              }
+            } else if (p.epi == EPI_RESID_F32) {
+              float *o = p.out_f32 + col;
 #pragma unroll
-          for (int j = 0; j < 32; ++j) {
-            const int t = t0 + c + j;
-            if (j < step && t < p.T) {
-              const float gv = __uint_as_float(g[j]), uv = __uint_as_float(u[j]);
-              const float a = gv / (1.0f + __expf(-gv)) * uv;
-              o[(size_t)t * p.ld_out] = __float2bfloat16_rn(a);
+              for (int j = 0; j < 32; ++j) {
+                const int t = t0 + c0 + j;
+                if (t < p.T) o[(size_t)t * p.ld_out] += __uint_as_float(v[j]);
+              }
+            } else {
+              float *o = p.out_f32 + col;
+#pragma unroll
+              for (int j = 0; j < 32; ++j) {
+                const int t = t0 + c0 + j;
+                if (t < p.T) o[(size_t)t * p.ld_out] = __uint_as_float(v[j]);
+              }
             }
           }
         }
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&tempty[buf]);
+        if (c_hi >= c_lo) {  // consumed: re-arm the contributors' flags for the next launch
+          epi_bar();
+          if (et == 0)
+            for (int cc = c_lo; cc <= c_hi; ++cc) p.fix_flags[cc] = 0;
+        }
       }
+      ++item;
     }
   }
   tc_fence_before();
@@ -228,32 +347,65 @@ int make_tmap_bf16_2d(CUtensorMap *out, const void *base, uint64_t rows, uint64_
 }
 
 int gemm_pick_bn(int T) {
-  const int c[5] = {16, 32, 64, 128, 256};
-  for (int i = 0; i < 5; ++i)
+  const int c[4] = {32, 64, 128, 256};
+  for (int i = 0; i < 4; ++i)
     if (T <= c[i]) return c[i];
   return 256;
 }
 
 size_t gemm_smem_bytes(int bn, bool dual, int stages) {
   size_t stage = (size_t)A_TILE_BYTES * (dual ? 2 : 1) + (size_t)bn * 128;
-  return 1024 + stage * stages + 8 * (2 * stages + 1) + 16;
+  return 1024 + stage * stages + 8 * (2 * stages + 4) + 16;
+}
+
+static int env_int(const char *name, int dflt) {
+  const char *e = getenv(name);
+  return e ? atoi(e) : dflt;
 }
 
 int gemm_pick_stages(int bn, bool dual) {
   static int env = -1;
-  if (env < 0) {
-    const char *e = getenv("SS_GEMM_STAGES");
-    env = e ? atoi(e) : 0;
-  }
+  if (env < 0) env = env_int("SS_GEMM_STAGES", 0);
   size_t stage = (size_t)A_TILE_BYTES * (dual ? 2 : 1) + (size_t)bn * 128;
-  // small stages: aim at two co-resident CTAs per SM (their prologues/epilogues overlap); big stages: one CTA
-  size_t budget = stage >= 32 * 1024 ? 200 * 1024 : 100 * 1024;
-  int st = (int)(budget / stage);
+  int st = (int)((size_t)208 * 1024 / stage);  // one persistent CTA per SM: use most of the 227 KB
   if (env > 0) st = env;
-  if (st > 8) st = 8;
+  if (st > 10) st = 10;
   while (st > 2 && gemm_smem_bytes(bn, dual, st) > 227 * 1024) --st;
   if (st < 2) st = 2;
   return st;
+}
+
+void gemm_plan(GemmLaunch &g, int n_sm) {
+  GemmParams &p = g.p;
+  static int env_band = -1, env_sched = -2, env_grid = -1;
+  if (env_band < 0) env_band = env_int("SS_GEMM_BAND", 0);
+  if (env_sched == -2) env_sched = env_int("SS_GEMM_SCHED", -1);
+  if (env_grid < 0) env_grid = env_int("SS_GEMM_GRID", 0);
+  int tiles = 0, col = 0;
+  for (int i = 0; i < 3; ++i) {
+    p.seg_tile0[i] = tiles;
+    p.seg_col[i] = col;
+    if (i < p.n_seg) {
+      tiles += (p.seg_rows[i] + GEMM_BM - 1) / GEMM_BM;
+      col += p.seg_rows[i];
+    } else {
+      p.seg_rows[i] = 0;
+    }
+  }
+  p.n_row_tiles = tiles;
+  p.bn = gemm_pick_bn(p.T);
+  p.n_t_tiles = (p.T + p.bn - 1) / p.bn;
+  p.stages = gemm_pick_stages(p.bn, g.dual);
+  const long long n_tiles = (long long)p.n_row_tiles * p.n_t_tiles;
+  const long long nkb = (p.K + GEMM_BK - 1) / GEMM_BK;
+  int max_grid = env_grid > 0 ? env_grid : n_sm;
+  if (max_grid > GEMM_MAX_GRID) max_grid = GEMM_MAX_GRID;
+  p.sched = (n_tiles >= 4LL * max_grid) ? SCHED_TILES : SCHED_STREAMK;
+  if (env_sched >= 0) p.sched = env_sched;
+  p.band = env_band > 0 ? env_band : (g.dual ? 8 : 16);
+  if (p.band > p.n_row_tiles) p.band = p.n_row_tiles;
+  const long long work = p.sched == SCHED_STREAMK ? n_tiles * nkb : n_tiles;
+  g.grid = (int)(work < max_grid ? work : max_grid);
 }
 
 cudaError_t gemm_init() {
@@ -264,16 +416,13 @@ cudaError_t gemm_init() {
 
 cudaError_t gemm_launch(const GemmLaunch &g) {
   const GemmParams &p = g.p;
-  int tiles = 0;
-  for (int i = 0; i < p.n_seg; ++i) tiles += (p.seg_rows[i] + GEMM_BM - 1) / GEMM_BM;
-  dim3 grid(tiles, (p.T + p.bn - 1) / p.bn, g.splits);
   size_t smem = gemm_smem_bytes(p.bn, g.dual, p.stages);
   const CUtensorMap *a1 = g.a[1] ? g.a[1] : g.a[0];
   const CUtensorMap *a2 = g.a[2] ? g.a[2] : g.a[0];
   if (g.dual)
-    gemm_kernel<true><<<grid, 192, smem, g.stream>>>(*g.a[0], *a1, *a2, *g.b, p);
+    gemm_kernel<true><<<g.grid, 192, smem, g.stream>>>(*g.a[0], *a1, *a2, *g.b, p);
   else
-    gemm_kernel<false><<<grid, 192, smem, g.stream>>>(*g.a[0], *a1, *a2, *g.b, p);
+    gemm_kernel<false><<<g.grid, 192, smem, g.stream>>>(*g.a[0], *a1, *a2, *g.b, p);
   count_launch();
   return cudaGetLastError();
 }

@@ -10,34 +10,50 @@ namespace ss {
 // ---------------------------------------------------------------------------------------------------------------
 // tcgen05 GEMM (gemm_tcgen05.cu).  Orientation ("swap-AB", used for every shape): the UMMA M dimension (128 TMEM
 // lanes) runs over OUTPUT FEATURES, i.e. rows of the weight matrix W[N,K]; the UMMA N dimension (TMEM columns,
-// bn in {16,32,64,128,256}) runs over TOKENS, rows of X[T,K].  out[t][n] = sum_k X[t,k] W[n,k].
+// bn in {32,64,128,256}) runs over TOKENS, rows of X[T,K].  out[t][n] = sum_k X[t,k] W[n,k].
+// Persistent: gridDim.x CTAs (<= #SMs, one per SM) walk a work list.  Two schedules:
+//   SCHED_STREAMK (few tiles, the HBM-bound decode case): the flattened (tile, k-block) units are cut into gridDim.x
+//     equal contiguous ranges; a tile cut between CTAs is fixed up in-kernel (the CTA holding the tile's first
+//     k-blocks adds the others' fp32 partials, in CTA order, then runs the epilogue) — every SM streams the same
+//     number of weight bytes whatever the tile count;
+//   SCHED_TILES (many tiles, the tensor-bound prefill case): whole tiles, round-robin, rasterised in bands of
+//     `band` weight-row tiles so that concurrently running CTAs share weight and activation tiles in L2.
 // ---------------------------------------------------------------------------------------------------------------
 constexpr int GEMM_BM = 128;  // weight rows per tile
 constexpr int GEMM_BK = 64;   // K elements per stage (= one 128-byte swizzle row of bf16)
 
-enum GemmEpilogue { EPI_F32 = 0, EPI_SWIGLU_BF16 = 1, EPI_BF16 = 2 };
+enum GemmEpilogue {
+  EPI_F32 = 0,          // out_f32[t][col] = acc
+  EPI_SWIGLU_BF16 = 1,  // dual: out_bf16[t][col] = silu(acc_gate) * acc_up
+  EPI_RESID_F32 = 2     // out_f32[t][col] += acc   (residual stream updated in place; each element once)
+};
+enum GemmSchedule { SCHED_STREAMK = 0, SCHED_TILES = 1 };
 
 struct GemmParams {
   int n_seg;            // 1..3 weight segments laid side by side in the output (q | k | v)
   int seg_rows[3];      // rows (output features) of each segment
-  int seg_tile0[3];     // first tile index of each segment
+  int seg_tile0[3];     // first row-tile index of each segment
   int seg_col[3];       // output column of each segment's row 0
+  int n_row_tiles;      // sum of the segments' row tiles
+  int n_t_tiles;        // ceil(T / bn)
   int T, K;             // tokens, reduction length
   int bn;               // tokens per tile (UMMA N)
   int stages;           // smem pipeline depth
-  int kb_per_split;     // k-blocks (of 64) per split; gridDim.z = splits
+  int sched;            // GemmSchedule
+  int band;             // SCHED_TILES: row tiles per raster band
   int epi;              // GemmEpilogue
   int ld_out;           // leading dimension (elements) of the output
-  long long split_stride;  // elements between consecutive splits' partial outputs (EPI_F32)
   float *out_f32;
   void *out_bf16;
+  float *fix_slots;     // SCHED_STREAMK: gridDim.x partial-accumulator slots of (dual ? 2 : 1) * bn * 128 floats
+  int *fix_flags;       // SCHED_STREAMK: gridDim.x flags, zero between launches (consumers reset them)
 };
 
 struct GemmLaunch {
   const CUtensorMap *a[3];  // weight maps, box {64, 128}; dual (SwiGLU): a[0] = gate, a[1] = up, n_seg = 1
   const CUtensorMap *b;     // activation map, box {64, bn}
   bool dual;
-  int splits;
+  int grid;                 // persistent CTAs
   GemmParams p;
   cudaStream_t stream;
 };
@@ -45,11 +61,17 @@ struct GemmLaunch {
 // Encode a 2-D bf16 row-major [rows, cols] tensor map with box {64 cols, box_rows}, SWIZZLE_128B.
 int make_tmap_bf16_2d(CUtensorMap *out, const void *base, uint64_t rows, uint64_t cols, uint32_t box_rows,
                       bool weight_like);
+// Fills sched / band / stages / n_*_tiles / grid from the problem shape; fix buffers must be set by the caller.
+void gemm_plan(GemmLaunch &g, int n_sm);
 cudaError_t gemm_launch(const GemmLaunch &g);
 cudaError_t gemm_init();  // sets max dynamic smem attributes once
-int gemm_pick_bn(int T);  // smallest of {16,32,64,128,256} >= min(T,256)
+int gemm_pick_bn(int T);  // smallest of {32,64,128,256} >= min(T,256)
 int gemm_pick_stages(int bn, bool dual);
 size_t gemm_smem_bytes(int bn, bool dual, int stages);
+constexpr int GEMM_MAX_GRID = 256;                       // upper bound on persistent CTAs (sizes the fix buffers)
+constexpr size_t GEMM_FIX_FLAG_BYTES = 1024;             // GEMM_MAX_GRID ints
+constexpr size_t GEMM_FIX_SLOT_BYTES = 2 * 256 * 128 * 4;  // worst case: dual, bn = 256
+inline size_t gemm_fix_bytes() { return GEMM_FIX_FLAG_BYTES + GEMM_MAX_GRID * GEMM_FIX_SLOT_BYTES; }
 
 // ---------------------------------------------------------------------------------------------------------------
 // element-wise / reduction kernels (elementwise.cu)

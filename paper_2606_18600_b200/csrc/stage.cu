@@ -34,14 +34,12 @@ static int cuda_fail(cudaError_t e, const char *where) {
     if (e__ != cudaSuccess) return cuda_fail(e__, #call); \
   } while (0)
 
-constexpr int S_MAX = 8;           // max K-splits of a projection
-constexpr int SPLIT_ROWS = 256;    // split-K is only used when T <= SPLIT_ROWS
 constexpr int MAX_WORKERS = 4096;  // upper bound on decode-attention worker warps (sizes the partial buffers)
 
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Carve {  // byte offsets into the workspace
-  size_t args, rope, x, h, qkv_part, q, kv_new, attn_out, proj_part, a, part_o, part_ml, cum_pages, meta, tok_seq,
+  size_t args, rope, x, h, qkv_part, q, kv_new, attn_out, fix, a, part_o, part_ml, cum_pages, meta, tok_seq,
       tok_pos, tile_cum, hl, logits, total;
 };
 
@@ -64,8 +62,6 @@ static Carve carve(const ss_model_dims *d) {
   const size_t Tm = (size_t)(d->max_tokens > d->max_seqs ? d->max_tokens : d->max_seqs);
   const size_t H = d->hidden, Hq = (size_t)d->n_q_heads * d->head_dim, Hkv = (size_t)d->n_kv_heads * d->head_dim;
   const size_t F = d->ffn, Nqkv = Hq + 2 * Hkv;
-  const size_t split_rows = (size_t)S_MAX * (Tm < (size_t)SPLIT_ROWS ? Tm : (size_t)SPLIT_ROWS);
-  const size_t part_rows = split_rows > Tm ? split_rows : Tm;
   const size_t n_slots = (size_t)MAX_WORKERS + (size_t)d->max_seqs * d->n_kv_heads;
   size_t o = 0;
   auto take = [&](size_t bytes) {
@@ -77,11 +73,11 @@ static Carve carve(const ss_model_dims *d) {
   c.rope = take((size_t)d->max_pos * (d->head_dim / 2) * 2 * sizeof(float));
   c.x = take(Tm * H * 4);
   c.h = take(Tm * H * 2);
-  c.qkv_part = take(part_rows * Nqkv * 4);
+  c.qkv_part = take(Tm * Nqkv * 4);
   c.q = take(Tm * Hq * 2);
   c.kv_new = take((size_t)d->max_seqs * 2 * Hkv * 2);
   c.attn_out = take(Tm * Hq * 2);
-  c.proj_part = take(part_rows * H * 4);
+  c.fix = take(gemm_fix_bytes());  // stream-K fix-up flags + partial-accumulator slots
   c.a = take(Tm * F * 2);
   c.part_o = take(n_slots * 16 * d->head_dim * 4);
   c.part_ml = take(n_slots * 32 * 4);
@@ -131,7 +127,6 @@ struct ss_stage {
   int64_t launches;
   std::map<int, Graph> graphs;  // key = batch*2 + tail
   bool use_graph;
-  int force_split[3];  // qkv, o, down (0 = heuristic)
   CallArgs *h_args;    // pinned host staging for the argument block
 
   size_t layer_kv_elems() const { return (size_t)num_pages * d.n_kv_heads * 16 * d.head_dim; }
@@ -215,9 +210,6 @@ int ss_stage_create(ss_stage **out, const ss_model_dims *dims, int l0, int l1, c
   st->stream = (cudaStream_t)cuda_stream;
   st->launches = 0;
   st->use_graph = (cuda_stream != nullptr) && env_int("SS_NO_GRAPH", 0) == 0;
-  st->force_split[0] = env_int("SS_SPLIT_QKV", 0);
-  st->force_split[1] = env_int("SS_SPLIT_O", 0);
-  st->force_split[2] = env_int("SS_SPLIT_DOWN", 0);
   st->h_args = nullptr;
 
   auto fail = [&](int code) {
@@ -253,6 +245,8 @@ int ss_stage_create(ss_stage **out, const ss_model_dims *dims, int l0, int l1, c
     }
     e = cudaMemcpyAsync(st->ws + c.rope, tab.data(), tab.size() * sizeof(float), cudaMemcpyHostToDevice, st->stream);
     if (e != cudaSuccess) return fail(cuda_fail(e, "rope upload"));
+    e = cudaMemsetAsync(st->ws + c.fix, 0, GEMM_FIX_FLAG_BYTES, st->stream);  // stream-K flags start (and stay) zero
+    if (e != cudaSuccess) return fail(cuda_fail(e, "fix flags memset"));
     e = cudaStreamSynchronize(st->stream);
     if (e != cudaSuccess) return fail(cuda_fail(e, "rope upload sync"));
   }
@@ -351,68 +345,30 @@ int64_t ss_stage_launch_count(const ss_stage *st) { return st ? st->launches : 0
 // ===================================================================================================================
 namespace ss {
 
-// K-split heuristic for the HBM-bound small-T case: enough CTAs to cover the SMs, each with a long enough K loop.
-static int pick_splits(const ss_stage *st, int tiles, int t_tiles, int nkb, int T, int forced) {
-  if (T > SPLIT_ROWS) return 1;
-  int s = 1;
-  if (forced > 0) {
-    s = forced;
-  } else if (tiles * t_tiles < st->n_sm) {
-    s = (st->n_sm + tiles * t_tiles - 1) / (tiles * t_tiles);
-    while (s > 1 && nkb / s < 16) --s;  // keep >= 16 k-blocks (1024 K elements) per CTA
-  }
-  if (s > S_MAX) s = S_MAX;
-  if (s > nkb) s = nkb;
-  if (s < 1) s = 1;
-  return s;
-}
-
-struct GemmOut {
-  int splits;
-  long long split_stride;
-};
-
-// one projection: out_f32 partials [splits][T][ld] (EPI_F32) or fused SwiGLU bf16 (dual)
+// one projection through the persistent tcgen05 GEMM
 static cudaError_t run_gemm(const ss_stage *st, const CUtensorMap *const a[3], int n_seg, const int rows[3],
-                            bool dual, const CUtensorMap bmaps[5], int T, int K, float *out_f32, void *out_bf16,
-                            int ld_out, int forced_split, GemmOut *res) {
+                            bool dual, const CUtensorMap bmaps[5], int T, int K, int epi, float *out_f32,
+                            void *out_bf16, int ld_out) {
   GemmLaunch g;
   memset(&g, 0, sizeof(g));
   GemmParams &p = g.p;
   p.n_seg = n_seg;
-  int tiles = 0, col = 0;
   for (int i = 0; i < 3; ++i) {
     g.a[i] = a[i];
     p.seg_rows[i] = i < n_seg ? rows[i] : 0;
-    p.seg_tile0[i] = tiles;
-    p.seg_col[i] = col;
-    if (i < n_seg) {
-      tiles += (rows[i] + GEMM_BM - 1) / GEMM_BM;
-      col += rows[i];
-    }
   }
   p.T = T;
   p.K = K;
-  p.bn = gemm_pick_bn(T);
-  p.stages = gemm_pick_stages(p.bn, dual);
-  const int nkb = (K + GEMM_BK - 1) / GEMM_BK;
-  const int t_tiles = (T + p.bn - 1) / p.bn;
-  int splits = dual ? 1 : pick_splits(st, tiles, t_tiles, nkb, T, forced_split);
-  p.kb_per_split = (nkb + splits - 1) / splits;
-  splits = (nkb + p.kb_per_split - 1) / p.kb_per_split;
-  p.epi = dual ? EPI_SWIGLU_BF16 : EPI_F32;
+  p.epi = epi;
   p.ld_out = ld_out;
-  p.split_stride = (long long)T * ld_out;
   p.out_f32 = out_f32;
   p.out_bf16 = out_bf16;
-  g.b = &bmaps[p.bn == 16 ? 0 : p.bn == 32 ? 1 : p.bn == 64 ? 2 : p.bn == 128 ? 3 : 4];
+  p.fix_flags = st->at<int>(st->c.fix);
+  p.fix_slots = (float *)(st->ws + st->c.fix + GEMM_FIX_FLAG_BYTES);
   g.dual = dual;
-  g.splits = splits;
   g.stream = st->stream;
-  if (res) {
-    res->splits = splits;
-    res->split_stride = p.split_stride;
-  }
+  gemm_plan(g, st->n_sm);
+  g.b = &bmaps[p.bn == 32 ? 1 : p.bn == 64 ? 2 : p.bn == 128 ? 3 : 4];
   return gemm_launch(g);
 }
 
@@ -432,7 +388,6 @@ static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T,
   float *x = st->at<float>(c.x);
   void *h = st->at<void>(c.h);
   float *qkv_part = st->at<float>(c.qkv_part);
-  float *proj_part = st->at<float>(c.proj_part);
   cudaStream_t s = st->stream;
 
   DecodePlan dplan{st->at<int32_t>(c.cum_pages), st->at<int32_t>(c.meta)};
@@ -446,17 +401,16 @@ static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T,
   for (int l = 0; l < st->L; ++l) {
     const ss_layer_weights &w = st->lw[l];
     const LayerMaps &m = st->maps[l];
-    GemmOut go;
-    {  // S2: QKV projection -> fp32 partials [splits][T][Hq+2Hkv]
+    {  // S2: QKV projection -> fp32 [T][Hq+2Hkv]
       const CUtensorMap *a[3] = {&m.wq, &m.wk, &m.wv};
       const int rows[3] = {Hq, Hkv, Hkv};
-      CKE(run_gemm(st, a, 3, rows, false, st->b_h, T, H, qkv_part, nullptr, Nqkv, st->force_split[0], &go));
+      CKE(run_gemm(st, a, 3, rows, false, st->b_h, T, H, EPI_F32, qkv_part, nullptr, Nqkv));
     }
     QkvPostParams qp;
     memset(&qp, 0, sizeof(qp));
     qp.qkv_part = qkv_part;
-    qp.splits = go.splits;
-    qp.split_stride = go.split_stride;
+    qp.splits = 1;
+    qp.split_stride = 0;
     qp.T = T; qp.n_q = d.n_q_heads; qp.n_kv = d.n_kv_heads; qp.d = dh;
     qp.qk_norm = d.qk_norm;
     qp.eps = d.rms_eps;
@@ -503,32 +457,28 @@ static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T,
     {  // S7: output projection, then S8: x1 = x + o Wo^T ; h2 = rmsnorm(x1; ln2)
       const CUtensorMap *a[3] = {&m.wo, nullptr, nullptr};
       const int rows[3] = {H, 0, 0};
-      CKE(run_gemm(st, a, 1, rows, false, st->b_attn, T, Hq, proj_part, nullptr, H, st->force_split[1], &go));
-      CKE(launch_residual_rmsnorm(x, proj_part, go.splits, go.split_stride, w.ln2, d.rms_eps, H, T, h, args, false,
-                                  s));
+      CKE(run_gemm(st, a, 1, rows, false, st->b_attn, T, Hq, EPI_RESID_F32, x, nullptr, H));
+      CKE(launch_residual_rmsnorm(x, nullptr, 0, 0, w.ln2, d.rms_eps, H, T, h, args, false, s));
     }
     {  // S9: gate/up + SwiGLU fused -> a bf16 [T,F]
       const CUtensorMap *a[3] = {&m.wg, &m.wu, nullptr};
       const int rows[3] = {F, 0, 0};
-      CKE(run_gemm(st, a, 1, rows, true, st->b_h, T, H, nullptr, st->at<void>(c.a), F, 0, &go));
+      CKE(run_gemm(st, a, 1, rows, true, st->b_h, T, H, EPI_SWIGLU_BF16, nullptr, st->at<void>(c.a), F));
     }
     {  // S10: down projection + residual, then the next layer's RMSNorm-1 (or the stage output)
       const CUtensorMap *a[3] = {&m.wd, nullptr, nullptr};
       const int rows[3] = {H, 0, 0};
-      CKE(run_gemm(st, a, 1, rows, false, st->b_a, T, F, proj_part, nullptr, H, st->force_split[2], &go));
+      CKE(run_gemm(st, a, 1, rows, false, st->b_a, T, F, EPI_RESID_F32, x, nullptr, H));
       const bool last = (l == st->L - 1);
       const void *next_ln = last ? nullptr : st->lw[l + 1].ln1;
-      CKE(launch_residual_rmsnorm(x, proj_part, go.splits, go.split_stride, next_ln, d.rms_eps, H, T, h, args, last,
-                                  s));
+      CKE(launch_residual_rmsnorm(x, nullptr, 0, 0, next_ln, d.rms_eps, H, T, h, args, last, s));
     }
   }
   if (tail) {  // S11: final norm of each sequence's last row, lm_head, argmax
-    GemmOut go;
     CKE(launch_final_norm_rows(x, args, decode, st->edge.final_norm, d.rms_eps, H, n_seqs, st->at<void>(c.hl), s));
     const CUtensorMap *a[3] = {&st->lm_map, nullptr, nullptr};
     const int rows[3] = {d.vocab, 0, 0};
-    // the partial buffer of the logits is the logits workspace itself (never split: V/128 tiles cover the SMs)
-    CKE(run_gemm(st, a, 1, rows, false, st->b_hl, n_seqs, H, st->at<float>(c.logits), nullptr, d.vocab, 1, &go));
+    CKE(run_gemm(st, a, 1, rows, false, st->b_hl, n_seqs, H, EPI_F32, st->at<float>(c.logits), nullptr, d.vocab));
     CKE(launch_logits_argmax(st->at<float>(c.logits), 1, 0, d.vocab, n_seqs, st->at<float>(c.logits), args, s));
   }
   return cudaSuccess;
@@ -635,93 +585,73 @@ int ss_stage_decode(ss_stage *st, int batch, const void *hidden_bf16, const int3
 // op-level entry points: the same GEMM kernel, stand-alone (per-kernel parity tests, profiling)
 // ===================================================================================================================
 namespace ss {
-__global__ void reduce_splits_kernel(const float *__restrict__ part, int splits, long long stride, long long n,
-                                     float *__restrict__ out) {
-  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
-    float v = part[i];
-    for (int s = 1; s < splits; ++s) v += part[(long long)s * stride + i];
-    out[i] = v;
+static int device_sms() {
+  static int n = 0;
+  if (n == 0) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+      n = 0;
   }
+  return n;
+}
+
+static int op_gemm(const void *x_dev, const void *w0, const void *w1, float *c_f32, void *c_bf16, int T, int N, int K,
+                   bool dual, void *scratch_dev, size_t scratch_bytes, void *cuda_stream) {
+  if (!x_dev || !w0 || (dual && !w1) || (!c_f32 && !c_bf16) || T <= 0 || N <= 0 || K <= 0 || !scratch_dev)
+    return SS_ERR_INVALID_ARG;
+  if (K % 8 != 0 || ((uintptr_t)x_dev & 15) || ((uintptr_t)w0 & 15) || (dual && ((uintptr_t)w1 & 15)) ||
+      ((uintptr_t)scratch_dev & 255))
+    return SS_ERR_UNSUPPORTED;
+  if (scratch_bytes < gemm_fix_bytes()) return SS_ERR_CAPACITY;
+  cudaError_t e = gemm_init();
+  if (e != cudaSuccess) return cuda_fail(e, "gemm_init");
+  const int n_sm = device_sms();
+  if (n_sm <= 0) return cuda_fail(cudaErrorNoDevice, "device_sms");
+  CUtensorMap ta, tu, tb;
+  GemmLaunch g;
+  memset(&g, 0, sizeof(g));
+  GemmParams &p = g.p;
+  p.n_seg = 1;
+  p.seg_rows[0] = N;
+  p.T = T;
+  p.K = K;
+  p.epi = dual ? EPI_SWIGLU_BF16 : EPI_F32;
+  p.ld_out = N;
+  p.out_f32 = c_f32;
+  p.out_bf16 = c_bf16;
+  p.fix_flags = (int *)scratch_dev;
+  p.fix_slots = (float *)((uint8_t *)scratch_dev + GEMM_FIX_FLAG_BYTES);
+  g.dual = dual;
+  g.stream = (cudaStream_t)cuda_stream;
+  gemm_plan(g, n_sm);
+  if (make_tmap_bf16_2d(&ta, w0, (uint64_t)N, (uint64_t)K, GEMM_BM, true) != 0 ||
+      (dual && make_tmap_bf16_2d(&tu, w1, (uint64_t)N, (uint64_t)K, GEMM_BM, true) != 0) ||
+      make_tmap_bf16_2d(&tb, x_dev, (uint64_t)T, (uint64_t)K, (uint32_t)p.bn, false) != 0) {
+    g_cuda_err = "cuTensorMapEncodeTiled failed";
+    return SS_ERR_CUDA;
+  }
+  g.a[0] = &ta;
+  g.a[1] = dual ? &tu : nullptr;
+  g.b = &tb;
+  e = gemm_launch(g);
+  if (e != cudaSuccess) return cuda_fail(e, "gemm_launch");
+  return SS_OK;
 }
 }  // namespace ss
 
 extern "C" {
 
-int ss_op_gemm_bf16(const void *x_dev, const void *w_dev, float *c_dev, int T, int N, int K, int splits,
-                    void *scratch_dev, void *cuda_stream) {
-  if (!x_dev || !w_dev || !c_dev || T <= 0 || N <= 0 || K <= 0 || splits < 1) return SS_ERR_INVALID_ARG;
-  if (K % 8 != 0 || ((uintptr_t)x_dev & 15) || ((uintptr_t)w_dev & 15)) return SS_ERR_UNSUPPORTED;
-  if (splits > 1 && !scratch_dev) return SS_ERR_INVALID_ARG;
-  cudaError_t e = gemm_init();
-  if (e != cudaSuccess) return cuda_fail(e, "gemm_init");
-  CUtensorMap ta, tb;
-  GemmLaunch g;
-  memset(&g, 0, sizeof(g));
-  GemmParams &p = g.p;
-  p.bn = gemm_pick_bn(T);
-  if (make_tmap_bf16_2d(&ta, w_dev, (uint64_t)N, (uint64_t)K, GEMM_BM, true) != 0 ||
-      make_tmap_bf16_2d(&tb, x_dev, (uint64_t)T, (uint64_t)K, (uint32_t)p.bn, false) != 0) {
-    g_cuda_err = "cuTensorMapEncodeTiled failed";
-    return SS_ERR_CUDA;
-  }
-  const int nkb = (K + GEMM_BK - 1) / GEMM_BK;
-  if (splits > nkb) splits = nkb;
-  p.n_seg = 1;
-  p.seg_rows[0] = N;
-  p.T = T; p.K = K;
-  p.stages = gemm_pick_stages(p.bn, false);
-  p.kb_per_split = (nkb + splits - 1) / splits;
-  splits = (nkb + p.kb_per_split - 1) / p.kb_per_split;
-  p.epi = EPI_F32;
-  p.ld_out = N;
-  p.split_stride = (long long)T * N;
-  p.out_f32 = splits > 1 ? (float *)scratch_dev : c_dev;
-  g.a[0] = &ta; g.b = &tb; g.dual = false; g.splits = splits; g.stream = (cudaStream_t)cuda_stream;
-  e = gemm_launch(g);
-  if (e != cudaSuccess) return cuda_fail(e, "gemm_launch");
-  if (splits > 1) {
-    const long long n = (long long)T * N;
-    int blocks = (int)((n + 255) / 256 > 4096 ? 4096 : (n + 255) / 256);
-    reduce_splits_kernel<<<blocks, 256, 0, (cudaStream_t)cuda_stream>>>((const float *)scratch_dev, splits, n, n,
-                                                                         c_dev);
-    count_launch();
-    e = cudaGetLastError();
-    if (e != cudaSuccess) return cuda_fail(e, "reduce_splits");
-  }
-  return SS_OK;
+size_t ss_op_gemm_scratch_bytes(void) { return gemm_fix_bytes(); }
+
+int ss_op_gemm_bf16(const void *x_dev, const void *w_dev, float *c_dev, int T, int N, int K, void *scratch_dev,
+                    size_t scratch_bytes, void *cuda_stream) {
+  return op_gemm(x_dev, w_dev, nullptr, c_dev, nullptr, T, N, K, false, scratch_dev, scratch_bytes, cuda_stream);
 }
 
 int ss_op_gemm_swiglu_bf16(const void *x_dev, const void *wg_dev, const void *wu_dev, void *a_dev, int T, int F,
-                           int K, void *cuda_stream) {
-  if (!x_dev || !wg_dev || !wu_dev || !a_dev || T <= 0 || F <= 0 || K <= 0) return SS_ERR_INVALID_ARG;
-  if (K % 8 != 0 || ((uintptr_t)x_dev & 15) || ((uintptr_t)wg_dev & 15) || ((uintptr_t)wu_dev & 15))
-    return SS_ERR_UNSUPPORTED;
-  cudaError_t e = gemm_init();
-  if (e != cudaSuccess) return cuda_fail(e, "gemm_init");
-  CUtensorMap tg, tu, tb;
-  GemmLaunch g;
-  memset(&g, 0, sizeof(g));
-  GemmParams &p = g.p;
-  p.bn = gemm_pick_bn(T);
-  if (make_tmap_bf16_2d(&tg, wg_dev, (uint64_t)F, (uint64_t)K, GEMM_BM, true) != 0 ||
-      make_tmap_bf16_2d(&tu, wu_dev, (uint64_t)F, (uint64_t)K, GEMM_BM, true) != 0 ||
-      make_tmap_bf16_2d(&tb, x_dev, (uint64_t)T, (uint64_t)K, (uint32_t)p.bn, false) != 0) {
-    g_cuda_err = "cuTensorMapEncodeTiled failed";
-    return SS_ERR_CUDA;
-  }
-  const int nkb = (K + GEMM_BK - 1) / GEMM_BK;
-  p.n_seg = 1;
-  p.seg_rows[0] = F;
-  p.T = T; p.K = K;
-  p.stages = gemm_pick_stages(p.bn, true);
-  p.kb_per_split = nkb;
-  p.epi = EPI_SWIGLU_BF16;
-  p.ld_out = F;
-  p.out_bf16 = a_dev;
-  g.a[0] = &tg; g.a[1] = &tu; g.b = &tb; g.dual = true; g.splits = 1; g.stream = (cudaStream_t)cuda_stream;
-  e = gemm_launch(g);
-  if (e != cudaSuccess) return cuda_fail(e, "gemm_launch");
-  return SS_OK;
+                           int K, void *scratch_dev, size_t scratch_bytes, void *cuda_stream) {
+  return op_gemm(x_dev, wg_dev, wu_dev, nullptr, a_dev, T, F, K, true, scratch_dev, scratch_bytes, cuda_stream);
 }
 
 }  // extern "C"
