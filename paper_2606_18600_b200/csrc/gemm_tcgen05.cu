@@ -280,11 +280,19 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
                 }
               }
             } else if (p.epi == EPI_RESID_F32) {
+              // all 32 loads of the residual are issued before the first store (a `+=` loop would serialise
+              // 32 dependent L2 round trips per chunk: the compiler cannot prove the stores do not alias the loads)
               float *o = p.out_f32 + col;
+              float xv[32];
 #pragma unroll
               for (int j = 0; j < 32; ++j) {
                 const int t = t0 + c0 + j;
-                if (t < p.T) o[(size_t)t * p.ld_out] += __uint_as_float(v[j]);
+                xv[j] = (t < p.T) ? __ldcg(o + (size_t)t * p.ld_out) : 0.f;
+              }
+#pragma unroll
+              for (int j = 0; j < 32; ++j) {
+                const int t = t0 + c0 + j;
+                if (t < p.T) o[(size_t)t * p.ld_out] = xv[j] + __uint_as_float(v[j]);
               }
             } else {
               float *o = p.out_f32 + col;
