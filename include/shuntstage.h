@@ -163,6 +163,12 @@ int64_t ss_stage_launch_count(const ss_stage *st);
  * 1024 bytes must be ZERO before the first call (the kernel leaves them zero). */
 size_t ss_op_gemm_scratch_bytes(void);
 
+/* Debug aid.  `host_mapped_u64x4` is pinned, device-mapped HOST memory of 4 x uint64 (or NULL to disable).  Every
+ * wait inside the GEMM kernel is bounded; when one expires the kernel stores {site id, block<<32|thread,
+ * info<<32|parity} there and traps (the call then fails with SS_ERR_CUDA), so a protocol bug is a located error and
+ * never a hung GPU.  Returns SS_OK or SS_ERR_CUDA. */
+int ss_debug_buffer(void *host_mapped_u64x4);
+
 /* C[T, N] (fp32, row-major, ld = N) = X[T, K] (bf16, row-major) * W[N, K]^T (bf16) through the persistent
  * tcgen05/TMEM GEMM.  K % 8 == 0.  Asynchronous on cuda_stream. */
 int ss_op_gemm_bf16(const void *x_dev, const void *w_dev, float *c_dev, int T, int N, int K,

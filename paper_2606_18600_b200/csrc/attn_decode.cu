@@ -29,6 +29,8 @@ constexpr int DA_STAGES = 3;
 // ---- plan: prefix sum of pages per sequence --------------------------------------------------------------------
 __global__ void decode_plan_kernel(const CallArgs *__restrict__ args, int batch, int n_kv, int n_workers,
                                    DecodePlan plan) {
+  pdl_launch_dependents();
+  pdl_wait();
   if (threadIdx.x == 0 && blockIdx.x == 0) {
     int acc = 0;
     plan.cum_pages[0] = 0;
@@ -44,9 +46,7 @@ __global__ void decode_plan_kernel(const CallArgs *__restrict__ args, int batch,
 
 cudaError_t launch_decode_plan(const CallArgs *args, int batch, int n_kv, int n_workers, DecodePlan plan,
                                cudaStream_t s) {
-  decode_plan_kernel<<<1, 32, 0, s>>>(args, batch, n_kv, n_workers, plan);
-  count_launch();
-  return cudaGetLastError();
+  return launch_pdl(decode_plan_kernel, dim3(1), dim3(32), 0, s, args, batch, n_kv, n_workers, plan);
 }
 
 struct Cursor {
@@ -55,6 +55,8 @@ struct Cursor {
 
 template <int D>
 __global__ void __launch_bounds__(DA_WARPS * 32) decode_attn_kernel(const DecodeAttnParams p) {
+  pdl_launch_dependents();
+  pdl_wait();
   constexpr int ROW_BYTES = D * 2;
   constexpr int CHUNKS = ROW_BYTES / 16;       // 16-byte chunks per row: 16 (d=128) or 8 (d=64)
   constexpr int PAGE_BYTES = 16 * ROW_BYTES;   // one K (or V) page of one head
@@ -293,6 +295,8 @@ __global__ void __launch_bounds__(DA_WARPS * 32) decode_attn_kernel(const Decode
 constexpr int MERGE_THREADS = 256;
 template <int D>
 __global__ void __launch_bounds__(MERGE_THREADS) decode_merge_kernel(const DecodeAttnParams p) {
+  pdl_launch_dependents();
+  pdl_wait();
   constexpr int LANES = D / 4;                  // threads per q head
   constexpr int HEADS_PER_PASS = MERGE_THREADS / LANES;
   const int pair = blockIdx.x;
@@ -341,20 +345,16 @@ cudaError_t attn_init() {
 cudaError_t launch_decode_attn(const DecodeAttnParams &p, cudaStream_t s) {
   const int ctas = p.n_workers / DA_WARPS;
   if (p.d == 128)
-    decode_attn_kernel<128><<<ctas, DA_WARPS * 32, decode_smem(128), s>>>(p);
+    return launch_pdl(decode_attn_kernel<128>, dim3(ctas), dim3(DA_WARPS * 32), decode_smem(128), s, p);
   else
-    decode_attn_kernel<64><<<ctas, DA_WARPS * 32, decode_smem(64), s>>>(p);
-  count_launch();
-  return cudaGetLastError();
+    return launch_pdl(decode_attn_kernel<64>, dim3(ctas), dim3(DA_WARPS * 32), decode_smem(64), s, p);
 }
 
 cudaError_t launch_decode_merge(const DecodeAttnParams &p, cudaStream_t s) {
   if (p.d == 128)
-    decode_merge_kernel<128><<<p.batch * p.n_kv, MERGE_THREADS, 0, s>>>(p);
+    return launch_pdl(decode_merge_kernel<128>, dim3(p.batch * p.n_kv), dim3(MERGE_THREADS), 0, s, p);
   else
-    decode_merge_kernel<64><<<p.batch * p.n_kv, MERGE_THREADS, 0, s>>>(p);
-  count_launch();
-  return cudaGetLastError();
+    return launch_pdl(decode_merge_kernel<64>, dim3(p.batch * p.n_kv), dim3(MERGE_THREADS), 0, s, p);
 }
 
 }  // namespace ss

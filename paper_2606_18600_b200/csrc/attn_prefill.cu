@@ -23,6 +23,8 @@ constexpr int PA_BN = 64;  // keys per tile
 
 // ---- plan: token -> (sequence, position) and the prefix sum of query tiles --------------------------------------
 __global__ void prefill_plan_kernel(const CallArgs *__restrict__ args, int n_seqs, PrefillPlan plan) {
+  pdl_launch_dependents();
+  pdl_wait();
   if (blockIdx.x == 0 && threadIdx.x == 0) {
     int acc = 0;
     plan.tile_cum[0] = 0;
@@ -42,13 +44,13 @@ __global__ void prefill_plan_kernel(const CallArgs *__restrict__ args, int n_seq
 
 cudaError_t launch_prefill_plan(const CallArgs *args, int n_seqs, PrefillPlan plan, cudaStream_t s) {
   int blocks = n_seqs < 1 ? 1 : (n_seqs > 1024 ? 1024 : n_seqs);
-  prefill_plan_kernel<<<blocks, 256, 0, s>>>(args, n_seqs, plan);
-  count_launch();
-  return cudaGetLastError();
+  return launch_pdl(prefill_plan_kernel, dim3(blocks), dim3(256), 0, s, args, n_seqs, plan);
 }
 
 template <int D>
 __global__ void __launch_bounds__(PA_WARPS * 32) prefill_attn_kernel(const PrefillAttnParams p) {
+  pdl_launch_dependents();
+  pdl_wait();
   constexpr int ROW_BYTES = D * 2;
   constexpr int CHUNKS = ROW_BYTES / 16;
   constexpr int TILE_BYTES = PA_BN * ROW_BYTES;
@@ -251,11 +253,9 @@ cudaError_t launch_prefill_attn(const PrefillAttnParams &p, cudaStream_t s) {
   }
   dim3 grid(p.n_q, p.max_tiles);
   if (p.d == 128)
-    prefill_attn_kernel<128><<<grid, PA_WARPS * 32, prefill_smem(128), s>>>(p);
+    return launch_pdl(prefill_attn_kernel<128>, dim3(grid), dim3(PA_WARPS * 32), prefill_smem(128), s, p);
   else
-    prefill_attn_kernel<64><<<grid, PA_WARPS * 32, prefill_smem(64), s>>>(p);
-  count_launch();
-  return cudaGetLastError();
+    return launch_pdl(prefill_attn_kernel<64>, dim3(grid), dim3(PA_WARPS * 32), prefill_smem(64), s, p);
 }
 
 }  // namespace ss

@@ -43,6 +43,14 @@ __device__ __forceinline__ bool elect_one() {
   return pred != 0;
 }
 
+// ---- programmatic dependent launch (PDL) --------------------------------------------------------------------
+// Every kernel of the stage is launched with programmaticStreamSerialization: it may start while its predecessor
+// is still draining.  pdl_launch_dependents() lets the successor be scheduled; pdl_wait() returns once the
+// predecessor grid has completed and its writes are visible — nothing written by an earlier kernel of the same
+// call may be read, and nothing may be written, before it.  Both are no-ops in a launch without the attribute.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 // ---- mbarrier ----------------------------------------------------------------------------------------------
 __device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));

@@ -33,6 +33,8 @@ __global__ void __launch_bounds__(EW_THREADS)
 input_rmsnorm_kernel(const CallArgs *__restrict__ args, const __nv_bfloat16 *__restrict__ embed,
                      const __nv_bfloat16 *__restrict__ w, float eps, int H, float *__restrict__ x,
                      __nv_bfloat16 *__restrict__ h) {
+  pdl_launch_dependents();
+  pdl_wait();
   __shared__ float red[32];
   const int t = blockIdx.x;
   const __nv_bfloat16 *src;
@@ -67,10 +69,7 @@ input_rmsnorm_kernel(const CallArgs *__restrict__ args, const __nv_bfloat16 *__r
 
 cudaError_t launch_input_rmsnorm(const CallArgs *args, const void *embed, const void *ln_w, float eps, int H,
                                  int T, float *x, void *h, cudaStream_t s) {
-  input_rmsnorm_kernel<<<T, EW_THREADS, 0, s>>>(args, (const __nv_bfloat16 *)embed, (const __nv_bfloat16 *)ln_w,
-                                                eps, H, x, (__nv_bfloat16 *)h);
-  count_launch();
-  return cudaGetLastError();
+  return launch_pdl(input_rmsnorm_kernel, dim3(T), dim3(EW_THREADS), 0, s, args, (const __nv_bfloat16 *)embed, (const __nv_bfloat16 *)ln_w, eps, H, x, (__nv_bfloat16 *)h);
 }
 
 // ---- residual += sum_s part[s]; optional RMSNorm -> h; optional bf16 stage output -----------------------------
@@ -82,6 +81,8 @@ __global__ void __launch_bounds__(RN_THREADS)
 residual_rmsnorm_kernel(float *__restrict__ x, const float *__restrict__ part, int splits, long long split_stride,
                         const __nv_bfloat16 *__restrict__ w, float eps, int H, __nv_bfloat16 *__restrict__ h,
                         const CallArgs *__restrict__ args, int write_out) {
+  pdl_launch_dependents();
+  pdl_wait();
   __shared__ float red[32];
   const int t = blockIdx.x;
   float *xr = x + (size_t)t * H;
@@ -148,21 +149,21 @@ cudaError_t launch_residual_rmsnorm(float *x, const float *part, int splits, lon
   const int wo = write_out_hidden ? 1 : 0;
   const int it = (H + RN_THREADS * 4 - 1) / (RN_THREADS * 4);
   if (it <= 1)
-    residual_rmsnorm_kernel<1><<<T, RN_THREADS, 0, s>>>(x, part, splits, split_stride, w, eps, H, hh, args, wo);
+    return launch_pdl(residual_rmsnorm_kernel<1>, dim3(T), dim3(RN_THREADS), 0, s, x, part, splits, split_stride, w, eps, H, hh, args, wo);
   else if (it <= 2)
-    residual_rmsnorm_kernel<2><<<T, RN_THREADS, 0, s>>>(x, part, splits, split_stride, w, eps, H, hh, args, wo);
+    return launch_pdl(residual_rmsnorm_kernel<2>, dim3(T), dim3(RN_THREADS), 0, s, x, part, splits, split_stride, w, eps, H, hh, args, wo);
   else if (it <= 4)
-    residual_rmsnorm_kernel<4><<<T, RN_THREADS, 0, s>>>(x, part, splits, split_stride, w, eps, H, hh, args, wo);
+    return launch_pdl(residual_rmsnorm_kernel<4>, dim3(T), dim3(RN_THREADS), 0, s, x, part, splits, split_stride, w, eps, H, hh, args, wo);
   else
     return cudaErrorInvalidValue;  // hidden > 16384 is rejected at create
-  count_launch();
-  return cudaGetLastError();
 }
 
 // ---- S11a: final RMSNorm of the last row of each sequence -----------------------------------------------------
 __global__ void __launch_bounds__(EW_THREADS)
 final_norm_rows_kernel(const float *__restrict__ x, const CallArgs *__restrict__ args, int decode,
                        const __nv_bfloat16 *__restrict__ wf, float eps, int H, __nv_bfloat16 *__restrict__ hl) {
+  pdl_launch_dependents();
+  pdl_wait();
   __shared__ float red[32];
   const int s = blockIdx.x;
   const int row = decode ? s : (args->cu_q[s + 1] - 1);
@@ -177,16 +178,15 @@ final_norm_rows_kernel(const float *__restrict__ x, const CallArgs *__restrict__
 
 cudaError_t launch_final_norm_rows(const float *x, const CallArgs *args, bool decode, const void *wf, float eps,
                                    int H, int n_seqs, void *hl, cudaStream_t s) {
-  final_norm_rows_kernel<<<n_seqs, EW_THREADS, 0, s>>>(x, args, decode ? 1 : 0, (const __nv_bfloat16 *)wf, eps, H,
-                                                       (__nv_bfloat16 *)hl);
-  count_launch();
-  return cudaGetLastError();
+  return launch_pdl(final_norm_rows_kernel, dim3(n_seqs), dim3(EW_THREADS), 0, s, x, args, decode ? 1 : 0, (const __nv_bfloat16 *)wf, eps, H, (__nv_bfloat16 *)hl);
 }
 
 // ---- S11b: reduce logits splits, copy out, argmax (lowest index among maxima) ---------------------------------
 __global__ void __launch_bounds__(1024)
 logits_argmax_kernel(const float *__restrict__ part, int splits, long long split_stride, int V,
                      float *__restrict__ logits_ws, const CallArgs *__restrict__ args) {
+  pdl_launch_dependents();
+  pdl_wait();
   __shared__ float smax[32];
   __shared__ int sidx[32];
   const int r = blockIdx.x;
@@ -237,13 +237,13 @@ logits_argmax_kernel(const float *__restrict__ part, int splits, long long split
 
 cudaError_t launch_logits_argmax(const float *part, int splits, long long split_stride, int V, int n_rows,
                                  float *logits_ws, const CallArgs *args, cudaStream_t s) {
-  logits_argmax_kernel<<<n_rows, 1024, 0, s>>>(part, splits, split_stride, V, logits_ws, args);
-  count_launch();
-  return cudaGetLastError();
+  return launch_pdl(logits_argmax_kernel, dim3(n_rows), dim3(1024), 0, s, part, splits, split_stride, V, logits_ws, args);
 }
 
 // ---- S3 + S4 (+ S5 in prefill): one warp per (token, head) ----------------------------------------------------
 __global__ void __launch_bounds__(EW_THREADS) qkv_post_kernel(const QkvPostParams p) {
+  pdl_launch_dependents();
+  pdl_wait();
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int n_heads = p.n_q + 2 * p.n_kv;
   const int head = blockIdx.y * (EW_THREADS / 32) + warp;
@@ -331,9 +331,7 @@ __global__ void __launch_bounds__(EW_THREADS) qkv_post_kernel(const QkvPostParam
 cudaError_t launch_qkv_post(const QkvPostParams &p, cudaStream_t s) {
   const int n_heads = p.n_q + 2 * p.n_kv;
   dim3 grid(p.T, (n_heads + EW_THREADS / 32 - 1) / (EW_THREADS / 32));
-  qkv_post_kernel<<<grid, EW_THREADS, 0, s>>>(p);
-  count_launch();
-  return cudaGetLastError();
+  return launch_pdl(qkv_post_kernel, dim3(grid), dim3(EW_THREADS), 0, s, p);
 }
 
 }  // namespace ss

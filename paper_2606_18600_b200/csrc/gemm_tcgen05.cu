@@ -8,9 +8,10 @@
 // At decode (T = 64..128) this streams every weight byte exactly once through full-width 128-row MMAs (the
 // HBM-bound case); at prefill (bn = 256) the same kernel is a 128x256 compute tile.
 //
-// CTA = 6 warps: warp 0 = TMA producer (one lane), warp 1 = TMEM allocator + MMA issuer (one lane), warps 2-5 =
-// epilogue (one TMEM lane quadrant each).  smem ring of `stages` x {A tile 128x64 (x2 when DUAL), B tile bn x 64},
-// SWIZZLE_128B, full/empty mbarriers; accumulators in TMEM, double-buffered when they fit so the epilogue of one
+// CTA = 7 warps: warp 0 = weight TMA producer (one lane), warp 6 = activation TMA producer (one lane), warp 1 = TMEM
+// allocator + MMA issuer (one lane), warps 2-5 = epilogue (one TMEM lane quadrant each).  Two smem rings, SWIZZLE_128B,
+// each with full/empty mbarriers: a deep one of weight tiles 128x64 (x2 when DUAL) and a shallow one of activation
+// tiles bn x 64 (the weight ring's depth is what bounds the HBM bytes in flight); accumulators in TMEM, double-buffered when they fit so the epilogue of one
 // work item overlaps the MMAs of the next; the producer runs ahead across work items.  Schedules: see internal.h
 // (stream-K with in-kernel fix-up for the decode shapes, band-rasterised whole tiles for the prefill shapes).
 // DUAL = gate and up tiles share the B tile and the epilogue writes silu(g)*u as bf16 (step S9), so [T,2F] never
@@ -28,6 +29,7 @@ namespace ss {
 
 constexpr int A_TILE_BYTES = GEMM_BM * GEMM_BK * 2;  // 16 KB
 constexpr int EPI_THREADS = 128;
+constexpr int GEMM_THREADS = 224;  // warp 0: TMA producer, 1: MMA issuer 0, 2-5: epilogue, 6: MMA issuer 1
 
 struct WorkItem {
   int row_tile, t_tile, kb0, kb1;
@@ -86,17 +88,36 @@ __device__ __forceinline__ int ld_acquire(const int *p) {
   asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
   return v;
 }
+// Debug aid: when a bounded wait expires, the site is recorded in host-mapped memory (if ss_debug_buffer() was
+// given one) before the trap, so that a protocol bug can be located without a debugger.
+__device__ unsigned long long *g_dbg = nullptr;
+__device__ __noinline__ void wait_expired(int site, uint32_t a, uint32_t b) {
+  if (g_dbg) {
+    g_dbg[1] = ((unsigned long long)blockIdx.x << 32) | threadIdx.x;
+    g_dbg[2] = ((unsigned long long)a << 32) | b;
+    g_dbg[0] = (unsigned long long)site;
+    __threadfence_system();
+  }
+  __trap();
+}
+__device__ __forceinline__ void mbar_wait_site(uint64_t *bar, uint32_t parity, int site, uint32_t info) {
+  uint32_t spins = 0;
+  while (!mbar_try_wait(bar, parity)) {
+    if (++spins > (1u << 24)) wait_expired(site, info, parity);
+  }
+}
 __device__ __forceinline__ void epi_bar() { asm volatile("bar.sync 1, 128;" ::: "memory"); }
 
 template <bool DUAL>
-__global__ void __launch_bounds__(192, 1)
+__global__ void __launch_bounds__(GEMM_THREADS, 1)
 gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUtensorMap ta1,
             const __grid_constant__ CUtensorMap ta2, const __grid_constant__ CUtensorMap tb, const GemmParams p) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t *base = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   const int bn = p.bn;
+  constexpr uint32_t a_bytes = A_TILE_BYTES * (DUAL ? 2 : 1);
   const uint32_t b_bytes = (uint32_t)bn * 128u;
-  const uint32_t stage_bytes = A_TILE_BYTES * (DUAL ? 2 : 1) + b_bytes;
+  const uint32_t stage_bytes = a_bytes + b_bytes;
   const int stages = p.stages;
   uint64_t *full = (uint64_t *)(base + (size_t)stages * stage_bytes);
   uint64_t *empty = full + stages;
@@ -107,11 +128,20 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int cta = blockIdx.x, grid = gridDim.x;
 
+  // One tcgen05.mma (M=128, K=16, operands in smem) occupies its issuing thread for ~128 cycles whatever N is
+  // (measured, profiles/r01_mma_issue_microbench.md), i.e. 4 KB of weights per 128 cycles: a single issuer
+  // cannot keep up with HBM at bn <= 128.  The HBM-bound schedule therefore runs TWO issuers (warps 1 and 6), each
+  // into its own accumulator; the epilogue adds the two.  Issuer (slot & 1) owns ring slot `slot` for the whole
+  // kernel: an mbarrier's single phase bit is only safe when all waits on it come, in order, from one thread (with
+  // k-blocks dealt alternately and an odd ring size a slot changed hands every round, a fast issuer could take a
+  // stale phase for its own and read a tile still in flight).
   const uint32_t acc_cols = (uint32_t)bn * (DUAL ? 2u : 1u);
-  const int nbuf = (2 * acc_cols <= 512) ? 2 : 1;
+  const int n_iss = p.issuers;
+  const int nbuf = (p.single_buf == 0 && 2 * n_iss * acc_cols <= 512) ? 2 : 1;
   uint32_t tmem_cols = 32;
-  while (tmem_cols < acc_cols * nbuf) tmem_cols <<= 1;
+  while (tmem_cols < acc_cols * n_iss * nbuf) tmem_cols <<= 1;
 
+  pdl_launch_dependents();
   if (warp == 0 && lane == 0) {
     tma_prefetch_desc(&ta0);
     if (DUAL || p.n_seg > 1) tma_prefetch_desc(&ta1);
@@ -122,7 +152,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
       mbar_init(&empty[i], 1);
     }
     for (int i = 0; i < 2; ++i) {
-      mbar_init(&tfull[i], 1);
+      mbar_init(&tfull[i], (uint32_t)n_iss);
       mbar_init(&tempty[i], 4);  // one arrival per epilogue warp
     }
     mbar_fence_init();
@@ -136,11 +166,19 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
   if (warp == 0) {
     if (lane == 0) {
       // ---------------- TMA producer ----------------
-      const uint64_t pol_w = l2_policy_evict_first();  // weights are streamed
+      // Weights are never written by the stage, so the first `stages` weight tiles are requested BEFORE waiting for
+      // the predecessor kernel (PDL): the ring is full of weights by the time the activations exist.
+      // (No integer division in the per-k-block loops of the single-thread roles: they are latency-bound, and a
+      // u32 divide by a runtime value cost ~0.1 us per k-block.)
+      const uint64_t pol_w = l2_policy_evict_first();  // weights are streamed once
       const uint64_t pol_x = l2_policy_evict_last();   // activations are re-read by every CTA
       WorkIter it(p, cta, grid);
       WorkItem w;
-      uint32_t n = 0;  // running k-block counter across items
+      int n = 0;        // running k-block counter across items (saturating use: only compared with `stages`)
+      int s = 0;        // = n % stages
+      uint32_t ph = 0;  // = (n / stages) & 1
+      bool waited = false;
+      int pend_kb[GEMM_MAX_STAGES], pend_t0[GEMM_MAX_STAGES];
       while (it.next(w)) {
         int seg = 0;
 #pragma unroll
@@ -149,62 +187,106 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
         const int row0 = (w.row_tile - p.seg_tile0[seg]) * GEMM_BM;
         const int t0 = w.t_tile * bn;
         const CUtensorMap *ta = DUAL ? &ta0 : (seg == 0 ? &ta0 : (seg == 1 ? &ta1 : &ta2));
-        for (int kb = w.kb0; kb < w.kb1; ++kb, ++n) {
-          const int s = n % stages;
-          const uint32_t ph = (n / stages) & 1u;
-          mbar_wait(&empty[s], ph ^ 1u);
+        for (int kb = w.kb0; kb < w.kb1; ++kb) {
+          if (!waited && n == stages) {  // ring primed with weights: now the activations of those k-blocks
+            pdl_wait();
+            waited = true;
+            for (int i = 0; i < stages; ++i)
+              tma_load_2d(base + (size_t)i * stage_bytes + a_bytes, &tb, &full[i], pend_kb[i] * GEMM_BK, pend_t0[i],
+                          pol_x);
+          }
+          mbar_wait_site(&empty[s], ph ^ 1u, 1, (uint32_t)s);
           uint8_t *st = base + (size_t)s * stage_bytes;
           mbar_expect_tx(&full[s], stage_bytes);
           tma_load_2d(st, ta, &full[s], kb * GEMM_BK, row0, pol_w);
           if (DUAL) tma_load_2d(st + A_TILE_BYTES, &ta1, &full[s], kb * GEMM_BK, row0, pol_w);
-          tma_load_2d(st + A_TILE_BYTES * (DUAL ? 2 : 1), &tb, &full[s], kb * GEMM_BK, t0, pol_x);
+          if (waited) {
+            tma_load_2d(st + a_bytes, &tb, &full[s], kb * GEMM_BK, t0, pol_x);
+          } else {
+            pend_kb[n] = kb;
+            pend_t0[n] = t0;
+            ++n;
+          }
+          if (++s == stages) {
+            s = 0;
+            ph ^= 1u;
+          }
         }
       }
+      if (!waited) {  // fewer k-blocks than stages
+        pdl_wait();
+        for (int i = 0; i < n; ++i)
+          tma_load_2d(base + (size_t)i * stage_bytes + a_bytes, &tb, &full[i], pend_kb[i] * GEMM_BK, pend_t0[i], pol_x);
+      }
     }
-  } else if (warp == 1) {
-    if (lane == 0) {
-      // ---------------- MMA issuer ----------------
+  } else if (warp == 1 || warp == 6) {
+    const int me = warp == 1 ? 0 : 1;
+    if (lane == 0 && me < n_iss) {
+      // ---------------- MMA issuer `me`: k-blocks with running index n = me (mod n_iss) ----------------
       const uint32_t idesc = umma_idesc_bf16(GEMM_BM, (uint32_t)bn);
       WorkIter it(p, cta, grid);
       WorkItem w;
       uint32_t n = 0, item = 0;
+      const uint32_t iss_mask = (uint32_t)n_iss - 1u;  // n_iss is 1 or 2
+      int ms = 0;        // = n % stages
+      uint32_t mph = 0;  // = (n / stages) & 1
       while (it.next(w)) {
         const uint32_t buf = item % nbuf, tph = (item / nbuf) & 1u;
-        mbar_wait(&tempty[buf], tph ^ 1u);  // epilogue has drained this accumulator
+        mbar_wait_site(&tempty[buf], tph ^ 1u, 2 + me, item);  // epilogue has drained this accumulator
         tc_fence_after();
-        const uint32_t acc_addr = tmem_base + buf * acc_cols;
+        const uint32_t acc_addr = tmem_base + (buf * n_iss + me) * acc_cols;
+        bool first = true;
         for (int kb = w.kb0; kb < w.kb1; ++kb, ++n) {
-          const int s = n % stages;
-          const uint32_t ph = (n / stages) & 1u;
-          mbar_wait(&full[s], ph);
+          const int s = ms;
+          const uint32_t ph = mph;
+          if (++ms == stages) {
+            ms = 0;
+            mph ^= 1u;
+          }
+          if (((uint32_t)s & iss_mask) != (uint32_t)me) continue;  // a slot always belongs to the same issuer
+          mbar_wait_site(&full[s], ph, 4 + me, n);
           tc_fence_after();
           const uint32_t st = smem_u32(base + (size_t)s * stage_bytes);
           const uint64_t da = umma_desc_k_sw128(st);
           const uint64_t da1 = umma_desc_k_sw128(st + A_TILE_BYTES);
-          const uint64_t db = umma_desc_k_sw128(st + A_TILE_BYTES * (DUAL ? 2 : 1));
+          const uint64_t db = umma_desc_k_sw128(st + a_bytes);
 #pragma unroll
           for (int k = 0; k < GEMM_BK / 16; ++k) {
-            const uint32_t acc = (kb > w.kb0 || k > 0) ? 1u : 0u;
+            const uint32_t acc = (!first || k > 0) ? 1u : 0u;
             umma_bf16(acc_addr, da + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc, acc);
             if (DUAL) umma_bf16(acc_addr + (uint32_t)bn, da1 + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc, acc);
           }
+          first = false;
           umma_commit(&empty[s]);  // frees the smem slot when these MMAs have read it
         }
-        umma_commit(&tfull[buf]);
+        umma_commit(&tfull[buf]);  // arrives at once if this issuer had no k-block in the item
         ++item;
       }
     }
-  } else {
+  } else if (warp >= 2 && warp < 6) {
     // ---------------- epilogue: TMEM -> registers -> (fix-up) -> global ----------------
+    pdl_wait();
     const int quad = warp & 3;
     const int r = quad * 32 + lane;  // row of the tile = TMEM lane
     const int et = threadIdx.x - 64; // 0..127
     WorkIter it(p, cta, grid);
     WorkItem w;
-    uint32_t item = 0;
+    uint32_t item = 0, n_run = 0;  // n_run: running k-block counter (the issuers' n) at the item's start
     const int nkb = it.nkb;
     while (it.next(w)) {
       const uint32_t buf = item % nbuf, tph = (item / nbuf) & 1u;
+      const uint32_t len = (uint32_t)(w.kb1 - w.kb0);
+      // which issuers accumulated anything in this item (an accumulator nobody wrote holds stale data): issuer
+      // (slot & 1) handles a k-block, slots run cyclically from n_run % stages
+      bool has0 = n_iss == 1, has1 = false;
+      if (n_iss == 2) {
+        uint32_t sl = n_run % (uint32_t)stages;
+        for (uint32_t j = 0; j < len && j < 3u; ++j) {
+          if (sl & 1u) has1 = true; else has0 = true;
+          if (++sl == (uint32_t)stages) sl = 0;
+        }
+      }
+      n_run += len;
       int seg = 0;
 #pragma unroll
       for (int i = 1; i < 3; ++i)
@@ -225,22 +307,35 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
         for (int cc = c_lo; cc <= c_hi; ++cc) {
           uint32_t spins = 0;
           while (ld_acquire(p.fix_flags + cc) == 0) {
-            if (++spins > (1u << 28)) __trap();
+            if (++spins > (1u << 24)) wait_expired(7, (uint32_t)cc, item);
           }
         }
       }
 
-      mbar_wait(&tfull[buf], tph);
+      mbar_wait_site(&tfull[buf], tph, 6, item);
       tc_fence_after();
-      const uint32_t tq = tmem_base + buf * acc_cols + ((uint32_t)(quad * 32) << 16);
+      const uint32_t tq = tmem_base + buf * n_iss * acc_cols + ((uint32_t)(quad * 32) << 16);
+      // 32 columns of the item's accumulator = sum over the issuers that contributed
+      auto ld_acc = [&](uint32_t c, uint32_t (&v)[32]) {
+        if (has0) tmem_ld_32x32(tq + c, v);
+        if (has1) {
+          uint32_t v1[32];
+          tmem_ld_32x32(tq + acc_cols + c, v1);
+          tmem_ld_wait();
+#pragma unroll
+          for (int j = 0; j < 32; ++j)
+            v[j] = has0 ? __float_as_uint(__uint_as_float(v[j]) + __uint_as_float(v1[j])) : v1[j];
+        } else {
+          tmem_ld_wait();
+        }
+      };
 
       if (!is_first) {
         // contributor: dump the raw fp32 accumulator(s) to this CTA's slot, [acc][col][row]
         float *slot = p.fix_slots + (size_t)cta * (DUAL ? 2 : 1) * bn * GEMM_BM;
         for (int c0 = 0; c0 < (int)acc_cols; c0 += 32) {
           uint32_t v[32];
-          tmem_ld_32x32(tq + (uint32_t)c0, v);
-          tmem_ld_wait();
+          ld_acc((uint32_t)c0, v);
 #pragma unroll
           for (int j = 0; j < 32; ++j) slot[(size_t)(c0 + j) * GEMM_BM + r] = __uint_as_float(v[j]);
         }
@@ -256,9 +351,8 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
       } else {
         for (int c0 = 0; c0 < bn; c0 += 32) {
           uint32_t v[32], u[32];
-          tmem_ld_32x32(tq + (uint32_t)c0, v);
-          if (DUAL) tmem_ld_32x32(tq + (uint32_t)(bn + c0), u);
-          tmem_ld_wait();
+          ld_acc((uint32_t)c0, v);
+          if (DUAL) ld_acc((uint32_t)(bn + c0), u);
           for (int cc = c_lo; cc <= c_hi; ++cc) {  // fixed order: deterministic sums
             const float *slot = p.fix_slots + (size_t)cc * (DUAL ? 2 : 1) * bn * GEMM_BM;
 #pragma unroll
@@ -362,7 +456,7 @@ int gemm_pick_bn(int T) {
 }
 
 size_t gemm_smem_bytes(int bn, bool dual, int stages) {
-  size_t stage = (size_t)A_TILE_BYTES * (dual ? 2 : 1) + (size_t)bn * 128;
+  const size_t stage = (size_t)A_TILE_BYTES * (dual ? 2 : 1) + (size_t)bn * 128;
   return 1024 + stage * stages + 8 * (2 * stages + 4) + 16;
 }
 
@@ -374,12 +468,9 @@ static int env_int(const char *name, int dflt) {
 int gemm_pick_stages(int bn, bool dual) {
   static int env = -1;
   if (env < 0) env = env_int("SS_GEMM_STAGES", 0);
-  size_t stage = (size_t)A_TILE_BYTES * (dual ? 2 : 1) + (size_t)bn * 128;
-  int st = (int)((size_t)208 * 1024 / stage);  // one persistent CTA per SM: use most of the 227 KB
-  if (env > 0) st = env;
-  if (st > 10) st = 10;
+  int st = env > 0 ? env : GEMM_MAX_STAGES;  // one persistent CTA per SM: use the 227 KB
+  if (st > GEMM_MAX_STAGES) st = GEMM_MAX_STAGES;
   while (st > 2 && gemm_smem_bytes(bn, dual, st) > 227 * 1024) --st;
-  if (st < 2) st = 2;
   return st;
 }
 
@@ -403,7 +494,6 @@ void gemm_plan(GemmLaunch &g, int n_sm) {
   p.n_row_tiles = tiles;
   p.bn = gemm_pick_bn(p.T);
   p.n_t_tiles = (p.T + p.bn - 1) / p.bn;
-  p.stages = gemm_pick_stages(p.bn, g.dual);
   const long long n_tiles = (long long)p.n_row_tiles * p.n_t_tiles;
   const long long nkb = (p.K + GEMM_BK - 1) / GEMM_BK;
   int max_grid = env_grid > 0 ? env_grid : n_sm;
@@ -412,8 +502,23 @@ void gemm_plan(GemmLaunch &g, int n_sm) {
   if (env_sched >= 0) p.sched = env_sched;
   p.band = env_band > 0 ? env_band : (g.dual ? 8 : 16);
   if (p.band > p.n_row_tiles) p.band = p.n_row_tiles;
+  p.stages = gemm_pick_stages(p.bn, g.dual);
+  {
+    static int env_iss = -1;
+    if (env_iss < 0) env_iss = env_int("SS_GEMM_ISSUERS", 0);
+    const int acc_cols = p.bn * (g.dual ? 2 : 1);
+    p.issuers = (p.sched == SCHED_STREAMK && 2 * acc_cols <= 512) ? 2 : 1;
+    if (env_iss == 1) p.issuers = 1;
+    static int env_sb = -1;
+    if (env_sb < 0) env_sb = env_int("SS_GEMM_SINGLE_BUF", 0);
+    p.single_buf = env_sb;
+  }
   const long long work = p.sched == SCHED_STREAMK ? n_tiles * nkb : n_tiles;
   g.grid = (int)(work < max_grid ? work : max_grid);
+}
+
+cudaError_t gemm_set_debug_buffer(unsigned long long *host_mapped) {
+  return cudaMemcpyToSymbol(g_dbg, &host_mapped, sizeof(host_mapped));
 }
 
 cudaError_t gemm_init() {
@@ -428,11 +533,8 @@ cudaError_t gemm_launch(const GemmLaunch &g) {
   const CUtensorMap *a1 = g.a[1] ? g.a[1] : g.a[0];
   const CUtensorMap *a2 = g.a[2] ? g.a[2] : g.a[0];
   if (g.dual)
-    gemm_kernel<true><<<g.grid, 192, smem, g.stream>>>(*g.a[0], *a1, *a2, *g.b, p);
-  else
-    gemm_kernel<false><<<g.grid, 192, smem, g.stream>>>(*g.a[0], *a1, *a2, *g.b, p);
-  count_launch();
-  return cudaGetLastError();
+    return launch_pdl_if(!g.no_pdl, gemm_kernel<true>, dim3(g.grid), dim3(GEMM_THREADS), smem, g.stream, *g.a[0], *a1, *a2, *g.b, p);
+  return launch_pdl_if(!g.no_pdl, gemm_kernel<false>, dim3(g.grid), dim3(GEMM_THREADS), smem, g.stream, *g.a[0], *a1, *a2, *g.b, p);
 }
 
 }  // namespace ss

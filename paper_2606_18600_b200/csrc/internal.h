@@ -21,6 +21,7 @@ namespace ss {
 // ---------------------------------------------------------------------------------------------------------------
 constexpr int GEMM_BM = 128;  // weight rows per tile
 constexpr int GEMM_BK = 64;   // K elements per stage (= one 128-byte swizzle row of bf16)
+constexpr int GEMM_MAX_STAGES = 12;
 
 enum GemmEpilogue {
   EPI_F32 = 0,          // out_f32[t][col] = acc
@@ -39,6 +40,8 @@ struct GemmParams {
   int T, K;             // tokens, reduction length
   int bn;               // tokens per tile (UMMA N)
   int stages;           // smem pipeline depth
+  int single_buf;       // debug: 1 = never double-buffer the TMEM accumulators
+  int issuers;          // MMA-issuing threads (2 on the HBM-bound schedule, see gemm_tcgen05.cu)
   int sched;            // GemmSchedule
   int band;             // SCHED_TILES: row tiles per raster band
   int epi;              // GemmEpilogue
@@ -53,6 +56,7 @@ struct GemmLaunch {
   const CUtensorMap *a[3];  // weight maps, box {64, 128}; dual (SwiGLU): a[0] = gate, a[1] = up, n_seg = 1
   const CUtensorMap *b;     // activation map, box {64, bn}
   bool dual;
+  bool no_pdl;              // weights may have been written by the preceding kernel (op-level entry points)
   int grid;                 // persistent CTAs
   GemmParams p;
   cudaStream_t stream;
@@ -65,6 +69,7 @@ int make_tmap_bf16_2d(CUtensorMap *out, const void *base, uint64_t rows, uint64_
 void gemm_plan(GemmLaunch &g, int n_sm);
 cudaError_t gemm_launch(const GemmLaunch &g);
 cudaError_t gemm_init();  // sets max dynamic smem attributes once
+cudaError_t gemm_set_debug_buffer(unsigned long long *host_mapped);  // see gemm_tcgen05.cu wait_expired()
 int gemm_pick_bn(int T);  // smallest of {32,64,128,256} >= min(T,256)
 int gemm_pick_stages(int bn, bool dual);
 size_t gemm_smem_bytes(int bn, bool dual, int stages);
@@ -168,5 +173,29 @@ struct PrefillAttnParams {
 cudaError_t launch_prefill_attn(const PrefillAttnParams &p, cudaStream_t s);
 
 void count_launch(int n = 1);  // stage.cu: per-thread launch counter hook
+bool pdl_enabled();            // stage.cu: false when SS_NO_PDL=1
+
+// Launch with the programmatic-stream-serialization attribute (PDL; see common.cuh) and count it.
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl_if(bool allow, void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem,
+                                 cudaStream_t s, Args &&...args) {
+  cudaLaunchConfig_t cfg;
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = (allow && pdl_enabled()) ? 1 : 0;
+  count_launch();
+  return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s,
+                              Args &&...args) {
+  return launch_pdl_if(true, kernel, grid, block, smem, s, static_cast<Args &&>(args)...);
+}
 
 }  // namespace ss

@@ -23,6 +23,14 @@ namespace ss {
 static thread_local int64_t g_launches = 0;
 static thread_local std::string g_cuda_err;
 void count_launch(int n) { g_launches += n; }
+bool pdl_enabled() {
+  static int v = -1;
+  if (v < 0) {
+    const char *e = getenv("SS_NO_PDL");
+    v = (e && atoi(e) != 0) ? 0 : 1;
+  }
+  return v == 1;
+}
 
 static int cuda_fail(cudaError_t e, const char *where) {
   g_cuda_err = std::string(where) + ": " + cudaGetErrorString(e);
@@ -616,13 +624,14 @@ static int op_gemm(const void *x_dev, const void *w0, const void *w1, float *c_f
   p.seg_rows[0] = N;
   p.T = T;
   p.K = K;
-  p.epi = dual ? EPI_SWIGLU_BF16 : EPI_F32;
+  p.epi = dual ? EPI_SWIGLU_BF16 : (env_int("SS_OP_GEMM_RESID", 0) ? EPI_RESID_F32 : EPI_F32);  // env: profiling only
   p.ld_out = N;
   p.out_f32 = c_f32;
   p.out_bf16 = c_bf16;
   p.fix_flags = (int *)scratch_dev;
   p.fix_slots = (float *)((uint8_t *)scratch_dev + GEMM_FIX_FLAG_BYTES);
   g.dual = dual;
+  g.no_pdl = true;  // the caller's weights may come straight out of a preceding kernel
   g.stream = (cudaStream_t)cuda_stream;
   gemm_plan(g, n_sm);
   if (make_tmap_bf16_2d(&ta, w0, (uint64_t)N, (uint64_t)K, GEMM_BM, true) != 0 ||
@@ -643,6 +652,11 @@ static int op_gemm(const void *x_dev, const void *w0, const void *w1, float *c_f
 extern "C" {
 
 size_t ss_op_gemm_scratch_bytes(void) { return gemm_fix_bytes(); }
+
+int ss_debug_buffer(void *host_mapped_u64x4) {
+  cudaError_t e = gemm_set_debug_buffer((unsigned long long *)host_mapped_u64x4);
+  return e == cudaSuccess ? SS_OK : cuda_fail(e, "ss_debug_buffer");
+}
 
 int ss_op_gemm_bf16(const void *x_dev, const void *w_dev, float *c_dev, int T, int N, int K, void *scratch_dev,
                     size_t scratch_bytes, void *cuda_stream) {
