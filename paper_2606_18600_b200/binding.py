@@ -22,7 +22,7 @@ ERRORS = {0: "SS_OK", -1: "SS_ERR_INVALID_ARG", -2: "SS_ERR_UNSUPPORTED", -3: "S
 EXPORTS = ["ss_stage_workspace_bytes", "ss_kv_page_bytes", "ss_stage_create", "ss_stage_destroy",
            "ss_kv_num_pages", "ss_kv_num_free", "ss_kv_alloc", "ss_kv_free", "ss_stage_prefill", "ss_stage_decode",
            "ss_stage_launch_count", "ss_op_gemm_scratch_bytes", "ss_op_gemm_bf16", "ss_op_gemm_swiglu_bf16", "ss_strerror",
-           "ss_last_cuda_error", "ss_version"]
+           "ss_last_cuda_error", "ss_version", "ss_debug_buffer"]
 
 
 class ss_model_dims(C.Structure):
@@ -85,6 +85,7 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
                                     C.c_void_p, C.c_void_p, C.c_void_p]
     lib.ss_stage_launch_count.restype = C.c_int64
     lib.ss_stage_launch_count.argtypes = [C.c_void_p]
+    lib.ss_debug_buffer.argtypes = [C.c_void_p]
     lib.ss_op_gemm_scratch_bytes.restype = C.c_size_t
     lib.ss_op_gemm_bf16.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p,
                                     C.c_size_t, C.c_void_p]
