@@ -49,6 +49,19 @@ def peaks():
     return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "source": "fallback"}
 
 
+def ncu_traffic(kernel, workload):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `kernel`, from the committed ncu --set full
+    capture (profiles/r01_traffic.json names its source); None when no capture exists for this workload."""
+    p = os.path.join(ROOT, "profiles", "r01_traffic.json")
+    try:
+        e = json.load(open(p)).get(kernel)
+    except (OSError, ValueError):
+        return None
+    if not e or e.get("workload") != workload:
+        return None
+    return e["dram_bytes_read"] + e["dram_bytes_write"]
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
@@ -477,7 +490,8 @@ def main():
         dom = res["dominant"]
         ach = dom["bytes"] / (dom["us"] * 1e-6) / 1e9
         line["roofline"] = {"bound": "hbm", "achieved": ach, "peak": pk["hbm_gbs"], "unit": "GB/s",
-                            "frac": ach / pk["hbm_gbs"], "traffic": None, "kernel": dom["kernel"],
+                            "frac": ach / pk["hbm_gbs"], "traffic": ncu_traffic(dom["kernel"], args.workload),
+                            "algorithmic_bytes": dom["bytes"], "kernel": dom["kernel"],
                             "us_per_launch": dom["us"], "peak_source": pk["source"]}
         step_gbs = res["bytes_per_step"] / (ms / K * 1e-3) / 1e9
         line["step_roofline"] = {"bound": "hbm", "algorithmic_GB_per_step": res["bytes_per_step"] / 1e9,
