@@ -1,0 +1,140 @@
+"""Parity at BASELINE.json's FULL layer shapes, in the launch configuration bench.py times (148-CTA stream-K GEMMs
+with two issuers at decode, band-rasterised 128x256 tiles at prefill, CUDA-graph replay with PDL edges), against
+the CPU oracle.  The oracle cannot run 20 layers x 34 GB in a test, so each case runs a 1-2 layer stage of the real
+width (hidden 8192 / 5120, FFN 28672 / 25600, 64/8 heads of 128) on the seed-0 workload draws; every decode row is
+compared, and for the 40,173-token recompute the rows of the two shortest requests (sequences are independent:
+oracle pin P9).  Tolerances: north_star's 2e-2 per stage / 1e-2 per layer (reading A15), KV pages per reading A13.
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import Oracle
+from paper_2606_18600_b200 import synth
+from tests import helpers as hp
+
+pytestmark = pytest.mark.gpu
+F32 = Oracle("f32")
+
+
+def _sub(shape, L):
+    return synth.ModelShape(shape.name, shape.hidden, shape.n_q, shape.n_kv, shape.d, shape.ffn, L, shape.eps,
+                            shape.theta, shape.qk_norm, shape.vocab)
+
+
+def _check_new_kv(gh, shape, pool_before, pool_oracle_r1, pool_gpu, ctx, bt, layer0_only=True):
+    """A13: (i) the GPU modified exactly the slots the oracle modified; (iii) layer-0 values equal or adjacent."""
+    changed_gpu = pool_gpu != pool_before
+    changed_orc = pool_oracle_r1 != pool_before
+    # a slot whose new value happens to equal the old bits is not 'changed' on either side: compare supports via
+    # the slot mask the block table defines
+    mask = np.zeros(pool_before.shape[2:5:2], dtype=bool)  # [pages, 16]
+    for b, c in enumerate(ctx):
+        mask[bt[b, c >> 4], c & 15] = True
+    outside = ~mask[None, None, :, None, :, None]
+    assert not (changed_gpu & outside).any(), "GPU wrote outside the new tokens' slots"
+    assert not (changed_orc & outside).any()
+    sel = np.broadcast_to(mask[None, None, :, None, :, None], pool_before.shape)
+    L = pool_before.shape[0]
+    ulp = gh.bf16_ulp_distance(pool_gpu[sel], pool_oracle_r1[sel]).reshape(L, -1)
+    a = synth.bf16_bits_to_f32(pool_gpu[sel]).reshape(L, -1)
+    b = synth.bf16_bits_to_f32(pool_oracle_r1[sel]).reshape(L, -1)
+    # near zero (cancellation in RoPE / the projections) an absolute bound replaces the ulp bound, as in
+    # tests/test_gpu_parity.py::_check_kv
+    ok0 = (ulp[0] <= 1) | (np.abs(a[0] - b[0]) <= 2e-3 * np.abs(b[0]).max())
+    eq0 = float((ulp[0] == 0).mean())
+    print(f"new KV, layer 0: equal {eq0:.4f}, outside 1 ulp / 2e-3 abs: {int((~ok0).sum())}; "
+          f"deeper layers max abs diff {float(np.abs(a - b).max()):.3e} (scale {float(np.abs(b).max()):.2f})")
+    # at K = 8192 the tensor cores' fp32 accumulation differs from the CPU loop by ~2e-4 relative, so ~6% of the
+    # bf16 roundings land on the neighbouring value (measured 0.94 equal at cfg-2; 0.97+ at the tiny width)
+    assert ok0.all() and eq0 >= 0.90
+    assert (np.abs(a - b) <= 1e-2 * np.abs(b).max()).all()
+
+
+@pytest.mark.parametrize("name", ["cfg2", "cfg3"])
+def test_full_width_decode_step_vs_oracle(name):
+    from tests import gpu_helpers as gh
+    full, ctx_fn = (synth.LLAMA70B, synth.cfg2_contexts) if name == "cfg2" else (synth.QWEN32B, synth.cfg3_contexts)
+    shape = _sub(full, 2)
+    ctx = ctx_fn(0).astype(np.int32)
+    B = len(ctx)
+    rng = np.random.default_rng(0)
+    pb = synth.paged_batch(rng, ctx, extra_tokens=2)
+    P = gh.Problem(shape, 0, n_pages=pb.n_pages_pool, max_tokens=B, max_seqs=B, max_blocks=pb.max_blocks,
+                   pool_fill="random")
+    try:
+        x = synth.bits(synth.hidden_rows(B, shape.hidden, 0))
+        pool_before = P.pool_cpu.copy()
+        pool_r0 = pool_before.copy()
+        want, _ = hp.run_oracle_decode(F32, shape, P.wb, pool_r0, ctx, pb.block_tables, x)
+        pool_r1 = pool_before.copy()
+        hp.run_oracle_decode(F32, shape, P.wb, pool_r1, ctx, pb.block_tables, x, rounding=1)
+        got = P.decode(ctx, pb.block_tables, x)
+        got2 = P.decode(ctx, pb.block_tables, x)          # graph replay on the same inputs: same bits
+        assert np.array_equal(got, got2)
+        err = hp.rel_err_rows(got, want)
+        l2 = float(np.linalg.norm(got - want) / np.linalg.norm(want))
+        print(f"{name}: 2-layer full-width decode, B={B}: max row rel err {err:.3e}, l2 rel {l2:.3e}")
+        assert err < 2e-2
+        _check_new_kv(gh, shape, pool_before, pool_r1, P.pool_bits(), ctx, pb.block_tables)
+    finally:
+        P.close()
+
+
+def test_full_width_recompute_prefill_and_migration_vs_oracle():
+    """cfg-4: one ss_stage_prefill over all 32 migrated requests (40,173 tokens, packed varlen), then one decode
+    step; the oracle follows the two shortest requests through the same two calls."""
+    from tests import gpu_helpers as gh
+    shape = _sub(synth.LLAMA70B, 1)
+    lens = synth.cfg4_lengths(0).astype(np.int32)
+    n, T = len(lens), int(lens.sum())
+    rng = np.random.default_rng(0)
+    pb = synth.paged_batch(rng, lens, extra_tokens=2)
+    P = gh.Problem(shape, 0, n_pages=pb.n_pages_pool, max_tokens=T, max_seqs=n, max_blocks=pb.max_blocks)
+    try:
+        g = torch.Generator().manual_seed(77)
+        x = synth.bits(synth.randn_bf16((T + n, shape.hidden), 1.0, g))
+        cu = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
+        got = P.prefill(lens, pb.block_tables, x[:T])
+        assert np.isfinite(got).all()
+        got_d = P.decode(lens, pb.block_tables, x[T:])
+        assert np.isfinite(got_d).all()
+        pool_gpu = P.pool_bits()
+
+        pick = np.argsort(lens)[:2]
+        rows = np.concatenate([np.arange(cu[s], cu[s + 1]) for s in pick])
+        sub_lens, sub_bt = lens[pick], pb.block_tables[pick]
+        pool = hp.new_pool(shape, pb.n_pages_pool, 1)
+        want, _, _ = hp.run_oracle_prefill(F32, shape, P.wb, pool, sub_lens, sub_bt, x[rows])
+        pool_r1 = hp.new_pool(shape, pb.n_pages_pool, 1)
+        want1, _, _ = hp.run_oracle_prefill(F32, shape, P.wb, pool_r1, sub_lens, sub_bt, x[rows], rounding=1)
+        err, err1, floor = (hp.rel_err_rows(got[rows], want), hp.rel_err_rows(got[rows], want1),
+                            hp.rel_err_rows(want1, want))
+        print(f"cfg4: recompute prefill, {len(rows)} oracle-checked rows of {T}: max row rel err vs R0 {err:.3e}, "
+              f"vs R1 {err1:.3e}; R1 vs R0 (what bf16 operands alone cost) {floor:.3e}")
+        # DESIGN.md reading A15b: at this width and with N(0, 0.02) weights (activations grow ~5x per layer, sharp
+        # softmax) rounding the GEMM operands to bf16 — which the paper's BF16 engine does and the oracle's R1 mode
+        # restates — moves a layer's output by 1.5e-2 of the row maximum by itself, so the 1e-2 per-layer bound is
+        # judged against R1 here; against R0 the 1-layer stage must meet the stage bound and not exceed that floor.
+        assert err1 < 1e-2 and err < 2e-2 and err <= 1.1 * floor
+        want_d, _ = hp.run_oracle_decode(F32, shape, P.wb, pool, sub_lens, sub_bt, x[T + pick])
+        want_d1, _ = hp.run_oracle_decode(F32, shape, P.wb, pool_r1, sub_lens, sub_bt, x[T + pick], rounding=1)
+        err_d, err_d1 = hp.rel_err_rows(got_d[pick], want_d), hp.rel_err_rows(got_d[pick], want_d1)
+        print(f"cfg4: decode step after the recompute, 2 oracle-checked rows: vs R0 {err_d:.3e}, vs R1 {err_d1:.3e}")
+        assert err_d1 < 1e-2 and err_d < 2e-2
+        # logical KV of the two requests (prompt + the decoded token): equal or adjacent bf16 values (A13 iii)
+        for i, s in enumerate(pick):
+            for kv in range(2):
+                a = hp.logical_kv(pool_gpu[0, kv], pb.block_tables[s], int(lens[s]) + 1)
+                b = hp.logical_kv(pool_r1[0, kv], sub_bt[i], int(lens[s]) + 1)
+                ulp = gh.bf16_ulp_distance(a, b)
+                fa, fb = synth.bf16_bits_to_f32(a), synth.bf16_bits_to_f32(b)
+                ok = (ulp <= 1) | (np.abs(fa - fb) <= 2e-3 * np.abs(fb).max())
+                assert ok.all() and (ulp == 0).mean() >= 0.90, (int(s), kv, int((~ok).sum()))
+        # pages of no sequence keep the sentinel (indexing, A13 i)
+        used = np.zeros(pb.n_pages_pool, dtype=bool)
+        for s in range(n):
+            used[pb.block_tables[s, : (int(lens[s]) + 1 + 15) // 16]] = True
+        assert (pool_gpu[:, :, ~used] == 0x7FC1).all()
+    finally:
+        P.close()
