@@ -49,6 +49,21 @@ def peaks():
     return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "source": "fallback"}
 
 
+def max_over_ranks(values, device):
+    """Replicas only: no data-path collective; the one exchange is this MAX all-reduce of the
+    ranks' device-timed milliseconds, so that the job's time is the slowest replica's."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(values), device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t]
+
+
+def whole_job_value(units_per_rank, world, ms_max):
+    """units all ranks processed / max-over-ranks time (weak scaling: per-GPU work is fixed)."""
+    return units_per_rank * world / (ms_max * 1e-3)
+
+
 def ncu_traffic(kernel, workload):
     """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `kernel`, from the committed ncu --set full
     capture (profiles/r01_traffic.json names its source); None when no capture exists for this workload."""
@@ -469,9 +484,7 @@ def main():
     e2e_ms = res["e2e"]["ms_per_step"] if res["e2e"] else None
     if world > 1:
         import torch.distributed as dist
-        t = torch.tensor([ms, e2e_ms or 0.0], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)          # max over ranks
-        ms, e2e_max = float(t[0]), float(t[1])
+        ms, e2e_max = max_over_ranks([ms, e2e_ms or 0.0], "cuda")
         e2e_ms = e2e_max if e2e_ms is not None else None
         dist.barrier()
         dist.destroy_process_group()
@@ -479,7 +492,7 @@ def main():
         return
     K = args.steps
     tokens_all = res["tokens"] * world
-    value = tokens_all / (ms * 1e-3)
+    value = whole_job_value(res["tokens"], world, ms)
     line = {"metric": metric, "value": value, "unit": unit, "n_gpus": world, "steps": K, "warmup": args.warmup,
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
             "data": "synthetic", "config": cfg, "clocks": res["clocks"], "gpu_launches": res["launches"]}

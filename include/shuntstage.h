@@ -122,6 +122,18 @@ int ss_kv_num_free(const ss_stage *st);
 int ss_kv_alloc(ss_stage *st, int n, int32_t *out_page_ids /* host, [n] */);   /* all-or-nothing */
 int ss_kv_free(ss_stage *st, int n, const int32_t *page_ids /* host, [n] */);  /* all-or-nothing */
 
+/* The same page allocator stand-alone: host-only, no device and no stage needed (a scheduler can size and drive a
+ * pool before any stage exists; the stage's ss_kv_* calls run this code on its own pool).  LIFO free list;
+ * ss_pool_alloc hands out n distinct free ids or nothing (SS_ERR_NO_PAGES); ss_pool_free returns n ids or nothing
+ * (SS_ERR_BAD_PAGE on an id out of range, already free, or repeated within the call).  Paged KV: PAPER.md:265, 271. */
+typedef struct ss_pool ss_pool;
+int ss_pool_create(ss_pool **out, int num_pages);
+int ss_pool_destroy(ss_pool *p);
+int ss_pool_num_pages(const ss_pool *p);
+int ss_pool_num_free(const ss_pool *p);
+int ss_pool_alloc(ss_pool *p, int n, int32_t *out_page_ids /* host, [n] */);
+int ss_pool_free(ss_pool *p, int n, const int32_t *page_ids /* host, [n] */);
+
 /*
  * Causal prefill of n_seqs packed sequences (steps S0-S11 of DESIGN.md; migration recompute).
  * Token i of sequence s sits in packed row cu_q[s]+i and at global position ctx_before[s]+i; it attends keys

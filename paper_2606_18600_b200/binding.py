@@ -22,7 +22,8 @@ ERRORS = {0: "SS_OK", -1: "SS_ERR_INVALID_ARG", -2: "SS_ERR_UNSUPPORTED", -3: "S
 EXPORTS = ["ss_stage_workspace_bytes", "ss_kv_page_bytes", "ss_stage_create", "ss_stage_destroy",
            "ss_kv_num_pages", "ss_kv_num_free", "ss_kv_alloc", "ss_kv_free", "ss_stage_prefill", "ss_stage_decode",
            "ss_stage_launch_count", "ss_op_gemm_scratch_bytes", "ss_op_gemm_bf16", "ss_op_gemm_swiglu_bf16", "ss_strerror",
-           "ss_last_cuda_error", "ss_version", "ss_debug_buffer"]
+           "ss_last_cuda_error", "ss_version", "ss_debug_buffer", "ss_pool_create", "ss_pool_destroy",
+           "ss_pool_num_pages", "ss_pool_num_free", "ss_pool_alloc", "ss_pool_free"]
 
 
 class ss_model_dims(C.Structure):
@@ -86,6 +87,12 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     lib.ss_stage_launch_count.restype = C.c_int64
     lib.ss_stage_launch_count.argtypes = [C.c_void_p]
     lib.ss_debug_buffer.argtypes = [C.c_void_p]
+    lib.ss_pool_create.argtypes = [C.POINTER(C.c_void_p), C.c_int]
+    lib.ss_pool_destroy.argtypes = [C.c_void_p]
+    lib.ss_pool_num_pages.argtypes = [C.c_void_p]
+    lib.ss_pool_num_free.argtypes = [C.c_void_p]
+    lib.ss_pool_alloc.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_int32)]
+    lib.ss_pool_free.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_int32)]
     lib.ss_op_gemm_scratch_bytes.restype = C.c_size_t
     lib.ss_op_gemm_bf16.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p,
                                     C.c_size_t, C.c_void_p]
@@ -264,3 +271,36 @@ def op_gemm_swiglu_bf16(x: torch.Tensor, wg: torch.Tensor, wu: torch.Tensor, str
     if rc != SS_OK:
         raise ShuntStageError(rc, "ss_op_gemm_swiglu_bf16")
     return a
+
+
+class PagePool:
+    """ss_pool_*: the stand-alone host page allocator (argument marshalling only)."""
+
+    def __init__(self, num_pages: int):
+        self.lib = load_library()
+        h = C.c_void_p()
+        rc = self.lib.ss_pool_create(C.byref(h), num_pages)
+        if rc != SS_OK:
+            raise ShuntStageError(rc, "ss_pool_create")
+        self.h = h
+
+    def num_pages(self) -> int:
+        return self.lib.ss_pool_num_pages(self.h)
+
+    def num_free(self) -> int:
+        return self.lib.ss_pool_num_free(self.h)
+
+    def alloc(self, n: int):
+        """returns (rc, list of ids)"""
+        buf = (C.c_int32 * max(n, 1))()
+        rc = self.lib.ss_pool_alloc(self.h, n, buf)
+        return rc, (list(buf[:n]) if rc == SS_OK else [])
+
+    def free(self, ids) -> int:
+        buf = (C.c_int32 * max(len(ids), 1))(*ids)
+        return self.lib.ss_pool_free(self.h, len(ids), buf)
+
+    def destroy(self):
+        if self.h:
+            self.lib.ss_pool_destroy(self.h)
+            self.h = None

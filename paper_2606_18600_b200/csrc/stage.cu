@@ -113,6 +113,52 @@ struct Graph {
 
 using namespace ss;
 
+// Host-side page allocator of the paged KV cache: a LIFO free list + a state byte per page.
+// All-or-nothing semantics; never touches the device.
+struct ss_pool {
+  int num_pages = 0;
+  std::vector<int32_t> free_list;
+  std::vector<uint8_t> is_free;
+  void init(int n) {
+    num_pages = n;
+    free_list.resize(n);
+    for (int i = 0; i < n; ++i) free_list[i] = n - 1 - i;  // pop gives 0,1,2,...
+    is_free.assign(n, 1);
+  }
+  int alloc(int n, int32_t *out) {
+    if (n < 0 || (n > 0 && !out)) return SS_ERR_INVALID_ARG;
+    if ((size_t)n > free_list.size()) return SS_ERR_NO_PAGES;
+    for (int i = 0; i < n; ++i) {
+      const int32_t id = free_list.back();
+      free_list.pop_back();
+      is_free[id] = 0;
+      out[i] = id;
+    }
+    return SS_OK;
+  }
+  int release(int n, const int32_t *ids) {
+    if (n < 0 || (n > 0 && !ids)) return SS_ERR_INVALID_ARG;
+    int bad = -1;  // validate first (all-or-nothing); 2 marks "seen in this call" so duplicates are caught in O(n)
+    for (int i = 0; i < n; ++i) {
+      const int32_t id = ids[i];
+      if (id < 0 || id >= num_pages || is_free[id] != 0) {
+        bad = i;
+        break;
+      }
+      is_free[id] = 2;
+    }
+    if (bad >= 0) {
+      for (int i = 0; i < bad; ++i) is_free[ids[i]] = 0;
+      return SS_ERR_BAD_PAGE;
+    }
+    for (int i = 0; i < n; ++i) {
+      is_free[ids[i]] = 1;
+      free_list.push_back(ids[i]);
+    }
+    return SS_OK;
+  }
+};
+
 struct ss_stage {
   ss_model_dims d;
   int l0, l1, L;
@@ -130,8 +176,7 @@ struct ss_stage {
   std::vector<LayerMaps> maps;
   CUtensorMap lm_map;
   CUtensorMap b_h[5], b_attn[5], b_a[5], b_hl[5];  // activation maps for bn = 16,32,64,128,256
-  std::vector<int32_t> free_list;
-  std::vector<uint8_t> is_free;
+  ss_pool pages;
   int64_t launches;
   std::map<int, Graph> graphs;  // key = batch*2 + tail
   bool use_graph;
@@ -290,9 +335,7 @@ int ss_stage_create(ss_stage **out, const ss_model_dims *dims, int l0, int l1, c
     return fail(SS_ERR_CUDA);
   }
 
-  st->free_list.resize(st->num_pages);
-  for (int i = 0; i < st->num_pages; ++i) st->free_list[i] = st->num_pages - 1 - i;  // pop gives 0,1,2,...
-  st->is_free.assign(st->num_pages, 1);
+  st->pages.init(st->num_pages);
   *out = st;
   return SS_OK;
 }
@@ -308,41 +351,32 @@ int ss_stage_destroy(ss_stage *st) {
 
 // ---- page pool --------------------------------------------------------------------------------------------------
 int ss_kv_num_pages(const ss_stage *st) { return st ? st->num_pages : SS_ERR_INVALID_ARG; }
-int ss_kv_num_free(const ss_stage *st) { return st ? (int)st->free_list.size() : SS_ERR_INVALID_ARG; }
-
+int ss_kv_num_free(const ss_stage *st) { return st ? (int)st->pages.free_list.size() : SS_ERR_INVALID_ARG; }
 int ss_kv_alloc(ss_stage *st, int n, int32_t *out_page_ids) {
-  if (!st || n < 0 || (n > 0 && !out_page_ids)) return SS_ERR_INVALID_ARG;
-  if ((size_t)n > st->free_list.size()) return SS_ERR_NO_PAGES;
-  for (int i = 0; i < n; ++i) {
-    const int32_t id = st->free_list.back();
-    st->free_list.pop_back();
-    st->is_free[id] = 0;
-    out_page_ids[i] = id;
-  }
-  return SS_OK;
+  return st ? st->pages.alloc(n, out_page_ids) : SS_ERR_INVALID_ARG;
+}
+int ss_kv_free(ss_stage *st, int n, const int32_t *page_ids) {
+  return st ? st->pages.release(n, page_ids) : SS_ERR_INVALID_ARG;
 }
 
-int ss_kv_free(ss_stage *st, int n, const int32_t *page_ids) {
-  if (!st || n < 0 || (n > 0 && !page_ids)) return SS_ERR_INVALID_ARG;
-  int bad = -1;  // validate first (all-or-nothing); 2 marks "seen in this call" so duplicates are caught in O(n)
-  for (int i = 0; i < n; ++i) {
-    const int32_t id = page_ids[i];
-    if (id < 0 || id >= st->num_pages || st->is_free[id] != 0) {
-      bad = i;
-      break;
-    }
-    st->is_free[id] = 2;
-  }
-  if (bad >= 0) {
-    for (int i = 0; i < bad; ++i) st->is_free[page_ids[i]] = 0;
-    return SS_ERR_BAD_PAGE;
-  }
-  for (int i = 0; i < n; ++i) {
-    st->is_free[page_ids[i]] = 1;
-    st->free_list.push_back(page_ids[i]);
-  }
+// the same allocator stand-alone (no device, no stage): what a scheduler sizing a pool ahead of a stage uses, and
+// what the CPU property tests drive
+int ss_pool_create(ss_pool **out, int num_pages) {
+  if (!out || num_pages < 0) return SS_ERR_INVALID_ARG;
+  ss_pool *p = new ss_pool();
+  p->init(num_pages);
+  *out = p;
   return SS_OK;
 }
+int ss_pool_destroy(ss_pool *p) {
+  if (!p) return SS_ERR_INVALID_ARG;
+  delete p;
+  return SS_OK;
+}
+int ss_pool_num_pages(const ss_pool *p) { return p ? p->num_pages : SS_ERR_INVALID_ARG; }
+int ss_pool_num_free(const ss_pool *p) { return p ? (int)p->free_list.size() : SS_ERR_INVALID_ARG; }
+int ss_pool_alloc(ss_pool *p, int n, int32_t *out_page_ids) { return p ? p->alloc(n, out_page_ids) : SS_ERR_INVALID_ARG; }
+int ss_pool_free(ss_pool *p, int n, const int32_t *page_ids) { return p ? p->release(n, page_ids) : SS_ERR_INVALID_ARG; }
 
 int64_t ss_stage_launch_count(const ss_stage *st) { return st ? st->launches : 0; }
 

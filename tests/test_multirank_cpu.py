@@ -1,0 +1,60 @@
+"""The N > 1 path of bench.py on CPU (gloo, world_size 2): replicas only, no data-path collective (DESIGN.md
+section 8; the paper's replicas are independent pipelines).  What is multi-rank is the timing
+rule (max over ranks, whole-job value) and the launch contract (rank 0 alone prints one JSON line)."""
+import json
+import os
+import subprocess
+import sys
+
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _worker(rank, world, port, out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    sys.path.insert(0, ROOT)
+    import bench
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    ms = [10.0, 12.5][rank]          # rank 1 is the slow replica
+    e2e = [11.0, 10.5][rank]
+    got = bench.max_over_ranks([ms, e2e], "cpu")
+    dist.barrier()
+    dist.destroy_process_group()
+    out.put((rank, got))
+
+
+def test_max_over_ranks_and_whole_job_value_gloo_world2():
+    sys.path.insert(0, ROOT)
+    import bench
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 29000 + os.getpid() % 2000
+    ps = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in ps:
+        p.start()
+    res = dict(q.get(timeout=120) for _ in ps)
+    for p in ps:
+        p.join(60)
+        assert p.exitcode == 0
+    assert res[0] == [12.5, 11.0] and res[1] == [12.5, 11.0]
+    # 64 tokens x 20 steps per rank, 2 ranks, slowest rank 12.5 ms in total
+    assert bench.whole_job_value(64 * 20, 2, 12.5) == 2 * 64 * 20 / 12.5e-3
+
+
+def test_reference_arm_under_torchrun_prints_one_line_from_rank0():
+    """`bench.py --impl reference` launched the way the driver launches N > 1: rank 0 alone runs the oracle and
+    prints; the other rank exits 0 without work."""
+    port = 31000 + os.getpid() % 2000
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr",
+           "127.0.0.1", "--master-port", str(port), os.path.join(ROOT, "bench.py"), "--gpus", "2", "--impl",
+           "reference", "--workload", "tiny", "--steps", "1", "--warmup", "0"]
+    r = subprocess.run(cmd, capture_output=True, text=True, timeout=600, cwd=ROOT)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["cpu_baseline"]["kind"] == "oracle" and d["value"] > 0
+    assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["unit"] == "tokens/s"
