@@ -136,10 +136,16 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
   // k-blocks dealt alternately and an odd ring size a slot changed hands every round, a fast issuer could take a
   // stale phase for its own and read a tile still in flight).
   const uint32_t acc_cols = (uint32_t)bn * (DUAL ? 2u : 1u);
+  // The tensor-bound schedule also runs two issuers, but SPLIT inside every k-block (p.split): issuer 0 takes the
+  // gate tile / tokens [0, bn/2), issuer 1 the up tile / tokens [bn/2, bn), into disjoint columns of ONE
+  // accumulator.  At N = 256 a single issuer leaves the tensor pipe idle while it commits and waits (187 vs 128
+  // cycles per MMA); two issuers keep it at the 128-cycle floor (profiles/r01_mma_issue_microbench.md).
   const int n_iss = p.issuers;
-  const int nbuf = (p.single_buf == 0 && 2 * n_iss * acc_cols <= 512) ? 2 : 1;
+  const bool split = p.split != 0;
+  const uint32_t acc_stride = split ? acc_cols : acc_cols * (uint32_t)n_iss;  // TMEM columns per buffer
+  const int nbuf = (p.single_buf == 0 && 2 * acc_stride <= 512) ? 2 : 1;
   uint32_t tmem_cols = 32;
-  while (tmem_cols < acc_cols * n_iss * nbuf) tmem_cols <<= 1;
+  while (tmem_cols < acc_stride * nbuf) tmem_cols <<= 1;
 
   pdl_launch_dependents();
   if (warp == 0 && lane == 0) {
@@ -149,7 +155,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
     tma_prefetch_desc(&tb);
     for (int i = 0; i < stages; ++i) {
       mbar_init(&full[i], 1);
-      mbar_init(&empty[i], 1);
+      mbar_init(&empty[i], split ? 2u : 1u);  // split: both issuers read every slot
     }
     for (int i = 0; i < 2; ++i) {
       mbar_init(&tfull[i], (uint32_t)n_iss);
@@ -170,8 +176,11 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
       // the predecessor kernel (PDL): the ring is full of weights by the time the activations exist.
       // (No integer division in the per-k-block loops of the single-thread roles: they are latency-bound, and a
       // u32 divide by a runtime value cost ~0.1 us per k-block.)
-      const uint64_t pol_w = l2_policy_evict_first();  // weights are streamed once
-      const uint64_t pol_x = l2_policy_evict_last();   // activations are re-read by every CTA
+      // stream-K (decode): weights are streamed once, activations are re-read by every CTA.  Tiles (prefill): a
+      // weight tile is re-read by every token tile of its band, so it must stay in L2 as well.
+      const uint64_t pol_w = p.w_policy == 0 ? l2_policy_evict_first()
+                                             : (p.w_policy == 1 ? l2_policy_evict_normal() : l2_policy_evict_last());
+      const uint64_t pol_x = l2_policy_evict_last();
       WorkIter it(p, cta, grid);
       WorkItem w;
       int n = 0;        // running k-block counter across items (saturating use: only compared with `stages`)
@@ -222,19 +231,26 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
   } else if (warp == 1 || warp == 6) {
     const int me = warp == 1 ? 0 : 1;
     if (lane == 0 && me < n_iss) {
-      // ---------------- MMA issuer `me`: k-blocks with running index n = me (mod n_iss) ----------------
-      const uint32_t idesc = umma_idesc_bf16(GEMM_BM, (uint32_t)bn);
+      // ---------------- MMA issuer `me` ----------------
+      // alternate mode: the k-blocks in ring slots s = me (mod n_iss), own accumulator; split mode: every k-block,
+      // own half (gate | up, or tokens [0,bn/2) | [bn/2,bn)) of the shared accumulator
+      const uint32_t idesc = umma_idesc_bf16(GEMM_BM, (uint32_t)((split && !DUAL) ? bn / 2 : bn));
+      const uint32_t a_off = (split && DUAL && me == 1) ? (uint32_t)A_TILE_BYTES : 0u;
+      const uint32_t b_off = (split && !DUAL && me == 1) ? (uint32_t)(bn / 2) * 128u : 0u;
+      const uint32_t acc_off = split ? (uint32_t)me * (DUAL ? (uint32_t)bn : (uint32_t)(bn / 2)) : (uint32_t)me * acc_cols;
+      const bool both = DUAL && !split;  // this issuer issues the gate AND the up MMA
       WorkIter it(p, cta, grid);
       WorkItem w;
       uint32_t n = 0, item = 0;
-      const uint32_t iss_mask = (uint32_t)n_iss - 1u;  // n_iss is 1 or 2
+      const uint32_t iss_mask = split ? 0u : (uint32_t)n_iss - 1u;  // n_iss is 1 or 2
+      const uint32_t my_slots = split ? 0u : (uint32_t)me;
       int ms = 0;        // = n % stages
       uint32_t mph = 0;  // = (n / stages) & 1
       while (it.next(w)) {
         const uint32_t buf = item % nbuf, tph = (item / nbuf) & 1u;
         mbar_wait_site(&tempty[buf], tph ^ 1u, 2 + me, item);  // epilogue has drained this accumulator
         tc_fence_after();
-        const uint32_t acc_addr = tmem_base + (buf * n_iss + me) * acc_cols;
+        const uint32_t acc_addr = tmem_base + buf * acc_stride + acc_off;
         bool first = true;
         for (int kb = w.kb0; kb < w.kb1; ++kb, ++n) {
           const int s = ms;
@@ -243,18 +259,20 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
             ms = 0;
             mph ^= 1u;
           }
-          if (((uint32_t)s & iss_mask) != (uint32_t)me) continue;  // a slot always belongs to the same issuer
+          if (((uint32_t)s & iss_mask) != my_slots) continue;  // a slot always belongs to the same issuer
           mbar_wait_site(&full[s], ph, 4 + me, n);
           tc_fence_after();
           const uint32_t st = smem_u32(base + (size_t)s * stage_bytes);
-          const uint64_t da = umma_desc_k_sw128(st);
+          const uint64_t da = umma_desc_k_sw128(st + a_off);
           const uint64_t da1 = umma_desc_k_sw128(st + A_TILE_BYTES);
-          const uint64_t db = umma_desc_k_sw128(st + a_bytes);
+          const uint64_t db = umma_desc_k_sw128(st + a_bytes + b_off);
 #pragma unroll
           for (int k = 0; k < GEMM_BK / 16; ++k) {
             const uint32_t acc = (!first || k > 0) ? 1u : 0u;
             umma_bf16(acc_addr, da + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc, acc);
-            if (DUAL) umma_bf16(acc_addr + (uint32_t)bn, da1 + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc, acc);
+            if (DUAL) {
+              if (both) umma_bf16(acc_addr + (uint32_t)bn, da1 + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc, acc);
+            }
           }
           first = false;
           umma_commit(&empty[s]);  // frees the smem slot when these MMAs have read it
@@ -278,8 +296,8 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
       const uint32_t len = (uint32_t)(w.kb1 - w.kb0);
       // which issuers accumulated anything in this item (an accumulator nobody wrote holds stale data): issuer
       // (slot & 1) handles a k-block, slots run cyclically from n_run % stages
-      bool has0 = n_iss == 1, has1 = false;
-      if (n_iss == 2) {
+      bool has0 = n_iss == 1 || split, has1 = false;
+      if (n_iss == 2 && !split) {
         uint32_t sl = n_run % (uint32_t)stages;
         for (uint32_t j = 0; j < len && j < 3u; ++j) {
           if (sl & 1u) has1 = true; else has0 = true;
@@ -314,7 +332,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
 
       mbar_wait_site(&tfull[buf], tph, 6, item);
       tc_fence_after();
-      const uint32_t tq = tmem_base + buf * n_iss * acc_cols + ((uint32_t)(quad * 32) << 16);
+      const uint32_t tq = tmem_base + buf * acc_stride + ((uint32_t)(quad * 32) << 16);
       // 32 columns of the item's accumulator = sum over the issuers that contributed
       auto ld_acc = [&](uint32_t c, uint32_t (&v)[32]) {
         if (has0) tmem_ld_32x32(tq + c, v);
@@ -507,8 +525,23 @@ void gemm_plan(GemmLaunch &g, int n_sm) {
     static int env_iss = -1;
     if (env_iss < 0) env_iss = env_int("SS_GEMM_ISSUERS", 0);
     const int acc_cols = p.bn * (g.dual ? 2 : 1);
-    p.issuers = (p.sched == SCHED_STREAMK && 2 * acc_cols <= 512) ? 2 : 1;
-    if (env_iss == 1) p.issuers = 1;
+    static int env_wpol = -2;
+    if (env_wpol == -2) env_wpol = env_int("SS_GEMM_WPOL", -1);
+    p.w_policy = p.sched == SCHED_STREAMK ? 0 : 2;
+    if (env_wpol >= 0) p.w_policy = env_wpol;
+    p.split = 0;
+    if (p.sched == SCHED_STREAMK) {
+      p.issuers = (2 * acc_cols <= 512) ? 2 : 1;
+    } else {
+      // measured: splitting each k-block between two issuers does not help here (the tensor pipe waits on L2, not
+      // on the issuer: 59% vs 66% active) — one issuer; SS_GEMM_ISSUERS=2 keeps the split path testable
+      p.issuers = env_iss == 2 ? 2 : 1;
+      p.split = env_iss == 2 ? 1 : 0;
+    }
+    if (env_iss == 1) {
+      p.issuers = 1;
+      p.split = 0;
+    }
     static int env_sb = -1;
     if (env_sb < 0) env_sb = env_int("SS_GEMM_SINGLE_BUF", 0);
     p.single_buf = env_sb;

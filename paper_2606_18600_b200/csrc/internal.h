@@ -40,6 +40,8 @@ struct GemmParams {
   int T, K;             // tokens, reduction length
   int bn;               // tokens per tile (UMMA N)
   int stages;           // smem pipeline depth
+  int w_policy;         // L2 policy of the weight loads: 0 evict_first, 1 evict_normal, 2 evict_last
+  int split;            // 1: the two issuers split every k-block (tensor-bound schedule); 0: they alternate k-blocks
   int single_buf;       // debug: 1 = never double-buffer the TMEM accumulators
   int issuers;          // MMA-issuing threads (2 on the HBM-bound schedule, see gemm_tcgen05.cu)
   int sched;            // GemmSchedule

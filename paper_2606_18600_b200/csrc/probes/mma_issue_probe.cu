@@ -9,7 +9,7 @@
 #include "../common.cuh"
 using namespace ss;
 
-struct P { int N; int groups; int mma_per_group; int commit_every; int issuers; int M; };
+struct P { int N; int groups; int mma_per_group; int commit_every; int issuers; int M; int same_acc; };
 
 __global__ void __launch_bounds__(128, 1) k(P p, long long *out) {
   extern __shared__ uint8_t smem_raw[];
@@ -26,7 +26,7 @@ __global__ void __launch_bounds__(128, 1) k(P p, long long *out) {
   const uint32_t tm = slot;
   if (lane == 0 && warp < p.issuers) {
     const uint32_t idesc = umma_idesc_bf16(p.M, p.N);
-    const uint32_t acc = tm + warp * 256;
+    const uint32_t acc = tm + (p.same_acc ? 0 : warp * 256);
     long long t0 = clock64();
     for (int g = 0; g < p.groups; ++g) {
       const uint32_t sa = smem_u32(base + (g & 3) * 16384);
@@ -52,15 +52,23 @@ int main() {
   int Ns[] = {16, 32, 64, 128, 256};
   printf("M N mma/grp commit_every issuers grid | issue clk/mma | total clk/mma\n");
   for (int M : {128, 64}) for (int grid : {1, 148}) for (int issuers : {1, 2}) for (int ce : {0, 1, 2}) for (int N : Ns) {
-    if (issuers == 2 && N > 128) continue;
     if (M == 64 && (grid == 1 || issuers == 2)) continue;
-    P p{N, 2000, 4, ce, issuers, M};
+    P p{N, 2000, 4, ce, issuers, M, 0};
     k<<<grid, 128, 200 * 1024>>>(p, d);
     cudaError_t e = cudaDeviceSynchronize();
     if (e != cudaSuccess) { printf("err %s\n", cudaGetErrorString(e)); return 1; }
     cudaMemcpy(h, d, 32, cudaMemcpyDeviceToHost);
     double n = 2000.0 * 4;
     printf("%3d %3d %d %d %d %3d | %7.1f | %7.1f\n", M, N, 4, ce, issuers, grid, h[0] / n, h[1] / n);
+  }
+  printf("two issuers, N=256, separate vs same accumulator, 8 MMAs per group (per issuer clk/MMA; pipe floor 128 per MMA => 256 when two issuers share the pipe)\n");
+  for (int same : {0, 1}) for (int ce : {0, 1}) for (int mpg : {4, 8}) {
+    P p{256, 2000, mpg, ce, 2, 128, same};
+    k<<<148, 128, 200 * 1024>>>(p, d);
+    if (cudaDeviceSynchronize() != cudaSuccess) { printf("err\n"); return 1; }
+    cudaMemcpy(h, d, 32, cudaMemcpyDeviceToHost);
+    double n = 2000.0 * mpg;
+    printf("same_acc=%d commit_every=%d mma/grp=%d | issuer0 %7.1f issuer1 %7.1f (total/MMA)\n", same, ce, mpg, h[1] / n, h[3] / n);
   }
   return 0;
 }
