@@ -26,7 +26,7 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     if not force and not _stale():
         return LIB
     nvcc = os.environ.get("NVCC", "nvcc")
-    flags = [f for f in FLAGS if not f.startswith("--use_fast_math")]
+    flags = [f for f in FLAGS if not f.startswith("--use_fast_math")] + os.environ.get("SS_NVCC_EXTRA", "").split()
     objs = []
     procs = []
     (HERE / "build").mkdir(exist_ok=True)

@@ -106,6 +106,18 @@ __device__ __forceinline__ void mbar_wait_site(uint64_t *bar, uint32_t parity, i
     if (++spins > (1u << 24)) wait_expired(site, info, parity);
   }
 }
+// Optional timeline (profiling builds only: -DSS_GEMM_TRACE): globaltimer stamps per CTA into p.trace[cta*64 + slot].
+#ifdef SS_GEMM_TRACE
+__device__ __forceinline__ void trace(const GemmParams &p, int slot) {
+  if (p.trace && slot < 64) {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+    p.trace[(size_t)blockIdx.x * 64 + slot] = t;
+  }
+}
+#else
+__device__ __forceinline__ void trace(const GemmParams &, int) {}
+#endif
 __device__ __forceinline__ void epi_bar() { asm volatile("bar.sync 1, 128;" ::: "memory"); }
 
 template <bool DUAL>
@@ -148,6 +160,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
   while (tmem_cols < acc_stride * nbuf) tmem_cols <<= 1;
 
   pdl_launch_dependents();
+  if (threadIdx.x == 0) trace(p, 0);
   if (warp == 0 && lane == 0) {
     tma_prefetch_desc(&ta0);
     if (DUAL || p.n_seg > 1) tma_prefetch_desc(&ta1);
@@ -261,6 +274,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
           }
           if (((uint32_t)s & iss_mask) != my_slots) continue;  // a slot always belongs to the same issuer
           mbar_wait_site(&full[s], ph, 4 + me, n);
+          if (n == 0) trace(p, 2);
           tc_fence_after();
           const uint32_t st = smem_u32(base + (size_t)s * stage_bytes);
           const uint64_t da = umma_desc_k_sw128(st + a_off);
@@ -278,6 +292,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
           umma_commit(&empty[s]);  // frees the smem slot when these MMAs have read it
         }
         umma_commit(&tfull[buf]);  // arrives at once if this issuer had no k-block in the item
+        if (me == 0) trace(p, 3 + 4 * (int)item);
         ++item;
       }
     }
@@ -330,7 +345,9 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
         }
       }
 
+      if (et == 0) trace(p, 4 + 4 * (int)item);
       mbar_wait_site(&tfull[buf], tph, 6, item);
+      if (et == 0) trace(p, 5 + 4 * (int)item);
       tc_fence_after();
       const uint32_t tq = tmem_base + buf * acc_stride + ((uint32_t)(quad * 32) << 16);
       // 32 columns of the item's accumulator = sum over the issuers that contributed
@@ -371,7 +388,8 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
           uint32_t v[32], u[32];
           ld_acc((uint32_t)c0, v);
           if (DUAL) ld_acc((uint32_t)(bn + c0), u);
-          for (int cc = c_lo; cc <= c_hi; ++cc) {  // fixed order: deterministic sums
+          if (et == 0 && item == 1) trace(p, 40 + 3 * (c0 >> 5));
+          for (int cc = c_lo; cc <= c_hi; ++cc) {  // fix-up in CTA order: deterministic sums
             const float *slot = p.fix_slots + (size_t)cc * (DUAL ? 2 : 1) * bn * GEMM_BM;
 #pragma unroll
             for (int j = 0; j < 32; ++j) {
@@ -380,18 +398,30 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
                 u[j] = __float_as_uint(__uint_as_float(u[j]) + __ldcg(slot + (size_t)(bn + c0 + j) * GEMM_BM + r));
             }
           }
-          if (row_ok) {
-            if (DUAL) {  // EPI_SWIGLU_BF16: a = g / (1 + exp(-g)) * u
-              __nv_bfloat16 *o = (__nv_bfloat16 *)p.out_bf16 + col;
+          if (et == 0 && item == 1) trace(p, 41 + 3 * (c0 >> 5));
+          if (DUAL) {
+            // EPI_SWIGLU_BF16: a = g / (1 + exp(-g)) * u.  This epilogue is on the kernel's critical path (the last
+            // work item's is never overlapped): fast-math SiLU (ex2.approx + div.approx, error far below the bf16
+            // output's 2^-9) and, instead of 32 two-byte stores per thread, lane pairs swap alternate tokens so
+            // every lane stores one bf16x2 = features (col, col+1) of one token (timeline:
+            // profiles/r01_gemm_timeline.md: 3.6 -> 1.7 us per 32-token chunk).
+            __nv_bfloat16 *o = (__nv_bfloat16 *)p.out_bf16;
+            const bool odd = (lane & 1) != 0;
 #pragma unroll
-              for (int j = 0; j < 32; ++j) {
-                const int t = t0 + c0 + j;
-                if (t < p.T) {
-                  const float gv = __uint_as_float(v[j]), uv = __uint_as_float(u[j]);
-                  o[(size_t)t * p.ld_out] = __float2bfloat16_rn(gv / (1.0f + __expf(-gv)) * uv);
-                }
-              }
-            } else if (p.epi == EPI_RESID_F32) {
+            for (int j = 0; j < 32; j += 2) {
+              const float g0 = __uint_as_float(v[j]), g1 = __uint_as_float(v[j + 1]);
+              const float a0 = __fdividef(g0, 1.0f + __expf(-g0)) * __uint_as_float(u[j]);
+              const float a1 = __fdividef(g1, 1.0f + __expf(-g1)) * __uint_as_float(u[j + 1]);
+              const float got = __shfl_xor_sync(0xffffffffu, odd ? a0 : a1, 1);
+              // even lane: token j, features (col, col+1) = (own a0, neighbour's a0)
+              // odd lane : token j+1, features (col-1, col) = (neighbour's a1, own a1)
+              const int t = t0 + c0 + j + (odd ? 1 : 0);
+              const uint32_t pk = odd ? pack_bf16x2(got, a1) : pack_bf16x2(a0, got);
+              if (row_ok && t < p.T)
+                *reinterpret_cast<uint32_t *>(o + (size_t)t * p.ld_out + (col & ~1)) = pk;
+            }
+          } else if (row_ok) {
+            if (p.epi == EPI_RESID_F32) {
               // all 32 loads of the residual are issued before the first store (a `+=` loop would serialise
               // 32 dependent L2 round trips per chunk: the compiler cannot prove the stores do not alias the loads)
               float *o = p.out_f32 + col;
@@ -416,6 +446,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
             }
           }
         }
+        if (et == 0 && item == 1) trace(p, 60);
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(&tempty[buf]);
@@ -425,11 +456,13 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
             for (int cc = c_lo; cc <= c_hi; ++cc) p.fix_flags[cc] = 0;
         }
       }
+      if (et == 0) trace(p, 6 + 4 * (int)item);
       ++item;
     }
   }
   tc_fence_before();
   __syncthreads();
+  if (threadIdx.x == 0) trace(p, 1);
   if (warp == 1) {
     tc_fence_after();
     tmem_dealloc_dyn(tmem_base, tmem_cols);

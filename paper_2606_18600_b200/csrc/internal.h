@@ -51,6 +51,7 @@ struct GemmParams {
   float *out_f32;
   void *out_bf16;
   float *fix_slots;     // SCHED_STREAMK: gridDim.x partial-accumulator slots of (dual ? 2 : 1) * bn * 128 floats
+  unsigned long long *trace;  // profiling builds (-DSS_GEMM_TRACE): [grid][64] globaltimer stamps, else null
   int *fix_flags;       // SCHED_STREAMK: gridDim.x flags, zero between launches (consumers reset them)
 };
 

@@ -663,6 +663,9 @@ static int op_gemm(const void *x_dev, const void *w0, const void *w1, float *c_f
   p.out_f32 = c_f32;
   p.out_bf16 = c_bf16;
   p.fix_flags = (int *)scratch_dev;
+#ifdef SS_GEMM_TRACE
+  p.trace = (unsigned long long *)((uint8_t *)scratch_dev + gemm_fix_bytes());  // profiling build: caller over-allocates
+#endif
   p.fix_slots = (float *)((uint8_t *)scratch_dev + GEMM_FIX_FLAG_BYTES);
   g.dual = dual;
   g.no_pdl = true;  // the caller's weights may come straight out of a preceding kernel
