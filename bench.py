@@ -32,7 +32,7 @@ def parse():
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "tiny"])
+    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "cfg5", "tiny"])
     ap.add_argument("--seed", type=int, default=0)
     ap.add_argument("--layers", type=int, default=0, help="override the stage depth (debug only; marks the line)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -139,6 +139,8 @@ def workload_spec(name, layers_override=0):
         shape, ctx, kind = synth.QWEN32B, synth.cfg3_contexts, "decode"
     elif name == "cfg4":
         shape, ctx, kind = synth.LLAMA70B, synth.cfg4_lengths, "prefill"
+    elif name == "cfg5":
+        shape, ctx, kind = synth.QWEN32B, None, "online"
     else:
         shape, ctx, kind = synth.TINY, synth.cfg1_contexts, "decode"
     L = layers_override or shape.n_layers
@@ -386,6 +388,50 @@ def run_prefill(args, shape, len_fn, rank, world):
     return res
 
 
+def run_online(args, shape, rank, world):
+    """cfg5: online mixed batches (96 decode rows + <= 4 prefill chunks of <= 512 tokens per ss_stage_prefill call)
+    driven by paper_2606_18600_b200/online.py over a page pool at ~85% occupancy; K timed iterations."""
+    import torch
+    from paper_2606_18600_b200 import binding, online
+    dev = torch.device(f"cuda:{int(os.environ.get('LOCAL_RANK', 0))}")
+    torch.cuda.set_device(dev)
+    K, W = args.steps, args.warmup
+    n_pages = online.OnlineDriver.pool_pages(args.seed)
+    S = online.N_DECODE + online.N_PREFILL
+    Tmax = online.N_DECODE + online.N_PREFILL * online.CHUNK
+    max_blocks = (8192 + 2048 + online.CHUNK) // 16 + 2
+    layers = gpu_weights(shape, dev, args.seed)
+    dims = binding.make_dims(shape, max_tokens=Tmax, max_seqs=S, max_blocks=max_blocks,
+                             max_pos=8192 + 2048 + online.CHUNK + 64)
+    st = binding.Stage(dims, 0, shape.n_layers, layers, None, n_pages=n_pages, device=dev)
+    g = torch.Generator(device=dev)
+    g.manual_seed(args.seed + 99)
+    _fill_randn(st.kv_pool.view(-1), g)
+    bank = torch.randn((Tmax, shape.hidden), generator=g, device=dev, dtype=torch.float32).to(torch.bfloat16)
+    out = torch.empty((Tmax, shape.hidden), dtype=torch.bfloat16, device=dev)
+    drv = online.OnlineDriver(st, shape, seed=args.seed, max_blocks=max_blocks, device=dev)
+    for _ in range(W):
+        drv.step(bank, out)
+    torch.cuda.synchronize(dev)
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+    sampler = ClockSampler(dev.index or 0)
+    sampler.start()
+    d0, p0, n0 = drv.stats["decode_tokens"], drv.stats["prefill_tokens"], st.launch_count()
+    t0 = time.perf_counter()
+    for _ in range(K):                       # each step ends with a stream sync (the scheduler reads the results)
+        drv.step(bank, out)
+    ms = (time.perf_counter() - t0) * 1e3
+    clocks = sampler.stop()
+    occ = drv.stats["occupancy"][W:]
+    res = {"ms": ms, "decode_tokens": drv.stats["decode_tokens"] - d0, "prefill_tokens": drv.stats["prefill_tokens"] - p0,
+           "launches": st.launch_count() - n0, "clocks": clocks, "occupancy": [min(occ), float(np.mean(occ)), max(occ)],
+           "dropped": drv.stats["dropped"], "finished": drv.stats["finished"], "pages": n_pages}
+    st.destroy()
+    return res
+
+
 # ---------------------------------------------------------------------------------------------------------------
 # CPU oracle timing (cpu_baseline leg and --impl reference): the oracle as it stands, on a bounded sample
 # ---------------------------------------------------------------------------------------------------------------
@@ -444,6 +490,7 @@ def main():
     cfg = {"workload": {"cfg2": "configs[1]: Llama-3.1-70B-shaped 20-layer decode stage, B=64, ctx lognormal(med 1024)",
                         "cfg3": "configs[2]: Qwen3-32B-shaped 16-layer decode stage, B=128, ctx lognormal(med 768)",
                         "cfg4": "configs[3]: migration recompute prefill, 70B shapes, 32 requests lognormal(med 1200)",
+                        "cfg5": "configs[4]: online mixed batches, Qwen3-32B shapes",
                         "tiny": "configs[0]: tiny Llama-style stage"}[args.workload],
            "layers": shape.n_layers, "hidden": shape.hidden, "ffn": shape.ffn, "heads": f"{shape.n_q}/{shape.n_kv}",
            "page_size": 16, "seed": args.seed, "parallelism": f"replicas x{world}",
@@ -455,6 +502,8 @@ def main():
     if args.impl == "reference":
         if rank != 0:
             return
+        if kind == "online":
+            raise SystemExit("--impl reference covers cfg2/cfg3/cfg4/tiny (the oracle has no online driver)")
         ts = []
         T = cores = desc = None
         for i in range(max(1, min(args.steps, 3)) + min(args.warmup, 1)):
@@ -478,6 +527,30 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{int(os.environ.get('LOCAL_RANK', 0))}"))
 
+    if kind == "online":
+        res = run_online(args, shape, rank, world)
+        ms = res["ms"]
+        if world > 1:
+            import torch.distributed as dist
+            ms = max_over_ranks([ms], "cuda")[0]
+            dist.barrier()
+            dist.destroy_process_group()
+        if rank != 0:
+            return
+        toks = res["decode_tokens"] + res["prefill_tokens"]
+        cfg["workload"] = "configs[4]: online mixed batches, Qwen3-32B shapes, 96 decode + 4 prefill chunks of 512"
+        line = {"metric": "online mixed-batch tokens/s (decode + prefill tokens per second of wall time, host "
+                          "scheduling and per-iteration H2D of block tables inside)",
+                "value": whole_job_value(toks, world, ms), "unit": "tokens/s", "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "bf16", "data": "synthetic", "config": cfg, "clocks": res["clocks"],
+                "gpu_launches": int(res["launches"]),
+                "decode_tokens_per_s": res["decode_tokens"] * world / (ms * 1e-3),
+                "prefill_tokens_per_s": res["prefill_tokens"] * world / (ms * 1e-3),
+                "pool": {"pages": res["pages"], "occupancy_min_mean_max": res["occupancy"], "dropped": res["dropped"],
+                         "finished": res["finished"]}}
+        print(json.dumps(line))
+        return
     res = run_decode(args, shape, len_fn, rank, world) if kind == "decode" else \
         run_prefill(args, shape, len_fn, rank, world)
     ms = res["ms"]

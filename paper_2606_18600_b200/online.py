@@ -1,0 +1,173 @@
+"""Online mixed-batch driver for BASELINE.json configs[4] ("cfg-5"): every iteration is ONE ss_stage_prefill call
+that combines 96 decode requests (q_len = 1 rows, first in the batch: reading A19) with up to 4 prefill chunks of
+<= 512 tokens from new requests, over a page pool kept near 85% occupancy (reading A18), as in the paper's online
+serving experiments (continuous batching of the Azure-trace-shaped load).
+
+Host scheduling only — slots, lengths, the ready FIFO, page bookkeeping through the stage's allocator
+(ss_kv_alloc / ss_kv_free) — no arithmetic of the method lives here; every step of the forward pass runs in the
+CUDA kernels behind the C-ABI.  Recipe (DESIGN.md section 3 / SURVEY 8(d) cfg-5), all draws from one
+numpy.random.default_rng(seed): decode slots start with ctx ~ LN(1024) in [16, 8192] and remaining output
+~ LN(250) in [1, 2048]; prefill slots hold a new request with prompt ~ LN(600) in [16, 2048] (2048 = the paper's
+prune), consumed <= 512 tokens per iteration; a finished prompt enters a ready FIFO (pages kept) and
+its slot takes a new request; a decode slot whose remaining output hits 0 frees its pages and takes the FIFO head
+(or, if the FIFO is empty, a fresh already-prefilled context); FIFO entries are dropped (pages freed) while the
+occupancy exceeds 0.85.
+"""
+from __future__ import annotations
+
+from collections import deque
+from dataclasses import dataclass, field
+
+import numpy as np
+import torch
+
+from . import synth
+
+PAGE = synth.PAGE
+N_DECODE, N_PREFILL, CHUNK = 96, 4, 512
+OCCUPANCY = 0.85
+
+
+@dataclass
+class Req:
+    pages: list = field(default_factory=list)
+    ctx: int = 0          # tokens cached
+    prompt: int = 0       # prefill slots: prompt length
+    remaining: int = 0    # decode slots: output tokens still to produce
+
+
+@dataclass
+class Iteration:
+    """What one call was given (host copies, for tests) and where its rows sit."""
+    cu_q: np.ndarray
+    ctx_before: np.ndarray
+    block_tables: np.ndarray
+    n_seqs: int
+    T: int
+
+
+class OnlineDriver:
+    def __init__(self, stage, shape: synth.ModelShape, seed: int = 0, max_blocks: int = 0, device="cuda:0"):
+        self.stage, self.shape, self.dev = stage, shape, torch.device(device)
+        self.rng = np.random.default_rng(seed)
+        self.max_blocks = max_blocks or (8192 + 2048 + CHUNK) // PAGE + 2
+        self.n_pages = stage.num_pages()
+        self.decode = [self._fresh_decode() for _ in range(N_DECODE)]
+        self.prefill = [self._fresh_prefill() for _ in range(N_PREFILL)]
+        self.fifo: deque = deque()
+        self.stats = {"decode_tokens": 0, "prefill_tokens": 0, "dropped": 0, "finished": 0, "occupancy": []}
+        S = N_DECODE + N_PREFILL
+        # pinned host staging + device copies of the per-call integer inputs
+        self.h_bt = torch.zeros((S, self.max_blocks), dtype=torch.int32).pin_memory()
+        self.h_cu = torch.zeros(S + 1, dtype=torch.int32).pin_memory()
+        self.h_ctx = torch.zeros(S, dtype=torch.int32).pin_memory()
+        self.d_bt = torch.zeros_like(self.h_bt, device=self.dev)
+        self.d_cu = torch.zeros_like(self.h_cu, device=self.dev)
+        self.d_ctx = torch.zeros_like(self.h_ctx, device=self.dev)
+
+    # ---- sizing (reading A18): pool = live pages at iteration 0 / 0.85 ----
+    @staticmethod
+    def _draw_decode(rng):
+        ctx = int(synth.lognormal_lengths(rng, 1, 1024, 16, 8192)[0])
+        rem = int(synth.lognormal_lengths(rng, 1, 250, 1, 2048)[0])
+        return ctx, rem
+
+    @staticmethod
+    def pool_pages(seed: int) -> int:
+        """Pages of the 96 initial decode contexts (same draws, same order as __init__) plus the prefill slots'
+        first chunks, divided by 0.85."""
+        rng = np.random.default_rng(seed)
+        live = sum((OnlineDriver._draw_decode(rng)[0] + 1 + PAGE - 1) // PAGE for _ in range(N_DECODE))
+        live += N_PREFILL * (CHUNK // PAGE)
+        return int(np.ceil(live / OCCUPANCY))
+
+    def _alloc(self, req: Req, n_tokens: int) -> bool:
+        need = (n_tokens + PAGE - 1) // PAGE - len(req.pages)
+        if need > 0:
+            if need > self.stage.num_free():
+                return False
+            req.pages += self.stage.kv_alloc(need)
+        return True
+
+    def _free(self, req: Req):
+        if req.pages:
+            self.stage.kv_free(req.pages)
+            req.pages = []
+
+    def _fresh_decode(self) -> Req:
+        """A decode request whose context is taken as already cached (its pages hold whatever the pool held: the
+        synthetic 'random KV pre-fill' of reading A21)."""
+        ctx, rem = self._draw_decode(self.rng)
+        r = Req(ctx=ctx, remaining=rem)
+        while not self._alloc(r, ctx + 1):      # pool too full for this draw: halve it (keeps the run going)
+            ctx = max(16, ctx // 2)
+            r.ctx = ctx
+        return r
+
+    def _fresh_prefill(self) -> Req:
+        return Req(prompt=int(synth.lognormal_lengths(self.rng, 1, 600, 16, 2048)[0]))
+
+    def occupancy(self) -> float:
+        return 1.0 - self.stage.num_free() / self.n_pages
+
+    # ---- one iteration: build the batch, call the stage, advance the state ----
+    def plan(self):
+        """Rows of this iteration: (request, q_len) for the 96 decode slots then the active prefill slots."""
+        rows = [(r, 1) for r in self.decode]
+        for r in self.prefill:
+            q = min(CHUNK, r.prompt - r.ctx)
+            if q > 0 and self._alloc(r, r.ctx + q):
+                rows.append((r, q))
+        for r, _ in rows[:N_DECODE]:
+            ok = self._alloc(r, r.ctx + 1)
+            assert ok, "page pool exhausted for a decode row (the 85% rule should prevent this)"
+        return rows
+
+    def step(self, hidden_bank: torch.Tensor, out: torch.Tensor) -> Iteration:
+        """hidden_bank: bf16 [>= T, H] device rows to feed (synthetic stage input); out: bf16 [>= T, H]."""
+        rows = self.plan()
+        n = len(rows)
+        q = np.array([ql for _, ql in rows], dtype=np.int32)
+        cu = np.concatenate([[0], np.cumsum(q)]).astype(np.int32)
+        T = int(cu[-1])
+        bt = self.h_bt.numpy()
+        for i, (r, _) in enumerate(rows):
+            bt[i, :len(r.pages)] = r.pages
+        self.h_cu.numpy()[:n + 1] = cu
+        self.h_ctx.numpy()[:n] = [r.ctx for r, _ in rows]
+        with torch.cuda.stream(self.stage.stream):
+            self.d_bt.copy_(self.h_bt, non_blocking=True)
+            self.d_cu.copy_(self.h_cu, non_blocking=True)
+            self.d_ctx.copy_(self.h_ctx, non_blocking=True)
+        self.stage.prefill(n, self.d_cu, self.d_ctx, self.d_bt, T, hidden=hidden_bank[:T], out_hidden=out[:T])
+        it = Iteration(cu.copy(), np.array([r.ctx for r, _ in rows], dtype=np.int32), bt[:n].copy(), n, T)
+        self.stage.synchronize()   # the host staging buffers are rewritten next iteration
+        self._advance(rows)
+        return it
+
+    def _advance(self, rows):
+        st = self.stats
+        for i, (r, ql) in enumerate(rows):
+            r.ctx += ql
+            if i < N_DECODE:
+                st["decode_tokens"] += 1
+                r.remaining -= 1
+                if r.remaining <= 0:
+                    self._free(r)
+                    st["finished"] += 1
+                    if self.fifo:
+                        nxt = self.fifo.popleft()
+                        nxt.remaining = int(synth.lognormal_lengths(self.rng, 1, 250, 1, 2048)[0])
+                        self.decode[i] = nxt
+                    else:
+                        self.decode[i] = self._fresh_decode()
+            else:
+                st["prefill_tokens"] += ql
+        for j, r in enumerate(self.prefill):
+            if r.prompt > 0 and r.ctx >= r.prompt:
+                self.fifo.append(r)
+                self.prefill[j] = self._fresh_prefill()
+        while self.fifo and self.occupancy() > OCCUPANCY:
+            self._free(self.fifo.pop())
+            st["dropped"] += 1
+        st["occupancy"].append(self.occupancy())
