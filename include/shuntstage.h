@@ -152,6 +152,19 @@ int ss_stage_prefill(ss_stage *st, int n_seqs,
                      const int32_t *block_tables, int max_blocks, int total_tokens,
                      void *out_hidden_bf16, float *out_logits, int32_t *out_argmax);
 
+/* Mixed iteration of online serving (continuous batching: decode requests and prefill chunks share one pass over the
+ * weights; the paper's online experiments; BASELINE.json configs[4]).  Same arguments, semantics
+ * and errors as ss_stage_prefill, plus one HOST hint: the first n_decode_rows sequences of the batch are decode
+ * requests, i.e. have q_len == 1 (cu_q[s+1] - cu_q[s] == 1 for s < n_decode_rows; "decode rows first").  Their
+ * attention then runs in the page-balanced GQA decode kernel instead of one 64-row causal tile per (row, head).
+ * Results are those of ss_stage_prefill on the same arguments.  A hint that does not hold is undefined behaviour.
+ * n_decode_rows = 0 is ss_stage_prefill; n_decode_rows = n_seqs = total_tokens is a decode step expressed through
+ * cu_q.  SS_ERR_INVALID_ARG if n_decode_rows < 0 or > n_seqs. */
+int ss_stage_mixed(ss_stage *st, int n_decode_rows, int n_seqs,
+                   const void *hidden_bf16, const int32_t *token_ids, const int32_t *cu_q,
+                   const int32_t *ctx_before, const int32_t *block_tables, int max_blocks, int total_tokens,
+                   void *out_hidden_bf16, float *out_logits, int32_t *out_argmax);
+
 /*
  * One decode iteration for `batch` sequences, one new token each (Table 2 "Decode" rows).
  * context_lens[b] = tokens already cached (A20); the new token's K/V are appended at that position by the

@@ -20,7 +20,8 @@ ERRORS = {0: "SS_OK", -1: "SS_ERR_INVALID_ARG", -2: "SS_ERR_UNSUPPORTED", -3: "S
           -4: "SS_ERR_NO_PAGES", -5: "SS_ERR_BAD_PAGE", -6: "SS_ERR_CUDA"}
 
 EXPORTS = ["ss_stage_workspace_bytes", "ss_kv_page_bytes", "ss_stage_create", "ss_stage_destroy",
-           "ss_kv_num_pages", "ss_kv_num_free", "ss_kv_alloc", "ss_kv_free", "ss_stage_prefill", "ss_stage_decode",
+           "ss_kv_num_pages", "ss_kv_num_free", "ss_kv_alloc", "ss_kv_free", "ss_stage_prefill", "ss_stage_mixed",
+           "ss_stage_decode",
            "ss_stage_launch_count", "ss_op_gemm_scratch_bytes", "ss_op_gemm_bf16", "ss_op_gemm_swiglu_bf16", "ss_strerror",
            "ss_last_cuda_error", "ss_version", "ss_debug_buffer", "ss_pool_create", "ss_pool_destroy",
            "ss_pool_num_pages", "ss_pool_num_free", "ss_pool_alloc", "ss_pool_free"]
@@ -82,6 +83,8 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     lib.ss_kv_free.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_int32)]
     lib.ss_stage_prefill.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                      C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.ss_stage_mixed.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                   C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.ss_stage_decode.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p,
                                     C.c_void_p, C.c_void_p, C.c_void_p]
     lib.ss_stage_launch_count.restype = C.c_int64
@@ -203,6 +206,15 @@ class Stage:
                                        _ptr(out_logits), _ptr(out_argmax))
         if check and rc != SS_OK:
             raise ShuntStageError(rc, "ss_stage_prefill")
+        return rc
+
+    def mixed(self, n_decode_rows, n_seqs, cu_q, ctx_before, block_tables, total_tokens, hidden=None, token_ids=None,
+              out_hidden=None, out_logits=None, out_argmax=None, check=True):
+        rc = self.lib.ss_stage_mixed(self.h, n_decode_rows, n_seqs, _ptr(hidden), _ptr(token_ids), _ptr(cu_q),
+                                     _ptr(ctx_before), _ptr(block_tables), block_tables.shape[1], total_tokens,
+                                     _ptr(out_hidden), _ptr(out_logits), _ptr(out_argmax))
+        if check and rc != SS_OK:
+            raise ShuntStageError(rc, "ss_stage_mixed")
         return rc
 
     def decode(self, batch, block_tables, context_lens, hidden=None, token_ids=None, out_hidden=None,

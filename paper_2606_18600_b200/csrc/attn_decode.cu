@@ -178,7 +178,7 @@ __global__ void __launch_bounds__(DA_WARPS * 32) decode_attn_kernel(const Decode
       const int page = bt[(size_t)cc.b * max_blocks + cc.pg];
       const uint8_t *src = (const uint8_t *)p.kv_new + ((size_t)cc.b * 2 * n_kv * D + (size_t)cc.h * D) * 2;
       const size_t goff = (((size_t)page * n_kv + cc.h) * 16 + r) * ROW_BYTES;
-      for (int idx = lane; idx < 2 * CHUNKS; idx += 32) {
+      for (int idx = lane; idx < (p.append ? 2 * CHUNKS : 0); idx += 32) {
         const int isv = idx / CHUNKS, ch = idx % CHUNKS;
         const uint4 val = *reinterpret_cast<const uint4 *>(src + (size_t)isv * n_kv * D * 2 + ch * 16);
         uint8_t *sdst = (isv ? vsm : ksm) + r * ROW_BYTES + ((ch ^ (r & 7)) << 4);

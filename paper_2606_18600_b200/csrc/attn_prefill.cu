@@ -22,14 +22,14 @@ constexpr int PA_BM = 64;  // query rows per CTA
 constexpr int PA_BN = 64;  // keys per tile
 
 // ---- plan: token -> (sequence, position) and the prefix sum of query tiles --------------------------------------
-__global__ void prefill_plan_kernel(const CallArgs *__restrict__ args, int n_seqs, PrefillPlan plan) {
+__global__ void prefill_plan_kernel(const CallArgs *__restrict__ args, int n_seqs, int seq0, PrefillPlan plan) {
   pdl_launch_dependents();
   pdl_wait();
   if (blockIdx.x == 0 && threadIdx.x == 0) {
     int acc = 0;
     plan.tile_cum[0] = 0;
     for (int s = 0; s < n_seqs; ++s) {
-      acc += (args->cu_q[s + 1] - args->cu_q[s] + PA_BM - 1) / PA_BM;
+      if (s >= seq0) acc += (args->cu_q[s + 1] - args->cu_q[s] + PA_BM - 1) / PA_BM;
       plan.tile_cum[s + 1] = acc;
     }
   }
@@ -42,9 +42,9 @@ __global__ void prefill_plan_kernel(const CallArgs *__restrict__ args, int n_seq
   }
 }
 
-cudaError_t launch_prefill_plan(const CallArgs *args, int n_seqs, PrefillPlan plan, cudaStream_t s) {
+cudaError_t launch_prefill_plan(const CallArgs *args, int n_seqs, int seq0, PrefillPlan plan, cudaStream_t s) {
   int blocks = n_seqs < 1 ? 1 : (n_seqs > 1024 ? 1024 : n_seqs);
-  return launch_pdl(prefill_plan_kernel, dim3(blocks), dim3(256), 0, s, args, n_seqs, plan);
+  return launch_pdl(prefill_plan_kernel, dim3(blocks), dim3(256), 0, s, args, n_seqs, seq0, plan);
 }
 
 template <int D>

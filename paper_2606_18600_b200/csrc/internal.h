@@ -152,6 +152,7 @@ struct DecodeAttnParams {
   void *out;                 // bf16 [B,Hq]
   const CallArgs *args;
   int n_workers;             // worker warps in the grid
+  int append;                // 1: write kv_new into the last page (decode step); 0: the token is already in the pool
   int warps_per_cta;
 };
 cudaError_t launch_decode_attn(const DecodeAttnParams &p, cudaStream_t s);
@@ -163,7 +164,8 @@ struct PrefillPlan {
   int32_t *tok_pos;          // [max_tokens]
   int32_t *tile_cum;         // [max_seqs+1] prefix sum of 64-row query tiles per sequence
 };
-cudaError_t launch_prefill_plan(const CallArgs *args, int n_seqs, PrefillPlan plan, cudaStream_t s);
+// seq0: the first seq0 sequences get no query tiles (mixed batches: their attention runs in the decode kernel)
+cudaError_t launch_prefill_plan(const CallArgs *args, int n_seqs, int seq0, PrefillPlan plan, cudaStream_t s);
 struct PrefillAttnParams {
   const void *q;             // bf16 [T,Hq]
   const void *kpool, *vpool;

@@ -421,7 +421,9 @@ static cudaError_t run_gemm(const ss_stage *st, const CUtensorMap *const a[3], i
   } while (0)
 
 // enqueue every kernel of one call; `decode` selects the q_len == 1 fast path
-static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T, bool tail) {
+// `n_dec` (prefill calls only): the first n_dec sequences are decode rows (q_len == 1) whose attention runs in the
+// decode kernel (mixed batches, reading A19)
+static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T, bool tail, int n_dec = 0) {
   const ss_model_dims &d = st->d;
   const int H = d.hidden, dh = d.head_dim, Hq = d.n_q_heads * dh, Hkv = d.n_kv_heads * dh, F = d.ffn;
   const int Nqkv = Hq + 2 * Hkv;
@@ -436,8 +438,10 @@ static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T,
   PrefillPlan pplan{st->at<int32_t>(c.tok_seq), st->at<int32_t>(c.tok_pos), st->at<int32_t>(c.tile_cum)};
   if (decode)
     CKE(launch_decode_plan(args, n_seqs, d.n_kv_heads, st->n_workers, dplan, s));
-  else
-    CKE(launch_prefill_plan(args, n_seqs, pplan, s));
+  else {
+    CKE(launch_prefill_plan(args, n_seqs, n_dec, pplan, s));
+    if (n_dec > 0) CKE(launch_decode_plan(args, n_dec, d.n_kv_heads, st->n_workers, dplan, s));
+  }
   CKE(launch_input_rmsnorm(args, st->edge.embed, st->lw[0].ln1, d.rms_eps, H, T, x, h, s));
 
   for (int l = 0; l < st->L; ++l) {
@@ -467,14 +471,14 @@ static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T,
     qp.decode = decode ? 1 : 0;
     CKE(launch_qkv_post(qp, s));  // S3, S4 (+S5 in prefill)
 
-    if (decode) {  // S5 + S6a
+    if (decode || n_dec > 0) {  // S5 + S6a (mixed call: the decode rows' K/V were appended by qkv_post already)
       DecodeAttnParams ap;
       memset(&ap, 0, sizeof(ap));
       ap.q = st->at<void>(c.q);
       ap.kv_new = st->at<void>(c.kv_new);
       ap.kpool = st->kpool(l); ap.vpool = st->vpool(l);
       ap.n_pages = st->num_pages;
-      ap.batch = n_seqs; ap.n_q = d.n_q_heads; ap.n_kv = d.n_kv_heads; ap.d = dh;
+      ap.batch = decode ? n_seqs : n_dec; ap.n_q = d.n_q_heads; ap.n_kv = d.n_kv_heads; ap.d = dh;
       ap.plan = dplan;
       ap.part_o = st->at<float>(c.part_o);
       ap.part_ml = st->at<float>(c.part_ml);
@@ -482,9 +486,11 @@ static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T,
       ap.args = args;
       ap.n_workers = st->n_workers;
       ap.warps_per_cta = 4;
+      ap.append = decode ? 1 : 0;
       CKE(launch_decode_attn(ap, s));
       CKE(launch_decode_merge(ap, s));
-    } else {  // S6b
+    }
+    if (!decode && n_dec < n_seqs) {  // S6b
       PrefillAttnParams ap;
       memset(&ap, 0, sizeof(ap));
       ap.q = st->at<void>(c.q);
@@ -493,7 +499,7 @@ static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T,
       ap.plan = pplan;
       ap.out = st->at<void>(c.attn_out);
       ap.args = args;
-      ap.max_tiles = (T + 63) / 64 + n_seqs;
+      ap.max_tiles = (T - n_dec + 63) / 64 + (n_seqs - n_dec);
       CKE(launch_prefill_attn(ap, s));
     }
     {  // S7: output projection, then S8: x1 = x + o Wo^T ; h2 = rmsnorm(x1; ln2)
@@ -557,6 +563,14 @@ extern "C" {
 int ss_stage_prefill(ss_stage *st, int n_seqs, const void *hidden_bf16, const int32_t *token_ids,
                      const int32_t *cu_q, const int32_t *ctx_before, const int32_t *block_tables, int max_blocks,
                      int total_tokens, void *out_hidden_bf16, float *out_logits, int32_t *out_argmax) {
+  return ss_stage_mixed(st, 0, n_seqs, hidden_bf16, token_ids, cu_q, ctx_before, block_tables, max_blocks,
+                        total_tokens, out_hidden_bf16, out_logits, out_argmax);
+}
+
+int ss_stage_mixed(ss_stage *st, int n_decode_rows, int n_seqs, const void *hidden_bf16, const int32_t *token_ids,
+                   const int32_t *cu_q, const int32_t *ctx_before, const int32_t *block_tables, int max_blocks,
+                   int total_tokens, void *out_hidden_bf16, float *out_logits, int32_t *out_argmax) {
+  if (n_decode_rows < 0 || n_decode_rows > n_seqs || n_decode_rows > total_tokens) return SS_ERR_INVALID_ARG;
   int rc = common_checks(st, n_seqs, total_tokens, hidden_bf16, token_ids, block_tables, max_blocks, ctx_before,
                          out_logits, out_argmax);
   if (rc != SS_OK) return rc;
@@ -569,9 +583,9 @@ int ss_stage_prefill(ss_stage *st, int n_seqs, const void *hidden_bf16, const in
   a.n_seqs = n_seqs; a.T = total_tokens; a.max_blocks = max_blocks;
   if ((rc = upload_args(st, a)) != SS_OK) return rc;
   const int64_t before = g_launches;
-  cudaError_t e = enqueue_forward(st, false, n_seqs, total_tokens, out_logits || out_argmax);
+  cudaError_t e = enqueue_forward(st, false, n_seqs, total_tokens, out_logits || out_argmax, n_decode_rows);
   st->launches += g_launches - before;
-  if (e != cudaSuccess) return cuda_fail(e, "ss_stage_prefill");
+  if (e != cudaSuccess) return cuda_fail(e, "ss_stage_mixed");
   return SS_OK;
 }
 

@@ -1,5 +1,5 @@
-"""Online mixed-batch driver for BASELINE.json configs[4] ("cfg-5"): every iteration is ONE ss_stage_prefill call
-that combines 96 decode requests (q_len = 1 rows, first in the batch: reading A19) with up to 4 prefill chunks of
+"""Online mixed-batch driver for BASELINE.json configs[4] ("cfg-5"): every iteration is ONE ss_stage_mixed call
+(ss_stage_prefill plus the host hint "the first 96 sequences are decode rows") that combines 96 decode requests (q_len = 1 rows, first in the batch: reading A19) with up to 4 prefill chunks of
 <= 512 tokens from new requests, over a page pool kept near 85% occupancy (reading A18), as in the paper's online
 serving experiments (continuous batching of the Azure-trace-shaped load).
 
@@ -47,8 +47,10 @@ class Iteration:
 
 
 class OnlineDriver:
-    def __init__(self, stage, shape: synth.ModelShape, seed: int = 0, max_blocks: int = 0, device="cuda:0"):
+    def __init__(self, stage, shape: synth.ModelShape, seed: int = 0, max_blocks: int = 0, device="cuda:0",
+                 use_mixed: bool = True):
         self.stage, self.shape, self.dev = stage, shape, torch.device(device)
+        self.use_mixed = use_mixed   # False: plain ss_stage_prefill (decode rows as 1-row causal tiles)
         self.rng = np.random.default_rng(seed)
         self.max_blocks = max_blocks or (8192 + 2048 + CHUNK) // PAGE + 2
         self.n_pages = stage.num_pages()
@@ -139,7 +141,8 @@ class OnlineDriver:
             self.d_bt.copy_(self.h_bt, non_blocking=True)
             self.d_cu.copy_(self.h_cu, non_blocking=True)
             self.d_ctx.copy_(self.h_ctx, non_blocking=True)
-        self.stage.prefill(n, self.d_cu, self.d_ctx, self.d_bt, T, hidden=hidden_bank[:T], out_hidden=out[:T])
+        self.stage.mixed(N_DECODE if self.use_mixed else 0, n, self.d_cu, self.d_ctx, self.d_bt, T,
+                         hidden=hidden_bank[:T], out_hidden=out[:T])
         it = Iteration(cu.copy(), np.array([r.ctx for r, _ in rows], dtype=np.int32), bt[:n].copy(), n, T)
         self.stage.synchronize()   # the host staging buffers are rewritten next iteration
         self._advance(rows)

@@ -294,6 +294,54 @@ def test_chunked_prefill_and_mixed_batch_on_gpu():
         P.close()
 
 
+@pytest.mark.parametrize("shape", [synth.TINY, synth.TINY_QWEN])
+def test_stage_mixed_decode_rows_first_vs_oracle(shape):
+    """ss_stage_mixed (continuous batching; reading A19): 3 decode rows (q_len 1, routed to the
+    decode attention kernel, their K/V appended by qkv_post) followed by 2 prefill chunks, one call; then the same
+    state advanced again with every row a decode row (n_decode_rows == n_seqs)."""
+    from paper_2606_18600_b200 import binding
+    lens = np.array([37, 16, 129, 90, 50], dtype=np.int32)           # totals after the mixed call
+    P, lens, pb, x = _problem(shape, seed=4, lens=lens, extra=8)
+    try:
+        bt = pb.block_tables
+        before = np.array([36, 15, 128, 30, 0], dtype=np.int32)       # rows 0-2 decode (q_len 1), 3-4 chunks
+        cu_full = np.concatenate([[0], np.cumsum(lens)]).astype(np.int32)
+        rows1 = np.concatenate([np.arange(cu_full[s], cu_full[s] + before[s]) for s in range(5)])
+        rows2 = np.concatenate([np.arange(cu_full[s] + before[s], cu_full[s + 1]) for s in range(5)])
+        pool0 = hp.new_pool(shape, pb.n_pages_pool, P.L)
+        keep = before > 0
+        hp.run_oracle_prefill(F32, shape, P.wb, pool0, before[keep], bt[keep], x[rows1])
+        w2, _, _ = hp.run_oracle_prefill(F32, shape, P.wb, pool0, lens, bt, x[rows2], ctx_before=before)
+        P.prefill(before[keep], bt[keep], x[rows1])
+        q = lens - before
+        cu = np.concatenate([[0], np.cumsum(q)]).astype(np.int32)
+        T = int(cu[-1])
+        out = torch.empty((T, shape.hidden), dtype=torch.bfloat16, device="cuda:0")
+        a = (P.i32(cu), P.i32(before), P.i32(bt), P.bf16(x[rows2]))
+        torch.cuda.synchronize()
+        P.stage.mixed(3, 5, a[0], a[1], a[2], T, hidden=a[3], out_hidden=out)
+        P.stage.synchronize()
+        g2 = f32b(out.cpu().view(torch.int16).numpy().view(np.uint16))
+        assert hp.rel_err_rows(g2, w2) < STAGE_TOL
+        mask = _written_mask(pool0.shape, bt, lens)
+        pg = P.pool_bits()
+        assert (pg[~mask] == 0x7FC1).all() and (pg[mask] != 0x7FC1).all()
+        # every row a decode row, through ss_stage_mixed
+        xs = x[int(lens.sum()):int(lens.sum()) + 5]
+        w3, _ = hp.run_oracle_decode(F32, shape, P.wb, pool0, lens, bt, xs)
+        out3 = torch.empty((5, shape.hidden), dtype=torch.bfloat16, device="cuda:0")
+        b = (P.i32(np.arange(6)), P.i32(lens), P.bf16(xs))
+        torch.cuda.synchronize()
+        P.stage.mixed(5, 5, b[0], b[1], a[2], 5, hidden=b[2], out_hidden=out3)
+        P.stage.synchronize()
+        assert hp.rel_err_rows(f32b(out3.cpu().view(torch.int16).numpy().view(np.uint16)), w3) < STAGE_TOL
+        # host-detectable misuse
+        assert P.stage.mixed(6, 5, b[0], b[1], a[2], 5, hidden=b[2], out_hidden=out3, check=False) == -1
+        assert P.stage.mixed(-1, 5, b[0], b[1], a[2], 5, hidden=b[2], out_hidden=out3, check=False) == -1
+    finally:
+        P.close()
+
+
 def test_token_ids_logits_and_argmax():
     """S0 embedding gather and S11 logits/argmax (Table 2 'Logits Calculation'; reading A14)."""
     shape = synth.TINY
