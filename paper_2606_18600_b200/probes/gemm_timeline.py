@@ -30,7 +30,7 @@ tr = sc[nfix:].view(torch.int64).cpu().numpy().reshape(256, 64)[:148].astype(np.
 t0 = tr[:, 0].min()
 rel = lambda a: (a - t0) / 1e3
 print(name, "kernel span us: start spread %.1f, end min/median/max %.1f %.1f %.1f" % (rel(tr[:, 0]).max(), rel(tr[:, 1]).min(), np.median(rel(tr[:, 1])), rel(tr[:, 1]).max()))
-print(" first full (issuer0 first tile landed): median %.1f max %.1f" % (np.median(rel(tr[:, 2])), rel(tr[:, 2]).max()))
+print(" setup done (barriers, TMEM) median %.2f; first TMA issued %.2f; first tile landed (issuer 0): median %.2f max %.2f" % (np.median((tr[:, 7] - tr[:, 0]) / 1e3), np.median((tr[:, 8] - tr[:, 0]) / 1e3), np.median((tr[:, 2] - tr[:, 0]) / 1e3), ((tr[:, 2] - tr[:, 0]) / 1e3).max()))
 nit = int(((tr[:, 3::4][:, :8] > 0).sum(axis=1)).max())
 for it in range(nit):
     b = 3 + 4 * it
