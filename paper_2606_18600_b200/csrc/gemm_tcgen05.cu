@@ -29,7 +29,8 @@ namespace ss {
 
 constexpr int A_TILE_BYTES = GEMM_BM * GEMM_BK * 2;  // 16 KB
 constexpr int EPI_THREADS = 128;
-constexpr int GEMM_THREADS = 224;  // warp 0: TMA producer, 1: MMA issuer 0, 2-5: epilogue, 6: MMA issuer 1
+constexpr int GEMM_THREADS = 352;  // warp 0: TMA producer, 1: MMA issuer 0, 6: MMA issuer 1, 2-5 and 7-10: epilogue
+constexpr int EPI_WARPS = 8;       // two warps per TMEM lane quadrant, taking alternate 32-column chunks
 
 struct WorkItem {
   int row_tile, t_tile, kb0, kb1;
@@ -118,7 +119,7 @@ __device__ __forceinline__ void trace(const GemmParams &p, int slot) {
 #else
 __device__ __forceinline__ void trace(const GemmParams &, int) {}
 #endif
-__device__ __forceinline__ void epi_bar() { asm volatile("bar.sync 1, 128;" ::: "memory"); }
+__device__ __forceinline__ void epi_bar() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
 
 template <bool DUAL>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
@@ -172,7 +173,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
     }
     for (int i = 0; i < 2; ++i) {
       mbar_init(&tfull[i], (uint32_t)n_iss);
-      mbar_init(&tempty[i], 4);  // one arrival per epilogue warp
+      mbar_init(&tempty[i], EPI_WARPS);  // one arrival per epilogue warp
     }
     mbar_fence_init();
   }
@@ -298,12 +299,15 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
         ++item;
       }
     }
-  } else if (warp >= 2 && warp < 6) {
+  } else if ((warp >= 2 && warp < 6) || (warp >= 7 && warp < 11)) {
     // ---------------- epilogue: TMEM -> registers -> (fix-up) -> global ----------------
     pdl_wait();
     const int quad = warp & 3;
     const int r = quad * 32 + lane;  // row of the tile = TMEM lane
-    const int et = threadIdx.x - 64; // 0..127
+    // The last work item's epilogue is never overlapped (it is the kernel's tail), so it is spread over 8 warps:
+    // warp (2..5 | 7..10) owns TMEM lane quadrant warp & 3 and group grp takes the 32-column chunks c0 = 32*grp (mod 64)
+    const int grp = warp >= 7 ? 1 : 0;
+    const int et = grp ? (int)threadIdx.x - 224 + 128 : (int)threadIdx.x - 64;  // 0..255
     WorkIter it(p, cta, grid);
     WorkItem w;
     uint32_t item = 0, n_run = 0;  // n_run: running k-block counter (the issuers' n) at the item's start
@@ -370,7 +374,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
       if (!is_first) {
         // contributor: dump the raw fp32 accumulator(s) to this CTA's slot, [acc][col][row]
         float *slot = p.fix_slots + (size_t)cta * (DUAL ? 2 : 1) * bn * GEMM_BM;
-        for (int c0 = 0; c0 < (int)acc_cols; c0 += 32) {
+        for (int c0 = grp * 32; c0 < (int)acc_cols; c0 += 64) {
           uint32_t v[32];
           ld_acc((uint32_t)c0, v);
 #pragma unroll
@@ -386,7 +390,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
           atomicExch(p.fix_flags + cta, 1);
         }
       } else {
-        for (int c0 = 0; c0 < bn; c0 += 32) {
+        for (int c0 = grp * 32; c0 < bn; c0 += 64) {
           uint32_t v[32], u[32];
           ld_acc((uint32_t)c0, v);
           if (DUAL) ld_acc((uint32_t)(bn + c0), u);
