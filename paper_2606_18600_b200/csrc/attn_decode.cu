@@ -23,8 +23,16 @@
 
 namespace ss {
 
-constexpr int DA_WARPS = 4;
-constexpr int DA_STAGES = 3;
+#ifndef SS_DA_WARPS
+#define SS_DA_WARPS 4
+#endif
+#ifndef SS_DA_STAGES
+#define SS_DA_STAGES 3
+#endif
+constexpr int DA_WARPS = SS_DA_WARPS;    // independent warp pipelines per CTA
+constexpr int DA_STAGES = SS_DA_STAGES;  // pages (K 4 KB + V 4 KB at d = 128) per warp ring
+int decode_attn_warps_per_cta() { return DA_WARPS; }
+int decode_attn_default_ctas_per_sm() { return (int)((size_t)220 * 1024 / ((size_t)DA_WARPS * DA_STAGES * 2 * 16 * 128 * 2)); }
 
 // ---- plan: prefix sum of pages per sequence --------------------------------------------------------------------
 __global__ void decode_plan_kernel(const CallArgs *__restrict__ args, int batch, int n_kv, int n_workers,

@@ -158,6 +158,8 @@ struct DecodeAttnParams {
 cudaError_t launch_decode_attn(const DecodeAttnParams &p, cudaStream_t s);
 cudaError_t launch_decode_merge(const DecodeAttnParams &p, cudaStream_t s);
 cudaError_t attn_init();
+int decode_attn_warps_per_cta();
+int decode_attn_default_ctas_per_sm();
 
 struct PrefillPlan {
   int32_t *tok_seq;          // [max_tokens]

@@ -275,9 +275,11 @@ int ss_stage_create(ss_stage **out, const ss_model_dims *dims, int l0, int l1, c
   if (e != cudaSuccess) return fail(cuda_fail(e, "cudaGetDevice"));
   e = cudaDeviceGetAttribute(&st->n_sm, cudaDevAttrMultiProcessorCount, dev);
   if (e != cudaSuccess) return fail(cuda_fail(e, "cudaDeviceGetAttribute"));
-  int ctas_per_sm = env_int("SS_ATTN_CTAS_PER_SM", 2);
-  st->n_workers = st->n_sm * ctas_per_sm * 4;
-  if (st->n_workers > MAX_WORKERS) st->n_workers = MAX_WORKERS / 4 * 4;
+  int ctas_per_sm = env_int("SS_ATTN_CTAS_PER_SM", decode_attn_default_ctas_per_sm());
+  if (ctas_per_sm < 1) ctas_per_sm = 1;
+  const int wpc = decode_attn_warps_per_cta();
+  st->n_workers = st->n_sm * ctas_per_sm * wpc;
+  if (st->n_workers > MAX_WORKERS) st->n_workers = MAX_WORKERS / wpc * wpc;
   if ((e = gemm_init()) != cudaSuccess) return fail(cuda_fail(e, "gemm_init"));
   if ((e = attn_init()) != cudaSuccess) return fail(cuda_fail(e, "attn_init"));
   if ((e = cudaMallocHost((void **)&st->h_args, sizeof(CallArgs))) != cudaSuccess)
@@ -485,7 +487,7 @@ static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T,
       ap.out = st->at<void>(c.attn_out);
       ap.args = args;
       ap.n_workers = st->n_workers;
-      ap.warps_per_cta = 4;
+      ap.warps_per_cta = decode_attn_warps_per_cta();
       ap.append = decode ? 1 : 0;
       CKE(launch_decode_attn(ap, s));
       CKE(launch_decode_merge(ap, s));
