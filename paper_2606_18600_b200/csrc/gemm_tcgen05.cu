@@ -505,7 +505,11 @@ int make_tmap_bf16_2d(CUtensorMap *out, const void *base, uint64_t rows, uint64_
   return r == CUDA_SUCCESS ? 0 : -(int)r - 1000;
 }
 
+static int env_int(const char *name, int dflt);
 int gemm_pick_bn(int T) {
+  static int env_bn = -1;
+  if (env_bn < 0) env_bn = env_int("SS_GEMM_BN", 0);  // experiments: force the token tile
+  if (env_bn > 0) return env_bn;
   const int c[4] = {32, 64, 128, 256};
   for (int i = 0; i < 4; ++i)
     if (T <= c[i]) return c[i];

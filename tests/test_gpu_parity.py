@@ -342,6 +342,49 @@ def test_stage_mixed_decode_rows_first_vs_oracle(shape):
         P.close()
 
 
+def test_P17_dyadic_case_kv_bits_exact():
+    """Reading A13, strict value pin: with projection weights +-2^-k, unit gains and small-integer hidden rows every
+    fp32 partial sum of the K/V projections is exact, so the result cannot depend on the summation order (tensor
+    core vs CPU loop): V at every position and K at position 0 (RoPE = identity there) must equal the oracle's
+    pages BIT FOR BIT."""
+    shape = synth.TINY
+    gh = _gh()
+    lens = np.array([1, 5, 16, 33], dtype=np.int32)
+    P, lens, pb, _ = _problem(shape, seed=9, lens=lens)
+    try:
+        g = torch.Generator().manual_seed(123)
+        for name in ("wq", "wk", "wv", "wo", "w_gate", "w_up", "w_down"):
+            w = P.tw[0][name]
+            sign = torch.randint(0, 2, w.shape, generator=g) * 2 - 1
+            expo = torch.randint(4, 8, w.shape, generator=g)
+            w.copy_((sign.float() * torch.pow(2.0, -expo.float())).to(torch.bfloat16))
+        for name in ("ln1", "ln2"):
+            for l in range(P.L):
+                P.tw[l][name].fill_(1.0)
+        for l in range(P.L):
+            for k, v in P.tw[l].items():
+                if v is not None:
+                    P.dw[l][k].copy_(v.to("cuda:0"))
+        wb = [{k: (None if v is None else synth.bits(v)) for k, v in w.items()} for w in P.tw]
+        T = int(lens.sum())
+        xi = torch.randint(-4, 5, (T, shape.hidden), generator=g).float()
+        xi[xi == 0] = 1.0
+        x = synth.bits(xi.to(torch.bfloat16))
+        pool = hp.new_pool(shape, pb.n_pages_pool, P.L)
+        hp.run_oracle_prefill(F32, shape, wb, pool, lens, pb.block_tables, x, rounding=1)
+        P.prefill(lens, pb.block_tables, x)
+        pg = P.pool_bits()
+        for s, n in enumerate(lens):
+            v_gpu = hp.logical_kv(pg[0, 1], pb.block_tables[s], int(n))
+            v_orc = hp.logical_kv(pool[0, 1], pb.block_tables[s], int(n))
+            assert np.array_equal(v_gpu, v_orc), f"V bits differ in sequence {s}"
+            k_gpu = hp.logical_kv(pg[0, 0], pb.block_tables[s], 1)
+            k_orc = hp.logical_kv(pool[0, 0], pb.block_tables[s], 1)
+            assert np.array_equal(k_gpu, k_orc), f"K bits at position 0 differ in sequence {s}"
+    finally:
+        P.close()
+
+
 def test_token_ids_logits_and_argmax():
     """S0 embedding gather and S11 logits/argmax (Table 2 'Logits Calculation'; reading A14)."""
     shape = synth.TINY
