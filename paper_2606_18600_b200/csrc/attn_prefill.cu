@@ -48,7 +48,7 @@ cudaError_t launch_prefill_plan(const CallArgs *args, int n_seqs, int seq0, Pref
 }
 
 template <int D>
-__global__ void __launch_bounds__(PA_WARPS * 32) prefill_attn_kernel(const PrefillAttnParams p) {
+__global__ void __launch_bounds__(PA_WARPS * 32, 3) prefill_attn_kernel(const PrefillAttnParams p) {
   pdl_launch_dependents();
   pdl_wait();
   constexpr int ROW_BYTES = D * 2;
@@ -57,8 +57,11 @@ __global__ void __launch_bounds__(PA_WARPS * 32) prefill_attn_kernel(const Prefi
   constexpr int KSTEPS = D / 16;
   constexpr int NT = D / 8;
   extern __shared__ __align__(128) uint8_t smem[];
-  uint8_t *q_s = smem;                       // [64][D]
-  uint8_t *kv_s = smem + PA_BM * ROW_BYTES;  // 2 x (K tile, V tile)
+  // smem = 2 x (K tile, V tile).  The Q tile is staged once through the SECOND buffer (free until the prefetch of
+  // key tile 1) and then lives in registers, so a CTA needs 64 KB and three fit on an SM (occupancy, not
+  // bandwidth, bounds this kernel: ncu showed 8 warps/SM with 56% of the cycles without an eligible warp).
+  uint8_t *kv_s = smem;
+  uint8_t *q_s = smem + 2 * TILE_BYTES;      // [PA_BM][D], aliases buffer 1
 
   const int head = blockIdx.x, slot = blockIdx.y;
   const int32_t *tile_cum = p.plan.tile_cum;
@@ -122,18 +125,21 @@ __global__ void __launch_bounds__(PA_WARPS * 32) prefill_attn_kernel(const Prefi
   for (int t = 0; t < NT; ++t) o[t][0] = o[t][1] = o[t][2] = o[t][3] = 0.f;
   float m_run[2] = {-INFINITY, -INFINITY}, l_run[2] = {0.f, 0.f};
 
+  {  // Q tile -> registers, then its smem (buffer 1) is free for the prefetch of key tile 1
+    cp_async_wait<0>();
+    __syncthreads();
+    const int mtx = lane >> 3, rr = lane & 7;
+    const int r = warp * 16 + (mtx & 1) * 8 + rr;
+    const uint32_t qb = smem_u32(q_s) + r * ROW_BYTES;
+#pragma unroll
+    for (int ks = 0; ks < KSTEPS; ++ks) ldmatrix_x4(qf[ks], qb + (((ks * 2 + (mtx >> 1)) ^ (r & 7)) << 4));
+    __syncthreads();
+  }
   for (int kt = 0; kt < n_kt; ++kt) {
     if (kt + 1 < n_kt) load_kv(kt + 1, (kt + 1) & 1);
     cp_async_commit();
     cp_async_wait<1>();
     __syncthreads();
-    if (kt == 0) {
-      const int mtx = lane >> 3, rr = lane & 7;
-      const int r = warp * 16 + (mtx & 1) * 8 + rr;
-      const uint32_t qb = smem_u32(q_s) + r * ROW_BYTES;
-#pragma unroll
-      for (int ks = 0; ks < KSTEPS; ++ks) ldmatrix_x4(qf[ks], qb + (((ks * 2 + (mtx >> 1)) ^ (r & 7)) << 4));
-    }
     const uint8_t *ksm = kv_s + (size_t)(kt & 1) * 2 * TILE_BYTES;
     const uint8_t *vsm = ksm + TILE_BYTES;
 
@@ -240,7 +246,7 @@ __global__ void __launch_bounds__(PA_WARPS * 32) prefill_attn_kernel(const Prefi
   }
 }
 
-static size_t prefill_smem(int d) { return (size_t)(PA_BM + 4 * PA_BN) * d * 2; }
+static size_t prefill_smem(int d) { return (size_t)(4 * PA_BN) * d * 2; }  // Q aliases the second K/V buffer
 
 cudaError_t launch_prefill_attn(const PrefillAttnParams &p, cudaStream_t s) {
   static bool inited = false;

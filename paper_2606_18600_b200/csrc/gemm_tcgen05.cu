@@ -39,9 +39,12 @@ struct WorkItem {
 // Per-CTA work list.  All roles of a CTA construct the same iterator and see the same items in the same order.
 struct WorkIter {
   int sched, nkb, n_row_tiles, n_t_tiles, band, G, c;
-  long long u, u_end;  // stream-K: unit cursor / end of this CTA's range
+  uint32_t u, u_end;   // stream-K: unit cursor / end of this CTA's range (units = (tile, k-block); < 2^31, gemm_plan)
+  uint32_t uq, ur;     // U / G, U % G
   int idx, n_tiles;    // tiles: next tile index
 
+  // 32-bit arithmetic only: every role runs this before its first instruction of real work, and a 64-bit divide is
+  // a ~200-cycle subroutine (the producer issued its first TMA load ~1 us after the CTA's setup was done)
   __device__ WorkIter(const GemmParams &p, int cta, int grid) {
     sched = p.sched;
     nkb = (p.K + GEMM_BK - 1) / GEMM_BK;
@@ -51,24 +54,26 @@ struct WorkIter {
     G = grid;
     c = cta;
     n_tiles = n_row_tiles * n_t_tiles;
-    const long long U = (long long)n_tiles * nkb;
-    u = (long long)c * U / G;
-    u_end = (long long)(c + 1) * U / G;
+    const uint32_t U = (uint32_t)n_tiles * (uint32_t)nkb;
+    uq = U / (uint32_t)G;
+    ur = U - uq * (uint32_t)G;
+    u = range_start(c);
+    u_end = range_start(c + 1);
     idx = c;
   }
-  // first unit of CTA cc's stream-K range
-  __device__ long long range_start(int cc) const { return (long long)cc * ((long long)n_tiles * nkb) / G; }
+  // first unit of CTA cc's stream-K range = floor(cc * U / G)
+  __device__ uint32_t range_start(int cc) const { return (uint32_t)cc * uq + ((uint32_t)cc * ur) / (uint32_t)G; }
 
   __device__ bool next(WorkItem &w) {
     if (sched == SCHED_STREAMK) {
       if (u >= u_end) return false;
-      const int tile = (int)(u / nkb);
-      w.kb0 = (int)(u - (long long)tile * nkb);
-      const long long left = u_end - u;
-      w.kb1 = (int)((long long)w.kb0 + left < (long long)nkb ? (long long)w.kb0 + left : (long long)nkb);
-      w.t_tile = tile / n_row_tiles;
-      w.row_tile = tile - w.t_tile * n_row_tiles;
-      u += w.kb1 - w.kb0;
+      const uint32_t tile = u / (uint32_t)nkb;
+      w.kb0 = (int)(u - tile * (uint32_t)nkb);
+      const uint32_t left = u_end - u;
+      w.kb1 = (int)min((uint32_t)w.kb0 + left, (uint32_t)nkb);
+      w.t_tile = (int)tile / n_row_tiles;
+      w.row_tile = (int)tile - w.t_tile * n_row_tiles;
+      u += (uint32_t)(w.kb1 - w.kb0);
       return true;
     }
     if (idx >= n_tiles) return false;
@@ -339,7 +344,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
       // stream-K fix-up bookkeeping
       int c_lo = 0, c_hi = -1;  // contributors [c_lo, c_hi] of a tile this CTA owns
       if (is_first && !is_last) {
-        const long long tile_end = ((long long)(w.t_tile * p.n_row_tiles + w.row_tile) + 1) * nkb;
+        const uint32_t tile_end = ((uint32_t)(w.t_tile * p.n_row_tiles + w.row_tile) + 1u) * (uint32_t)nkb;
         c_lo = cta + 1;
         c_hi = cta;
         while (c_hi + 1 < grid && it.range_start(c_hi + 1) < tile_end) ++c_hi;
@@ -567,6 +572,7 @@ void gemm_plan(GemmLaunch &g, int n_sm) {
   const bool full_waves = n_tiles >= max_grid && n_tiles * 100 >= waves * max_grid * (p.n_t_tiles >= 2 ? 70 : 88);
   p.sched = (n_tiles >= 4LL * max_grid || full_waves) ? SCHED_TILES : SCHED_STREAMK;
   if (env_sched >= 0) p.sched = env_sched;
+  if (n_tiles * nkb >= (1LL << 31)) p.sched = SCHED_TILES;  // the stream-K unit cursor is 32-bit
   p.band = env_band > 0 ? env_band : (g.dual ? 8 : 16);
   if (p.band > p.n_row_tiles) p.band = p.n_row_tiles;
   p.stages = gemm_pick_stages(p.bn, g.dual);
