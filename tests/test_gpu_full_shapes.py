@@ -138,3 +138,35 @@ def test_full_width_recompute_prefill_and_migration_vs_oracle():
         assert (pool_gpu[:, :, ~used] == 0x7FC1).all()
     finally:
         P.close()
+
+
+def test_full_vocab_logits_and_argmax_vs_oracle():
+    """S11 at the real width (Table 2 'Logits Calculation'; reading A12: V = 128,256 with the
+    Llama shapes, A14 for the argmax): a 1-layer stage with final norm + lm_head, one decode step of 64 rows."""
+    from tests import gpu_helpers as gh
+    shape = _sub(synth.LLAMA70B, 1)
+    assert shape.vocab == 128256
+    ctx = np.minimum(synth.cfg2_contexts(0), 600).astype(np.int32)      # the tail does not depend on the context
+    B = len(ctx)
+    rng = np.random.default_rng(1)
+    pb = synth.paged_batch(rng, ctx, extra_tokens=2)
+    P = gh.Problem(shape, 0, n_pages=pb.n_pages_pool, max_tokens=B, max_seqs=B, max_blocks=pb.max_blocks,
+                   pool_fill="random", with_edge=True)
+    try:
+        x = synth.bits(synth.hidden_rows(B, shape.hidden, 3))
+        eb = {k: synth.bits(v) for k, v in P.edge_cpu.items()}
+        pool = P.pool_cpu.copy()
+        y, _ = hp.run_oracle_decode(F32, shape, P.wb, pool, ctx, pb.block_tables, x)
+        wl, wa, wm = F32.logits(hp.odims(shape), y, eb["final_norm"], eb["lm_head"])
+        _, lg, am = P.decode(ctx, pb.block_tables, x, logits=True)
+        # (i) the argmax kernel is bit-exact on the GPU's own fp32 logits, ties -> lowest index
+        assert np.array_equal(am, np.argmax(lg, axis=1).astype(np.int32))
+        # (ii) ids equal the oracle's wherever the oracle's top-2 margin exceeds 8x the measured logit error
+        lerr = float(np.abs(lg - wl).max())
+        safe = wm > 8 * lerr
+        print(f"V={shape.vocab}: logit max abs err {lerr:.3e} (logit scale {float(np.abs(wl).max()):.2f}); "
+              f"rows over margin {int(safe.sum())}/{B}; argmax equal on {int((am == wa).sum())}/{B} rows")
+        assert np.array_equal(am[safe], wa[safe])
+        assert hp.rel_err_rows(lg, wl) < 2e-2
+    finally:
+        P.close()
