@@ -9,11 +9,13 @@
 // at (b,h) boundaries into segments; each segment yields one partial (m, l, O[G x d]) in slot `worker + pair`,
 // which is unique and monotone along the flattened order.  decode_merge combines the segments of a pair.
 //
-// A warp is an independent pipeline: cp.async 16-byte copies of whole pages into its private XOR-swizzled smem
-// ring (no block barrier anywhere), ldmatrix + mma.sync m16n8k16 with the G query heads of the group as the M rows
+// A warp is an independent pipeline: one lane issues the TMA loads of whole pages (2-D boxes of 16 rows x 64
+// columns, SWIZZLE_128B) into the warp's private smem ring, completion on the warp's own mbarriers (no block
+// barrier anywhere), ldmatrix + mma.sync m16n8k16 with the G query heads of the group as the M rows
 // (each K/V byte feeds all G heads), online softmax in fp32 with quad shuffles.  The warp that owns a sequence's
 // last page writes the new token's K/V (bf16, post-RoPE, from qkv_post) into that page — in smem for its own use
 // and in the pool — which is the fused append of step S5.
+#include <cuda.h>
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 #include <stdlib.h>
@@ -27,12 +29,16 @@ namespace ss {
 #define SS_DA_WARPS 4
 #endif
 #ifndef SS_DA_STAGES
-#define SS_DA_STAGES 3
+#define SS_DA_STAGES 2
 #endif
+// Measured (same-box A/B, cfg-2 / cfg-3 step): the kernel is bound by the latency of each warp's dependent chain
+// (QK mma -> softmax -> PV mma per page), not by bytes in flight or by the load instructions: 8 warps/SM with 3-stage
+// rings 7.57 / 5.34 ms; 12 warps/SM with 2-stage rings (4 warps x 3 CTAs, register-limited) 7.43 / 5.21 ms; fewer,
+// deeper rings (7x4, 6x4, 5x5) slower.
 constexpr int DA_WARPS = SS_DA_WARPS;    // independent warp pipelines per CTA
 constexpr int DA_STAGES = SS_DA_STAGES;  // pages (K 4 KB + V 4 KB at d = 128) per warp ring
 int decode_attn_warps_per_cta() { return DA_WARPS; }
-int decode_attn_default_ctas_per_sm() { return (int)((size_t)220 * 1024 / ((size_t)DA_WARPS * DA_STAGES * 2 * 16 * 128 * 2)); }
+int decode_attn_default_ctas_per_sm() { return (int)((size_t)226 * 1024 / (1024 + 1024 + (size_t)DA_WARPS * DA_STAGES * 2 * 16 * 128 * 2)); }
 
 // ---- plan: prefix sum of pages per sequence --------------------------------------------------------------------
 __global__ void decode_plan_kernel(const CallArgs *__restrict__ args, int batch, int n_kv, int n_workers,
@@ -61,8 +67,15 @@ struct Cursor {
   int b, h, pg, pages_b;
 };
 
+// smem image of one K (or V) page as TMA writes it: D/64 halves of [16 rows][128 B], SWIZZLE_128B inside each half
+// (16-byte chunk c of row r sits at chunk c ^ (r & 7)): byte offset of chunk `ch` (0 .. D/8-1) of row `row`
+__device__ __forceinline__ int page_off(int row, int ch) {
+  return (ch >> 3) * 2048 + row * 128 + (((ch & 7) ^ (row & 7)) << 4);
+}
+
 template <int D>
-__global__ void __launch_bounds__(DA_WARPS * 32) decode_attn_kernel(const DecodeAttnParams p) {
+__global__ void __launch_bounds__(DA_WARPS * 32)
+decode_attn_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodeAttnParams p) {
   pdl_launch_dependents();
   pdl_wait();
   constexpr int ROW_BYTES = D * 2;
@@ -70,10 +83,20 @@ __global__ void __launch_bounds__(DA_WARPS * 32) decode_attn_kernel(const Decode
   constexpr int PAGE_BYTES = 16 * ROW_BYTES;   // one K (or V) page of one head
   constexpr int KSTEPS = D / 16;
   constexpr int NT = D / 8;                    // output n-tiles
-  extern __shared__ __align__(128) uint8_t smem[];
+  extern __shared__ uint8_t smem_raw[];
+  __shared__ uint64_t page_bar[DA_WARPS][DA_STAGES];  // one mbarrier per ring slot of each warp
+  uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);  // swizzle atoms are 1 KB
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int w = blockIdx.x * DA_WARPS + warp;
   uint8_t *ring = smem + (size_t)warp * DA_STAGES * 2 * PAGE_BYTES;
+  uint64_t *bars = page_bar[warp];
+  if (lane == 0) {
+#pragma unroll
+    for (int i = 0; i < DA_STAGES; ++i) mbar_init(&bars[i], 1);
+    mbar_fence_init();
+    tma_prefetch_desc(&kv_map);
+  }
+  __syncwarp();
 
   const int total = p.plan.meta[0], quota = p.plan.meta[1];
   const int g0 = w * quota;
@@ -113,20 +136,22 @@ __global__ void __launch_bounds__(DA_WARPS * 32) decode_attn_kernel(const Decode
       }
     }
   };
+  // one page = K tile + V tile of one (page, kv head): D/64 TMA boxes of {64 columns, 16 rows} each, issued by one
+  // lane; the pool of this layer is one 2-D tensor [K rows | V rows] x D (rows = (page * n_kv + head) * 16 + slot)
+  const uint64_t pol = l2_policy_evict_first();  // every K/V byte is read once per step
+  const int v_row0 = p.n_pages * n_kv * 16;
   auto issue_load = [&](const Cursor &c, int slot) {
-    const int page = bt[(size_t)c.b * max_blocks + c.pg];
-    const size_t off = ((size_t)page * n_kv + c.h) * 16 * D;
-    const uint8_t *ks = (const uint8_t *)(kpool + off);
-    const uint8_t *vs = (const uint8_t *)(vpool + off);
-    uint8_t *kd = ring + (size_t)slot * 2 * PAGE_BYTES;
-    uint8_t *vd = kd + PAGE_BYTES;
+    if (lane == 0) {
+      const int page = bt[(size_t)c.b * max_blocks + c.pg];
+      const int row = (page * n_kv + c.h) * 16;
+      uint8_t *kd = ring + (size_t)slot * 2 * PAGE_BYTES;
+      fence_proxy_async();  // the slot's previous contents were read through the generic proxy (ldmatrix)
+      mbar_expect_tx(&bars[slot], 2 * PAGE_BYTES);
 #pragma unroll
-    for (int i = 0; i < PAGE_BYTES / 16 / 32; ++i) {
-      const int idx = i * 32 + lane;
-      const int r = idx / CHUNKS, ch = idx % CHUNKS;
-      const int dst = r * ROW_BYTES + ((ch ^ (r & 7)) << 4);
-      cp_async16(kd + dst, ks + (size_t)idx * 16);
-      cp_async16(vd + dst, vs + (size_t)idx * 16);
+      for (int hf = 0; hf < D / 64; ++hf) {
+        tma_load_2d(kd + hf * 2048, &kv_map, &bars[slot], hf * 64, row, pol);
+        tma_load_2d(kd + PAGE_BYTES + hf * 2048, &kv_map, &bars[slot], hf * 64, v_row0 + row, pol);
+      }
     }
   };
 
@@ -137,7 +162,6 @@ __global__ void __launch_bounds__(DA_WARPS * 32) decode_attn_kernel(const Decode
       issue_load(lc, i);
       advance(lc);
     }
-    cp_async_commit();
   }
 
   const float sl2 = 1.4426950408889634f / sqrtf((float)D);  // log2(e) / sqrt(d)
@@ -148,13 +172,11 @@ __global__ void __launch_bounds__(DA_WARPS * 32) decode_attn_kernel(const Decode
   const int qrow = lane >> 2, qcol = (lane & 3) * 2;
 
   for (int i = 0; i < n; ++i) {
-    if (i + DA_STAGES - 1 < n) {
+    if (i + DA_STAGES - 1 < n) {  // the slot was drained in iteration i - 1 (its trailing __syncwarp)
       issue_load(lc, (i + DA_STAGES - 1) % DA_STAGES);
       advance(lc);
     }
-    cp_async_commit();
-    cp_async_wait<DA_STAGES - 1>();
-    __syncwarp();
+    mbar_wait(&bars[i % DA_STAGES], (uint32_t)(i / DA_STAGES) & 1u);
 
     const int ctx = args->ctx[cc.b];
     if (!seg_open) {
@@ -189,7 +211,7 @@ __global__ void __launch_bounds__(DA_WARPS * 32) decode_attn_kernel(const Decode
       for (int idx = lane; idx < (p.append ? 2 * CHUNKS : 0); idx += 32) {
         const int isv = idx / CHUNKS, ch = idx % CHUNKS;
         const uint4 val = *reinterpret_cast<const uint4 *>(src + (size_t)isv * n_kv * D * 2 + ch * 16);
-        uint8_t *sdst = (isv ? vsm : ksm) + r * ROW_BYTES + ((ch ^ (r & 7)) << 4);
+        uint8_t *sdst = (isv ? vsm : ksm) + page_off(r, ch);
         *reinterpret_cast<uint4 *>(sdst) = val;
         uint8_t *gdst = (uint8_t *)(isv ? p.vpool : p.kpool) + goff + ch * 16;
         *reinterpret_cast<uint4 *>(gdst) = val;
@@ -198,7 +220,7 @@ __global__ void __launch_bounds__(DA_WARPS * 32) decode_attn_kernel(const Decode
       // NaN) cannot reach the output; their scores are overwritten with -inf below
       for (int idx = lane; idx < (15 - r) * CHUNKS; idx += 32) {
         const int rr2 = r + 1 + idx / CHUNKS, ch = idx % CHUNKS;
-        *reinterpret_cast<uint4 *>(vsm + rr2 * ROW_BYTES + (ch << 4)) = make_uint4(0u, 0u, 0u, 0u);
+        *reinterpret_cast<uint4 *>(vsm + page_off(rr2, ch)) = make_uint4(0u, 0u, 0u, 0u);
       }
       __syncwarp();
     }
@@ -208,12 +230,12 @@ __global__ void __launch_bounds__(DA_WARPS * 32) decode_attn_kernel(const Decode
     {
       const int mtx = lane >> 3, rr = lane & 7;
       const int tok = (mtx >> 1) * 8 + rr;
-      const uint32_t kbase = smem_u32(ksm) + tok * ROW_BYTES;
+      const uint32_t kbase = smem_u32(ksm);
 #pragma unroll
       for (int ks = 0; ks < KSTEPS; ++ks) {
         const int ch = ks * 2 + (mtx & 1);
         uint32_t kb[4];
-        ldmatrix_x4(kb, kbase + ((ch ^ (tok & 7)) << 4));
+        ldmatrix_x4(kb, kbase + page_off(tok, ch));
         mma_bf16_16816(s0, qf[ks], kb[0], kb[1]);
         mma_bf16_16816(s1, qf[ks], kb[2], kb[3]);
       }
@@ -258,12 +280,12 @@ __global__ void __launch_bounds__(DA_WARPS * 32) decode_attn_kernel(const Decode
     {
       const int mtx = lane >> 3, rr = lane & 7;
       const int tok = (mtx & 1) * 8 + rr;
-      const uint32_t vbase = smem_u32(vsm) + tok * ROW_BYTES;
+      const uint32_t vbase = smem_u32(vsm);
 #pragma unroll
       for (int t2 = 0; t2 < NT / 2; ++t2) {
         const int ch = t2 * 2 + (mtx >> 1);
         uint32_t vb[4];
-        ldmatrix_x4_trans(vb, vbase + ((ch ^ (tok & 7)) << 4));
+        ldmatrix_x4_trans(vb, vbase + page_off(tok, ch));
         float *oa = o[2 * t2], *ob = o[2 * t2 + 1];
         oa[0] *= a0; oa[1] *= a0; oa[2] *= a1; oa[3] *= a1;
         ob[0] *= a0; ob[1] *= a0; ob[2] *= a1; ob[3] *= a1;
@@ -340,7 +362,7 @@ __global__ void __launch_bounds__(MERGE_THREADS) decode_merge_kernel(const Decod
   }
 }
 
-static size_t decode_smem(int d) { return (size_t)DA_WARPS * DA_STAGES * 2 * 16 * d * 2; }
+static size_t decode_smem(int d) { return 1024 + (size_t)DA_WARPS * DA_STAGES * 2 * 16 * d * 2; }  // + alignment slack
 
 cudaError_t attn_init() {
   cudaError_t e =
@@ -353,9 +375,9 @@ cudaError_t attn_init() {
 cudaError_t launch_decode_attn(const DecodeAttnParams &p, cudaStream_t s) {
   const int ctas = p.n_workers / DA_WARPS;
   if (p.d == 128)
-    return launch_pdl(decode_attn_kernel<128>, dim3(ctas), dim3(DA_WARPS * 32), decode_smem(128), s, p);
+    return launch_pdl(decode_attn_kernel<128>, dim3(ctas), dim3(DA_WARPS * 32), decode_smem(128), s, *p.kv_map, p);
   else
-    return launch_pdl(decode_attn_kernel<64>, dim3(ctas), dim3(DA_WARPS * 32), decode_smem(64), s, p);
+    return launch_pdl(decode_attn_kernel<64>, dim3(ctas), dim3(DA_WARPS * 32), decode_smem(64), s, *p.kv_map, p);
 }
 
 cudaError_t launch_decode_merge(const DecodeAttnParams &p, cudaStream_t s) {

@@ -144,6 +144,7 @@ struct DecodeAttnParams {
   const void *q;             // bf16 [B,Hq]
   const void *kv_new;        // bf16 [B,2*Hkv]
   void *kpool, *vpool;       // this layer
+  const CUtensorMap *kv_map; // this layer's pool as a 2-D bf16 tensor [2 * n_pages * n_kv * 16 rows, d], box {64, 16}
   int n_pages;
   int batch, n_q, n_kv, d;
   DecodePlan plan;

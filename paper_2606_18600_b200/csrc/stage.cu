@@ -102,6 +102,7 @@ static Carve carve(const ss_model_dims *d) {
 
 struct LayerMaps {
   CUtensorMap wq, wk, wv, wo, wg, wu, wd;
+  CUtensorMap kv;  // this layer's K and V pools: [2 * num_pages * n_kv * 16 rows, head_dim], box {64, 16}
 };
 
 struct Graph {
@@ -322,6 +323,8 @@ int ss_stage_create(ss_stage **out, const ss_model_dims *dims, int l0, int l1, c
     rc |= make_tmap_bf16_2d(&m.wg, w.w_gate, F, H, GEMM_BM, true);
     rc |= make_tmap_bf16_2d(&m.wu, w.w_up, F, H, GEMM_BM, true);
     rc |= make_tmap_bf16_2d(&m.wd, w.w_down, H, F, GEMM_BM, true);
+    rc |= make_tmap_bf16_2d(&m.kv, st->kpool(l), (uint64_t)2 * st->num_pages * dims->n_kv_heads * 16,
+                            (uint64_t)dims->head_dim, 16, true);
   }
   if (rc == 0 && edge && edge->lm_head)
     rc |= make_tmap_bf16_2d(&st->lm_map, edge->lm_head, (uint64_t)dims->vocab, H, GEMM_BM, true);
@@ -479,6 +482,7 @@ static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T,
       ap.q = st->at<void>(c.q);
       ap.kv_new = st->at<void>(c.kv_new);
       ap.kpool = st->kpool(l); ap.vpool = st->vpool(l);
+      ap.kv_map = &st->maps[l].kv;
       ap.n_pages = st->num_pages;
       ap.batch = decode ? n_seqs : n_dec; ap.n_q = d.n_q_heads; ap.n_kv = d.n_kv_heads; ap.d = dh;
       ap.plan = dplan;
