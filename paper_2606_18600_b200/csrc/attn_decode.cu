@@ -38,7 +38,7 @@ namespace ss {
 constexpr int DA_WARPS = SS_DA_WARPS;    // independent warp pipelines per CTA
 constexpr int DA_STAGES = SS_DA_STAGES;  // pages (K 4 KB + V 4 KB at d = 128) per warp ring
 int decode_attn_warps_per_cta() { return DA_WARPS; }
-int decode_attn_default_ctas_per_sm() { return (int)((size_t)226 * 1024 / (1024 + 1024 + (size_t)DA_WARPS * DA_STAGES * 2 * 16 * 128 * 2)); }
+int decode_attn_default_ctas_per_sm() { return (int)((size_t)228 * 1024 / (1024 + (size_t)DA_WARPS * DA_STAGES * (2 * 16 * 128 * 2 + 8))); }
 
 // ---- plan: prefix sum of pages per sequence --------------------------------------------------------------------
 __global__ void decode_plan_kernel(const CallArgs *__restrict__ args, int batch, int n_kv, int n_workers,
@@ -73,7 +73,10 @@ __device__ __forceinline__ int page_off(int row, int ch) {
   return (ch >> 3) * 2048 + row * 128 + (((ch & 7) ^ (row & 7)) << 4);
 }
 
-template <int D>
+// HI: the GQA group has more than 8 query heads, i.e. rows 8-15 of the 16-row MMA tile are live too.  The paper's
+// models have G = 8: with HI = false the accumulators, query fragments and softmax statistics of rows 8-15 do not
+// exist (about 45 registers fewer: more resident warps, which is what bounds this kernel).
+template <int D, bool HI>
 __global__ void __launch_bounds__(DA_WARPS * 32)
 decode_attn_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodeAttnParams p) {
   pdl_launch_dependents();
@@ -83,13 +86,12 @@ decode_attn_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodeAttnP
   constexpr int PAGE_BYTES = 16 * ROW_BYTES;   // one K (or V) page of one head
   constexpr int KSTEPS = D / 16;
   constexpr int NT = D / 8;                    // output n-tiles
-  extern __shared__ uint8_t smem_raw[];
-  __shared__ uint64_t page_bar[DA_WARPS][DA_STAGES];  // one mbarrier per ring slot of each warp
-  uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);  // swizzle atoms are 1 KB
+  extern __shared__ __align__(1024) uint8_t smem[];   // swizzle atoms are 1 KB: the rings start 1 KB-aligned
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int w = blockIdx.x * DA_WARPS + warp;
   uint8_t *ring = smem + (size_t)warp * DA_STAGES * 2 * PAGE_BYTES;
-  uint64_t *bars = page_bar[warp];
+  // one mbarrier per ring slot of each warp, behind the rings
+  uint64_t *bars = (uint64_t *)(smem + (size_t)DA_WARPS * DA_STAGES * 2 * PAGE_BYTES) + warp * DA_STAGES;
   if (lane == 0) {
 #pragma unroll
     for (int i = 0; i < DA_STAGES; ++i) mbar_init(&bars[i], 1);
@@ -165,9 +167,10 @@ decode_attn_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodeAttnP
   }
 
   const float sl2 = 1.4426950408889634f / sqrtf((float)D);  // log2(e) / sqrt(d)
-  uint32_t qf[KSTEPS][4];
-  float o[NT][4];
-  float m_run[2], l_run[2];
+  constexpr int RW = HI ? 2 : 1;   // live 8-row groups
+  uint32_t qf[KSTEPS][2 * RW];     // [ks][rowgroup * 2 + khalf]
+  float o[NT][2 * RW];             // [n-tile][rowgroup * 2 + col]
+  float m_run[RW], l_run[RW];
   bool seg_open = false;
   const int qrow = lane >> 2, qcol = (lane & 3) * 2;
 
@@ -186,14 +189,21 @@ decode_attn_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodeAttnP
       for (int ks = 0; ks < KSTEPS; ++ks) {
         const int c = ks * 16 + qcol;
         qf[ks][0] = (qrow < G) ? *reinterpret_cast<const uint32_t *>(qb + (size_t)qrow * D + c) : 0u;
-        qf[ks][2] = (qrow < G) ? *reinterpret_cast<const uint32_t *>(qb + (size_t)qrow * D + c + 8) : 0u;
-        qf[ks][1] = (qrow + 8 < G) ? *reinterpret_cast<const uint32_t *>(qb + (size_t)(qrow + 8) * D + c) : 0u;
-        qf[ks][3] = (qrow + 8 < G) ? *reinterpret_cast<const uint32_t *>(qb + (size_t)(qrow + 8) * D + c + 8) : 0u;
+        qf[ks][1] = (qrow < G) ? *reinterpret_cast<const uint32_t *>(qb + (size_t)qrow * D + c + 8) : 0u;
+        if (HI) {
+          qf[ks][2] = (qrow + 8 < G) ? *reinterpret_cast<const uint32_t *>(qb + (size_t)(qrow + 8) * D + c) : 0u;
+          qf[ks][3] = (qrow + 8 < G) ? *reinterpret_cast<const uint32_t *>(qb + (size_t)(qrow + 8) * D + c + 8) : 0u;
+        }
       }
 #pragma unroll
-      for (int t = 0; t < NT; ++t) o[t][0] = o[t][1] = o[t][2] = o[t][3] = 0.f;
-      m_run[0] = m_run[1] = -INFINITY;
-      l_run[0] = l_run[1] = 0.f;
+      for (int t = 0; t < NT; ++t)
+#pragma unroll
+        for (int e = 0; e < 2 * RW; ++e) o[t][e] = 0.f;
+#pragma unroll
+      for (int r = 0; r < RW; ++r) {
+        m_run[r] = -INFINITY;
+        l_run[r] = 0.f;
+      }
       seg_open = true;
     }
 
@@ -225,8 +235,20 @@ decode_attn_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodeAttnP
       __syncwarp();
     }
 
-    // ---- S = Q K^T for the 16 tokens of the page: two n-tiles of 8 tokens
-    float s0[4] = {0.f, 0.f, 0.f, 0.f}, s1[4] = {0.f, 0.f, 0.f, 0.f};
+    // ---- S = Q K^T for the 16 tokens of the page: two n-tiles of 8 tokens; s[tile][rowgroup * 2 + col]
+    float sc[2][2 * RW];
+#pragma unroll
+    for (int e = 0; e < 2 * RW; ++e) sc[0][e] = sc[1][e] = 0.f;
+    auto mma_rows = [&](float (&d)[2 * RW], const uint32_t (&a)[2 * RW], uint32_t b0, uint32_t b1) {
+      if constexpr (HI) {
+        const uint32_t af[4] = {a[0], a[2], a[1], a[3]};  // PTX order: (row, k-lo), (row+8, k-lo), (row, k-hi), (row+8, k-hi)
+        float df[4] = {d[0], d[1], d[2], d[3]};
+        mma_bf16_16816(df, af, b0, b1);
+        d[0] = df[0]; d[1] = df[1]; d[2] = df[2]; d[3] = df[3];
+      } else {
+        mma_bf16_16816_lo(d, a[0], a[1], b0, b1);
+      }
+    };
     {
       const int mtx = lane >> 3, rr = lane & 7;
       const int tok = (mtx >> 1) * 8 + rr;
@@ -236,46 +258,40 @@ decode_attn_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodeAttnP
         const int ch = ks * 2 + (mtx & 1);
         uint32_t kb[4];
         ldmatrix_x4(kb, kbase + page_off(tok, ch));
-        mma_bf16_16816(s0, qf[ks], kb[0], kb[1]);
-        mma_bf16_16816(s1, qf[ks], kb[2], kb[3]);
+        mma_rows(sc[0], qf[ks], kb[0], kb[1]);
+        mma_rows(sc[1], qf[ks], kb[2], kb[3]);
       }
     }
     // mask tokens past the sequence end (only on the last page)
     if (n_valid < 16) {
-      if (qcol >= n_valid) s0[0] = s0[2] = -INFINITY;
-      if (qcol + 1 >= n_valid) s0[1] = s0[3] = -INFINITY;
-      if (qcol + 8 >= n_valid) s1[0] = s1[2] = -INFINITY;
-      if (qcol + 9 >= n_valid) s1[1] = s1[3] = -INFINITY;
+#pragma unroll
+      for (int r = 0; r < RW; ++r) {
+        if (qcol >= n_valid) sc[0][2 * r] = -INFINITY;
+        if (qcol + 1 >= n_valid) sc[0][2 * r + 1] = -INFINITY;
+        if (qcol + 8 >= n_valid) sc[1][2 * r] = -INFINITY;
+        if (qcol + 9 >= n_valid) sc[1][2 * r + 1] = -INFINITY;
+      }
     }
-    // ---- online softmax (rows qrow and qrow+8), statistics across the quad
-    float mx0 = fmaxf(fmaxf(s0[0], s0[1]), fmaxf(s1[0], s1[1]));
-    float mx1 = fmaxf(fmaxf(s0[2], s0[3]), fmaxf(s1[2], s1[3]));
-    mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 1));
-    mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 2));
-    mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 1));
-    mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 2));
-    const float mn0 = fmaxf(m_run[0], mx0), mn1 = fmaxf(m_run[1], mx1);
-    const float a0 = exp2f((m_run[0] - mn0) * sl2), a1 = exp2f((m_run[1] - mn1) * sl2);
-    m_run[0] = mn0;
-    m_run[1] = mn1;
-    float pr0[4], pr1[4];
-    pr0[0] = exp2f((s0[0] - mn0) * sl2); pr0[1] = exp2f((s0[1] - mn0) * sl2);
-    pr0[2] = exp2f((s0[2] - mn1) * sl2); pr0[3] = exp2f((s0[3] - mn1) * sl2);
-    pr1[0] = exp2f((s1[0] - mn0) * sl2); pr1[1] = exp2f((s1[1] - mn0) * sl2);
-    pr1[2] = exp2f((s1[2] - mn1) * sl2); pr1[3] = exp2f((s1[3] - mn1) * sl2);
-    float rs0 = pr0[0] + pr0[1] + pr1[0] + pr1[1];
-    float rs1 = pr0[2] + pr0[3] + pr1[2] + pr1[3];
-    rs0 += __shfl_xor_sync(0xffffffffu, rs0, 1);
-    rs0 += __shfl_xor_sync(0xffffffffu, rs0, 2);
-    rs1 += __shfl_xor_sync(0xffffffffu, rs1, 1);
-    rs1 += __shfl_xor_sync(0xffffffffu, rs1, 2);
-    l_run[0] = l_run[0] * a0 + rs0;
-    l_run[1] = l_run[1] * a1 + rs1;
-    uint32_t pa[4];
-    pa[0] = pack_bf16x2(pr0[0], pr0[1]);
-    pa[1] = pack_bf16x2(pr0[2], pr0[3]);
-    pa[2] = pack_bf16x2(pr1[0], pr1[1]);
-    pa[3] = pack_bf16x2(pr1[2], pr1[3]);
+    // ---- online softmax per live row group, statistics across the quad
+    float alpha[RW];
+    uint32_t pa[2 * RW];  // [rowgroup * 2 + khalf] : P as the A fragment of the PV product (k = the 16 tokens)
+#pragma unroll
+    for (int r = 0; r < RW; ++r) {
+      float mx = fmaxf(fmaxf(sc[0][2 * r], sc[0][2 * r + 1]), fmaxf(sc[1][2 * r], sc[1][2 * r + 1]));
+      mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 1));
+      mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 2));
+      const float mn = fmaxf(m_run[r], mx);
+      alpha[r] = exp2f((m_run[r] - mn) * sl2);
+      m_run[r] = mn;
+      const float p00 = exp2f((sc[0][2 * r] - mn) * sl2), p01 = exp2f((sc[0][2 * r + 1] - mn) * sl2);
+      const float p10 = exp2f((sc[1][2 * r] - mn) * sl2), p11 = exp2f((sc[1][2 * r + 1] - mn) * sl2);
+      float rs = p00 + p01 + p10 + p11;
+      rs += __shfl_xor_sync(0xffffffffu, rs, 1);
+      rs += __shfl_xor_sync(0xffffffffu, rs, 2);
+      l_run[r] = l_run[r] * alpha[r] + rs;
+      pa[2 * r] = pack_bf16x2(p00, p01);      // tokens 0-7 (k-lo)
+      pa[2 * r + 1] = pack_bf16x2(p10, p11);  // tokens 8-15 (k-hi)
+    }
     // ---- O = O * alpha + P V
     {
       const int mtx = lane >> 3, rr = lane & 7;
@@ -286,11 +302,13 @@ decode_attn_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodeAttnP
         const int ch = t2 * 2 + (mtx >> 1);
         uint32_t vb[4];
         ldmatrix_x4_trans(vb, vbase + page_off(tok, ch));
-        float *oa = o[2 * t2], *ob = o[2 * t2 + 1];
-        oa[0] *= a0; oa[1] *= a0; oa[2] *= a1; oa[3] *= a1;
-        ob[0] *= a0; ob[1] *= a0; ob[2] *= a1; ob[3] *= a1;
-        mma_bf16_16816(o[2 * t2], pa, vb[0], vb[1]);
-        mma_bf16_16816(o[2 * t2 + 1], pa, vb[2], vb[3]);
+#pragma unroll
+        for (int r = 0; r < RW; ++r) {
+          o[2 * t2][2 * r] *= alpha[r]; o[2 * t2][2 * r + 1] *= alpha[r];
+          o[2 * t2 + 1][2 * r] *= alpha[r]; o[2 * t2 + 1][2 * r + 1] *= alpha[r];
+        }
+        mma_rows(o[2 * t2], pa, vb[0], vb[1]);
+        mma_rows(o[2 * t2 + 1], pa, vb[2], vb[3]);
       }
     }
 
@@ -306,11 +324,13 @@ decode_attn_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodeAttnP
           *reinterpret_cast<float2 *>(po + (size_t)qrow * D + t * 8 + qcol) = make_float2(o[t][0], o[t][1]);
         if ((lane & 3) == 0) *reinterpret_cast<float2 *>(pml + qrow * 2) = make_float2(m_run[0], l_run[0]);
       }
-      if (qrow + 8 < G) {
+      if constexpr (HI) {
+        if (qrow + 8 < G) {
 #pragma unroll
-        for (int t = 0; t < NT; ++t)
-          *reinterpret_cast<float2 *>(po + (size_t)(qrow + 8) * D + t * 8 + qcol) = make_float2(o[t][2], o[t][3]);
-        if ((lane & 3) == 0) *reinterpret_cast<float2 *>(pml + (qrow + 8) * 2) = make_float2(m_run[1], l_run[1]);
+          for (int t = 0; t < NT; ++t)
+            *reinterpret_cast<float2 *>(po + (size_t)(qrow + 8) * D + t * 8 + qcol) = make_float2(o[t][2], o[t][3]);
+          if ((lane & 3) == 0) *reinterpret_cast<float2 *>(pml + (qrow + 8) * 2) = make_float2(m_run[1], l_run[1]);
+        }
       }
       seg_open = false;
     }
@@ -362,22 +382,35 @@ __global__ void __launch_bounds__(MERGE_THREADS) decode_merge_kernel(const Decod
   }
 }
 
-static size_t decode_smem(int d) { return 1024 + (size_t)DA_WARPS * DA_STAGES * 2 * 16 * d * 2; }  // + alignment slack
+static size_t decode_smem(int d) { return (size_t)DA_WARPS * DA_STAGES * (2 * 16 * d * 2 + 8); }  // rings + mbarriers
+
+template <int D, bool HI>
+static cudaError_t set_smem() {
+  cudaError_t e = cudaFuncSetAttribute(decode_attn_kernel<D, HI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       (int)decode_smem(D));
+  if (e != cudaSuccess) return e;
+  // several CTAs per SM are the point of this kernel: ask for the largest shared-memory carve-out
+  return cudaFuncSetAttribute(decode_attn_kernel<D, HI>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                              cudaSharedmemCarveoutMaxShared);
+}
 
 cudaError_t attn_init() {
-  cudaError_t e =
-      cudaFuncSetAttribute(decode_attn_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)decode_smem(128));
-  if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(decode_attn_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                              (int)decode_smem(64));
+  cudaError_t e;
+  if ((e = set_smem<128, false>()) != cudaSuccess) return e;
+  if ((e = set_smem<128, true>()) != cudaSuccess) return e;
+  if ((e = set_smem<64, false>()) != cudaSuccess) return e;
+  return set_smem<64, true>();
 }
 
 cudaError_t launch_decode_attn(const DecodeAttnParams &p, cudaStream_t s) {
   const int ctas = p.n_workers / DA_WARPS;
+  const bool hi = p.n_q / p.n_kv > 8;
+  const dim3 g(ctas), b(DA_WARPS * 32);
   if (p.d == 128)
-    return launch_pdl(decode_attn_kernel<128>, dim3(ctas), dim3(DA_WARPS * 32), decode_smem(128), s, *p.kv_map, p);
-  else
-    return launch_pdl(decode_attn_kernel<64>, dim3(ctas), dim3(DA_WARPS * 32), decode_smem(64), s, *p.kv_map, p);
+    return hi ? launch_pdl(decode_attn_kernel<128, true>, g, b, decode_smem(128), s, *p.kv_map, p)
+              : launch_pdl(decode_attn_kernel<128, false>, g, b, decode_smem(128), s, *p.kv_map, p);
+  return hi ? launch_pdl(decode_attn_kernel<64, true>, g, b, decode_smem(64), s, *p.kv_map, p)
+            : launch_pdl(decode_attn_kernel<64, false>, g, b, decode_smem(64), s, *p.kv_map, p);
 }
 
 cudaError_t launch_decode_merge(const DecodeAttnParams &p, cudaStream_t s) {

@@ -221,4 +221,14 @@ __device__ __forceinline__ void mma_bf16_16816(float (&d)[4], const uint32_t (&a
       : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
 }
 
+// The same MMA when only rows 0-7 of the 16-row A tile are live (a[1] = a[3] = 0, C rows 8-15 = 0): the results
+// of rows 8-15 go to two scratch registers, so the caller keeps 2 accumulator registers per tile instead of 4.
+__device__ __forceinline__ void mma_bf16_16816_lo(float (&d)[2], uint32_t a0, uint32_t a2, uint32_t b0, uint32_t b1) {
+  float j2, j3;
+  asm volatile(
+      "mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%10,%10};"
+      : "+f"(d[0]), "+f"(d[1]), "=f"(j2), "=f"(j3)
+      : "r"(a0), "r"(0u), "r"(a2), "r"(0u), "r"(b0), "r"(b1), "f"(0.f));
+}
+
 }  // namespace ss
