@@ -48,5 +48,20 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     return LIB
 
 
+PLACE_LIB = HERE / "libshuntplace.so"
+
+
+def build_placement(force: bool = False) -> Path:
+    """libshuntplace.so: the host-only estimator + placement optimizer (csrc/placement.cpp), plain g++."""
+    src = CSRC / "placement.cpp"
+    hdr = HERE.parent / "include" / "shuntplace.h"
+    if not force and PLACE_LIB.exists() and PLACE_LIB.stat().st_mtime >= max(src.stat().st_mtime, hdr.stat().st_mtime):
+        return PLACE_LIB
+    cmd = [os.environ.get("CXX", "g++"), "-O2", "-std=c++17", "-fPIC", "-shared", "-Wall", str(src), "-o", str(PLACE_LIB)]
+    subprocess.run(cmd, check=True)
+    return PLACE_LIB
+
+
 if __name__ == "__main__":
+    print(build_placement(force=True))
     print(build(force=True, verbose=True))
