@@ -182,6 +182,16 @@ int ss_stage_decode(ss_stage *st, int batch,
 /* Number of kernels the stage launched (directly or inside replayed graphs) since creation. */
 int64_t ss_stage_launch_count(const ss_stage *st);
 
+/* Migration by KV transfer (the alternative to recomputation the paper measures; SURVEY
+ * 8(f) NEXT-4).  ss_kv_export gathers the n pages `page_ids_dev[0..n)` (DEVICE int32) of every layer of the stage into
+ * the caller's contiguous DEVICE buffer, laid out [layer][K/V][i][h_kv][16][d] bf16 (n * ss_kv_page_bytes() bytes) —
+ * the message a GPU-to-GPU copy carries; ss_kv_import scatters such a buffer into the pages `page_ids_dev` of this
+ * stage's pool (ids chosen by the importing side, e.g. from ss_kv_alloc).  Byte-exact copies, enqueued on the stage's
+ * stream.  Errors: SS_ERR_INVALID_ARG (null / n <= 0), SS_ERR_UNSUPPORTED (buffer not 16-byte aligned),
+ * SS_ERR_CAPACITY (buffer too small).  Page ids out of range are undefined behaviour. */
+int ss_kv_export(ss_stage *st, int n, const int32_t *page_ids_dev, void *buf_dev, size_t buf_bytes);
+int ss_kv_import(ss_stage *st, int n, const int32_t *page_ids_dev, const void *buf_dev, size_t buf_bytes);
+
 /* ---- op-level entry points (the same kernels the stage uses; for per-kernel parity tests and profiling) -- */
 
 /* Scratch (dev, 256-byte aligned) the op-level GEMMs need for the stream-K fix-up: >= this many bytes, whose first

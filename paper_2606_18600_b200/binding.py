@@ -24,7 +24,7 @@ EXPORTS = ["ss_stage_workspace_bytes", "ss_kv_page_bytes", "ss_stage_create", "s
            "ss_stage_decode",
            "ss_stage_launch_count", "ss_op_gemm_scratch_bytes", "ss_op_gemm_bf16", "ss_op_gemm_swiglu_bf16", "ss_strerror",
            "ss_last_cuda_error", "ss_version", "ss_debug_buffer", "ss_pool_create", "ss_pool_destroy",
-           "ss_pool_num_pages", "ss_pool_num_free", "ss_pool_alloc", "ss_pool_free"]
+           "ss_pool_num_pages", "ss_pool_num_free", "ss_pool_alloc", "ss_pool_free", "ss_kv_export", "ss_kv_import"]
 
 
 class ss_model_dims(C.Structure):
@@ -90,6 +90,8 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     lib.ss_stage_launch_count.restype = C.c_int64
     lib.ss_stage_launch_count.argtypes = [C.c_void_p]
     lib.ss_debug_buffer.argtypes = [C.c_void_p]
+    lib.ss_kv_export.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_size_t]
+    lib.ss_kv_import.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_size_t]
     lib.ss_pool_create.argtypes = [C.POINTER(C.c_void_p), C.c_int]
     lib.ss_pool_destroy.argtypes = [C.c_void_p]
     lib.ss_pool_num_pages.argtypes = [C.c_void_p]
@@ -224,6 +226,18 @@ class Stage:
                                       _ptr(out_logits), _ptr(out_argmax))
         if check and rc != SS_OK:
             raise ShuntStageError(rc, "ss_stage_decode")
+        return rc
+
+    def kv_export(self, page_ids: torch.Tensor, buf: torch.Tensor, check=True):
+        rc = self.lib.ss_kv_export(self.h, page_ids.numel(), _ptr(page_ids), _ptr(buf), buf.numel() * buf.element_size())
+        if check and rc != SS_OK:
+            raise ShuntStageError(rc, "ss_kv_export")
+        return rc
+
+    def kv_import(self, page_ids: torch.Tensor, buf: torch.Tensor, check=True):
+        rc = self.lib.ss_kv_import(self.h, page_ids.numel(), _ptr(page_ids), _ptr(buf), buf.numel() * buf.element_size())
+        if check and rc != SS_OK:
+            raise ShuntStageError(rc, "ss_kv_import")
         return rc
 
     def launch_count(self) -> int:

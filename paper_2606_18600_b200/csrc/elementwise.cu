@@ -334,4 +334,27 @@ cudaError_t launch_qkv_post(const QkvPostParams &p, cudaStream_t s) {
   return launch_pdl(qkv_post_kernel, dim3(grid), dim3(EW_THREADS), 0, s, p);
 }
 
+// ---- KV migration by transfer (NEXT-4): gather a request's pages out of the layer-major pool into one contiguous
+// buffer [L][K/V][n][n_kv][16][d] (what a GPU-to-GPU copy would carry), and the reverse scatter.  One (layer, K/V,
+// page) piece is n_kv * 16 * d contiguous bf16 (32 KB at the paper's shapes); pure HBM copy, 16 bytes per thread. ----
+__global__ void __launch_bounds__(256)
+kv_pages_copy_kernel(uint4 *__restrict__ pool, uint4 *__restrict__ buf, const int32_t *__restrict__ page_ids, int n,
+                     int n_pages_pool, int piece_vec /* uint4 per piece */, int to_buffer) {
+  pdl_launch_dependents();
+  pdl_wait();
+  const int piece = blockIdx.x;              // = (layer * 2 + kv) * n + i
+  const int lk = piece / n, i = piece - lk * n;
+  uint4 *pp = pool + ((size_t)lk * n_pages_pool + page_ids[i]) * piece_vec;
+  uint4 *bp = buf + (size_t)piece * piece_vec;
+  for (int v = threadIdx.x; v < piece_vec; v += 256) {
+    if (to_buffer) bp[v] = pp[v]; else pp[v] = bp[v];
+  }
+}
+
+cudaError_t launch_kv_pages_copy(void *pool, void *buf, const int32_t *page_ids, int n, int n_layers, int n_pages_pool,
+                                 int piece_bytes, bool to_buffer, cudaStream_t s) {
+  return launch_pdl(kv_pages_copy_kernel, dim3(n_layers * 2 * n), dim3(256), 0, s, (uint4 *)pool, (uint4 *)buf, page_ids,
+                    n, n_pages_pool, piece_bytes / 16, to_buffer ? 1 : 0);
+}
+
 }  // namespace ss

@@ -180,6 +180,10 @@ struct PrefillAttnParams {
 };
 cudaError_t launch_prefill_attn(const PrefillAttnParams &p, cudaStream_t s);
 
+// gather (to_buffer) / scatter n pages of every layer between the pool and a contiguous [L][2][n][n_kv][16][d] buffer
+cudaError_t launch_kv_pages_copy(void *pool, void *buf, const int32_t *page_ids, int n, int n_layers, int n_pages_pool,
+                                 int piece_bytes, bool to_buffer, cudaStream_t s);
+
 void count_launch(int n = 1);  // stage.cu: per-thread launch counter hook
 bool pdl_enabled();            // stage.cu: false when SS_NO_PDL=1
 

@@ -385,6 +385,24 @@ int ss_pool_free(ss_pool *p, int n, const int32_t *page_ids) { return p ? p->rel
 
 int64_t ss_stage_launch_count(const ss_stage *st) { return st ? st->launches : 0; }
 
+static int kv_copy(ss_stage *st, int n, const int32_t *page_ids_dev, void *buf, size_t buf_bytes, bool to_buffer) {
+  if (!st || n <= 0 || !page_ids_dev || !buf) return SS_ERR_INVALID_ARG;
+  if ((uintptr_t)buf & 15) return SS_ERR_UNSUPPORTED;
+  const size_t piece = (size_t)st->d.n_kv_heads * 16 * st->d.head_dim * 2;
+  if (buf_bytes < (size_t)st->L * 2 * n * piece) return SS_ERR_CAPACITY;
+  const int64_t before = g_launches;
+  cudaError_t e = launch_kv_pages_copy(st->pool, buf, page_ids_dev, n, st->L, st->num_pages, (int)piece, to_buffer,
+                                       st->stream);
+  st->launches += g_launches - before;
+  return e == cudaSuccess ? SS_OK : cuda_fail(e, "ss_kv_export/import");
+}
+int ss_kv_export(ss_stage *st, int n, const int32_t *page_ids_dev, void *buf_dev, size_t buf_bytes) {
+  return kv_copy(st, n, page_ids_dev, buf_dev, buf_bytes, true);
+}
+int ss_kv_import(ss_stage *st, int n, const int32_t *page_ids_dev, const void *buf_dev, size_t buf_bytes) {
+  return kv_copy(st, n, page_ids_dev, const_cast<void *>(buf_dev), buf_bytes, false);
+}
+
 }  // extern "C"
 
 // ===================================================================================================================

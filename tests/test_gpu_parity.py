@@ -385,6 +385,54 @@ def test_P17_dyadic_case_kv_bits_exact():
         P.close()
 
 
+def test_migration_by_kv_transfer_is_bit_exact():
+    """instead of recomputing, move a request's KV pages to another stage
+    instance (ss_kv_export -> copy -> ss_kv_import into freshly allocated pages).  The exported message equals the
+    numpy gather of the pool byte for byte, the importer's logical KV equals the exporter's, and the next decode
+    step on the destination is bit-identical to the same step on the source."""
+    shape = synth.TINY_QWEN
+    gh = _gh()
+    A, lens, pb, x = _problem(shape, seed=6, lens=[70, 33, 150, 16], extra=20)
+    B = gh.Problem(shape, 6, n_pages=pb.n_pages_pool + 7, max_tokens=64, max_seqs=16, max_blocks=pb.max_blocks)
+    try:
+        bt = pb.block_tables
+        T = int(lens.sum())
+        A.prefill(lens, bt, x[:T])
+        need = [(int(n) + 1 + 15) // 16 for n in lens]                # pages incl. the next token's slot
+        src_ids = np.concatenate([bt[s, :need[s]] for s in range(len(lens))]).astype(np.int32)
+        n = len(src_ids)
+        page_bytes = A.L * 2 * shape.n_kv * 16 * shape.d * 2
+        buf = torch.empty(n * page_bytes // 2, dtype=torch.bfloat16, device="cuda:0")
+        A.stage.kv_export(A.i32(src_ids), buf)
+        A.stage.synchronize()
+        msg = buf.cpu().view(torch.int16).numpy().view(np.uint16).reshape(A.L, 2, n, shape.n_kv, 16, shape.d)
+        assert np.array_equal(msg, A.pool_bits()[:, :, src_ids])      # byte-exact gather
+        # destination: its own allocator hands out the pages (a different physical placement)
+        B.stage.kv_alloc(5)                                           # shift the ids
+        dst_ids = np.array(B.stage.kv_alloc(n), dtype=np.int32)[::-1].copy()
+        B.stage.kv_import(B.i32(dst_ids), buf)
+        bt_b = np.zeros_like(bt)
+        o = 0
+        for s in range(len(lens)):
+            bt_b[s, :need[s]] = dst_ids[o:o + need[s]]
+            o += need[s]
+        pa, pq = A.pool_bits(), B.pool_bits()
+        for s, ln in enumerate(lens):
+            for l in range(A.L):
+                for kv in range(2):
+                    assert np.array_equal(hp.logical_kv(pa[l, kv], bt[s], int(ln)), hp.logical_kv(pq[l, kv], bt_b[s], int(ln)))
+        xs = x[T:T + len(lens)]
+        ya = A.decode(lens, bt, xs)
+        yb = B.decode(lens, bt_b, xs)
+        assert np.array_equal(ya, yb)                                 # output-preserving, bit for bit
+        # misuse
+        assert B.stage.kv_import(B.i32(dst_ids), buf[:8], check=False) == -3      # SS_ERR_CAPACITY
+        assert B.stage.kv_export(B.i32(dst_ids[:0]), buf, check=False) == -1      # n <= 0
+    finally:
+        A.close()
+        B.close()
+
+
 def test_token_ids_logits_and_argmax():
     """S0 embedding gather and S11 logits/argmax (Table 2 'Logits Calculation'; reading A14)."""
     shape = synth.TINY
