@@ -32,7 +32,7 @@ def parse():
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "cfg5", "tiny"])
+    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "cfg5", "migrate", "tiny"])
     ap.add_argument("--seed", type=int, default=0)
     ap.add_argument("--layers", type=int, default=0, help="override the stage depth (debug only; marks the line)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -141,6 +141,8 @@ def workload_spec(name, layers_override=0):
         shape, ctx, kind = synth.LLAMA70B, synth.cfg4_lengths, "prefill"
     elif name == "cfg5":
         shape, ctx, kind = synth.QWEN32B, None, "online"
+    elif name == "migrate":
+        shape, ctx, kind = synth.LLAMA70B, None, "migrate"
     else:
         shape, ctx, kind = synth.TINY, synth.cfg1_contexts, "decode"
     L = layers_override or shape.n_layers
@@ -388,6 +390,50 @@ def run_prefill(args, shape, len_fn, rank, world):
     return res
 
 
+def run_migrate(args, shape):
+    """SURVEY 8(f) NEXT-4 / the paper's Fig. 5 question: migrate one request of context L
+    by RECOMPUTATION (one ss_stage_prefill of its L tokens) or by KV TRANSFER (ss_kv_export gather -> GPU-to-GPU copy
+    -> ss_kv_import scatter).  One GPU here: gather and scatter are measured, the link is modelled at NVLink 5's
+    900 GB/s per direction (stated in the output)."""
+    import torch
+    from paper_2606_18600_b200 import binding
+    dev = torch.device("cuda:0")
+    torch.cuda.set_device(dev)
+    lengths = [1024, 4096, 16384, 65536]
+    Lmax = lengths[-1]
+    n_pages = Lmax // 16 + 8
+    layers = gpu_weights(shape, dev, args.seed)
+    dims = binding.make_dims(shape, max_tokens=Lmax, max_seqs=1, max_blocks=n_pages, max_pos=Lmax + 64)
+    st = binding.Stage(dims, 0, shape.n_layers, layers, None, n_pages=n_pages, device=dev)
+    g = torch.Generator(device=dev)
+    g.manual_seed(args.seed + 7)
+    x = torch.randn((Lmax, shape.hidden), generator=g, device=dev, dtype=torch.float32).to(torch.bfloat16)
+    out = torch.empty_like(x)
+    perm = torch.randperm(n_pages, generator=g, device=dev).to(torch.int32)
+    bt = perm.view(1, -1).contiguous()
+    ctxb = torch.zeros(1, dtype=torch.int32, device=dev)
+    page_bytes = shape.n_layers * 2 * shape.hkv * 16 * 2
+    rows = []
+    for L in lengths:
+        cu = torch.tensor([0, L], dtype=torch.int32, device=dev)
+        n = (L + 15) // 16
+        ids = perm[:n].contiguous()
+        buf = torch.empty(n * page_bytes // 2, dtype=torch.bfloat16, device=dev)
+        st.prefill(1, cu, ctxb, bt, L, hidden=x[:L], out_hidden=out[:L])       # warm-up (also fills the pages)
+        rec = cuda_time_ms(st.stream, lambda i: st.prefill(1, cu, ctxb, bt, L, hidden=x[:L], out_hidden=out[:L]), 1)
+        st.kv_export(ids, buf); st.kv_import(ids, buf)
+        reps = 5
+        ex = cuda_time_ms(st.stream, lambda i: st.kv_export(ids, buf), reps) / reps
+        im = cuda_time_ms(st.stream, lambda i: st.kv_import(ids, buf), reps) / reps
+        nbytes = n * page_bytes
+        link = nbytes / 900e9 * 1e3
+        rows.append({"context": L, "kv_bytes": nbytes, "recompute_ms": rec, "export_ms": ex, "import_ms": im,
+                     "export_GBs": 2 * nbytes / (ex * 1e-3) / 1e9, "link_ms_modelled_900GBs": link,
+                     "transfer_ms": ex + link + im, "recompute_over_transfer": rec / (ex + link + im)})
+    st.destroy()
+    return rows
+
+
 def run_online(args, shape, rank, world):
     """cfg5: online mixed batches (96 decode rows + <= 4 prefill chunks of <= 512 tokens per ss_stage_prefill call)
     driven by paper_2606_18600_b200/online.py over a page pool at ~85% occupancy; K timed iterations."""
@@ -491,6 +537,7 @@ def main():
                         "cfg3": "configs[2]: Qwen3-32B-shaped 16-layer decode stage, B=128, ctx lognormal(med 768)",
                         "cfg4": "configs[3]: migration recompute prefill, 70B shapes, 32 requests lognormal(med 1200)",
                         "cfg5": "configs[4]: online mixed batches, Qwen3-32B shapes",
+                        "migrate": "migration of one request: recomputation vs KV transfer",
                         "tiny": "configs[0]: tiny Llama-style stage"}[args.workload],
            "layers": shape.n_layers, "hidden": shape.hidden, "ffn": shape.ffn, "heads": f"{shape.n_q}/{shape.n_kv}",
            "page_size": 16, "seed": args.seed, "parallelism": f"replicas x{world}",
@@ -502,7 +549,7 @@ def main():
     if args.impl == "reference":
         if rank != 0:
             return
-        if kind == "online":
+        if kind in ("online", "migrate"):
             raise SystemExit("--impl reference covers cfg2/cfg3/cfg4/tiny (the oracle has no online driver)")
         ts = []
         T = cores = desc = None
@@ -527,6 +574,16 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{int(os.environ.get('LOCAL_RANK', 0))}"))
 
+    if kind == "migrate":
+        if rank != 0:
+            return
+        rows = run_migrate(args, shape)
+        print(json.dumps({"metric": "migration of one request: recomputation vs KV transfer (ms)", "n_gpus": 1,
+                          "dtype": "bf16", "data": "synthetic",
+                          "config": {"workload": "70B-shaped 20-layer stage, one request, contexts 1K-64K",
+                                     "link": "modelled: NVLink 5, 900 GB/s per direction (single-GPU box)"},
+                          "rows": rows}))
+        return
     if kind == "online":
         res = run_online(args, shape, rank, world)
         ms = res["ms"]
