@@ -182,6 +182,18 @@ int ss_stage_decode(ss_stage *st, int batch,
 /* Number of kernels the stage launched (directly or inside replayed graphs) since creation. */
 int64_t ss_stage_launch_count(const ss_stage *st);
 
+/* Tensor parallelism inside a stage.  A rank of a D_TP-way stage is an
+ * ordinary ss_stage created with that rank's SHARD: dims.n_q_heads, n_kv_heads and ffn divided by D_TP (hidden
+ * unchanged), wq/wk/wv and w_gate/w_up = the rank's rows, wo = the rank's columns [H, Hq/D_TP] and w_down = [H, F/D_TP]
+ * (each a contiguous matrix), norms replicated, and its own KV pool holding only its kv heads.  Once an all-reduce is
+ * registered here the O and down projections produce fp32 partials [T, H] and the stage calls
+ *     fn(partial, T * H, user, cuda_stream)
+ * twice per layer (the two all-reduces of Eq. 3) — fn must enqueue, on `cuda_stream`, an in-place SUM of `partial`
+ * across the ranks (e.g. ncclAllReduce) and return without synchronising — then adds the sum to the fp32 residual.
+ * Decode steps are not graph-captured in this mode.  fn = NULL returns the stage to single-GPU operation. */
+typedef void (*ss_allreduce_fn)(float *partial_dev, size_t count, void *user, void *cuda_stream);
+int ss_stage_set_allreduce(ss_stage *st, ss_allreduce_fn fn, void *user);
+
 /* Migration by KV transfer (the alternative to recomputation the paper measures; SURVEY
  * 8(f) NEXT-4).  ss_kv_export gathers the n pages `page_ids_dev[0..n)` (DEVICE int32) of every layer of the stage into
  * the caller's contiguous DEVICE buffer, laid out [layer][K/V][i][h_kv][16][d] bf16 (n * ss_kv_page_bytes() bytes) —

@@ -24,7 +24,10 @@ EXPORTS = ["ss_stage_workspace_bytes", "ss_kv_page_bytes", "ss_stage_create", "s
            "ss_stage_decode",
            "ss_stage_launch_count", "ss_op_gemm_scratch_bytes", "ss_op_gemm_bf16", "ss_op_gemm_swiglu_bf16", "ss_strerror",
            "ss_last_cuda_error", "ss_version", "ss_debug_buffer", "ss_pool_create", "ss_pool_destroy",
-           "ss_pool_num_pages", "ss_pool_num_free", "ss_pool_alloc", "ss_pool_free", "ss_kv_export", "ss_kv_import"]
+           "ss_pool_num_pages", "ss_pool_num_free", "ss_pool_alloc", "ss_pool_free", "ss_kv_export", "ss_kv_import", "ss_stage_set_allreduce"]
+
+
+ALLREDUCE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p)
 
 
 class ss_model_dims(C.Structure):
@@ -90,6 +93,7 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     lib.ss_stage_launch_count.restype = C.c_int64
     lib.ss_stage_launch_count.argtypes = [C.c_void_p]
     lib.ss_debug_buffer.argtypes = [C.c_void_p]
+    lib.ss_stage_set_allreduce.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
     lib.ss_kv_export.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_size_t]
     lib.ss_kv_import.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_size_t]
     lib.ss_pool_create.argtypes = [C.POINTER(C.c_void_p), C.c_int]
@@ -227,6 +231,24 @@ class Stage:
         if check and rc != SS_OK:
             raise ShuntStageError(rc, "ss_stage_decode")
         return rc
+
+    def set_allreduce(self, fn):
+        """fn(partial: float32 torch view of the workspace, stream_ptr: int) -> None: enqueue an in-place sum across
+        the tensor-parallel ranks on that stream (see paper_2606_18600_b200/tp.py).  None clears it."""
+        if fn is None:
+            self._ar_cb = None
+            rc = self.lib.ss_stage_set_allreduce(self.h, None, None)
+        else:
+            ws, base = self.workspace, self.workspace.data_ptr()
+
+            def tramp(ptr, count, user, stream):
+                off = ptr - base
+                fn(ws[off:off + 4 * count].view(torch.float32), stream)
+
+            self._ar_cb = ALLREDUCE_FN(tramp)          # keep the trampoline alive
+            rc = self.lib.ss_stage_set_allreduce(self.h, C.cast(self._ar_cb, C.c_void_p), None)
+        if rc != SS_OK:
+            raise ShuntStageError(rc, "ss_stage_set_allreduce")
 
     def kv_export(self, page_ids: torch.Tensor, buf: torch.Tensor, check=True):
         rc = self.lib.ss_kv_export(self.h, page_ids.numel(), _ptr(page_ids), _ptr(buf), buf.numel() * buf.element_size())

@@ -47,7 +47,7 @@ constexpr int MAX_WORKERS = 4096;  // upper bound on decode-attention worker war
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Carve {  // byte offsets into the workspace
-  size_t args, rope, x, h, qkv_part, q, kv_new, attn_out, fix, a, part_o, part_ml, cum_pages, meta, tok_seq,
+  size_t args, rope, x, h, qkv_part, q, kv_new, attn_out, fix, a, part_o, part_ml, cum_pages, meta, tp_part, tok_seq,
       tok_pos, tile_cum, hl, logits, total;
 };
 
@@ -91,6 +91,7 @@ static Carve carve(const ss_model_dims *d) {
   c.part_ml = take(n_slots * 32 * 4);
   c.cum_pages = take(((size_t)d->max_seqs + 1) * 4);
   c.meta = take(16);
+  c.tp_part = take(Tm * H * 4);  // tensor-parallel mode: fp32 partial of the O / down projection
   c.tok_seq = take(Tm * 4);
   c.tok_pos = take(Tm * 4);
   c.tile_cum = take(((size_t)d->max_seqs + 1) * 4);
@@ -181,6 +182,8 @@ struct ss_stage {
   int64_t launches;
   std::map<int, Graph> graphs;  // key = batch*2 + tail
   bool use_graph;
+  ss_allreduce_fn allreduce;  // non-null: tensor-parallel shard (ss_stage_set_allreduce)
+  void *allreduce_user;
   CallArgs *h_args;    // pinned host staging for the argument block
 
   size_t layer_kv_elems() const { return (size_t)num_pages * d.n_kv_heads * 16 * d.head_dim; }
@@ -265,6 +268,8 @@ int ss_stage_create(ss_stage **out, const ss_model_dims *dims, int l0, int l1, c
   st->launches = 0;
   st->use_graph = (cuda_stream != nullptr) && env_int("SS_NO_GRAPH", 0) == 0;
   st->h_args = nullptr;
+  st->allreduce = nullptr;
+  st->allreduce_user = nullptr;
 
   auto fail = [&](int code) {
     if (st->h_args) cudaFreeHost(st->h_args);
@@ -385,6 +390,13 @@ int ss_pool_free(ss_pool *p, int n, const int32_t *page_ids) { return p ? p->rel
 
 int64_t ss_stage_launch_count(const ss_stage *st) { return st ? st->launches : 0; }
 
+int ss_stage_set_allreduce(ss_stage *st, ss_allreduce_fn fn, void *user) {
+  if (!st) return SS_ERR_INVALID_ARG;
+  st->allreduce = fn;
+  st->allreduce_user = user;
+  return SS_OK;
+}
+
 static int kv_copy(ss_stage *st, int n, const int32_t *page_ids_dev, void *buf, size_t buf_bytes, bool to_buffer) {
   if (!st || n <= 0 || !page_ids_dev || !buf) return SS_ERR_INVALID_ARG;
   if ((uintptr_t)buf & 15) return SS_ERR_UNSUPPORTED;
@@ -457,6 +469,8 @@ static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T,
   float *qkv_part = st->at<float>(c.qkv_part);
   cudaStream_t s = st->stream;
 
+  const bool tp = st->allreduce != nullptr;
+  float *tp_part = st->at<float>(c.tp_part);
   DecodePlan dplan{st->at<int32_t>(c.cum_pages), st->at<int32_t>(c.meta)};
   PrefillPlan pplan{st->at<int32_t>(c.tok_seq), st->at<int32_t>(c.tok_pos), st->at<int32_t>(c.tile_cum)};
   if (decode)
@@ -529,8 +543,14 @@ static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T,
     {  // S7: output projection, then S8: x1 = x + o Wo^T ; h2 = rmsnorm(x1; ln2)
       const CUtensorMap *a[3] = {&m.wo, nullptr, nullptr};
       const int rows[3] = {H, 0, 0};
-      CKE(run_gemm(st, a, 1, rows, false, st->b_attn, T, Hq, EPI_RESID_F32, x, nullptr, H));
-      CKE(launch_residual_rmsnorm(x, nullptr, 0, 0, w.ln2, d.rms_eps, H, T, h, args, false, s));
+      if (!tp) {
+        CKE(run_gemm(st, a, 1, rows, false, st->b_attn, T, Hq, EPI_RESID_F32, x, nullptr, H));
+        CKE(launch_residual_rmsnorm(x, nullptr, 0, 0, w.ln2, d.rms_eps, H, T, h, args, false, s));
+      } else {  // this rank's partial over its heads -> all-reduce -> x += sum (two per layer)
+        CKE(run_gemm(st, a, 1, rows, false, st->b_attn, T, Hq, EPI_F32, tp_part, nullptr, H));
+        st->allreduce(tp_part, (size_t)T * H, st->allreduce_user, (void *)s);
+        CKE(launch_residual_rmsnorm(x, tp_part, 1, 0, w.ln2, d.rms_eps, H, T, h, args, false, s));
+      }
     }
     {  // S9: gate/up + SwiGLU fused -> a bf16 [T,F]
       const CUtensorMap *a[3] = {&m.wg, &m.wu, nullptr};
@@ -540,10 +560,16 @@ static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T,
     {  // S10: down projection + residual, then the next layer's RMSNorm-1 (or the stage output)
       const CUtensorMap *a[3] = {&m.wd, nullptr, nullptr};
       const int rows[3] = {H, 0, 0};
-      CKE(run_gemm(st, a, 1, rows, false, st->b_a, T, F, EPI_RESID_F32, x, nullptr, H));
       const bool last = (l == st->L - 1);
       const void *next_ln = last ? nullptr : st->lw[l + 1].ln1;
-      CKE(launch_residual_rmsnorm(x, nullptr, 0, 0, next_ln, d.rms_eps, H, T, h, args, last, s));
+      if (!tp) {
+        CKE(run_gemm(st, a, 1, rows, false, st->b_a, T, F, EPI_RESID_F32, x, nullptr, H));
+        CKE(launch_residual_rmsnorm(x, nullptr, 0, 0, next_ln, d.rms_eps, H, T, h, args, last, s));
+      } else {
+        CKE(run_gemm(st, a, 1, rows, false, st->b_a, T, F, EPI_F32, tp_part, nullptr, H));
+        st->allreduce(tp_part, (size_t)T * H, st->allreduce_user, (void *)s);
+        CKE(launch_residual_rmsnorm(x, tp_part, 1, 0, next_ln, d.rms_eps, H, T, h, args, last, s));
+      }
     }
   }
   if (tail) {  // S11: final norm of each sequence's last row, lm_head, argmax
@@ -626,7 +652,7 @@ int ss_stage_decode(ss_stage *st, int batch, const void *hidden_bf16, const int3
   a.n_seqs = batch; a.T = batch; a.max_blocks = max_blocks;
   if ((rc = upload_args(st, a)) != SS_OK) return rc;
   const bool tail = out_logits || out_argmax;
-  if (!st->use_graph) {
+  if (!st->use_graph || st->allreduce) {  // a tensor-parallel shard calls back into the caller: never captured
     const int64_t before = g_launches;
     cudaError_t e = enqueue_forward(st, true, batch, batch, tail);
     st->launches += g_launches - before;

@@ -58,3 +58,53 @@ def test_reference_arm_under_torchrun_prints_one_line_from_rank0():
     d = json.loads(lines[0])
     assert d["impl"] == "reference" and d["cpu_baseline"]["kind"] == "oracle" and d["value"] > 0
     assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["unit"] == "tokens/s"
+
+
+def _tp_worker(rank, world, port, out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    sys.path.insert(0, ROOT)
+    from paper_2606_18600_b200 import synth, tp
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    shape = synth.TINY_QWEN
+    w = {k: (None if v is None else v.float()) for k, v in synth.layer_weights(shape, 0, 3).items()}
+    ws = tp.shard_layer_weights(w, rank, world, shape)
+    g = torch.Generator().manual_seed(5)
+    T = 9
+    h = torch.randn((T, shape.hidden), generator=g)
+    o_full = torch.randn((T, shape.hq), generator=g)          # attention output, all heads
+    # rank's slice of the heads -> partial of the O projection -> all-reduce (first all-reduce of the layer)
+    hq = shape.hq // world
+    part_o = o_full[:, rank * hq:(rank + 1) * hq] @ ws["wo"].T
+    dist.all_reduce(part_o)
+    # FFN: rank's FFN columns -> partial of the down projection -> all-reduce (second one)
+    a = torch.nn.functional.silu(h @ ws["w_gate"].T) * (h @ ws["w_up"].T)
+    part_d = a @ ws["w_down"].T
+    dist.all_reduce(part_d)
+    # the rank's q/k/v rows are whole heads of the full projections
+    q_r = h @ ws["wq"].T
+    k_r = h @ ws["wk"].T
+    want_o = o_full @ w["wo"].T
+    want_d = (torch.nn.functional.silu(h @ w["w_gate"].T) * (h @ w["w_up"].T)) @ w["w_down"].T
+    q_full, k_full = h @ w["wq"].T, h @ w["wk"].T
+    hkv = shape.hkv // world
+    ok = (torch.allclose(part_o, want_o, rtol=1e-5, atol=1e-5) and torch.allclose(part_d, want_d, rtol=1e-5, atol=1e-5)
+          and torch.equal(q_r, q_full[:, rank * hq:(rank + 1) * hq]) and torch.equal(k_r, k_full[:, rank * hkv:(rank + 1) * hkv]))
+    dist.barrier()
+    dist.destroy_process_group()
+    out.put((rank, bool(ok)))
+
+
+def test_tensor_parallel_sharding_algebra_gloo_world2():
+    """NEXT-1 on CPU: with the layer cut by tp.shard_layer_weights, the ranks' partials of the O and down projections
+    all-reduce (gloo, world_size 2) to the unsharded projections, and each rank's q/k rows are whole heads."""
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 33000 + os.getpid() % 2000
+    ps = [ctx.Process(target=_tp_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in ps:
+        p.start()
+    res = dict(q.get(timeout=120) for _ in ps)
+    for p in ps:
+        p.join(60)
+        assert p.exitcode == 0
+    assert res == {0: True, 1: True}
