@@ -181,22 +181,32 @@ cudaError_t launch_final_norm_rows(const float *x, const CallArgs *args, bool de
   return launch_pdl(final_norm_rows_kernel, dim3(n_seqs), dim3(EW_THREADS), 0, s, x, args, decode ? 1 : 0, (const __nv_bfloat16 *)wf, eps, H, (__nv_bfloat16 *)hl);
 }
 
-// ---- S11b: reduce logits splits, copy out, argmax (lowest index among maxima) ---------------------------------
+// ---- S11b: copy the logits out and argmax (lowest index among maxima), two passes: AM_SPLITS CTAs per row scan a
+// slice of the vocabulary each (64 rows x 128,256 fp32 = 33 MB: one CTA per row would leave most SMs idle), then one
+// warp per row combines the slices' (max, index) pairs in slice order.
+constexpr int AM_SPLITS = 16;
+__device__ __forceinline__ void argmax_combine(float &best, int &bi, float ob, int oi) {
+  if (ob > best || (ob == best && oi < bi)) {
+    best = ob;
+    bi = oi;
+  }
+}
+
 __global__ void __launch_bounds__(1024)
-logits_argmax_kernel(const float *__restrict__ part, int splits, long long split_stride, int V,
-                     float *__restrict__ logits_ws, const CallArgs *__restrict__ args) {
+logits_argmax_part_kernel(const float *__restrict__ logits, int V, const CallArgs *__restrict__ args,
+                          float *__restrict__ part_max, int *__restrict__ part_idx) {
   pdl_launch_dependents();
   pdl_wait();
   __shared__ float smax[32];
   __shared__ int sidx[32];
-  const int r = blockIdx.x;
+  const int r = blockIdx.x, sp = blockIdx.y;
+  const int per = (V + AM_SPLITS - 1) / AM_SPLITS;
+  const int j0 = sp * per, j1 = min(V, j0 + per);
   float *outl = args->out_logits ? args->out_logits + (size_t)r * V : nullptr;
   float best = -INFINITY;
   int bi = 0x7fffffff;
-  for (int j = threadIdx.x; j < V; j += blockDim.x) {
-    float v = part[(size_t)r * V + j];
-    for (int s = 1; s < splits; ++s) v += part[(size_t)s * split_stride + (size_t)r * V + j];
-    if (splits > 1) logits_ws[(size_t)r * V + j] = v;
+  for (int j = j0 + threadIdx.x; j < j1; j += blockDim.x) {
+    const float v = logits[(size_t)r * V + j];
     if (outl) outl[j] = v;
     if (v > best) {  // j ascending per thread: strict > keeps the lowest index
       best = v;
@@ -204,14 +214,8 @@ logits_argmax_kernel(const float *__restrict__ part, int splits, long long split
     }
   }
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    const float ob = __shfl_xor_sync(0xffffffffu, best, o);
-    const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
-    if (ob > best || (ob == best && oi < bi)) {
-      best = ob;
-      bi = oi;
-    }
-  }
+  for (int o = 16; o > 0; o >>= 1)
+    argmax_combine(best, bi, __shfl_xor_sync(0xffffffffu, best, o), __shfl_xor_sync(0xffffffffu, bi, o));
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   if (lane == 0) {
     smax[warp] = best;
@@ -223,21 +227,36 @@ logits_argmax_kernel(const float *__restrict__ part, int splits, long long split
     best = lane < nw ? smax[lane] : -INFINITY;
     bi = lane < nw ? sidx[lane] : 0x7fffffff;
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-      const float ob = __shfl_xor_sync(0xffffffffu, best, o);
-      const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
-      if (ob > best || (ob == best && oi < bi)) {
-        best = ob;
-        bi = oi;
-      }
+    for (int o = 16; o > 0; o >>= 1)
+      argmax_combine(best, bi, __shfl_xor_sync(0xffffffffu, best, o), __shfl_xor_sync(0xffffffffu, bi, o));
+    if (lane == 0) {
+      part_max[r * AM_SPLITS + sp] = best;
+      part_idx[r * AM_SPLITS + sp] = bi;
     }
-    if (lane == 0 && args->out_argmax) args->out_argmax[r] = bi;
   }
 }
 
-cudaError_t launch_logits_argmax(const float *part, int splits, long long split_stride, int V, int n_rows,
-                                 float *logits_ws, const CallArgs *args, cudaStream_t s) {
-  return launch_pdl(logits_argmax_kernel, dim3(n_rows), dim3(1024), 0, s, part, splits, split_stride, V, logits_ws, args);
+__global__ void __launch_bounds__(32)
+logits_argmax_final_kernel(const float *__restrict__ part_max, const int *__restrict__ part_idx,
+                           const CallArgs *__restrict__ args) {
+  pdl_launch_dependents();
+  pdl_wait();
+  const int r = blockIdx.x, lane = threadIdx.x;
+  float best = lane < AM_SPLITS ? part_max[r * AM_SPLITS + lane] : -INFINITY;
+  int bi = lane < AM_SPLITS ? part_idx[r * AM_SPLITS + lane] : 0x7fffffff;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1)
+    argmax_combine(best, bi, __shfl_xor_sync(0xffffffffu, best, o), __shfl_xor_sync(0xffffffffu, bi, o));
+  if (lane == 0 && args->out_argmax) args->out_argmax[r] = bi;
+}
+
+cudaError_t launch_logits_argmax(const float *logits, int V, int n_rows, float *part_max, int *part_idx,
+                                 const CallArgs *args, cudaStream_t s) {
+  cudaError_t e = launch_pdl(logits_argmax_part_kernel, dim3(n_rows, AM_SPLITS), dim3(1024), 0, s, logits, V, args,
+                             part_max, part_idx);
+  if (e != cudaSuccess) return e;
+  return launch_pdl(logits_argmax_final_kernel, dim3(n_rows), dim3(32), 0, s, (const float *)part_max,
+                    (const int *)part_idx, args);
 }
 
 // ---- S3 + S4 (+ S5 in prefill): one warp per (token, head) ----------------------------------------------------

@@ -571,6 +571,7 @@ void gemm_plan(GemmLaunch &g, int n_sm) {
   const long long waves = (n_tiles + max_grid - 1) / max_grid;
   const bool full_waves = n_tiles >= max_grid && n_tiles * 100 >= waves * max_grid * (p.n_t_tiles >= 2 ? 70 : 88);
   p.sched = (n_tiles >= 4LL * max_grid || full_waves) ? SCHED_TILES : SCHED_STREAMK;
+  if (p.n_t_tiles == 1) p.sched = SCHED_STREAMK;  // HBM-bound whatever the tile count (lm_head: 1,002-1,187 tiles = 6.8-8.02 waves)
   if (env_sched >= 0) p.sched = env_sched;
   if (n_tiles * nkb >= (1LL << 31)) p.sched = SCHED_TILES;  // the stream-K unit cursor is 32-bit
   p.band = env_band > 0 ? env_band : (g.dual ? 8 : 16);
@@ -582,10 +583,13 @@ void gemm_plan(GemmLaunch &g, int n_sm) {
     const int acc_cols = p.bn * (g.dual ? 2 : 1);
     static int env_wpol = -2;
     if (env_wpol == -2) env_wpol = env_int("SS_GEMM_WPOL", -1);
-    p.w_policy = p.sched == SCHED_STREAMK ? 0 : 2;
+    // one token tile (T <= 256): every weight byte is read once, whatever the schedule (e.g. the lm_head at decode:
+    // 1,002 row tiles -> whole-tile schedule, but HBM-bound like the stream-K shapes)
+    const bool hbm_bound = p.sched == SCHED_STREAMK || p.n_t_tiles == 1;
+    p.w_policy = hbm_bound ? 0 : 2;
     if (env_wpol >= 0) p.w_policy = env_wpol;
     p.split = 0;
-    if (p.sched == SCHED_STREAMK) {
+    if (hbm_bound) {
       p.issuers = (2 * acc_cols <= 512) ? 2 : 1;
     } else {
       // measured: splitting each k-block between two issuers does not help here (the tensor pipe waits on L2, not

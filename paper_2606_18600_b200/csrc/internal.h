@@ -107,9 +107,10 @@ cudaError_t launch_residual_rmsnorm(float *x, const float *part, int splits, lon
 // gather the last row of each sequence: hl[s,:] = bf16(rmsnorm(x[last(s),:]) * wf)
 cudaError_t launch_final_norm_rows(const float *x, const CallArgs *args, bool decode, const void *wf, float eps,
                                    int H, int n_seqs, void *hl, cudaStream_t s);
-// logits = sum of splits -> out (args->out_logits or internal), argmax (lowest index among maxima)
-cudaError_t launch_logits_argmax(const float *part, int splits, long long split_stride, int V, int n_rows,
-                                 float *logits_ws, const CallArgs *args, cudaStream_t s);
+// logits -> args->out_logits (when non-null) and argmax (lowest index among maxima) -> args->out_argmax;
+// part_max / part_idx: n_rows * 16 scratch entries each
+cudaError_t launch_logits_argmax(const float *logits, int V, int n_rows, float *part_max, int *part_idx,
+                                 const CallArgs *args, cudaStream_t s);
 
 struct QkvPostParams {
   const float *qkv_part;   // [splits][T][Hq+2Hkv]

@@ -47,7 +47,7 @@ constexpr int MAX_WORKERS = 4096;  // upper bound on decode-attention worker war
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Carve {  // byte offsets into the workspace
-  size_t args, rope, x, h, qkv_part, q, kv_new, attn_out, fix, a, part_o, part_ml, cum_pages, meta, tp_part, tok_seq,
+  size_t args, rope, x, h, qkv_part, q, kv_new, attn_out, fix, a, part_o, part_ml, cum_pages, meta, tp_part, am_part, tok_seq,
       tok_pos, tile_cum, hl, logits, total;
 };
 
@@ -91,6 +91,7 @@ static Carve carve(const ss_model_dims *d) {
   c.part_ml = take(n_slots * 32 * 4);
   c.cum_pages = take(((size_t)d->max_seqs + 1) * 4);
   c.meta = take(16);
+  c.am_part = take((size_t)d->max_seqs * 16 * 8);  // argmax partials: 16 (max, index) pairs per row
   c.tp_part = take(Tm * H * 4);  // tensor-parallel mode: fp32 partial of the O / down projection
   c.tok_seq = take(Tm * 4);
   c.tok_pos = take(Tm * 4);
@@ -577,7 +578,8 @@ static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T,
     const CUtensorMap *a[3] = {&st->lm_map, nullptr, nullptr};
     const int rows[3] = {d.vocab, 0, 0};
     CKE(run_gemm(st, a, 1, rows, false, st->b_hl, n_seqs, H, EPI_F32, st->at<float>(c.logits), nullptr, d.vocab));
-    CKE(launch_logits_argmax(st->at<float>(c.logits), 1, 0, d.vocab, n_seqs, st->at<float>(c.logits), args, s));
+    CKE(launch_logits_argmax(st->at<float>(c.logits), d.vocab, n_seqs, st->at<float>(c.am_part),
+                             (int *)(st->ws + c.am_part + (size_t)d.max_seqs * 16 * 4), args, s));
   }
   return cudaSuccess;
 }
