@@ -144,8 +144,14 @@ def _check_kv(pool_gpu, pool_r1, mask, first_layer_only_ulp=True):
         assert np.abs(a - b).max() <= 1e-2 * np.abs(b).max()
 
 
+# groups of 12 and 16 query heads per kv head: rows 8-15 of the decode kernel's MMA tile are live (its HI variant)
+G12 = synth.ModelShape("tiny-g12", 256, 12, 1, 64, 688, 2, 1e-5, 5e5, 0, 512)
+G16 = synth.ModelShape("tiny-g16-d128", 512, 16, 1, 128, 1024, 2, 1e-6, 1e6, 1, 512)
+
+
 @pytest.mark.parametrize("shape,proj_std,ref", [(synth.TINY, 0.02, 0), (synth.TINY, 0.08, 0), (synth.TINY, 0.16, 1),
-                                                (synth.TINY_QWEN, 0.02, 0), (synth.TINY128, 0.05, 0)])
+                                                (synth.TINY_QWEN, 0.02, 0), (synth.TINY128, 0.05, 0),
+                                                (G12, 0.04, 0), (G16, 0.04, 0)])
 def test_stage_prefill_then_decode_vs_oracle(shape, proj_std, ref):
     """ref = 0: judged against the plain fp32 oracle (R0).  ref = 1: the 'sharp' variant of reading A21 (weights x8,
     peaked softmax): there the oracle's own R1-vs-R0 distance is 6e-2 (any engine that materialises bf16
