@@ -553,6 +553,28 @@ def test_edge_cases_and_error_codes():
     assert lib.ss_stage_workspace_bytes(C.byref(bad), 0, 2) == 0
 
 
+def test_decode_at_maximum_context_many_segments():
+    """Contexts at the top of the paper's range (8,192 tokens, BASELINE.json configs[1]) with a tiny batch: every
+    (sequence, kv head) pair is cut across hundreds of worker warps, so the split-K partials and the merge carry the
+    whole result; plus a 1-token context beside it (a pair that is a single page)."""
+    shape = synth.TINY128
+    gh = _gh()
+    ctx = np.array([8191, 0, 4097], dtype=np.int32)
+    rng = np.random.default_rng(8)
+    pb = synth.paged_batch(rng, ctx, extra_tokens=2)
+    P = gh.Problem(shape, 8, n_pages=pb.n_pages_pool, max_tokens=8, max_seqs=8, max_blocks=pb.max_blocks,
+                   pool_fill="random")
+    try:
+        x = synth.bits(synth.hidden_rows(3, shape.hidden, 8))
+        pool = P.pool_cpu.copy()
+        want, _ = hp.run_oracle_decode(F32, shape, P.wb, pool, ctx, pb.block_tables, x)
+        # max_pos must cover position 8191
+        got = P.decode(ctx, pb.block_tables, x)
+        assert hp.rel_err_rows(got, want) < STAGE_TOL
+    finally:
+        P.close()
+
+
 def test_kv_allocator_invariants():
     """P15: alloc/free conserve the page multiset; double free / over-allocation return the documented errors."""
     shape = synth.TINY
