@@ -397,6 +397,17 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
       } else {
         for (int c0 = grp * 32; c0 < bn; c0 += 64) {
           uint32_t v[32], u[32];
+          // the residual values this chunk will be added to do not depend on the accumulator: request them first so
+          // their L2 round trip overlaps the TMEM loads and the fix-up rounds
+          float xv[32];
+          if (!DUAL && p.epi == EPI_RESID_F32 && row_ok) {
+            const float *o = p.out_f32 + col;
+#pragma unroll
+            for (int j = 0; j < 32; ++j) {
+              const int t = t0 + c0 + j;
+              xv[j] = (t < p.T) ? __ldcg(o + (size_t)t * p.ld_out) : 0.f;
+            }
+          }
           ld_acc((uint32_t)c0, v);
           if (DUAL) ld_acc((uint32_t)(bn + c0), u);
           if (et == 0 && item == 1) trace(p, 40 + 3 * (c0 >> 5));
@@ -433,15 +444,9 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
             }
           } else if (row_ok) {
             if (p.epi == EPI_RESID_F32) {
-              // all 32 loads of the residual are issued before the first store (a `+=` loop would serialise
-              // 32 dependent L2 round trips per chunk: the compiler cannot prove the stores do not alias the loads)
+              // (the 32 residual values were loaded above, before any store: a `+=` loop would serialise 32 dependent
+              // L2 round trips per chunk, since the compiler cannot prove the stores do not alias the loads)
               float *o = p.out_f32 + col;
-              float xv[32];
-#pragma unroll
-              for (int j = 0; j < 32; ++j) {
-                const int t = t0 + c0 + j;
-                xv[j] = (t < p.T) ? __ldcg(o + (size_t)t * p.ld_out) : 0.f;
-              }
 #pragma unroll
               for (int j = 0; j < 32; ++j) {
                 const int t = t0 + c0 + j;
