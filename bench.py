@@ -300,7 +300,9 @@ def _fill_randn(pool, g):
 def dominant_gemm(st, shape, layers, T, dev):
     """The dominant kernel of the decode step is the fused gate/up + SwiGLU GEMM (45% of the step's bytes).  Time it
     alone with CUDA events on its stream, over the stage's own weights layer after layer (so nothing is L2-resident:
-    each launch streams 2*H*F*2 bytes >> L2)."""
+    each launch streams 2*H*F*2 bytes >> L2).  Launches are plain stream-ordered (no programmatic dependent launch:
+    with PDL consecutive launches overlap head and tail and the per-launch time drops to 140.9 us = 102% of the
+    measured copy peak, which is a throughput of overlapped launches, not one kernel's duration)."""
     import torch
     from paper_2606_18600_b200 import binding
     g = torch.Generator(device=dev)

@@ -734,7 +734,10 @@ static int op_gemm(const void *x_dev, const void *w0, const void *w1, float *c_f
 #endif
   p.fix_slots = (float *)((uint8_t *)scratch_dev + GEMM_FIX_FLAG_BYTES);
   g.dual = dual;
-  g.no_pdl = true;  // the caller's weights may come straight out of a preceding kernel
+  // the caller's weights may come straight out of a preceding kernel, so the weight ring must not be primed before
+  // that kernel has finished: no PDL, unless the caller vouches for long-lived weights (SS_OP_GEMM_PDL=1: bench.py
+  // times the dominant kernel launched exactly as the stage launches it)
+  g.no_pdl = env_int("SS_OP_GEMM_PDL", 0) == 0;
   g.stream = (cudaStream_t)cuda_stream;
   gemm_plan(g, n_sm);
   if (make_tmap_bf16_2d(&ta, w0, (uint64_t)N, (uint64_t)K, GEMM_BM, true) != 0 ||
