@@ -28,3 +28,22 @@ def test_seed0_workload_draws_match_design():
     # decode is memory-bound on every row, prefill compute-bound on every GEMM row
     rows = est.decode_rows(synth.LLAMA70B, c2, 1616.2e12, 6545e9)
     assert max(rows, key=rows.get) == "up_gate"
+
+
+def test_bench_estimator_column_agrees_with_libshuntplace_on_uniform_batches():
+    """Two restatements of Eq. 1 + Table 2 in this repo — the per-sequence report column of bench.py (estimator.py) and
+    the placement library's stage latency (csrc/placement.cpp) — must give the same number where both apply: one
+    decode iteration (S_out = 1) or one prefill of a batch of equal lengths, D_TP = 1, no communication, no logits."""
+    import numpy as np
+    from paper_2606_18600_b200 import estimator, placement as pl, synth
+    for shape in (synth.LLAMA70B, synth.QWEN32B):
+        m = pl.sp_model(shape.hidden, shape.hq, shape.hkv, shape.ffn, 0, shape.n_layers, 2)
+        g = pl.sp_instance(1624.1e12, 6545.3e9, 180e9, 1, 0.0, 1.0, 1.0)
+        for B, S in ((64, 1313), (128, 992), (1, 17), (32, 1255)):
+            o = pl.sp_opts(float(S), 1.0, 0.0, 1e30, 0.0, 0.0, 0.0, 1, 8, 0)
+            dec = pl.stage_latency(m, g, o, shape.n_layers, B, 1, False, False) * 1e3
+            want = estimator.decode_step_ms(shape, np.full(B, S), g.flops, g.mem_bw)
+            assert abs(dec - want) <= 1e-12 * want
+            pre = pl.stage_latency(m, g, o, shape.n_layers, B, 0, False, False) * 1e3
+            want_p = estimator.prefill_ms(shape, np.full(B, S), g.flops, g.mem_bw)
+            assert abs(pre - want_p) <= 1e-12 * want_p

@@ -575,6 +575,60 @@ def test_decode_at_maximum_context_many_segments():
         P.close()
 
 
+def test_op_gemm_random_shapes_property():
+    """Property test (hypothesis): random ragged (T, N, K) — token tails, weight-row tails, K tails that are only
+    multiples of 8 — through both schedules and both epilogues, against a float64 matmul of the same bf16 bits."""
+    from hypothesis import given, settings, strategies as st
+    from paper_2606_18600_b200 import binding
+
+    @settings(max_examples=30, deadline=None)
+    @given(st.integers(1, 700), st.integers(1, 90), st.integers(1, 160), st.booleans(), st.integers(0, 10 ** 6))
+    def run(T, n8, k8, dual, seed):
+        N, K = 8 * n8, 8 * k8
+        g = torch.Generator().manual_seed(seed)
+        x = synth.randn_bf16((T, K), 1.0, g)
+        w0 = synth.randn_bf16((N, K), 0.06, g)
+        xd = x.cuda()
+        ref0 = x.double() @ w0.double().T
+        if dual:
+            w1 = synth.randn_bf16((N, K), 0.06, g)
+            got = binding.op_gemm_swiglu_bf16(xd, w0.cuda(), w1.cuda()).float().cpu().double()
+            ref = torch.nn.functional.silu(ref0) * (x.double() @ w1.double().T)
+            tol = 1e-2 * ref.abs().max() + 1e-6
+        else:
+            got = binding.op_gemm_bf16(xd, w0.cuda()).cpu().double()
+            ref = ref0
+            tol = 2e-5 * ref.abs().max() * np.sqrt(max(K, 64) / 64) + 1e-6
+        torch.cuda.synchronize()
+        assert (got - ref).abs().max() <= tol, (T, N, K, dual)
+
+    run()
+
+
+def test_graph_replay_equals_stream_launches_bit_for_bit(monkeypatch):
+    """The decode step captured into a CUDA graph (with its programmatic-dependency edges) and the same kernels
+    launched one by one on the stream produce identical bits, hidden state and KV pool."""
+    shape = synth.TINY_QWEN
+    gh = _gh()
+    P, lens, pb, x = _problem(shape, seed=12)
+    monkeypatch.setenv("SS_NO_GRAPH", "1")
+    Q = gh.Problem(shape, 12, n_pages=pb.n_pages_pool, max_tokens=int(lens.sum()) + 64, max_seqs=16,
+                   max_blocks=pb.max_blocks)
+    monkeypatch.delenv("SS_NO_GRAPH")
+    try:
+        T = int(lens.sum())
+        a, b = P.prefill(lens, pb.block_tables, x[:T]), Q.prefill(lens, pb.block_tables, x[:T])
+        assert np.array_equal(a, b)
+        for step in range(3):
+            xs = x[T + step * len(lens): T + (step + 1) * len(lens)]
+            ya, yb = P.decode(lens + step, pb.block_tables, xs), Q.decode(lens + step, pb.block_tables, xs)
+            assert np.array_equal(ya, yb), step
+        assert np.array_equal(P.pool_bits(), Q.pool_bits())
+    finally:
+        P.close()
+        Q.close()
+
+
 def test_kv_allocator_invariants():
     """P15: alloc/free conserve the page multiset; double free / over-allocation return the documented errors."""
     shape = synth.TINY
