@@ -259,70 +259,78 @@ cudaError_t launch_logits_argmax(const float *logits, int V, int n_rows, float *
                     (const int *)part_idx, args);
 }
 
-// ---- S3 + S4 (+ S5 in prefill): one warp per (token, head) ----------------------------------------------------
+// ---- S3 + S4 (+ S5 in prefill): one HALF-warp per (token, head) -------------------------------------------------
+// Lane l of the half-warp owns V = d/32 consecutive elements of the low half, [V*l, V*l + V), and their rotation
+// partners in the high half (c + d/2), so every access is one vector load / store (16 B at d = 128) and RoPE is
+// thread-local; the per-head RMSNorm statistic is a 4-step shuffle inside the half-warp.
+template <int V>  // V = d / 32: 4 (d = 128) or 2 (d = 64)
 __global__ void __launch_bounds__(EW_THREADS) qkv_post_kernel(const QkvPostParams p) {
   pdl_launch_dependents();
   pdl_wait();
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int hw = threadIdx.x >> 4, l = threadIdx.x & 15;
   const int n_heads = p.n_q + 2 * p.n_kv;
-  const int head = blockIdx.y * (EW_THREADS / 32) + warp;
+  const int head = blockIdx.y * (EW_THREADS / 16) + hw;
   const int t = blockIdx.x;
-  if (head >= n_heads) return;
+  const bool active = head < n_heads;
   const int d = p.d, half = d >> 1;
-  const int ldq = n_heads * d;
-  const float *src = p.qkv_part + (size_t)t * ldq + (size_t)head * d;
-  // lane owns pairs (c, c+half) for c = lane, lane+32 (d = 128) or c = lane (d = 64)
-  float lo[2], hi[2];
-  const int npair = half >> 5;  // 1 or 2
+  const int c = V * l;
+  float lo[V], hi[V];
 #pragma unroll
-  for (int i = 0; i < 2; ++i) {
-    lo[i] = hi[i] = 0.f;
-    if (i < npair) {
-      const int c = lane + 32 * i;
-      float a = src[c], b = src[c + half];
-      for (int s = 1; s < p.splits; ++s) {
-        a += src[(size_t)s * p.split_stride + c];
-        b += src[(size_t)s * p.split_stride + c + half];
+  for (int i = 0; i < V; ++i) lo[i] = hi[i] = 0.f;
+  const int ldq = n_heads * d;
+  if (active) {
+    const float *src = p.qkv_part + (size_t)t * ldq + (size_t)head * d;
+    for (int s = 0; s < p.splits; ++s) {
+      const float *sp = src + (size_t)s * p.split_stride;
+      if (V == 4) {
+        const float4 a = *reinterpret_cast<const float4 *>(sp + c), b = *reinterpret_cast<const float4 *>(sp + c + half);
+        lo[0] += a.x; lo[1] += a.y; lo[2] += a.z; lo[3] += a.w;
+        hi[0] += b.x; hi[1] += b.y; hi[2] += b.z; hi[3] += b.w;
+      } else {
+        const float2 a = *reinterpret_cast<const float2 *>(sp + c), b = *reinterpret_cast<const float2 *>(sp + c + half);
+        lo[0] += a.x; lo[1] += a.y;
+        hi[0] += b.x; hi[1] += b.y;
       }
-      lo[i] = a;
-      hi[i] = b;
     }
   }
   const bool is_q = head < p.n_q;
   const bool is_k = !is_q && head < p.n_q + p.n_kv;
-  int pos, seq;
-  if (p.decode) {
-    seq = t;
-    pos = p.args->ctx[t];
-  } else {
-    seq = p.tok_seq[t];
-    pos = p.tok_pos[t];
+  int pos = 0, seq = 0;
+  if (active) {
+    if (p.decode) {
+      seq = t;
+      pos = p.args->ctx[t];
+    } else {
+      seq = p.tok_seq[t];
+      pos = p.tok_pos[t];
+    }
   }
-  if (is_q || is_k) {
-    if (p.qk_norm) {
-      float ss = 0.f;
+  if (p.qk_norm) {  // every lane takes part in the shuffles; the result is used by q / k heads only
+    float ss = 0.f;
 #pragma unroll
-      for (int i = 0; i < 2; ++i) ss += lo[i] * lo[i] + hi[i] * hi[i];
-      ss = warp_sum(ss);
+    for (int i = 0; i < V; ++i) ss += lo[i] * lo[i] + hi[i] * hi[i];
+#pragma unroll
+    for (int o = 8; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
+    if (active && (is_q || is_k)) {
       const float inv = 1.0f / sqrtf(ss / (float)d + p.eps);
       const __nv_bfloat16 *g = (const __nv_bfloat16 *)(is_q ? p.q_norm : p.k_norm);
 #pragma unroll
-      for (int i = 0; i < 2; ++i)
-        if (i < npair) {
-          const int c = lane + 32 * i;
-          lo[i] = lo[i] * inv * __bfloat162float(g[c]);
-          hi[i] = hi[i] * inv * __bfloat162float(g[c + half]);
-        }
-    }
-    const float2 *rt = reinterpret_cast<const float2 *>(p.rope) + (size_t)pos * half;
-#pragma unroll
-    for (int i = 0; i < 2; ++i)
-      if (i < npair) {
-        const float2 cs = rt[lane + 32 * i];
-        const float a = lo[i], b = hi[i];
-        lo[i] = a * cs.x - b * cs.y;
-        hi[i] = b * cs.x + a * cs.y;
+      for (int i = 0; i < V; ++i) {
+        lo[i] = lo[i] * inv * __bfloat162float(g[c + i]);
+        hi[i] = hi[i] * inv * __bfloat162float(g[c + half + i]);
       }
+    }
+  }
+  if (!active) return;
+  if (is_q || is_k) {
+    const float2 *rt = reinterpret_cast<const float2 *>(p.rope) + (size_t)pos * half + c;
+#pragma unroll
+    for (int i = 0; i < V; ++i) {
+      const float2 cs = rt[i];
+      const float a = lo[i], b = hi[i];
+      lo[i] = a * cs.x - b * cs.y;
+      hi[i] = b * cs.x + a * cs.y;
+    }
   }
   __nv_bfloat16 *dst;
   if (is_q) {
@@ -338,19 +346,21 @@ __global__ void __launch_bounds__(EW_THREADS) qkv_post_kernel(const QkvPostParam
       dst = pool + (((size_t)page * p.n_kv + hk) * 16 + (size_t)(pos & 15)) * d;
     }
   }
-#pragma unroll
-  for (int i = 0; i < 2; ++i)
-    if (i < npair) {
-      const int c = lane + 32 * i;
-      dst[c] = __float2bfloat16_rn(lo[i]);
-      dst[c + half] = __float2bfloat16_rn(hi[i]);
-    }
+  if (V == 4) {
+    *reinterpret_cast<uint2 *>(dst + c) = make_uint2(pack_bf16x2(lo[0], lo[1]), pack_bf16x2(lo[2], lo[3]));
+    *reinterpret_cast<uint2 *>(dst + c + half) = make_uint2(pack_bf16x2(hi[0], hi[1]), pack_bf16x2(hi[2], hi[3]));
+  } else {
+    *reinterpret_cast<uint32_t *>(dst + c) = pack_bf16x2(lo[0], lo[1]);
+    *reinterpret_cast<uint32_t *>(dst + c + half) = pack_bf16x2(hi[0], hi[1]);
+  }
 }
 
 cudaError_t launch_qkv_post(const QkvPostParams &p, cudaStream_t s) {
   const int n_heads = p.n_q + 2 * p.n_kv;
-  dim3 grid(p.T, (n_heads + EW_THREADS / 32 - 1) / (EW_THREADS / 32));
-  return launch_pdl(qkv_post_kernel, dim3(grid), dim3(EW_THREADS), 0, s, p);
+  const int per_block = EW_THREADS / 16;
+  dim3 grid(p.T, (n_heads + per_block - 1) / per_block);
+  if (p.d == 128) return launch_pdl(qkv_post_kernel<4>, dim3(grid), dim3(EW_THREADS), 0, s, p);
+  return launch_pdl(qkv_post_kernel<2>, dim3(grid), dim3(EW_THREADS), 0, s, p);
 }
 
 // ---- KV migration by transfer (NEXT-4): gather a request's pages out of the layer-major pool into one contiguous
