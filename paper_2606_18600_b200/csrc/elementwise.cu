@@ -75,8 +75,9 @@ cudaError_t launch_input_rmsnorm(const CallArgs *args, const void *embed, const 
 // ---- residual += sum_s part[s]; optional RMSNorm -> h; optional bf16 stage output -----------------------------
 // One CTA of 1024 threads per token row; the whole row lives in registers (IT float4 per thread, H <= IT*4096), all
 // loads are issued before any use, and x is read and written exactly once.
-constexpr int RN_THREADS = 1024;
-template <int IT>
+// Few rows (decode): 1024 threads per row for latency.  Many rows (prefill): 256 threads per row, so 8 rows are in
+// flight per SM and the block reduction is two warps deep instead of 32.
+template <int IT, int RN_THREADS>
 __global__ void __launch_bounds__(RN_THREADS)
 residual_rmsnorm_kernel(float *__restrict__ x, const float *__restrict__ part, int splits, long long split_stride,
                         const __nv_bfloat16 *__restrict__ w, float eps, int H, __nv_bfloat16 *__restrict__ h,
@@ -147,15 +148,21 @@ cudaError_t launch_residual_rmsnorm(float *x, const float *part, int splits, lon
   const __nv_bfloat16 *w = (const __nv_bfloat16 *)ln_w;
   __nv_bfloat16 *hh = (__nv_bfloat16 *)h;
   const int wo = write_out_hidden ? 1 : 0;
-  const int it = (H + RN_THREADS * 4 - 1) / (RN_THREADS * 4);
-  if (it <= 1)
-    return launch_pdl(residual_rmsnorm_kernel<1>, dim3(T), dim3(RN_THREADS), 0, s, x, part, splits, split_stride, w, eps, H, hh, args, wo);
-  else if (it <= 2)
-    return launch_pdl(residual_rmsnorm_kernel<2>, dim3(T), dim3(RN_THREADS), 0, s, x, part, splits, split_stride, w, eps, H, hh, args, wo);
-  else if (it <= 4)
-    return launch_pdl(residual_rmsnorm_kernel<4>, dim3(T), dim3(RN_THREADS), 0, s, x, part, splits, split_stride, w, eps, H, hh, args, wo);
-  else
-    return cudaErrorInvalidValue;  // hidden > 16384 is rejected at create
+  auto go = [&](auto kernel, int threads) {
+    return launch_pdl(kernel, dim3(T), dim3(threads), 0, s, x, part, splits, split_stride, w, eps, H, hh, args, wo);
+  };
+  if (T >= 512 && H <= 16 * 256 * 4) {  // many rows: 256 threads each
+    const int it = (H + 1023) / 1024;
+    if (it <= 2) return go(residual_rmsnorm_kernel<2, 256>, 256);
+    if (it <= 4) return go(residual_rmsnorm_kernel<4, 256>, 256);
+    if (it <= 8) return go(residual_rmsnorm_kernel<8, 256>, 256);
+    return go(residual_rmsnorm_kernel<16, 256>, 256);
+  }
+  const int it = (H + 4095) / 4096;
+  if (it <= 1) return go(residual_rmsnorm_kernel<1, 1024>, 1024);
+  if (it <= 2) return go(residual_rmsnorm_kernel<2, 1024>, 1024);
+  if (it <= 4) return go(residual_rmsnorm_kernel<4, 1024>, 1024);
+  return cudaErrorInvalidValue;  // hidden > 16384 is rejected at create
 }
 
 // ---- S11a: final RMSNorm of the last row of each sequence -----------------------------------------------------
