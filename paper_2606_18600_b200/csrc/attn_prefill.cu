@@ -207,9 +207,13 @@ __global__ void __launch_bounds__(PA_WARPS * 32, 3) prefill_attn_kernel(const Pr
     rs1 += __shfl_xor_sync(0xffffffffu, rs1, 2);
     l_run[0] = l_run[0] * a0 + rs0;
     l_run[1] = l_run[1] * a1 + rs1;
+    // the running maxima settle after the first few key tiles: skip the 64 multiplies when no row of the warp moved
+    // (alpha == 1 exactly then, so skipping changes no bit)
+    if (__any_sync(0xffffffffu, a0 != 1.0f || a1 != 1.0f)) {
 #pragma unroll
-    for (int t = 0; t < NT; ++t) {
-      o[t][0] *= a0; o[t][1] *= a0; o[t][2] *= a1; o[t][3] *= a1;
+      for (int t = 0; t < NT; ++t) {
+        o[t][0] *= a0; o[t][1] *= a0; o[t][2] *= a1; o[t][3] *= a1;
+      }
     }
     // ---- O += P V
     {
