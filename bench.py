@@ -32,7 +32,7 @@ def parse():
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "cfg5", "migrate", "tiny"])
+    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "cfg5", "migrate", "pipeline", "tiny"])
     ap.add_argument("--seed", type=int, default=0)
     ap.add_argument("--layers", type=int, default=0, help="override the stage depth (debug only; marks the line)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -143,6 +143,8 @@ def workload_spec(name, layers_override=0):
         shape, ctx, kind = synth.QWEN32B, None, "online"
     elif name == "migrate":
         shape, ctx, kind = synth.LLAMA70B, None, "migrate"
+    elif name == "pipeline":
+        shape, ctx, kind = synth.LLAMA70B, synth.cfg2_contexts, "pipeline"
     else:
         shape, ctx, kind = synth.TINY, synth.cfg1_contexts, "decode"
     L = layers_override or shape.n_layers
@@ -436,6 +438,79 @@ def run_migrate(args, shape):
     return rows
 
 
+def run_pipeline(args, shape, ctx_fn):
+    """SURVEY 8(f) NEXT-2 / Eq. 5: an 80-layer 70B-shaped model cut into 4 stages, evenly (20 x 4) and
+    unevenly (12 + 28 + 20 + 20, the paper's asymmetric partitioning).  The box has ONE B200, so each
+    stage is measured alone, exactly as its own GPU would run it (cfg-2 micro-batch, B = 64; the last stage with the
+    final norm + lm_head + argmax tail); the hop between stages is MODELLED (one [B, H] bf16 message over NVLink 5,
+    900 GB/s + 10 us).  With M >= P micro-batches in flight (paper_2606_18600_b200/pipeline.py) every tick delivers one
+    micro-batch iteration, so throughput = B / (max_i L^i + hop): the slowest stage sets it."""
+    import torch
+    from paper_2606_18600_b200 import binding, estimator, synth
+    dev = torch.device("cuda:0")
+    torch.cuda.set_device(dev)
+    K, W = args.steps, args.warmup
+    pk = peaks()
+    rng = np.random.default_rng(args.seed)
+    ctx0 = ctx_fn(args.seed).astype(np.int32)
+    B = len(ctx0)
+    steps = 2 * (K + W) + 4
+    pb = synth.paged_batch(rng, ctx0, extra_tokens=steps + 1)
+    splits = {"even": [20, 20, 20, 20], "uneven": [12, 28, 20, 20]}
+    depths = sorted({l for v in splits.values() for l in v})
+    layers = gpu_weights(synth.ModelShape(shape.name, shape.hidden, shape.n_q, shape.n_kv, shape.d, shape.ffn,
+                                          max(depths), shape.eps, shape.theta, shape.qk_norm, shape.vocab), dev, args.seed)
+    g = torch.Generator(device=dev)
+    g.manual_seed(args.seed + 99)
+    edge = {"embed": None, "final_norm": torch.ones(shape.hidden, device=dev, dtype=torch.bfloat16),
+            "lm_head": (torch.randn((shape.vocab, shape.hidden), generator=g, device=dev) * 0.02).to(torch.bfloat16)}
+    bank = [torch.randn((B, shape.hidden), generator=g, device=dev, dtype=torch.float32).to(torch.bfloat16)
+            for _ in range(8)]
+    bt = torch.from_numpy(pb.block_tables).to(dev)
+    ctx_steps = torch.from_numpy(ctx0[None, :] + np.arange(steps, dtype=np.int32)[:, None]).to(dev).contiguous()
+    out = torch.empty((B, shape.hidden), dtype=torch.bfloat16, device=dev)
+    am = torch.empty((B,), dtype=torch.int32, device=dev)
+    measured, launches = {}, 0
+    sampler = ClockSampler(0)
+    sampler.start()
+    for l in depths:
+        for tail in (False, True):
+            if tail and l != splits["even"][-1] and l != splits["uneven"][-1]:
+                continue
+            dims = binding.make_dims(shape, max_tokens=B, max_seqs=B, max_blocks=pb.max_blocks,
+                                     max_pos=int(ctx0.max()) + steps + 64, n_layers_total=80)
+            st = binding.Stage(dims, 80 - l if tail else 0, 80 if tail else l, layers[:l], edge if tail else None,
+                               n_pages=pb.n_pages_pool, device=dev)
+            _fill_randn(st.kv_pool.view(-1), g)
+            torch.cuda.synchronize(dev)
+            no = [0]
+
+            def one(i):
+                kw = dict(out_argmax=am) if tail else dict(out_hidden=out)
+                st.decode(B, bt, ctx_steps[no[0]], hidden=bank[no[0] % 8], **kw)
+                no[0] += 1
+
+            for i in range(W):
+                one(i)
+            n0 = st.launch_count()
+            measured[(l, tail)] = cuda_time_ms(st.stream, one, K) / K
+            launches += st.launch_count() - n0
+            st.destroy()
+    clocks = sampler.stop()
+    hop_ms = (B * shape.hidden * 2 / 900e9 + 10e-6) * 1e3
+    rows = []
+    for name, cut in splits.items():
+        Li = [measured[(l, i == len(cut) - 1)] for i, l in enumerate(cut)]
+        est = [estimator.decode_step_ms(synth.ModelShape(shape.name, shape.hidden, shape.n_q, shape.n_kv, shape.d,
+                                                         shape.ffn, l, shape.eps, shape.theta, shape.qk_norm, shape.vocab),
+                                        ctx0, pk["bf16_tflops"] * 1e12, pk["hbm_gbs"] * 1e9) for l in cut]
+        rows.append({"split": name, "layers": cut, "stage_ms_measured": Li, "stage_ms_estimator_no_tail": est,
+                     "max_stage_ms": max(Li), "sum_stage_ms": sum(Li), "hop_ms_modelled": hop_ms,
+                     "tokens_per_s": B / ((max(Li) + hop_ms) * 1e-3),
+                     "token_latency_ms": sum(Li) + (len(cut) - 1) * hop_ms})
+    return rows, B, launches, clocks
+
+
 def run_online(args, shape, rank, world):
     """cfg5: online mixed batches (96 decode rows + <= 4 prefill chunks of <= 512 tokens per ss_stage_prefill call)
     driven by paper_2606_18600_b200/online.py over a page pool at ~85% occupancy; K timed iterations."""
@@ -540,6 +615,7 @@ def main():
                         "cfg4": "configs[3]: migration recompute prefill, 70B shapes, 32 requests lognormal(med 1200)",
                         "cfg5": "configs[4]: online mixed batches, Qwen3-32B shapes",
                         "migrate": "migration of one request: recomputation vs KV transfer",
+                        "pipeline": "80-layer 70B-shaped model in 4 stages (even / uneven), per-stage decode latency",
                         "tiny": "configs[0]: tiny Llama-style stage"}[args.workload],
            "layers": shape.n_layers, "hidden": shape.hidden, "ffn": shape.ffn, "heads": f"{shape.n_q}/{shape.n_kv}",
            "page_size": 16, "seed": args.seed, "parallelism": f"replicas x{world}",
@@ -551,7 +627,7 @@ def main():
     if args.impl == "reference":
         if rank != 0:
             return
-        if kind in ("online", "migrate"):
+        if kind in ("online", "migrate", "pipeline"):
             raise SystemExit("--impl reference covers cfg2/cfg3/cfg4/tiny (the oracle has no online driver)")
         ts = []
         T = cores = desc = None
@@ -584,6 +660,20 @@ def main():
                           "dtype": "bf16", "data": "synthetic",
                           "config": {"workload": "70B-shaped 20-layer stage, one request, contexts 1K-64K",
                                      "link": "modelled: NVLink 5, 900 GB/s per direction (single-GPU box)"},
+                          "rows": rows}))
+        return
+    if kind == "pipeline":
+        if rank != 0:
+            return
+        rows, B, launches, clocks = run_pipeline(args, shape, len_fn)
+        best = max(r["tokens_per_s"] for r in rows)
+        print(json.dumps({"metric": "4-stage pipeline decode tokens/s, throughput = B / (max_i L^i + hop) (Eq. 5)",
+                          "value": best, "unit": "tokens/s", "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+                          "higher_is_better": True, "dtype": "bf16", "data": "synthetic", "gpu_launches": int(launches),
+                          "clocks": clocks,
+                          "config": {"workload": "80-layer 70B-shaped model in 4 stages, cfg-2 micro-batch (B=64) per "
+                                                 "stage per tick; stages measured one at a time on one B200, hop modelled "
+                                                 "(NVLink 5: 900 GB/s + 10 us)", "micro_batches": ">= 4 (pipeline full)"},
                           "rows": rows}))
         return
     if kind == "online":

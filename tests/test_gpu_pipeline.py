@@ -98,3 +98,111 @@ def test_uneven_three_stage_pipeline_vs_oracle():
     finally:
         for st in stages:
             st.destroy()
+
+
+# ---- two processes, one stage each, micro-batched (paper_2606_18600_b200/pipeline.py) --------------------------------
+# The box has one GPU: both ranks open cuda:0 and talk through gloo with host staging (wire="host"); the ranks never
+# wait on each other inside a kernel, only in the host-side exchange.  What must hold: the pipelined run generates
+# exactly the tokens of the same two stages called one after the other in ONE process (same kernels, same shapes).
+_CUTS2 = [(0, 2), (2, 6)]
+_LENS2 = [np.array([21, 64, 5], dtype=np.int32), np.array([130, 17], dtype=np.int32)]
+_ITERS2 = 4
+
+
+def _pipe_problem():
+    base = synth.TINY_QWEN
+    shape = synth.ModelShape(base.name, base.hidden, base.n_q, base.n_kv, base.d, base.ffn, 6, base.eps, base.theta,
+                             base.qk_norm, base.vocab)
+    rng = np.random.default_rng(33)
+    all_lens = np.concatenate(_LENS2)
+    pb = synth.paged_batch(rng, all_lens, extra_tokens=_ITERS2 + 1, pool_factor=1.5)
+    batches, r0 = [], 0
+    for lens in _LENS2:
+        batches.append(dict(lens=lens, block_tables=pb.block_tables[r0:r0 + len(lens)],
+                            prompt=rng.integers(0, shape.vocab, int(lens.sum())).astype(np.int32)))
+        r0 += len(lens)
+    return shape, pb, batches
+
+
+def _build_stage(shape, pb, l0, l1):
+    tw, _ = hp.weights_bits(shape, 33)
+    edge = {k: v.to(DEV) for k, v in synth.edge_weights(shape, 33).items()}
+    L = shape.n_layers
+    T = int(max(l.sum() for l in _LENS2))
+    dims = binding.make_dims(shape, max_tokens=T + 8, max_seqs=8, max_blocks=pb.max_blocks, n_layers_total=L)
+    dw = [{k: (None if v is None else v.to(DEV)) for k, v in tw[l].items()} for l in range(l0, l1)]
+    e = {"embed": edge["embed"] if l0 == 0 else None, "final_norm": edge["final_norm"] if l1 == L else None,
+         "lm_head": edge["lm_head"] if l1 == L else None}
+    return binding.Stage(dims, l0, l1, dw, e, n_pages=pb.n_pages_pool, device=DEV)
+
+
+def _pipe_rank(rank, world, port, q):
+    import os
+    import torch.distributed as dist
+    from paper_2606_18600_b200 import pipeline
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    shape, pb, batches = _pipe_problem()
+    st = _build_stage(shape, pb, *_CUTS2[rank])
+    try:
+        pl = pipeline.StagePipeline(st, rank, world, batches, _ITERS2, shape.hidden, DEV, wire="host")
+        gen = pl.run()
+        launches = st.launch_count()
+    finally:
+        st.destroy()
+    dist.barrier()
+    dist.destroy_process_group()
+    q.put((rank, {k: v.tolist() for k, v in gen.items()}, launches))
+
+
+def test_two_process_microbatched_pipeline_equals_in_process_chain():
+    import os
+    import torch.multiprocessing as mp
+    shape, pb, batches = _pipe_problem()
+    # in-process chain: stage 0 then stage 1, micro-batch after micro-batch, greedy feedback
+    stages = [_build_stage(shape, pb, *c) for c in _CUTS2]
+    want = {}
+    try:
+        for j, b in enumerate(batches):
+            lens = b["lens"]
+            n, T = len(lens), int(lens.sum())
+            cu = _i32(np.concatenate([[0], np.cumsum(lens)]))
+            bt, zero = _i32(b["block_tables"]), _i32(np.zeros_like(lens))
+            tok = _i32(b["prompt"])
+            for t in range(_ITERS2):
+                rows = T if t == 0 else n
+                h = torch.empty((rows, shape.hidden), dtype=torch.bfloat16, device=DEV)
+                am = torch.empty((n,), dtype=torch.int32, device=DEV)
+                torch.cuda.synchronize()
+                if t == 0:
+                    stages[0].prefill(n, cu, zero, bt, T, token_ids=tok, out_hidden=h)
+                    stages[0].synchronize()
+                    stages[1].prefill(n, cu, zero, bt, T, hidden=h, out_argmax=am)
+                else:
+                    ctx = _i32(lens + t - 1)
+                    torch.cuda.synchronize()
+                    stages[0].decode(n, bt, ctx, token_ids=tok, out_hidden=h)
+                    stages[0].synchronize()
+                    stages[1].decode(n, bt, ctx, hidden=h, out_argmax=am)
+                stages[1].synchronize()
+                want[(t, j)] = am.cpu().tolist()
+                tok = am
+    finally:
+        for st in stages:
+            st.destroy()
+    ctx_mp = mp.get_context("spawn")
+    q = ctx_mp.Queue()
+    port = 35000 + os.getpid() % 2000
+    ps = [ctx_mp.Process(target=_pipe_rank, args=(r, 2, port, q)) for r in range(2)]
+    for p in ps:
+        p.start()
+    res = {}
+    for _ in ps:
+        r, gen, launches = q.get(timeout=300)
+        res[r] = (gen, launches)
+    for p in ps:
+        p.join(120)
+        assert p.exitcode == 0
+    assert {tuple(k): v for k, v in res[1][0].items()} == want
+    assert res[0][0] == {} and res[0][1] > 0 and res[1][1] > 0           # both ranks launched their own kernels
+    assert len(want) == _ITERS2 * len(batches) and len({tuple(v) for v in want.values()}) > 1

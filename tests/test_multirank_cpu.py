@@ -108,3 +108,100 @@ def test_tensor_parallel_sharding_algebra_gloo_world2():
         p.join(60)
         assert p.exitcode == 0
     assert res == {0: True, 1: True}
+
+
+# ---- NEXT-2: the micro-batched pipeline driver (paper_2606_18600_b200/pipeline.py) on gloo, host logic only ----
+_PIPE_H, _PIPE_N, _PIPE_T = 6, [3, 5, 2, 4], [7, 9, 4, 6]     # hidden size, sequences and prompt tokens per micro-batch
+
+
+def _toy_stage(r, P):
+    """a stand-in for a stage's arithmetic (exact in fp32): embeds on stage 0, emits tokens on the last stage"""
+    def compute(t, j, inp, out):
+        x = inp
+        if r == 0:
+            x = (inp.to(torch.float32) % 13).unsqueeze(1) + 0.5 * torch.arange(_PIPE_H, dtype=torch.float32) + t
+        x = x * (r + 2) + j + 1
+        if r == P - 1:
+            x = (x[:out.numel()].sum(1).to(torch.int64) % 101).to(torch.int32)
+        out.copy_(x)
+    return compute
+
+
+def _toy_prompt(j):
+    return (torch.arange(_PIPE_T[j], dtype=torch.int32) * 3 + j) % 29
+
+
+def _pipe_worker(rank, world, port, M, n_iters, out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    sys.path.insert(0, ROOT)
+    from paper_2606_18600_b200 import pipeline
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    drv = pipeline.PipelineRank(rank, world, M, n_iters, _PIPE_H, rows=lambda t, j: _PIPE_T[j] if t == 0 else _PIPE_N[j],
+                                n_tok=lambda j: _PIPE_N[j], compute=_toy_stage(rank, world), first_tokens=_toy_prompt,
+                                hidden_dtype=torch.float32, wire="host")
+    gen = drv.run()
+    dist.barrier()
+    dist.destroy_process_group()
+    out.put((rank, {k: v.tolist() for k, v in gen.items()}, drv.ticks))
+
+
+def _pipe_sequential(P, M, n_iters):
+    want = {}
+    for j in range(M):
+        tok = _toy_prompt(j)
+        for t in range(n_iters):
+            x = tok
+            for r in range(P):
+                rows = _PIPE_T[j] if t == 0 else _PIPE_N[j]
+                o = torch.empty((_PIPE_N[j],), dtype=torch.int32) if r == P - 1 else torch.empty((rows, _PIPE_H))
+                _toy_stage(r, P)(t, j, x, o)
+                x = o
+            want[(t, j)] = x.tolist()
+            tok = x
+    return want
+
+
+def test_pipeline_schedule_closed_forms():
+    sys.path.insert(0, ROOT)
+    from paper_2606_18600_b200 import pipeline
+    # full pipeline (M >= P): one item per tick, n_items + P - 1 ticks (fill + drain), the max-of-stages regime of Eq. 5
+    for P, M, n in [(1, 1, 5), (2, 2, 3), (3, 4, 6), (4, 4, 2), (4, 9, 3)]:
+        assert pipeline.item_starts(P, M, n) == list(range(M * n)) and pipeline.n_ticks(P, M, n) == M * n + P - 1
+    # M < P: every iteration of a micro-batch waits for its own tokens: P ticks per iteration, P - M of them bubbles
+    for P, M, n in [(3, 1, 4), (4, 2, 3), (5, 3, 2)]:
+        s = pipeline.item_starts(P, M, n)
+        assert all(s[t * M + j] == t * P + j for t in range(n) for j in range(M))
+        assert pipeline.n_ticks(P, M, n) == (n - 1) * P + M - 1 + P
+    # causality for arbitrary (P, M): stage 0 never runs (t, j) before the last stage finished (t - 1, j)
+    for P in range(1, 6):
+        for M in range(1, 7):
+            s = pipeline.item_starts(P, M, 4)
+            assert all(s[k] >= s[k - M] + P for k in range(M, len(s))) and all(b > a for a, b in zip(s, s[1:]))
+
+
+def _run_pipe(world, M, n_iters):
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 33000 + (os.getpid() * 7 + world * 13 + M) % 2000
+    ps = [ctx.Process(target=_pipe_worker, args=(r, world, port, M, n_iters, q)) for r in range(world)]
+    for p in ps:
+        p.start()
+    res = {}
+    for _ in ps:
+        r, gen, ticks = q.get(timeout=180)
+        res[r] = (gen, ticks)
+    for p in ps:
+        p.join(60)
+        assert p.exitcode == 0
+    return res
+
+
+def test_pipeline_driver_gloo_world3_full_and_bubbled():
+    sys.path.insert(0, ROOT)
+    from paper_2606_18600_b200 import pipeline
+    for M in (4, 2):                                         # M >= P: full pipeline; M < P: bubbles
+        res = _run_pipe(3, M, 4)
+        want = _pipe_sequential(3, M, 4)
+        assert {tuple(k): v for k, v in res[2][0].items()} == want       # the last stage saw every (t, j), right values
+        assert res[0][0] == {} and res[1][0] == {}
+        assert all(res[r][1] == pipeline.n_ticks(3, M, 4) for r in range(3))
