@@ -32,7 +32,7 @@ def parse():
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "cfg5", "migrate", "pipeline", "tiny"])
+    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "cfg5", "migrate", "pipeline", "estimator", "tiny"])
     ap.add_argument("--seed", type=int, default=0)
     ap.add_argument("--layers", type=int, default=0, help="override the stage depth (debug only; marks the line)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -145,6 +145,8 @@ def workload_spec(name, layers_override=0):
         shape, ctx, kind = synth.LLAMA70B, None, "migrate"
     elif name == "pipeline":
         shape, ctx, kind = synth.LLAMA70B, synth.cfg2_contexts, "pipeline"
+    elif name == "estimator":
+        shape, ctx, kind = synth.LLAMA70B, None, "estimator"
     else:
         shape, ctx, kind = synth.TINY, synth.cfg1_contexts, "decode"
     L = layers_override or shape.n_layers
@@ -511,6 +513,85 @@ def run_pipeline(args, shape, ctx_fn):
     return rows, B, launches, clocks
 
 
+def run_estimator(args, shape):
+    """SURVEY 8(f) NEXT-3, the Fig. 8 question asked of this B200: how well does the paper's static
+    estimator (Eq. 1 + Table 2, computed by libshuntplace's sp_stage_latency) predict a stage's measured latency?  The
+    paper's protocol: S_in = 763, S_out = 232, static batches of 1-32, pipeline depths PP2 / PP4 / PP8 of an 80-layer
+    70B-shaped model (40 / 20 / 10 layers per stage; TP1), prefill latency and the total over the 232 decode
+    iterations, MAPE over the configurations.  Two predictions: with the peaks of MEASURED_PEAKS.json, and after the
+    paper's "one-time hardware calibration (FLOPS, memory bandwidth)": effective FLOPS from ONE measured prefill and
+    effective bandwidth from ONE measured decode run (20 layers, batch 32), applied to every other configuration."""
+    import torch
+    from paper_2606_18600_b200 import binding, placement, synth
+    dev = torch.device("cuda:0")
+    torch.cuda.set_device(dev)
+    pk = peaks()
+    S_in, S_out = 763, 232
+    depths, batches = [10, 20, 40], [1, 2, 4, 8, 16, 32]
+    mk = lambda l: synth.ModelShape(shape.name, shape.hidden, shape.n_q, shape.n_kv, shape.d, shape.ffn, l, shape.eps,
+                                    shape.theta, shape.qk_norm, shape.vocab)
+    layers = gpu_weights(mk(max(depths)), dev, args.seed)
+    g = torch.Generator(device=dev)
+    g.manual_seed(args.seed + 5)
+    Bmax = max(batches)
+    x = torch.randn((Bmax * S_in, shape.hidden), generator=g, device=dev, dtype=torch.float32).to(torch.bfloat16)
+    out = torch.empty_like(x)
+    rows, launches = [], 0
+    sampler = ClockSampler(0)
+    sampler.start()
+    for l in depths:
+        for B in batches:
+            lens = np.full(B, S_in, dtype=np.int32)
+            pb = synth.paged_batch(np.random.default_rng(args.seed), lens, extra_tokens=S_out + 2)
+            dims = binding.make_dims(shape, max_tokens=B * S_in, max_seqs=B, max_blocks=pb.max_blocks,
+                                     max_pos=S_in + S_out + 64, n_layers_total=80)
+            st = binding.Stage(dims, 0, l, layers[:l], None, n_pages=pb.n_pages_pool, device=dev)
+            i32 = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.int32)).to(dev)
+            cu, zero, bt = i32(np.arange(B + 1) * S_in), i32(np.zeros(B)), i32(pb.block_tables)
+            ctx = i32(S_in + np.arange(S_out)[:, None] + np.zeros((1, B), dtype=np.int32))
+            T = B * S_in
+            torch.cuda.synchronize(dev)
+            n0 = st.launch_count()
+            pre = lambda i: st.prefill(B, cu, zero, bt, T, hidden=x[:T], out_hidden=out[:T])
+            pre(0)
+            pre_ms = cuda_time_ms(st.stream, pre, 2) / 2
+            dec = lambda i: st.decode(B, bt, ctx[i], hidden=x[i * B:(i + 1) * B], out_hidden=out[:B])
+            for i in range(3):
+                dec(i)
+            dec_ms = cuda_time_ms(st.stream, dec, S_out)
+            launches += st.launch_count() - n0
+            st.destroy()
+            rows.append({"layers": l, "B": B, "prefill_ms": pre_ms, "decode_total_ms": dec_ms})
+    clocks = sampler.stop()
+    m = placement.sp_model(shape.hidden, shape.hq, shape.hkv, shape.ffn, 0, 80, 2)
+    o = placement.sp_opts(s_in=S_in, s_out=S_out, alpha_inter=0.0, beta_inter=1e30, beam=1, max_stages=8)
+
+    def predict(flops, bw, l, B, phase):
+        inst = placement.sp_instance(flops, bw, 180e9, 1, 0.0, 1.0, 1.0)
+        return 1e3 * placement.stage_latency(m, inst, o, l, B, phase, False, False)
+
+    peak_f, peak_b = pk["bf16_tflops"] * 1e12, pk["hbm_gbs"] * 1e9
+    cal = next(r for r in rows if r["layers"] == 20 and r["B"] == 32)
+    # one-time calibration: the estimator is linear in 1/FLOPS when compute-bound and in 1/BW when memory-bound
+    f_eff = peak_f * predict(peak_f, 1e30, 20, 32, 0) / cal["prefill_ms"]
+    b_eff = peak_b * predict(1e30, peak_b, 20, 32, 1) / cal["decode_total_ms"]
+    errs = {"peaks": [], "calibrated": []}
+    for r in rows:
+        meas = r["prefill_ms"] + r["decode_total_ms"]
+        for name, (f, b) in {"peaks": (peak_f, peak_b), "calibrated": (f_eff, b_eff)}.items():
+            pred = predict(f, b, r["layers"], r["B"], 0) + predict(f, b, r["layers"], r["B"], 1)
+            r[f"predicted_ms_{name}"] = pred
+            r[f"err_pct_{name}"] = 100.0 * (pred - meas) / meas
+            if not (name == "calibrated" and r is cal):
+                errs[name].append(abs(pred - meas) / meas)
+    return {"rows": rows, "mape_pct_peaks": 100 * float(np.mean(errs["peaks"])),
+            "mape_pct_calibrated": 100 * float(np.mean(errs["calibrated"])),
+            "max_err_pct_calibrated": 100 * float(np.max(errs["calibrated"])),
+            "calibration": {"config": "20 layers, B=32", "flops_eff_TFLOPs": f_eff / 1e12, "bw_eff_GBs": b_eff / 1e9,
+                            "peaks": {"bf16_tflops": pk["bf16_tflops"], "hbm_gbs": pk["hbm_gbs"]}},
+            "launches": launches, "clocks": clocks}
+
+
 def run_online(args, shape, rank, world):
     """cfg5: online mixed batches (96 decode rows + <= 4 prefill chunks of <= 512 tokens per ss_stage_prefill call)
     driven by paper_2606_18600_b200/online.py over a page pool at ~85% occupancy; K timed iterations."""
@@ -616,6 +697,7 @@ def main():
                         "cfg5": "configs[4]: online mixed batches, Qwen3-32B shapes",
                         "migrate": "migration of one request: recomputation vs KV transfer",
                         "pipeline": "80-layer 70B-shaped model in 4 stages (even / uneven), per-stage decode latency",
+                        "estimator": "estimator accuracy (Fig. 8 protocol), 70B shapes",
                         "tiny": "configs[0]: tiny Llama-style stage"}[args.workload],
            "layers": shape.n_layers, "hidden": shape.hidden, "ffn": shape.ffn, "heads": f"{shape.n_q}/{shape.n_kv}",
            "page_size": 16, "seed": args.seed, "parallelism": f"replicas x{world}",
@@ -627,7 +709,7 @@ def main():
     if args.impl == "reference":
         if rank != 0:
             return
-        if kind in ("online", "migrate", "pipeline"):
+        if kind in ("online", "migrate", "pipeline", "estimator"):
             raise SystemExit("--impl reference covers cfg2/cfg3/cfg4/tiny (the oracle has no online driver)")
         ts = []
         T = cores = desc = None
@@ -661,6 +743,21 @@ def main():
                           "config": {"workload": "70B-shaped 20-layer stage, one request, contexts 1K-64K",
                                      "link": "modelled: NVLink 5, 900 GB/s per direction (single-GPU box)"},
                           "rows": rows}))
+        return
+    if kind == "estimator":
+        if rank != 0:
+            return
+        r = run_estimator(args, shape)
+        print(json.dumps({"metric": "MAPE of the paper's static estimator against measured stage latency (prefill of "
+                                    "763 tokens + 232 decode iterations), percent", "value": r["mape_pct_calibrated"],
+                          "unit": "percent", "higher_is_better": False, "n_gpus": 1, "dtype": "bf16",
+                          "data": "synthetic", "gpu_launches": int(r["launches"]), "clocks": r["clocks"],
+                          "mape_pct_with_measured_peaks": r["mape_pct_peaks"],
+                          "mape_pct_after_one_time_calibration": r["mape_pct_calibrated"],
+                          "max_err_pct_after_calibration": r["max_err_pct_calibrated"], "calibration": r["calibration"],
+                          "config": {"workload": "Fig. 8 protocol on one B200: 70B shapes, stages of 10 / 20 / 40 layers "
+                                                 "(PP8 / PP4 / PP2, TP1), batch 1-32, S_in 763, S_out 232",
+                                     "paper_mape_pct": 6.63}, "rows": r["rows"]}))
         return
     if kind == "pipeline":
         if rank != 0:
