@@ -25,12 +25,40 @@ constexpr int PA_BN = 64;  // keys per tile
 __global__ void prefill_plan_kernel(const CallArgs *__restrict__ args, int n_seqs, int seq0, PrefillPlan plan) {
   pdl_launch_dependents();
   pdl_wait();
-  if (blockIdx.x == 0 && threadIdx.x == 0) {
-    int acc = 0;
-    plan.tile_cum[0] = 0;
-    for (int s = 0; s < n_seqs; ++s) {
-      if (s >= seq0) acc += (args->cu_q[s + 1] - args->cu_q[s] + PA_BM - 1) / PA_BM;
-      plan.tile_cum[s + 1] = acc;
+  if (blockIdx.x == 0) {
+    __shared__ int n_tiles_s;
+    if (threadIdx.x == 0) {
+      int acc = 0;
+      plan.tile_cum[0] = 0;
+      for (int s = 0; s < n_seqs; ++s) {
+        if (s >= seq0) acc += (args->cu_q[s + 1] - args->cu_q[s] + PA_BM - 1) / PA_BM;
+        plan.tile_cum[s + 1] = acc;
+      }
+      n_tiles_s = acc;
+    }
+    __syncthreads();
+    // launch order = heaviest tile first (keys attended = context + causal prefix): the grid is dispatched in
+    // blockIdx order, and a causal batch in natural order would start its most expensive tiles last
+    const int n = min(n_tiles_s, plan.max_tiles);
+    int32_t *key = plan.tile_order + plan.max_tiles;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+      int lo = 0, hi = n_seqs;
+      while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (plan.tile_cum[mid] <= i) lo = mid; else hi = mid;
+      }
+      const int q_len = args->cu_q[lo + 1] - args->cu_q[lo];
+      key[i] = args->ctx[lo] + min(q_len, (i - plan.tile_cum[lo] + 1) * PA_BM);
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {  // rank sort (stable): n is a few hundred, once per call
+      const int k = key[i];
+      int rank = 0;
+      for (int j = 0; j < n; ++j) {
+        const int kj = key[j];
+        rank += (kj > k || (kj == k && j < i)) ? 1 : 0;
+      }
+      plan.tile_order[rank] = i;
     }
   }
   for (int s = blockIdx.x; s < n_seqs; s += gridDim.x) {
@@ -63,9 +91,10 @@ __global__ void __launch_bounds__(PA_WARPS * 32, 3) prefill_attn_kernel(const Pr
   uint8_t *kv_s = smem;
   uint8_t *q_s = smem + 2 * TILE_BYTES;      // [PA_BM][D], aliases buffer 1
 
-  const int head = blockIdx.x, slot = blockIdx.y;
+  const int head = blockIdx.x;
   const int32_t *tile_cum = p.plan.tile_cum;
-  if (slot >= tile_cum[p.n_seqs]) return;
+  if ((int)blockIdx.y >= tile_cum[p.n_seqs]) return;
+  const int slot = p.plan.tile_order[blockIdx.y];
   int lo = 0, hi = p.n_seqs;  // tile_cum[lo] <= slot < tile_cum[hi]
   while (hi - lo > 1) {
     const int mid = (lo + hi) >> 1;

@@ -167,6 +167,8 @@ struct PrefillPlan {
   int32_t *tok_seq;          // [max_tokens]
   int32_t *tok_pos;          // [max_tokens]
   int32_t *tile_cum;         // [max_seqs+1] prefix sum of 64-row query tiles per sequence
+  int32_t *tile_order;       // [2 * max_tiles]: launch slot -> tile, heaviest (most keys) first; second half = sort keys
+  int max_tiles;             // capacity: max_tokens / 64 + max_seqs + 1
 };
 // seq0: the first seq0 sequences get no query tiles (mixed batches: their attention runs in the decode kernel)
 cudaError_t launch_prefill_plan(const CallArgs *args, int n_seqs, int seq0, PrefillPlan plan, cudaStream_t s);

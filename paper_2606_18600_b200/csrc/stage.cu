@@ -48,7 +48,7 @@ static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Carve {  // byte offsets into the workspace
   size_t args, rope, x, h, qkv_part, q, kv_new, attn_out, fix, a, part_o, part_ml, cum_pages, meta, tp_part, am_part, tok_seq,
-      tok_pos, tile_cum, hl, logits, total;
+      tok_pos, tile_cum, tile_order, hl, logits, total;
 };
 
 static bool dims_ok(const ss_model_dims *d, int l0, int l1, int *why) {
@@ -96,6 +96,7 @@ static Carve carve(const ss_model_dims *d) {
   c.tok_seq = take(Tm * 4);
   c.tok_pos = take(Tm * 4);
   c.tile_cum = take(((size_t)d->max_seqs + 1) * 4);
+  c.tile_order = take(2 * (Tm / 64 + (size_t)d->max_seqs + 1) * 4);
   c.hl = take((size_t)d->max_seqs * H * 2);
   c.logits = take(d->vocab > 0 ? (size_t)d->max_seqs * d->vocab * 4 : 0);
   c.total = o;
@@ -473,7 +474,8 @@ static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T,
   const bool tp = st->allreduce != nullptr;
   float *tp_part = st->at<float>(c.tp_part);
   DecodePlan dplan{st->at<int32_t>(c.cum_pages), st->at<int32_t>(c.meta)};
-  PrefillPlan pplan{st->at<int32_t>(c.tok_seq), st->at<int32_t>(c.tok_pos), st->at<int32_t>(c.tile_cum)};
+  PrefillPlan pplan{st->at<int32_t>(c.tok_seq), st->at<int32_t>(c.tok_pos), st->at<int32_t>(c.tile_cum),
+                    st->at<int32_t>(c.tile_order), (int)(d.max_tokens / 64 + d.max_seqs + 1)};
   if (decode)
     CKE(launch_decode_plan(args, n_seqs, d.n_kv_heads, st->n_workers, dplan, s));
   else {
