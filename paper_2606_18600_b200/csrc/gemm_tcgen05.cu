@@ -595,7 +595,10 @@ void gemm_plan(GemmLaunch &g, int n_sm) {
     if (env_wpol >= 0) p.w_policy = env_wpol;
     p.split = 0;
     if (hbm_bound) {
-      p.issuers = (2 * acc_cols <= 512) ? 2 : 1;
+      // two issuers (one accumulator set each) only while BOTH sets still fit twice in TMEM: with 2 x 256 columns
+      // per item there is no second buffer and the epilogue stops the main loop (T = 256 down projection 119 -> 113 us,
+      // O 51.5 -> 45.5 us, T = 128 gate/up 155.6 -> 153.9 us with one issuer)
+      p.issuers = (4 * acc_cols <= 512) ? 2 : 1;
     } else {
       // measured: splitting each k-block between two issuers does not help here (the tensor pipe waits on L2, not
       // on the issuer: 59% vs 66% active) — one issuer; SS_GEMM_ISSUERS=2 keeps the split path testable
