@@ -520,10 +520,13 @@ int gemm_pick_bn(int T) {
   static int env_bn = -1;
   if (env_bn < 0) env_bn = env_int("SS_GEMM_BN", 0);  // experiments: force the token tile
   if (env_bn > 0) return env_bn;
-  const int c[4] = {32, 64, 128, 256};
-  for (int i = 0; i < 4; ++i)
-    if (T <= c[i]) return c[i];
-  return 256;
+  // the narrowest multiple of 32 columns that covers T in ceil(T / 256) token tiles: a UMMA costs tensor-pipe time and
+  // smem reads in proportion to N, and from ~128 tokens on the decode GEMMs are near the roofline's ridge (256 flop
+  // per weight byte at T = 256 against 1,624 TFLOP/s / 6,545 GB/s = 248), so padded columns are not free
+  if (T <= 32) return 32;
+  const int n_t = (T + 255) / 256;
+  const int per = (T + n_t - 1) / n_t;
+  return (per + 31) / 32 * 32;
 }
 
 size_t gemm_smem_bytes(int bn, bool dual, int stages) {

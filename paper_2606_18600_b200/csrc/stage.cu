@@ -179,7 +179,7 @@ struct ss_stage {
   int n_workers;
   std::vector<LayerMaps> maps;
   CUtensorMap lm_map;
-  CUtensorMap b_h[5], b_attn[5], b_a[5], b_hl[5];  // activation maps for bn = 16,32,64,128,256
+  CUtensorMap b_h[9], b_attn[9], b_a[9], b_hl[9];  // activation maps for bn = 16 and 32, 64, ..., 256 (index bn / 32)
   ss_pool pages;
   int64_t launches;
   std::map<int, Graph> graphs;  // key = batch*2 + tail
@@ -335,8 +335,8 @@ int ss_stage_create(ss_stage **out, const ss_model_dims *dims, int l0, int l1, c
   }
   if (rc == 0 && edge && edge->lm_head)
     rc |= make_tmap_bf16_2d(&st->lm_map, edge->lm_head, (uint64_t)dims->vocab, H, GEMM_BM, true);
-  const int bns[5] = {16, 32, 64, 128, 256};
-  for (int i = 0; i < 5 && rc == 0; ++i) {
+  const int bns[9] = {16, 32, 64, 96, 128, 160, 192, 224, 256};
+  for (int i = 0; i < 9 && rc == 0; ++i) {
     rc |= make_tmap_bf16_2d(&st->b_h[i], st->ws + c.h, Tm, H, bns[i], false);
     rc |= make_tmap_bf16_2d(&st->b_attn[i], st->ws + c.attn_out, Tm, Hq, bns[i], false);
     rc |= make_tmap_bf16_2d(&st->b_a[i], st->ws + c.a, Tm, F, bns[i], false);
@@ -447,7 +447,7 @@ static cudaError_t run_gemm(const ss_stage *st, const CUtensorMap *const a[3], i
   g.dual = dual;
   g.stream = st->stream;
   gemm_plan(g, st->n_sm);
-  g.b = &bmaps[p.bn == 32 ? 1 : p.bn == 64 ? 2 : p.bn == 128 ? 3 : 4];
+  g.b = &bmaps[p.bn / 32];
   return gemm_launch(g);
 }
 
