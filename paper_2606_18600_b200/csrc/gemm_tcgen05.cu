@@ -388,7 +388,8 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(&tempty[buf]);
-        __threadfence();
+        // publish: the barrier orders every epilogue thread's stores before thread 0's gpu-scope fence, which is
+        // cumulative, so one fence (not one per thread before the barrier as well) is on the tile owner's critical path
         epi_bar();
         if (et == 0) {
           __threadfence();
