@@ -348,13 +348,8 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
         c_lo = cta + 1;
         c_hi = cta;
         while (c_hi + 1 < grid && it.range_start(c_hi + 1) < tile_end) ++c_hi;
-        for (int cc = c_lo; cc <= c_hi; ++cc) {
-          uint32_t spins = 0;
-          while (ld_acquire(p.fix_flags + cc) == 0) {
-            if (++spins > (1u << 24)) wait_expired(7, (uint32_t)cc, item);
-          }
-        }
       }
+      bool polled = false;  // the contributors' flags are awaited as late as possible: just before the first fix-up add
 
       if (et == 0) trace(p, 4 + 4 * (int)item);
       mbar_wait_site(&tfull[buf], tph, 6, item);
@@ -412,6 +407,17 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
           ld_acc((uint32_t)c0, v);
           if (DUAL) ld_acc((uint32_t)(bn + c0), u);
           if (et == 0 && item == 1) trace(p, 40 + 3 * (c0 >> 5));
+          if (!polled) {
+            // with this chunk's residual values requested and its accumulator in registers, so that both round trips
+            // overlap the contributors' dump + publish (cfg-2 step 7.355 -> 7.30 ms, cfg-3 5.148 -> 5.12 ms, same box)
+            polled = true;
+            for (int cc = c_lo; cc <= c_hi; ++cc) {
+              uint32_t spins = 0;
+              while (ld_acquire(p.fix_flags + cc) == 0) {
+                if (++spins > (1u << 24)) wait_expired(7, (uint32_t)cc, item);
+              }
+            }
+          }
           for (int cc = c_lo; cc <= c_hi; ++cc) {  // fix-up in CTA order: deterministic sums
             const float *slot = p.fix_slots + (size_t)cc * (DUAL ? 2 : 1) * bn * GEMM_BM;
 #pragma unroll
