@@ -225,6 +225,26 @@ int ss_op_gemm_bf16(const void *x_dev, const void *w_dev, float *c_dev, int T, i
 int ss_op_gemm_swiglu_bf16(const void *x_dev, const void *wg_dev, const void *wu_dev, void *a_dev,
                            int T, int F, int K, void *scratch_dev, size_t scratch_bytes, void *cuda_stream);
 
+/* Shared Tensor Store attach (Section 5.2 "Concurrent initialization", Figure 7).  The paper keeps
+ * the weight tensors and the KV-cache space in a separate per-node process and shares them with the inference engine
+ * "in a zero-copy manner through CUDA IPC handles", so that a replacement engine can be initialised beside the serving
+ * one without a second copy of either.  These calls are that mechanism and nothing more (plain cudaMalloc / cudaIpc*;
+ * no kernel): the STORE process allocates one arena with ss_store_alloc (a whole cudaMalloc allocation, hence
+ * exportable), fills it (ss_store_upload, or any device copy) and hands the 64-byte handle of ss_store_export to the
+ * engines by whatever channel it likes; every ENGINE process calls ss_store_attach, which maps the same physical
+ * memory and returns its device address in that process, carves weights and KV pool out of it at the offsets the store
+ * published, and passes those pointers to ss_stage_create (all of whose device inputs are borrowed).  An engine must
+ * ss_stage_destroy before ss_store_detach; the store must outlive every attachment.  `handle` is HOST memory of
+ * SS_IPC_HANDLE_BYTES.  A handle cannot be opened by the process that exported it (CUDA's rule).  Errors:
+ * SS_ERR_INVALID_ARG (null argument / zero bytes), SS_ERR_CUDA (see ss_last_cuda_error). */
+#define SS_IPC_HANDLE_BYTES 64
+int ss_store_alloc(void **dev_ptr_out, size_t bytes);
+int ss_store_free(void *dev_ptr);
+int ss_store_upload(void *dst_dev, const void *src_host, size_t bytes);   /* synchronous host -> arena copy */
+int ss_store_export(const void *dev_ptr, void *handle_out /* host, SS_IPC_HANDLE_BYTES */);
+int ss_store_attach(const void *handle /* host, SS_IPC_HANDLE_BYTES */, void **dev_ptr_out);
+int ss_store_detach(void *dev_ptr);
+
 const char *ss_strerror(int code);
 const char *ss_last_cuda_error(void); /* text of the last CUDA error seen by this thread ("" if none) */
 const char *ss_version(void);

@@ -24,7 +24,8 @@ EXPORTS = ["ss_stage_workspace_bytes", "ss_kv_page_bytes", "ss_stage_create", "s
            "ss_stage_decode",
            "ss_stage_launch_count", "ss_op_gemm_scratch_bytes", "ss_op_gemm_bf16", "ss_op_gemm_swiglu_bf16", "ss_strerror",
            "ss_last_cuda_error", "ss_version", "ss_debug_buffer", "ss_pool_create", "ss_pool_destroy",
-           "ss_pool_num_pages", "ss_pool_num_free", "ss_pool_alloc", "ss_pool_free", "ss_kv_export", "ss_kv_import", "ss_stage_set_allreduce"]
+           "ss_pool_num_pages", "ss_pool_num_free", "ss_pool_alloc", "ss_pool_free", "ss_kv_export", "ss_kv_import", "ss_stage_set_allreduce",
+           "ss_store_alloc", "ss_store_free", "ss_store_upload", "ss_store_export", "ss_store_attach", "ss_store_detach"]
 
 
 ALLREDUCE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p)
@@ -102,6 +103,12 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     lib.ss_pool_num_free.argtypes = [C.c_void_p]
     lib.ss_pool_alloc.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_int32)]
     lib.ss_pool_free.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_int32)]
+    lib.ss_store_alloc.argtypes = [C.POINTER(C.c_void_p), C.c_size_t]
+    lib.ss_store_free.argtypes = [C.c_void_p]
+    lib.ss_store_upload.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t]
+    lib.ss_store_export.argtypes = [C.c_void_p, C.c_void_p]
+    lib.ss_store_attach.argtypes = [C.c_void_p, C.POINTER(C.c_void_p)]
+    lib.ss_store_detach.argtypes = [C.c_void_p]
     lib.ss_op_gemm_scratch_bytes.restype = C.c_size_t
     lib.ss_op_gemm_bf16.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p,
                                     C.c_size_t, C.c_void_p]

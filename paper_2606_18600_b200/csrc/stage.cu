@@ -34,6 +34,7 @@ bool pdl_enabled() {
 
 static int cuda_fail(cudaError_t e, const char *where) {
   g_cuda_err = std::string(where) + ": " + cudaGetErrorString(e);
+  cudaGetLastError();  // reported through the return code: do not leave a non-sticky error for the caller's next CUDA call
   return SS_ERR_CUDA;
 }
 #define CK(call)                                          \
@@ -389,6 +390,43 @@ int ss_pool_num_pages(const ss_pool *p) { return p ? p->num_pages : SS_ERR_INVAL
 int ss_pool_num_free(const ss_pool *p) { return p ? (int)p->free_list.size() : SS_ERR_INVALID_ARG; }
 int ss_pool_alloc(ss_pool *p, int n, int32_t *out_page_ids) { return p ? p->alloc(n, out_page_ids) : SS_ERR_INVALID_ARG; }
 int ss_pool_free(ss_pool *p, int n, const int32_t *page_ids) { return p ? p->release(n, page_ids) : SS_ERR_INVALID_ARG; }
+
+// ---- Shared Tensor Store attach: plain cudaMalloc + CUDA IPC, no kernel ------------------------
+static_assert(sizeof(cudaIpcMemHandle_t) == SS_IPC_HANDLE_BYTES, "handle size");
+int ss_store_alloc(void **dev_ptr_out, size_t bytes) {
+  if (!dev_ptr_out || bytes == 0) return SS_ERR_INVALID_ARG;
+  CK(cudaMalloc(dev_ptr_out, bytes));
+  return SS_OK;
+}
+int ss_store_free(void *dev_ptr) {
+  if (!dev_ptr) return SS_ERR_INVALID_ARG;
+  CK(cudaFree(dev_ptr));
+  return SS_OK;
+}
+int ss_store_upload(void *dst_dev, const void *src_host, size_t bytes) {
+  if (!dst_dev || !src_host) return SS_ERR_INVALID_ARG;
+  if (bytes) CK(cudaMemcpy(dst_dev, src_host, bytes, cudaMemcpyHostToDevice));
+  return SS_OK;
+}
+int ss_store_export(const void *dev_ptr, void *handle_out) {
+  if (!dev_ptr || !handle_out) return SS_ERR_INVALID_ARG;
+  cudaIpcMemHandle_t h;
+  CK(cudaIpcGetMemHandle(&h, const_cast<void *>(dev_ptr)));
+  memcpy(handle_out, &h, sizeof(h));
+  return SS_OK;
+}
+int ss_store_attach(const void *handle, void **dev_ptr_out) {
+  if (!handle || !dev_ptr_out) return SS_ERR_INVALID_ARG;
+  cudaIpcMemHandle_t h;
+  memcpy(&h, handle, sizeof(h));
+  CK(cudaIpcOpenMemHandle(dev_ptr_out, h, cudaIpcMemLazyEnablePeerAccess));
+  return SS_OK;
+}
+int ss_store_detach(void *dev_ptr) {
+  if (!dev_ptr) return SS_ERR_INVALID_ARG;
+  CK(cudaIpcCloseMemHandle(dev_ptr));
+  return SS_OK;
+}
 
 int64_t ss_stage_launch_count(const ss_stage *st) { return st ? st->launches : 0; }
 
