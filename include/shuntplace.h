@@ -81,6 +81,22 @@ int sp_evaluate(const sp_model *m, const sp_instance *types, int n_types, const 
 int sp_optimize(const sp_model *m, const sp_instance *types, int n_types, const int32_t *avail, const sp_opts *o,
                 sp_placement *out);
 
+/* Request dispatch over the pipelines a placement produced (the global server routes requests to
+ * pipelines; "load balancing via a weighted round-robin policy based on the throughput of each
+ * pipeline").  The paper names the policy, not the variant; reading: SMOOTH weighted round-robin — every
+ * pick adds each pipeline's weight to its running credit, takes the pipeline with the largest credit (lowest index on
+ * ties) and charges it the sum of the weights — which spreads a heavy pipeline's turns instead of bursting them and is
+ * deterministic.  Weights are the pipelines' throughputs (rps of sp_placement, or measured); weight 0 = no traffic (a
+ * pipeline being drained for replacement, section 5.2: the server "stops routing requests to the old pipeline ... and
+ * shunts the request path to the new pipeline").  Changing a weight keeps the credits of the others and clears that
+ * pipeline's own.  Returns: create 0 / -1 (n <= 0, null, negative or non-finite weight); next = pipeline index, or -1
+ * if every weight is 0; set_weight 0 / -1. */
+typedef struct sp_wrr sp_wrr;
+int sp_wrr_create(sp_wrr **out, int n, const double *weights);
+int sp_wrr_destroy(sp_wrr *w);
+int sp_wrr_next(sp_wrr *w);
+int sp_wrr_set_weight(sp_wrr *w, int i, double weight);
+
 #ifdef __cplusplus
 }
 #endif

@@ -159,3 +159,30 @@ def brute_force(m: Model, types, o: Opts, avail=None):
                 if r["batch"] > 0 and (best is None or r["score"] > best[0]["score"]):
                     best = (r, inst, layers)
     return best
+
+
+# ---- request dispatch (weighted round-robin on pipeline throughput; smooth variant) ----
+def wrr_sequence(weights, n, changes=None):
+    """The first n picks.  Each pick: credit_i += w_i for every pipeline with w_i > 0; choose the largest credit (lowest
+    index on ties); credit_chosen -= sum of the positive weights.  `changes` = {pick index: (pipeline, new weight)} applied
+    BEFORE that pick (the changed pipeline's credit restarts at 0).  -1 when no pipeline has a positive weight."""
+    w = [float(x) for x in weights]
+    credit = [0.0] * len(w)
+    out = []
+    for k in range(n):
+        if changes and k in changes:
+            i, nw = changes[k]
+            w[i], credit[i] = float(nw), 0.0
+        live = [i for i in range(len(w)) if w[i] > 0]
+        if not live:
+            out.append(-1)
+            continue
+        for i in live:
+            credit[i] += w[i]
+        best = live[0]
+        for i in live:
+            if credit[i] > credit[best]:
+                best = i
+        credit[best] -= sum(w[i] for i in live)
+        out.append(best)
+    return out

@@ -7,6 +7,7 @@
 #include <string.h>
 
 #include <algorithm>
+#include <cmath>
 #include <vector>
 
 namespace {
@@ -184,6 +185,50 @@ int sp_optimize(const sp_model *m, const sp_instance *types, int n_types, const 
         found = true;
       }
   return found ? 0 : 1;
+}
+
+// ---- request dispatch: smooth weighted round-robin over pipelines (reading in shuntplace.h) ----------
+struct sp_wrr {
+  std::vector<double> weight, credit;
+};
+
+int sp_wrr_create(sp_wrr **out, int n, const double *weights) {
+  if (!out || !weights || n <= 0) return -1;
+  for (int i = 0; i < n; ++i)
+    if (!(weights[i] >= 0.0) || !std::isfinite(weights[i])) return -1;
+  sp_wrr *w = new sp_wrr();
+  w->weight.assign(weights, weights + n);
+  w->credit.assign(n, 0.0);
+  *out = w;
+  return 0;
+}
+
+int sp_wrr_destroy(sp_wrr *w) {
+  if (!w) return -1;
+  delete w;
+  return 0;
+}
+
+int sp_wrr_next(sp_wrr *w) {
+  if (!w) return -1;
+  double total = 0.0;
+  int best = -1;
+  for (size_t i = 0; i < w->weight.size(); ++i) {
+    if (w->weight[i] <= 0.0) continue;
+    w->credit[i] += w->weight[i];
+    total += w->weight[i];
+    if (best < 0 || w->credit[i] > w->credit[best]) best = (int)i;
+  }
+  if (best < 0) return -1;
+  w->credit[best] -= total;
+  return best;
+}
+
+int sp_wrr_set_weight(sp_wrr *w, int i, double weight) {
+  if (!w || i < 0 || i >= (int)w->weight.size() || !(weight >= 0.0) || !std::isfinite(weight)) return -1;
+  w->weight[i] = weight;
+  w->credit[i] = 0.0;
+  return 0;
 }
 
 }  // extern "C"

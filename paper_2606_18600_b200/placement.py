@@ -7,7 +7,8 @@ import ctypes as C
 from . import build as _build
 
 SP_MAX_STAGES = 64
-EXPORTS = ["sp_stage_latency", "sp_max_batch", "sp_evaluate", "sp_optimize"]
+EXPORTS = ["sp_stage_latency", "sp_max_batch", "sp_evaluate", "sp_optimize", "sp_wrr_create", "sp_wrr_destroy",
+           "sp_wrr_next", "sp_wrr_set_weight"]
 
 
 class sp_model(C.Structure):
@@ -48,6 +49,10 @@ def load_library() -> C.CDLL:
                                     C.POINTER(sp_placement)]
         lib.sp_optimize.argtypes = [C.POINTER(sp_model), C.POINTER(sp_instance), C.c_int, C.POINTER(C.c_int32),
                                     C.POINTER(sp_opts), C.POINTER(sp_placement)]
+        lib.sp_wrr_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.POINTER(C.c_double)]
+        lib.sp_wrr_destroy.argtypes = [C.c_void_p]
+        lib.sp_wrr_next.argtypes = [C.c_void_p]
+        lib.sp_wrr_set_weight.argtypes = [C.c_void_p, C.c_int, C.c_double]
         _LIB = lib
     return _LIB
 
@@ -81,3 +86,26 @@ def optimize(model, types, opts, avail=None):
     if rc < 0:
         raise ValueError("sp_optimize: bad input")
     return rc, p
+
+
+class Dispatcher:
+    """sp_wrr_*: smooth weighted round-robin over pipelines, weights = their throughputs."""
+
+    def __init__(self, weights):
+        self.lib = load_library()
+        self.h = C.c_void_p()
+        arr = (C.c_double * max(len(weights), 1))(*[float(w) for w in weights])
+        if self.lib.sp_wrr_create(C.byref(self.h), len(weights), arr) != 0:
+            raise ValueError("sp_wrr_create: bad input")
+
+    def next(self) -> int:
+        return self.lib.sp_wrr_next(self.h)
+
+    def set_weight(self, i: int, w: float) -> None:
+        if self.lib.sp_wrr_set_weight(self.h, i, float(w)) != 0:
+            raise ValueError("sp_wrr_set_weight: bad input")
+
+    def close(self) -> None:
+        if self.h:
+            self.lib.sp_wrr_destroy(self.h)
+            self.h = C.c_void_p()

@@ -32,6 +32,7 @@ def test_library_exports_every_declared_symbol():
     lib = pl.load_library()
     import re
     hdr = open(pl._build.HERE.parent / "include" / "shuntplace.h").read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
     declared = set(re.findall(r"\b(sp_[a-z_]+)\s*\(", hdr))
     assert declared == set(pl.EXPORTS)
     out = subprocess.run(["nm", "-D", "--defined-only", str(pl._build.PLACE_LIB)], capture_output=True, text=True).stdout
@@ -186,3 +187,58 @@ def test_paper_shaped_cluster_llama70b():
         print(f"k={k}: stages {[(['L4x4', 'A10Gx4', 'L40Sx4'][t], l) for t, l in zip(inst, p.layers[:p.n_stages])]}, "
               f"B={p.batch}, rps={p.rps:.3f}, prefill {p.prefill_s:.2f}s decode {p.decode_s:.2f}s, score {p.score:.4f}")
     assert scores[1] >= scores[0] * (1 - 1e-12)
+
+
+# ---- request dispatch: weighted round-robin on pipeline throughput -------------------------------
+def test_wrr_oracle_pins():
+    # the textbook worked example of smooth weighted round-robin: weights 5, 1, 1 -> a a b a c a a, then it repeats
+    assert po.wrr_sequence([5, 1, 1], 14) == [0, 0, 1, 0, 2, 0, 0] * 2
+    # equal weights degenerate to plain round-robin; a single pipeline takes everything; all-zero -> -1
+    assert po.wrr_sequence([3, 3, 3, 3], 8) == [0, 1, 2, 3, 0, 1, 2, 3]
+    assert po.wrr_sequence([0.7], 3) == [0, 0, 0] and po.wrr_sequence([0, 0], 2) == [-1, -1]
+    rng = random.Random(11)
+    for _ in range(50):
+        w = [rng.randint(0, 9) for _ in range(rng.randint(1, 6))]
+        W = sum(w)
+        if W == 0:
+            continue
+        seq = po.wrr_sequence(w, 3 * W)
+        # integer weights: every window of one period holds exactly w_i picks of pipeline i ...
+        for start in (0, W, 2 * W):
+            assert [seq[start:start + W].count(i) for i in range(len(w))] == w
+        # ... and at every prefix each pipeline is within one request of its share (what "smooth" means)
+        cnt = [0] * len(w)
+        for n, i in enumerate(seq, 1):
+            cnt[i] += 1
+            assert all(abs(cnt[j] - n * w[j] / W) < 1.0 + 1e-9 for j in range(len(w)))
+
+
+def test_wrr_library_matches_oracle_including_drain_and_shunt():
+    rng = random.Random(5)
+    for trial in range(30):
+        n = rng.randint(1, 7)
+        w = [rng.choice([0.0, rng.uniform(0.1, 40.0)]) if trial % 3 else float(rng.randint(1, 9)) for _ in range(n)]
+        # a pipeline is drained (weight 0) at some pick and a replacement comes up later (section 5.2)
+        victim = rng.randrange(n)
+        changes = {17: (victim, 0.0), 41: (victim, rng.uniform(0.5, 30.0))}
+        want = po.wrr_sequence(w, 80, changes)
+        d = pl.Dispatcher(w)
+        got = []
+        for k in range(80):
+            if k in changes:
+                d.set_weight(*changes[k])
+            got.append(d.next())
+        d.close()
+        assert got == want
+        assert victim not in got[17:41]
+    with pytest.raises(ValueError):
+        pl.Dispatcher([1.0, -2.0])
+    with pytest.raises(ValueError):
+        pl.Dispatcher([])
+    with pytest.raises(ValueError):
+        pl.Dispatcher([float("nan")])
+    d = pl.Dispatcher([1.0])
+    with pytest.raises(ValueError):
+        d.set_weight(3, 1.0)
+    d.close()
+    assert pl.load_library().sp_wrr_next(None) == -1 and pl.load_library().sp_wrr_destroy(None) == -1
