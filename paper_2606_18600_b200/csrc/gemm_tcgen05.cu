@@ -625,6 +625,24 @@ void gemm_plan(GemmLaunch &g, int n_sm) {
   }
   const long long work = p.sched == SCHED_STREAMK ? n_tiles * nkb : n_tiles;
   g.grid = (int)(work < max_grid ? work : max_grid);
+  {
+    // Stream-K over FEWER tiles than SMs (O / down projections: 40-64 row tiles): a grid that is a multiple of the tile
+    // count cuts every tile into the same whole number of CTA ranges with aligned boundaries, so an owner waits for
+    // exactly k - 1 contributors and no CTA holds pieces of two tiles (148 CTAs over 40 tiles = 3.7 ranges per tile:
+    // 3-4 contributors, most CTAs with two short items).  HBM does not need all 148 SMs to be saturated, the fix-up
+    // tail is what these short GEMMs lose (profiles/r01_v7_cfg3_layer.md).  Same box, alternating: cfg-2 step
+    // 7.287 -> 7.217 ms (grid 128 for 64 tiles), cfg-3 5.10 -> 5.02 ms (grid 120 for 40 tiles); stand-alone O
+    // projection 29.0 -> 26.9 us, down 56.4 -> 53.9 us at T = 128.  Only when that grid keeps >= 80% of the SMs: the
+    // 80-tile QKV projection on 80 CTAs went 36.2 -> 39.3 us at cfg-2 (31.1 -> 30.0 at cfg-3).  Half-integer cuts (140
+    // CTAs for 40 tiles, 120 for 80) measured between the two or within noise of this rule; not used.
+    static int env_al = -1;
+    if (env_al < 0) env_al = env_int("SS_GEMM_ALIGN", 1);
+    if (env_al > 0 && p.sched == SCHED_STREAMK && n_tiles < max_grid && work >= max_grid) {
+      const int nt = (int)n_tiles;
+      const int aligned = (max_grid / nt) * nt;
+      if (aligned * 10 >= max_grid * 8) g.grid = aligned;
+    }
+  }
 }
 
 cudaError_t gemm_set_debug_buffer(unsigned long long *host_mapped) {
