@@ -16,13 +16,23 @@
  *                       reconstruct the KV cache (§5.1).
  *
  * All pointers named "dev" are CUDA device pointers, all others are host pointers.  Nothing in this header is
- * a torch type.  The library never allocates or frees device memory: weights, KV pool, workspace, inputs and
+ * a torch type.  A stage never allocates or frees device memory: weights, KV pool, workspace, inputs and
  * outputs are BORROWED from the caller (this mirrors the paper's engine, which attaches to tensors owned by the
  * Shared Tensor Store).  Borrowed pointers must stay valid and unchanged until ss_stage_destroy.
+ * The one exception in the library is the store side of that mechanism itself: ss_store_alloc / ss_store_free wrap
+ * cudaMalloc / cudaFree so that the arena is a whole allocation and therefore exportable over CUDA IPC.
  *
  * Calls enqueue work on the stage's CUDA stream and return; results are valid after the caller synchronises
  * that stream.  Errors that the host can detect are returned synchronously and nothing is enqueued.  A stage
  * is not thread-safe; distinct stages are independent.
+ *
+ * Environment variables read by the library (all at ss_stage_create, none afterwards; there are no others in a
+ * product build — the GEMM tuning overrides exist only in builds compiled with -DSS_TUNE):
+ *   SS_DEBUG=1    every call first runs the device-side contract checks described at ss_stage_debug_info and waits
+ *                 for their verdict (one stream synchronisation per call);
+ *   SS_NO_GRAPH=1 ss_stage_decode enqueues its kernels directly instead of replaying a captured CUDA graph;
+ *   SS_NO_PDL=1   kernels are launched without programmatic dependent launch (plain stream order).
+ * The last two change scheduling only, never results (tests compare them bit for bit).
  *
  * Readings of points the paper leaves open are listed in DESIGN.md ("Readings"), numbered A1..A22 after
  * SURVEY.md §8(c).
@@ -189,9 +199,10 @@ int64_t ss_stage_launch_count(const ss_stage *st);
  * registered here the O and down projections produce fp32 partials [T, H] and the stage calls
  *     fn(partial, T * H, user, cuda_stream)
  * twice per layer (the two all-reduces of Eq. 3) — fn must enqueue, on `cuda_stream`, an in-place SUM of `partial`
- * across the ranks (e.g. ncclAllReduce) and return without synchronising — then adds the sum to the fp32 residual.
+ * across the ranks (e.g. ncclAllReduce) and return 0 without synchronising — then adds the sum to the fp32 residual.
+ * A non-zero return aborts the call: nothing further is enqueued and the stage call returns SS_ERR_CUDA.
  * Decode steps are not graph-captured in this mode.  fn = NULL returns the stage to single-GPU operation. */
-typedef void (*ss_allreduce_fn)(float *partial_dev, size_t count, void *user, void *cuda_stream);
+typedef int (*ss_allreduce_fn)(float *partial_dev, size_t count, void *user, void *cuda_stream);
 int ss_stage_set_allreduce(ss_stage *st, ss_allreduce_fn fn, void *user);
 
 /* Migration by KV transfer (the alternative to recomputation the paper measures; SURVEY
@@ -203,6 +214,26 @@ int ss_stage_set_allreduce(ss_stage *st, ss_allreduce_fn fn, void *user);
  * SS_ERR_CAPACITY (buffer too small).  Page ids out of range are undefined behaviour. */
 int ss_kv_export(ss_stage *st, int n, const int32_t *page_ids_dev, void *buf_dev, size_t buf_bytes);
 int ss_kv_import(ss_stage *st, int n, const int32_t *page_ids_dev, const void *buf_dev, size_t buf_bytes);
+
+/* Device-side contract checks: block tables, context lengths, cu_q and token ids live in
+ * device memory, so the host cannot validate them, and in a normal run a violation is undefined behaviour (a page id
+ * out of range writes outside the pool).  In a stage created while SS_DEBUG=1 is set, ss_stage_prefill / mixed / decode
+ * and ss_kv_export / import first run a checking kernel and synchronise: every listed page id of positions
+ * [0, ctx + q_len) must lie in [0, num_pages); ctx >= 0; ctx + q_len <= max_blocks * 16 and <= dims.max_pos; cu_q[0] = 0,
+ * cu_q[n_seqs] = total_tokens, q_len >= 1 (= 1 for the decode rows of a mixed call); token ids in [0, vocab).  On a
+ * violation the call returns SS_ERR_INVALID_ARG, nothing else is enqueued (pool and workspace untouched), and
+ * ss_stage_debug_info reports the first violation found: out = {code, sequence (-1: none), index, offending value} with
+ * code 1 page id out of range (index = block-table column, or position in page_ids for export / import), 2 ctx + q_len
+ * beyond the listed pages, 3 beyond max_pos, 4 token id out of range (index = token), 5 malformed cu_q, 6 negative
+ * context.  Returns 1 if the stage runs with the checks on, 0 if not, SS_ERR_INVALID_ARG on null arguments. */
+int ss_stage_debug_info(const ss_stage *st, int32_t out[4]);
+
+/* Debug aid: device address and size of one of the stage's workspace tensors, as the last call left it (valid after the
+ * caller synchronises the stream).  Names: "x" fp32 [T,H] residual stream (after a call: the stage output before the
+ * bf16 hand-off); "h" bf16 [T,H] last RMSNorm output; "qkv" fp32 [T,Hq+2Hkv] last QKV projection (S2); "q" bf16 [T,Hq]
+ * last layer's queries after QK-norm + RoPE (S3, S4); "attn" bf16 [T,Hq] last attention output (S6); "a" bf16 [T,F] last
+ * SwiGLU output (S9).  Used by the per-step parity tests.  SS_ERR_INVALID_ARG on an unknown name. */
+int ss_stage_debug_tap(const ss_stage *st, const char *name, void **dev_ptr_out, size_t *bytes_out);
 
 /* ---- op-level entry points (the same kernels the stage uses; for per-kernel parity tests and profiling) -- */
 

@@ -25,10 +25,10 @@ EXPORTS = ["ss_stage_workspace_bytes", "ss_kv_page_bytes", "ss_stage_create", "s
            "ss_stage_launch_count", "ss_op_gemm_scratch_bytes", "ss_op_gemm_bf16", "ss_op_gemm_swiglu_bf16", "ss_strerror",
            "ss_last_cuda_error", "ss_version", "ss_debug_buffer", "ss_pool_create", "ss_pool_destroy",
            "ss_pool_num_pages", "ss_pool_num_free", "ss_pool_alloc", "ss_pool_free", "ss_kv_export", "ss_kv_import", "ss_stage_set_allreduce",
-           "ss_store_alloc", "ss_store_free", "ss_store_upload", "ss_store_export", "ss_store_attach", "ss_store_detach"]
+           "ss_stage_debug_tap", "ss_stage_debug_info", "ss_store_alloc", "ss_store_free", "ss_store_upload", "ss_store_export", "ss_store_attach", "ss_store_detach"]
 
 
-ALLREDUCE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p)
+ALLREDUCE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p)
 
 
 class ss_model_dims(C.Structure):
@@ -94,6 +94,8 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     lib.ss_stage_launch_count.restype = C.c_int64
     lib.ss_stage_launch_count.argtypes = [C.c_void_p]
     lib.ss_debug_buffer.argtypes = [C.c_void_p]
+    lib.ss_stage_debug_info.argtypes = [C.c_void_p, C.POINTER(C.c_int32)]
+    lib.ss_stage_debug_tap.argtypes = [C.c_void_p, C.c_char_p, C.POINTER(C.c_void_p), C.POINTER(C.c_size_t)]
     lib.ss_stage_set_allreduce.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
     lib.ss_kv_export.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_size_t]
     lib.ss_kv_import.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_size_t]
@@ -249,8 +251,13 @@ class Stage:
             ws, base = self.workspace, self.workspace.data_ptr()
 
             def tramp(ptr, count, user, stream):
-                off = ptr - base
-                fn(ws[off:off + 4 * count].view(torch.float32), stream)
+                try:                                   # an exception must not be lost inside the C call
+                    off = ptr - base
+                    fn(ws[off:off + 4 * count].view(torch.float32), stream)
+                    return 0
+                except Exception as exc:               # noqa: BLE001 - reported through the return code
+                    self._ar_error = exc
+                    return 1
 
             self._ar_cb = ALLREDUCE_FN(tramp)          # keep the trampoline alive
             rc = self.lib.ss_stage_set_allreduce(self.h, C.cast(self._ar_cb, C.c_void_p), None)
@@ -268,6 +275,26 @@ class Stage:
         if check and rc != SS_OK:
             raise ShuntStageError(rc, "ss_kv_import")
         return rc
+
+    def debug_info(self):
+        """(checks_on, [code, sequence, index, value]) of ss_stage_debug_info."""
+        out = (C.c_int32 * 4)()
+        rc = self.lib.ss_stage_debug_info(self.h, out)
+        if rc < 0:
+            raise ShuntStageError(rc, "ss_stage_debug_info")
+        return bool(rc), list(out)
+
+    def debug_tap(self, name: str, rows: int) -> torch.Tensor:
+        """ss_stage_debug_tap as a torch view of the workspace: the first `rows` rows of tensor `name`."""
+        p, n = C.c_void_p(), C.c_size_t()
+        rc = self.lib.ss_stage_debug_tap(self.h, name.encode(), C.byref(p), C.byref(n))
+        if rc != SS_OK:
+            raise ShuntStageError(rc, "ss_stage_debug_tap")
+        off = p.value - self.workspace.data_ptr()
+        d = self.dims
+        cap = max(d.max_tokens, d.max_seqs)
+        dt = torch.float32 if name in ("x", "qkv") else torch.bfloat16
+        return self.workspace[off:off + n.value].view(dt).view(cap, -1)[:rows]
 
     def launch_count(self) -> int:
         return int(self.lib.ss_stage_launch_count(self.h))
@@ -291,9 +318,10 @@ class Stage:
 _SCRATCH = {}
 
 
-def _op_scratch(device) -> torch.Tensor:
-    """Zero-initialised stream-K fix-up scratch for the op-level GEMMs (one per device, torch memory)."""
-    key = str(device)
+def _op_scratch(device, stream_ptr: int) -> torch.Tensor:
+    """Zero-initialised stream-K fix-up scratch for the op-level GEMMs: one per (device, stream), because two GEMMs in
+    flight on different streams must not share fix-up flags (torch memory)."""
+    key = (str(device), stream_ptr)
     if key not in _SCRATCH:
         n = load_library().ss_op_gemm_scratch_bytes()
         _SCRATCH[key] = torch.zeros(n, dtype=torch.uint8, device=device)
@@ -301,15 +329,20 @@ def _op_scratch(device) -> torch.Tensor:
     return _SCRATCH[key]
 
 
+def _op_stream(stream):
+    return stream if stream is not None else torch.cuda.current_stream()
+
+
 def op_gemm_bf16(x: torch.Tensor, w: torch.Tensor, stream=None) -> torch.Tensor:
     """C[T,N] fp32 = x[T,K] bf16 @ w[N,K]^T bf16 through the tcgen05 GEMM kernel."""
     lib = load_library()
     T, K = x.shape
     N = w.shape[0]
-    c = torch.empty((T, N), dtype=torch.float32, device=x.device)
-    sc = _op_scratch(x.device)
-    s = stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream
-    rc = lib.ss_op_gemm_bf16(_ptr(x), _ptr(w), _ptr(c), T, N, K, _ptr(sc), sc.numel(), s)
+    st = _op_stream(stream)
+    with torch.cuda.stream(st):                      # the output belongs to the stream the kernel runs on
+        c = torch.empty((T, N), dtype=torch.float32, device=x.device)
+    sc = _op_scratch(x.device, st.cuda_stream)
+    rc = lib.ss_op_gemm_bf16(_ptr(x), _ptr(w), _ptr(c), T, N, K, _ptr(sc), sc.numel(), st.cuda_stream)
     if rc != SS_OK:
         raise ShuntStageError(rc, "ss_op_gemm_bf16")
     return c
@@ -319,10 +352,12 @@ def op_gemm_swiglu_bf16(x: torch.Tensor, wg: torch.Tensor, wu: torch.Tensor, str
     lib = load_library()
     T, K = x.shape
     F = wg.shape[0]
-    a = torch.empty((T, F), dtype=torch.bfloat16, device=x.device)
-    sc = _op_scratch(x.device)
-    s = stream.cuda_stream if stream is not None else torch.cuda.current_stream().cuda_stream
-    rc = lib.ss_op_gemm_swiglu_bf16(_ptr(x), _ptr(wg), _ptr(wu), _ptr(a), T, F, K, _ptr(sc), sc.numel(), s)
+    st = _op_stream(stream)
+    with torch.cuda.stream(st):
+        a = torch.empty((T, F), dtype=torch.bfloat16, device=x.device)
+    sc = _op_scratch(x.device, st.cuda_stream)
+    rc = lib.ss_op_gemm_swiglu_bf16(_ptr(x), _ptr(wg), _ptr(wu), _ptr(a), T, F, K, _ptr(sc), sc.numel(),
+                                    st.cuda_stream)
     if rc != SS_OK:
         raise ShuntStageError(rc, "ss_op_gemm_swiglu_bf16")
     return a

@@ -281,15 +281,15 @@ __global__ void __launch_bounds__(PA_WARPS * 32, 3) prefill_attn_kernel(const Pr
 
 static size_t prefill_smem(int d) { return (size_t)(4 * PA_BN) * d * 2; }  // Q aliases the second K/V buffer
 
+cudaError_t prefill_attn_init() {  // per device: called from ss_stage_create
+  cudaError_t e = cudaFuncSetAttribute(prefill_attn_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       (int)prefill_smem(128));
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(prefill_attn_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              (int)prefill_smem(64));
+}
+
 cudaError_t launch_prefill_attn(const PrefillAttnParams &p, cudaStream_t s) {
-  static bool inited = false;
-  if (!inited) {
-    cudaFuncSetAttribute(prefill_attn_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                         (int)prefill_smem(128));
-    cudaFuncSetAttribute(prefill_attn_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                         (int)prefill_smem(64));
-    inited = true;
-  }
   dim3 grid(p.n_q, p.max_tiles);
   if (p.d == 128)
     return launch_pdl(prefill_attn_kernel<128>, dim3(grid), dim3(PA_WARPS * 32), prefill_smem(128), s, p);

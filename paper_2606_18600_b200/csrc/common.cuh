@@ -74,11 +74,25 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t *bar, uint32_t parity) {
       : "memory");
   return ok != 0;
 }
-// Bounded wait: a protocol bug becomes a trap (reported as a CUDA error) instead of a hung GPU.
+// Bounded waits: a protocol bug becomes a trap (reported as a CUDA error) instead of a hung GPU.  The bound is WALL
+// CLOCK (10 s on %globaltimer, looked at once per 65,536 polls), not an iteration count: under a debugger, a sanitizer
+// or a co-running stream that keeps this grid's other CTAs off the SMs for a while, a correct kernel only waits longer.
+constexpr unsigned long long WAIT_LIMIT_NS = 10ull * 1000ull * 1000ull * 1000ull;
+__device__ __forceinline__ bool wait_expired_ns(uint32_t &polls, unsigned long long &t0) {
+  if ((++polls & 0xffffu) != 0) return false;
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+  if (t0 == 0) {
+    t0 = t;
+    return false;
+  }
+  return t - t0 > WAIT_LIMIT_NS;
+}
 __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
-  uint32_t spins = 0;
+  uint32_t polls = 0;
+  unsigned long long t0 = 0;
   while (!mbar_try_wait(bar, parity)) {
-    if (++spins > (1u << 26)) __trap();
+    if (wait_expired_ns(polls, t0)) __trap();
   }
 }
 

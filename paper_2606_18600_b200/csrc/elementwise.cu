@@ -393,4 +393,72 @@ cudaError_t launch_kv_pages_copy(void *pool, void *buf, const int32_t *page_ids,
                     n, n_pages_pool, piece_bytes / 16, to_buffer ? 1 : 0);
 }
 
+// ---- SS_DEBUG=1: device-side contract checks (SURVEY.md section 8(b) "Errors"; include/shuntstage.h) -----------------
+// One CTA walks the call's sequences before anything else is enqueued: ctx >= 0, q_len >= 1 (== 1 for the decode rows),
+// cu_q consistent with T, ctx + q_len within the listed pages (max_blocks * 16) and within the RoPE table, every page id
+// of positions [0, ctx + q_len) inside the pool, token ids inside the vocabulary.  The FIRST violation (lowest thread
+// wins the CAS) is recorded as err = {code, sequence, index, value}.
+__global__ void __launch_bounds__(256)
+debug_validate_kernel(const CallArgs *__restrict__ args, DebugCheck c, int32_t *__restrict__ err) {
+  auto fail = [&](int code, int seq, int idx, int val) {
+    if (atomicCAS(err, 0, code) == 0) {
+      err[1] = seq;
+      err[2] = idx;
+      err[3] = val;
+    }
+  };
+  const int n = args->n_seqs;
+  if (threadIdx.x == 0 && !c.decode) {
+    if (args->cu_q[0] != 0) fail(SS_DBG_BAD_CU_Q, 0, 0, args->cu_q[0]);
+    if (args->cu_q[n] != args->T) fail(SS_DBG_BAD_CU_Q, n, n, args->cu_q[n]);
+  }
+  for (int s = 0; s < n; ++s) {
+    const int ctx = args->ctx[s];
+    const int q_len = c.decode ? 1 : args->cu_q[s + 1] - args->cu_q[s];
+    if (threadIdx.x == 0) {
+      if (ctx < 0) fail(SS_DBG_BAD_CTX, s, 0, ctx);
+      if (q_len < 1 || (s < c.n_decode_rows && q_len != 1)) fail(SS_DBG_BAD_CU_Q, s, s, q_len);
+      if ((long long)ctx + q_len > (long long)args->max_blocks * 16) fail(SS_DBG_BEYOND_PAGES, s, args->max_blocks, ctx + q_len);
+      if ((long long)ctx + q_len > (long long)c.max_pos) fail(SS_DBG_BEYOND_MAX_POS, s, c.max_pos, ctx + q_len);
+    }
+    if (ctx < 0 || q_len < 1) continue;
+    long long need = ((long long)ctx + q_len + 15) >> 4;
+    if (need > args->max_blocks) need = args->max_blocks;
+    const int32_t *bt = args->block_tables + (size_t)s * args->max_blocks;
+    for (int i = threadIdx.x; i < (int)need; i += blockDim.x) {
+      const int pg = bt[i];
+      if (pg < 0 || pg >= c.num_pages) fail(SS_DBG_BAD_PAGE, s, i, pg);
+    }
+  }
+  if (args->token_ids)
+    for (int t = threadIdx.x; t < args->T; t += blockDim.x) {
+      const int id = args->token_ids[t];
+      if (id < 0 || id >= c.vocab) fail(SS_DBG_BAD_TOKEN, -1, t, id);
+    }
+}
+
+cudaError_t launch_debug_validate(const CallArgs *args, const DebugCheck &c, int32_t *err, cudaStream_t s) {
+  count_launch();
+  debug_validate_kernel<<<1, 256, 0, s>>>(args, c, err);
+  return cudaGetLastError();
+}
+
+__global__ void __launch_bounds__(256)
+debug_validate_pages_kernel(const int32_t *__restrict__ ids, int n, int num_pages, int32_t *__restrict__ err) {
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    const int pg = ids[i];
+    if ((pg < 0 || pg >= num_pages) && atomicCAS(err, 0, SS_DBG_BAD_PAGE) == 0) {
+      err[1] = -1;
+      err[2] = i;
+      err[3] = pg;
+    }
+  }
+}
+
+cudaError_t launch_debug_validate_pages(const int32_t *ids, int n, int num_pages, int32_t *err, cudaStream_t s) {
+  count_launch();
+  debug_validate_pages_kernel<<<(n + 255) / 256 > 64 ? 64 : (n + 255) / 256, 256, 0, s>>>(ids, n, num_pages, err);
+  return cudaGetLastError();
+}
+
 }  // namespace ss

@@ -107,9 +107,10 @@ __device__ __noinline__ void wait_expired(int site, uint32_t a, uint32_t b) {
   __trap();
 }
 __device__ __forceinline__ void mbar_wait_site(uint64_t *bar, uint32_t parity, int site, uint32_t info) {
-  uint32_t spins = 0;
+  uint32_t polls = 0;
+  unsigned long long t0 = 0;
   while (!mbar_try_wait(bar, parity)) {
-    if (++spins > (1u << 24)) wait_expired(site, info, parity);
+    if (wait_expired_ns(polls, t0)) wait_expired(site, info, parity);
   }
 }
 // Optional timeline (profiling builds only: -DSS_GEMM_TRACE): globaltimer stamps per CTA into p.trace[cta*64 + slot].
@@ -154,13 +155,8 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
   // k-blocks dealt alternately and an odd ring size a slot changed hands every round, a fast issuer could take a
   // stale phase for its own and read a tile still in flight).
   const uint32_t acc_cols = (uint32_t)bn * (DUAL ? 2u : 1u);
-  // The tensor-bound schedule also runs two issuers, but SPLIT inside every k-block (p.split): issuer 0 takes the
-  // gate tile / tokens [0, bn/2), issuer 1 the up tile / tokens [bn/2, bn), into disjoint columns of ONE
-  // accumulator.  At N = 256 a single issuer leaves the tensor pipe idle while it commits and waits (187 vs 128
-  // cycles per MMA); two issuers keep it at the 128-cycle floor (profiles/r01_mma_issue_microbench.md).
   const int n_iss = p.issuers;
-  const bool split = p.split != 0;
-  const uint32_t acc_stride = split ? acc_cols : acc_cols * (uint32_t)n_iss;  // TMEM columns per buffer
+  const uint32_t acc_stride = acc_cols * (uint32_t)n_iss;  // TMEM columns per buffer
   const int nbuf = (p.single_buf == 0 && 2 * acc_stride <= 512) ? 2 : 1;
   uint32_t tmem_cols = 32;
   while (tmem_cols < acc_stride * nbuf) tmem_cols <<= 1;
@@ -174,7 +170,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
     tma_prefetch_desc(&tb);
     for (int i = 0; i < stages; ++i) {
       mbar_init(&full[i], 1);
-      mbar_init(&empty[i], split ? 2u : 1u);  // split: both issuers read every slot
+      mbar_init(&empty[i], 1u);
     }
     for (int i = 0; i < 2; ++i) {
       mbar_init(&tfull[i], (uint32_t)n_iss);
@@ -253,18 +249,14 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
     const int me = warp == 1 ? 0 : 1;
     if (lane == 0 && me < n_iss) {
       // ---------------- MMA issuer `me` ----------------
-      // alternate mode: the k-blocks in ring slots s = me (mod n_iss), own accumulator; split mode: every k-block,
-      // own half (gate | up, or tokens [0,bn/2) | [bn/2,bn)) of the shared accumulator
-      const uint32_t idesc = umma_idesc_bf16(GEMM_BM, (uint32_t)((split && !DUAL) ? bn / 2 : bn));
-      const uint32_t a_off = (split && DUAL && me == 1) ? (uint32_t)A_TILE_BYTES : 0u;
-      const uint32_t b_off = (split && !DUAL && me == 1) ? (uint32_t)(bn / 2) * 128u : 0u;
-      const uint32_t acc_off = split ? (uint32_t)me * (DUAL ? (uint32_t)bn : (uint32_t)(bn / 2)) : (uint32_t)me * acc_cols;
-      const bool both = DUAL && !split;  // this issuer issues the gate AND the up MMA
+      // the k-blocks in ring slots s = me (mod n_iss), into this issuer's own accumulator
+      const uint32_t idesc = umma_idesc_bf16(GEMM_BM, (uint32_t)bn);
+      const uint32_t acc_off = (uint32_t)me * acc_cols;
       WorkIter it(p, cta, grid);
       WorkItem w;
       uint32_t n = 0, item = 0;
-      const uint32_t iss_mask = split ? 0u : (uint32_t)n_iss - 1u;  // n_iss is 1 or 2
-      const uint32_t my_slots = split ? 0u : (uint32_t)me;
+      const uint32_t iss_mask = (uint32_t)n_iss - 1u;  // n_iss is 1 or 2
+      const uint32_t my_slots = (uint32_t)me;
       int ms = 0;        // = n % stages
       uint32_t mph = 0;  // = (n / stages) & 1
       while (it.next(w)) {
@@ -285,16 +277,14 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
           if (n == 0) trace(p, 2);
           tc_fence_after();
           const uint32_t st = smem_u32(base + (size_t)s * stage_bytes);
-          const uint64_t da = umma_desc_k_sw128(st + a_off);
+          const uint64_t da = umma_desc_k_sw128(st);
           const uint64_t da1 = umma_desc_k_sw128(st + A_TILE_BYTES);
-          const uint64_t db = umma_desc_k_sw128(st + a_bytes + b_off);
+          const uint64_t db = umma_desc_k_sw128(st + a_bytes);
 #pragma unroll
           for (int k = 0; k < GEMM_BK / 16; ++k) {
             const uint32_t acc = (!first || k > 0) ? 1u : 0u;
             umma_bf16(acc_addr, da + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc, acc);
-            if (DUAL) {
-              if (both) umma_bf16(acc_addr + (uint32_t)bn, da1 + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc, acc);
-            }
+            if (DUAL) umma_bf16(acc_addr + (uint32_t)bn, da1 + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc, acc);
           }
           first = false;
           umma_commit(&empty[s]);  // frees the smem slot when these MMAs have read it
@@ -322,8 +312,8 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
       const uint32_t len = (uint32_t)(w.kb1 - w.kb0);
       // which issuers accumulated anything in this item (an accumulator nobody wrote holds stale data): issuer
       // (slot & 1) handles a k-block, slots run cyclically from n_run % stages
-      bool has0 = n_iss == 1 || split, has1 = false;
-      if (n_iss == 2 && !split) {
+      bool has0 = n_iss == 1, has1 = false;
+      if (n_iss == 2) {
         uint32_t sl = n_run % (uint32_t)stages;
         for (uint32_t j = 0; j < len && j < 3u; ++j) {
           if (sl & 1u) has1 = true; else has0 = true;
@@ -412,9 +402,10 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
             // overlap the contributors' dump + publish (cfg-2 step 7.355 -> 7.30 ms, cfg-3 5.148 -> 5.12 ms, same box)
             polled = true;
             for (int cc = c_lo; cc <= c_hi; ++cc) {
-              uint32_t spins = 0;
+              uint32_t polls = 0;
+              unsigned long long t0w = 0;
               while (ld_acquire(p.fix_flags + cc) == 0) {
-                if (++spins > (1u << 24)) wait_expired(7, (uint32_t)cc, item);
+                if (wait_expired_ns(polls, t0w)) wait_expired(7, (uint32_t)cc, item);
               }
             }
           }
@@ -522,11 +513,20 @@ int make_tmap_bf16_2d(CUtensorMap *out, const void *base, uint64_t rows, uint64_
   return r == CUDA_SUCCESS ? 0 : -(int)r - 1000;
 }
 
-static int env_int(const char *name, int dflt);
+// Tuning overrides exist only in builds with -DSS_TUNE (SS_NVCC_EXTRA=-DSS_TUNE python -m paper_2606_18600_b200.build):
+// the product library reads no environment variable on this path.
+#ifdef SS_TUNE
+static int tune(const char *name, int dflt) {
+  const char *e = getenv(name);
+  return e ? atoi(e) : dflt;
+}
+#else
+static inline int tune(const char *, int dflt) { return dflt; }
+#endif
+
 int gemm_pick_bn(int T) {
-  static int env_bn = -1;
-  if (env_bn < 0) env_bn = env_int("SS_GEMM_BN", 0);  // experiments: force the token tile
-  if (env_bn > 0) return env_bn;
+  const int forced = tune("SS_GEMM_BN", 0);
+  if (forced > 0) return forced;
   // the narrowest multiple of 32 columns that covers T in ceil(T / 256) token tiles: a UMMA costs tensor-pipe time and
   // smem reads in proportion to N, and from ~128 tokens on the decode GEMMs are near the roofline's ridge (256 flop
   // per weight byte at T = 256 against 1,624 TFLOP/s / 6,545 GB/s = 248), so padded columns are not free
@@ -541,26 +541,15 @@ size_t gemm_smem_bytes(int bn, bool dual, int stages) {
   return 1024 + stage * stages + 8 * (2 * stages + 4) + 16;
 }
 
-static int env_int(const char *name, int dflt) {
-  const char *e = getenv(name);
-  return e ? atoi(e) : dflt;
-}
-
 int gemm_pick_stages(int bn, bool dual) {
-  static int env = -1;
-  if (env < 0) env = env_int("SS_GEMM_STAGES", 0);
-  int st = env > 0 ? env : GEMM_MAX_STAGES;  // one persistent CTA per SM: use the 227 KB
-  if (st > GEMM_MAX_STAGES) st = GEMM_MAX_STAGES;
+  int st = tune("SS_GEMM_STAGES", GEMM_MAX_STAGES);  // one persistent CTA per SM: use the 227 KB
+  if (st > GEMM_MAX_STAGES || st < 2) st = GEMM_MAX_STAGES;
   while (st > 2 && gemm_smem_bytes(bn, dual, st) > 227 * 1024) --st;
   return st;
 }
 
 void gemm_plan(GemmLaunch &g, int n_sm) {
   GemmParams &p = g.p;
-  static int env_band = -1, env_sched = -2, env_grid = -1;
-  if (env_band < 0) env_band = env_int("SS_GEMM_BAND", 0);
-  if (env_sched == -2) env_sched = env_int("SS_GEMM_SCHED", -1);
-  if (env_grid < 0) env_grid = env_int("SS_GEMM_GRID", 0);
   int tiles = 0, col = 0;
   for (int i = 0; i < 3; ++i) {
     p.seg_tile0[i] = tiles;
@@ -577,7 +566,7 @@ void gemm_plan(GemmLaunch &g, int n_sm) {
   p.n_t_tiles = (p.T + p.bn - 1) / p.bn;
   const long long n_tiles = (long long)p.n_row_tiles * p.n_t_tiles;
   const long long nkb = (p.K + GEMM_BK - 1) / GEMM_BK;
-  int max_grid = env_grid > 0 ? env_grid : n_sm;
+  int max_grid = tune("SS_GEMM_GRID", n_sm);
   if (max_grid > GEMM_MAX_GRID) max_grid = GEMM_MAX_GRID;
   // whole tiles when the last wave is nearly full (>= 88% of the CTAs busy; 70% once there are several token
   // tiles, i.e. the problem is tensor-bound anyway) or there are many waves; stream-K
@@ -587,41 +576,25 @@ void gemm_plan(GemmLaunch &g, int n_sm) {
   const bool full_waves = n_tiles >= max_grid && n_tiles * 100 >= waves * max_grid * (p.n_t_tiles >= 2 ? 70 : 88);
   p.sched = (n_tiles >= 4LL * max_grid || full_waves) ? SCHED_TILES : SCHED_STREAMK;
   if (p.n_t_tiles == 1) p.sched = SCHED_STREAMK;  // HBM-bound whatever the tile count (lm_head: 1,002-1,187 tiles = 6.8-8.02 waves)
-  if (env_sched >= 0) p.sched = env_sched;
+  p.sched = tune("SS_GEMM_SCHED", p.sched);
   if (n_tiles * nkb >= (1LL << 31)) p.sched = SCHED_TILES;  // the stream-K unit cursor is 32-bit
-  p.band = env_band > 0 ? env_band : (g.dual ? 8 : 16);
+  p.band = tune("SS_GEMM_BAND", g.dual ? 8 : 16);
   if (p.band > p.n_row_tiles) p.band = p.n_row_tiles;
   p.stages = gemm_pick_stages(p.bn, g.dual);
   {
-    static int env_iss = -1;
-    if (env_iss < 0) env_iss = env_int("SS_GEMM_ISSUERS", 0);
     const int acc_cols = p.bn * (g.dual ? 2 : 1);
-    static int env_wpol = -2;
-    if (env_wpol == -2) env_wpol = env_int("SS_GEMM_WPOL", -1);
     // one token tile (T <= 256): every weight byte is read once, whatever the schedule (e.g. the lm_head at decode:
     // 1,002 row tiles -> whole-tile schedule, but HBM-bound like the stream-K shapes)
     const bool hbm_bound = p.sched == SCHED_STREAMK || p.n_t_tiles == 1;
-    p.w_policy = hbm_bound ? 0 : 2;
-    if (env_wpol >= 0) p.w_policy = env_wpol;
-    p.split = 0;
-    if (hbm_bound) {
-      // two issuers (one accumulator set each) only while BOTH sets still fit twice in TMEM: with 2 x 256 columns
-      // per item there is no second buffer and the epilogue stops the main loop (T = 256 down projection 119 -> 113 us,
-      // O 51.5 -> 45.5 us, T = 128 gate/up 155.6 -> 153.9 us with one issuer)
-      p.issuers = (4 * acc_cols <= 512) ? 2 : 1;
-    } else {
-      // measured: splitting each k-block between two issuers does not help here (the tensor pipe waits on L2, not
-      // on the issuer: 59% vs 66% active) — one issuer; SS_GEMM_ISSUERS=2 keeps the split path testable
-      p.issuers = env_iss == 2 ? 2 : 1;
-      p.split = env_iss == 2 ? 1 : 0;
-    }
-    if (env_iss == 1) {
-      p.issuers = 1;
-      p.split = 0;
-    }
-    static int env_sb = -1;
-    if (env_sb < 0) env_sb = env_int("SS_GEMM_SINGLE_BUF", 0);
-    p.single_buf = env_sb;
+    p.w_policy = tune("SS_GEMM_WPOL", hbm_bound ? 0 : 2);
+    // HBM-bound: two issuers (one accumulator set each) only while BOTH sets still fit twice in TMEM: with 2 x 256
+    // columns per item there is no second buffer and the epilogue stops the main loop (T = 256 down projection
+    // 119 -> 113 us, O 51.5 -> 45.5 us, T = 128 gate/up 155.6 -> 153.9 us with one issuer).  Tensor-bound: one issuer
+    // (the tensor pipe waits on L2 there, not on the issuing thread).
+    p.issuers = (hbm_bound && 4 * acc_cols <= 512) ? 2 : 1;
+    const int forced_iss = tune("SS_GEMM_ISSUERS", 0);
+    if (forced_iss == 1 || (forced_iss == 2 && 2 * acc_cols <= 512)) p.issuers = forced_iss;
+    p.single_buf = tune("SS_GEMM_SINGLE_BUF", 0);
   }
   const long long work = p.sched == SCHED_STREAMK ? n_tiles * nkb : n_tiles;
   g.grid = (int)(work < max_grid ? work : max_grid);
@@ -630,14 +603,12 @@ void gemm_plan(GemmLaunch &g, int n_sm) {
     // count cuts every tile into the same whole number of CTA ranges with aligned boundaries, so an owner waits for
     // exactly k - 1 contributors and no CTA holds pieces of two tiles (148 CTAs over 40 tiles = 3.7 ranges per tile:
     // 3-4 contributors, most CTAs with two short items).  HBM does not need all 148 SMs to be saturated, the fix-up
-    // tail is what these short GEMMs lose (profiles/r01_v7_cfg3_layer.md).  Same box, alternating: cfg-2 step
+    // tail is what these short GEMMs lose.  Same box, alternating: cfg-2 step
     // 7.287 -> 7.217 ms (grid 128 for 64 tiles), cfg-3 5.10 -> 5.02 ms (grid 120 for 40 tiles); stand-alone O
     // projection 29.0 -> 26.9 us, down 56.4 -> 53.9 us at T = 128.  Only when that grid keeps >= 80% of the SMs: the
     // 80-tile QKV projection on 80 CTAs went 36.2 -> 39.3 us at cfg-2 (31.1 -> 30.0 at cfg-3).  Half-integer cuts (140
     // CTAs for 40 tiles, 120 for 80) measured between the two or within noise of this rule; not used.
-    static int env_al = -1;
-    if (env_al < 0) env_al = env_int("SS_GEMM_ALIGN", 1);
-    if (env_al > 0 && p.sched == SCHED_STREAMK && n_tiles < max_grid && work >= max_grid) {
+    if (tune("SS_GEMM_ALIGN", 1) > 0 && p.sched == SCHED_STREAMK && n_tiles < max_grid && work >= max_grid) {
       const int nt = (int)n_tiles;
       const int aligned = (max_grid / nt) * nt;
       if (aligned * 10 >= max_grid * 8) g.grid = aligned;

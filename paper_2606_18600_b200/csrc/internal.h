@@ -41,7 +41,6 @@ struct GemmParams {
   int bn;               // tokens per tile (UMMA N)
   int stages;           // smem pipeline depth
   int w_policy;         // L2 policy of the weight loads: 0 evict_first, 1 evict_normal, 2 evict_last
-  int split;            // 1: the two issuers split every k-block (tensor-bound schedule); 0: they alternate k-blocks
   int single_buf;       // debug: 1 = never double-buffer the TMEM accumulators
   int issuers;          // MMA-issuing threads (2 on the HBM-bound schedule, see gemm_tcgen05.cu)
   int sched;            // GemmSchedule
@@ -73,7 +72,7 @@ void gemm_plan(GemmLaunch &g, int n_sm);
 cudaError_t gemm_launch(const GemmLaunch &g);
 cudaError_t gemm_init();  // sets max dynamic smem attributes once
 cudaError_t gemm_set_debug_buffer(unsigned long long *host_mapped);  // see gemm_tcgen05.cu wait_expired()
-int gemm_pick_bn(int T);  // smallest of {32,64,128,256} >= min(T,256)
+int gemm_pick_bn(int T);  // 32 for T <= 32, else the narrowest multiple of 32 covering T in ceil(T / 256) token tiles
 int gemm_pick_stages(int bn, bool dual);
 size_t gemm_smem_bytes(int bn, bool dual, int stages);
 constexpr int GEMM_MAX_GRID = 256;                       // upper bound on persistent CTAs (sizes the fix buffers)
@@ -182,10 +181,22 @@ struct PrefillAttnParams {
   int max_tiles;             // upper bound on query tiles = ceil(T/64) + n_seqs
 };
 cudaError_t launch_prefill_attn(const PrefillAttnParams &p, cudaStream_t s);
+cudaError_t prefill_attn_init();
 
 // gather (to_buffer) / scatter n pages of every layer between the pool and a contiguous [L][2][n][n_kv][16][d] buffer
 cudaError_t launch_kv_pages_copy(void *pool, void *buf, const int32_t *page_ids, int n, int n_layers, int n_pages_pool,
                                  int piece_bytes, bool to_buffer, cudaStream_t s);
+
+// SS_DEBUG=1 contract checks (elementwise.cu): codes of the device error word, mirrored in include/shuntstage.h
+enum { SS_DBG_BAD_PAGE = 1, SS_DBG_BEYOND_PAGES = 2, SS_DBG_BEYOND_MAX_POS = 3, SS_DBG_BAD_TOKEN = 4, SS_DBG_BAD_CU_Q = 5,
+       SS_DBG_BAD_CTX = 6 };
+struct DebugCheck {
+  int decode;          // 1: ss_stage_decode (q_len == 1 everywhere, cu_q unused)
+  int n_decode_rows;   // mixed call: the first rows must have q_len == 1
+  int num_pages, max_pos, vocab;
+};
+cudaError_t launch_debug_validate(const CallArgs *args, const DebugCheck &c, int32_t *err /* dev [4], zeroed */, cudaStream_t s);
+cudaError_t launch_debug_validate_pages(const int32_t *ids, int n, int num_pages, int32_t *err, cudaStream_t s);
 
 void count_launch(int n = 1);  // stage.cu: per-thread launch counter hook
 bool pdl_enabled();            // stage.cu: false when SS_NO_PDL=1

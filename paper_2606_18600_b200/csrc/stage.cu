@@ -1,8 +1,9 @@
 // stage.cu — host runtime and C-ABI of libshuntstage.so (include/shuntstage.h): argument validation, workspace
 // carving, TMA descriptors, the per-layer kernel sequence of ss_stage_decode / ss_stage_prefill (steps S0-S11 of
 // DESIGN.md; Table 2 of the paper), CUDA-graph capture of the decode step, and the host-side
-// page allocator.  The library never allocates device memory (the paper's engine attaches to tensors owned by
-// the Shared Tensor Store).
+// page allocator.  A stage never allocates device memory (the paper's engine attaches to tensors owned by
+// the Shared Tensor Store); the only cudaMalloc in the library is ss_store_alloc, the store side of
+// that mechanism.
 #include <cuda.h>
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
@@ -48,7 +49,7 @@ constexpr int MAX_WORKERS = 4096;  // upper bound on decode-attention worker war
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Carve {  // byte offsets into the workspace
-  size_t args, rope, x, h, qkv_part, q, kv_new, attn_out, fix, a, part_o, part_ml, cum_pages, meta, tp_part, am_part, tok_seq,
+  size_t args, err, rope, x, h, qkv_part, q, kv_new, attn_out, fix, a, part_o, part_ml, cum_pages, meta, tp_part, am_part, tok_seq,
       tok_pos, tile_cum, tile_order, hl, logits, total;
 };
 
@@ -79,6 +80,7 @@ static Carve carve(const ss_model_dims *d) {
     return at;
   };
   c.args = take(sizeof(CallArgs));
+  c.err = take(16);  // SS_DEBUG device error word {code, sequence, index, value}
   c.rope = take((size_t)d->max_pos * (d->head_dim / 2) * 2 * sizeof(float));
   c.x = take(Tm * H * 4);
   c.h = take(Tm * H * 2);
@@ -187,7 +189,11 @@ struct ss_stage {
   bool use_graph;
   ss_allreduce_fn allreduce;  // non-null: tensor-parallel shard (ss_stage_set_allreduce)
   void *allreduce_user;
-  CallArgs *h_args;    // pinned host staging for the argument block
+  CallArgs *h_args;    // pinned host staging for the argument block (+ 4 ints behind it: the SS_DEBUG error word)
+  cudaEvent_t args_ev; // the last H2D copy out of h_args (the host must not overwrite the block before it has run)
+  bool debug;          // SS_DEBUG=1 at create: every call validates its device-side arguments first
+  int32_t dbg_info[4]; // last violation {code, sequence, index, value}
+  int32_t *h_err() const { return (int32_t *)(h_args + 1); }
 
   size_t layer_kv_elems() const { return (size_t)num_pages * d.n_kv_heads * 16 * d.head_dim; }
   __nv_bfloat16 *kpool(int l) const { return (__nv_bfloat16 *)pool + (size_t)l * 2 * layer_kv_elems(); }
@@ -271,11 +277,15 @@ int ss_stage_create(ss_stage **out, const ss_model_dims *dims, int l0, int l1, c
   st->launches = 0;
   st->use_graph = (cuda_stream != nullptr) && env_int("SS_NO_GRAPH", 0) == 0;
   st->h_args = nullptr;
+  st->args_ev = nullptr;
+  st->debug = env_int("SS_DEBUG", 0) != 0;
+  memset(st->dbg_info, 0, sizeof(st->dbg_info));
   st->allreduce = nullptr;
   st->allreduce_user = nullptr;
 
   auto fail = [&](int code) {
     if (st->h_args) cudaFreeHost(st->h_args);
+    if (st->args_ev) cudaEventDestroy(st->args_ev);
     delete st;
     return code;
   };
@@ -284,15 +294,18 @@ int ss_stage_create(ss_stage **out, const ss_model_dims *dims, int l0, int l1, c
   if (e != cudaSuccess) return fail(cuda_fail(e, "cudaGetDevice"));
   e = cudaDeviceGetAttribute(&st->n_sm, cudaDevAttrMultiProcessorCount, dev);
   if (e != cudaSuccess) return fail(cuda_fail(e, "cudaDeviceGetAttribute"));
-  int ctas_per_sm = env_int("SS_ATTN_CTAS_PER_SM", decode_attn_default_ctas_per_sm());
+  int ctas_per_sm = decode_attn_default_ctas_per_sm();
   if (ctas_per_sm < 1) ctas_per_sm = 1;
   const int wpc = decode_attn_warps_per_cta();
   st->n_workers = st->n_sm * ctas_per_sm * wpc;
   if (st->n_workers > MAX_WORKERS) st->n_workers = MAX_WORKERS / wpc * wpc;
   if ((e = gemm_init()) != cudaSuccess) return fail(cuda_fail(e, "gemm_init"));
   if ((e = attn_init()) != cudaSuccess) return fail(cuda_fail(e, "attn_init"));
-  if ((e = cudaMallocHost((void **)&st->h_args, sizeof(CallArgs))) != cudaSuccess)
+  if ((e = prefill_attn_init()) != cudaSuccess) return fail(cuda_fail(e, "prefill_attn_init"));
+  if ((e = cudaMallocHost((void **)&st->h_args, sizeof(CallArgs) + 16)) != cudaSuccess)
     return fail(cuda_fail(e, "cudaMallocHost"));
+  if ((e = cudaEventCreateWithFlags(&st->args_ev, cudaEventDisableTiming)) != cudaSuccess)
+    return fail(cuda_fail(e, "cudaEventCreate"));
 
   // RoPE table: cos/sin in double, stored fp32 (reading A10)
   {
@@ -358,6 +371,7 @@ int ss_stage_destroy(ss_stage *st) {
   for (auto &g : st->graphs)
     if (g.second.exec) cudaGraphExecDestroy(g.second.exec);
   if (st->h_args) cudaFreeHost(st->h_args);
+  if (st->args_ev) cudaEventDestroy(st->args_ev);
   delete st;
   return SS_OK;
 }
@@ -430,6 +444,30 @@ int ss_store_detach(void *dev_ptr) {
 
 int64_t ss_stage_launch_count(const ss_stage *st) { return st ? st->launches : 0; }
 
+int ss_stage_debug_info(const ss_stage *st, int32_t out[4]) {
+  if (!st || !out) return SS_ERR_INVALID_ARG;
+  memcpy(out, st->dbg_info, 16);
+  return st->debug ? 1 : 0;
+}
+
+int ss_stage_debug_tap(const ss_stage *st, const char *name, void **dev_ptr_out, size_t *bytes_out) {
+  if (!st || !name || !dev_ptr_out || !bytes_out) return SS_ERR_INVALID_ARG;
+  const ss_model_dims &d = st->d;
+  const size_t Tm = (size_t)(d.max_tokens > d.max_seqs ? d.max_tokens : d.max_seqs);
+  const size_t H = d.hidden, Hq = (size_t)d.n_q_heads * d.head_dim, Hkv = (size_t)d.n_kv_heads * d.head_dim;
+  const struct { const char *n; size_t off, bytes; } taps[] = {
+      {"x", st->c.x, Tm * H * 4},       {"h", st->c.h, Tm * H * 2},
+      {"qkv", st->c.qkv_part, Tm * (Hq + 2 * Hkv) * 4}, {"q", st->c.q, Tm * Hq * 2},
+      {"attn", st->c.attn_out, Tm * Hq * 2}, {"a", st->c.a, Tm * (size_t)d.ffn * 2}};
+  for (const auto &t : taps)
+    if (strcmp(t.n, name) == 0) {
+      *dev_ptr_out = st->ws + t.off;
+      *bytes_out = t.bytes;
+      return SS_OK;
+    }
+  return SS_ERR_INVALID_ARG;
+}
+
 int ss_stage_set_allreduce(ss_stage *st, ss_allreduce_fn fn, void *user) {
   if (!st) return SS_ERR_INVALID_ARG;
   st->allreduce = fn;
@@ -437,11 +475,20 @@ int ss_stage_set_allreduce(ss_stage *st, ss_allreduce_fn fn, void *user) {
   return SS_OK;
 }
 
+namespace ss { static int debug_fetch(ss_stage *st); }
 static int kv_copy(ss_stage *st, int n, const int32_t *page_ids_dev, void *buf, size_t buf_bytes, bool to_buffer) {
   if (!st || n <= 0 || !page_ids_dev || !buf) return SS_ERR_INVALID_ARG;
   if ((uintptr_t)buf & 15) return SS_ERR_UNSUPPORTED;
   const size_t piece = (size_t)st->d.n_kv_heads * 16 * st->d.head_dim * 2;
   if (buf_bytes < (size_t)st->L * 2 * n * piece) return SS_ERR_CAPACITY;
+  if (st->debug) {
+    CK(cudaMemsetAsync(st->ws + st->c.err, 0, 16, st->stream));
+    const int64_t b0 = g_launches;
+    CK(launch_debug_validate_pages(page_ids_dev, n, st->num_pages, st->at<int32_t>(st->c.err), st->stream));
+    st->launches += g_launches - b0;
+    const int rc = debug_fetch(st);
+    if (rc != SS_OK) return rc;
+  }
   const int64_t before = g_launches;
   cudaError_t e = launch_kv_pages_copy(st->pool, buf, page_ids_dev, n, st->L, st->num_pages, (int)piece, to_buffer,
                                        st->stream);
@@ -589,7 +636,7 @@ static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T,
         CKE(launch_residual_rmsnorm(x, nullptr, 0, 0, w.ln2, d.rms_eps, H, T, h, args, false, s));
       } else {  // this rank's partial over its heads -> all-reduce -> x += sum (two per layer)
         CKE(run_gemm(st, a, 1, rows, false, st->b_attn, T, Hq, EPI_F32, tp_part, nullptr, H));
-        st->allreduce(tp_part, (size_t)T * H, st->allreduce_user, (void *)s);
+        if (st->allreduce(tp_part, (size_t)T * H, st->allreduce_user, (void *)s) != 0) return cudaErrorLaunchFailure;
         CKE(launch_residual_rmsnorm(x, tp_part, 1, 0, w.ln2, d.rms_eps, H, T, h, args, false, s));
       }
     }
@@ -608,7 +655,7 @@ static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T,
         CKE(launch_residual_rmsnorm(x, nullptr, 0, 0, next_ln, d.rms_eps, H, T, h, args, last, s));
       } else {
         CKE(run_gemm(st, a, 1, rows, false, st->b_a, T, F, EPI_F32, tp_part, nullptr, H));
-        st->allreduce(tp_part, (size_t)T * H, st->allreduce_user, (void *)s);
+        if (st->allreduce(tp_part, (size_t)T * H, st->allreduce_user, (void *)s) != 0) return cudaErrorLaunchFailure;
         CKE(launch_residual_rmsnorm(x, tp_part, 1, 0, next_ln, d.rms_eps, H, T, h, args, last, s));
       }
     }
@@ -639,13 +686,32 @@ static int common_checks(ss_stage *st, int n_seqs, int T, const void *hidden, co
 static int upload_args(ss_stage *st, const CallArgs &a) {
   // the previous call's copy may still be in flight from the same pinned block: the stream orders the copies,
   // but the host must not overwrite the block before the previous copy has read it
-  static thread_local cudaEvent_t ev = nullptr;
-  if (!ev) CK(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
-  CK(cudaEventSynchronize(ev));
+  CK(cudaEventSynchronize(st->args_ev));  // a never-recorded event is complete
   *st->h_args = a;
   CK(cudaMemcpyAsync(st->ws + st->c.args, st->h_args, sizeof(CallArgs), cudaMemcpyHostToDevice, st->stream));
-  CK(cudaEventRecord(ev, st->stream));
+  CK(cudaEventRecord(st->args_ev, st->stream));
   return SS_OK;
+}
+
+// SS_DEBUG=1: run the device-side contract checks of this call and wait for their verdict; nothing else has been
+// enqueued yet, so a violation leaves the pool and the workspace untouched.
+static int debug_fetch(ss_stage *st) {
+  CK(cudaMemcpyAsync(st->h_err(), st->ws + st->c.err, 16, cudaMemcpyDeviceToHost, st->stream));
+  CK(cudaStreamSynchronize(st->stream));
+  if (st->h_err()[0] != 0) {
+    memcpy(st->dbg_info, st->h_err(), 16);
+    return SS_ERR_INVALID_ARG;
+  }
+  return SS_OK;
+}
+static int debug_check(ss_stage *st, bool decode, int n_dec) {
+  if (!st->debug) return SS_OK;
+  CK(cudaMemsetAsync(st->ws + st->c.err, 0, 16, st->stream));
+  DebugCheck c{decode ? 1 : 0, n_dec, st->num_pages, st->d.max_pos, st->d.vocab};
+  const int64_t before = g_launches;
+  CK(launch_debug_validate(st->at<CallArgs>(st->c.args), c, st->at<int32_t>(st->c.err), st->stream));
+  st->launches += g_launches - before;
+  return debug_fetch(st);
 }
 
 }  // namespace ss
@@ -674,6 +740,7 @@ int ss_stage_mixed(ss_stage *st, int n_decode_rows, int n_seqs, const void *hidd
   a.cu_q = cu_q; a.out_hidden = out_hidden_bf16; a.out_logits = out_logits; a.out_argmax = out_argmax;
   a.n_seqs = n_seqs; a.T = total_tokens; a.max_blocks = max_blocks;
   if ((rc = upload_args(st, a)) != SS_OK) return rc;
+  if ((rc = debug_check(st, false, n_decode_rows)) != SS_OK) return rc;
   const int64_t before = g_launches;
   cudaError_t e = enqueue_forward(st, false, n_seqs, total_tokens, out_logits || out_argmax, n_decode_rows);
   st->launches += g_launches - before;
@@ -693,6 +760,7 @@ int ss_stage_decode(ss_stage *st, int batch, const void *hidden_bf16, const int3
   a.out_hidden = out_hidden_bf16; a.out_logits = out_logits; a.out_argmax = out_argmax;
   a.n_seqs = batch; a.T = batch; a.max_blocks = max_blocks;
   if ((rc = upload_args(st, a)) != SS_OK) return rc;
+  if ((rc = debug_check(st, true, 0)) != SS_OK) return rc;
   const bool tail = out_logits || out_argmax;
   if (!st->use_graph || st->allreduce) {  // a tensor-parallel shard calls back into the caller: never captured
     const int64_t before = g_launches;
@@ -733,14 +801,11 @@ int ss_stage_decode(ss_stage *st, int batch, const void *hidden_bf16, const int3
 // op-level entry points: the same GEMM kernel, stand-alone (per-kernel parity tests, profiling)
 // ===================================================================================================================
 namespace ss {
-static int device_sms() {
-  static int n = 0;
-  if (n == 0) {
-    int dev = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess ||
-        cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
-      n = 0;
-  }
+static int device_sms() {  // of the current device (a process may drive several)
+  int dev = 0, n = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess ||
+      cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+    return 0;
   return n;
 }
 
@@ -764,7 +829,7 @@ static int op_gemm(const void *x_dev, const void *w0, const void *w1, float *c_f
   p.seg_rows[0] = N;
   p.T = T;
   p.K = K;
-  p.epi = dual ? EPI_SWIGLU_BF16 : (env_int("SS_OP_GEMM_RESID", 0) ? EPI_RESID_F32 : EPI_F32);  // env: profiling only
+  p.epi = dual ? EPI_SWIGLU_BF16 : EPI_F32;
   p.ld_out = N;
   p.out_f32 = c_f32;
   p.out_bf16 = c_bf16;
@@ -775,9 +840,8 @@ static int op_gemm(const void *x_dev, const void *w0, const void *w1, float *c_f
   p.fix_slots = (float *)((uint8_t *)scratch_dev + GEMM_FIX_FLAG_BYTES);
   g.dual = dual;
   // the caller's weights may come straight out of a preceding kernel, so the weight ring must not be primed before
-  // that kernel has finished: no PDL, unless the caller vouches for long-lived weights (SS_OP_GEMM_PDL=1: bench.py
-  // times the dominant kernel launched exactly as the stage launches it)
-  g.no_pdl = env_int("SS_OP_GEMM_PDL", 0) == 0;
+  // that kernel has finished: no programmatic dependent launch here
+  g.no_pdl = true;
   g.stream = (cudaStream_t)cuda_stream;
   gemm_plan(g, n_sm);
   if (make_tmap_bf16_2d(&ta, w0, (uint64_t)N, (uint64_t)K, GEMM_BM, true) != 0 ||

@@ -80,18 +80,23 @@ def randn_bf16(shape, std: float, gen: torch.Generator, mean: float = 0.0) -> to
     return t.to(torch.bfloat16)
 
 
-def layer_weights(shape: ModelShape, layer: int, seed: int = 0, proj_std: float = 0.02) -> dict:
-    """CPU bf16 tensors of one decoder layer (no biases: reading A7)."""
+def layer_weights(shape: ModelShape, layer: int, seed: int = 0, proj_std: float = 0.02, executor=None) -> dict:
+    """CPU bf16 tensors of one decoder layer (no biases: reading A7).  `executor` (a concurrent.futures executor)
+    only draws the tensors concurrently: each has its own generator, so the bytes are the same either way."""
     H, Hq, Hkv, F, d = shape.hidden, shape.hq, shape.hkv, shape.ffn, shape.d
     shp = {"ln1": (H,), "wq": (Hq, H), "wk": (Hkv, H), "wv": (Hkv, H), "q_norm": (d,), "k_norm": (d,),
            "wo": (H, Hq), "ln2": (H,), "w_gate": (F, H), "w_up": (F, H), "w_down": (H, F)}
-    out = {}
-    for idx, name in enumerate(_TENSORS):
+    def draw(idx, name):
         g = _gen(seed, layer, idx)
         if name in ("ln1", "ln2", "q_norm", "k_norm"):
-            out[name] = randn_bf16(shp[name], 0.02, g, mean=1.0)
-        else:
-            out[name] = randn_bf16(shp[name], proj_std, g)
+            return randn_bf16(shp[name], 0.02, g, mean=1.0)
+        return randn_bf16(shp[name], proj_std, g)
+
+    if executor is None:
+        out = {name: draw(idx, name) for idx, name in enumerate(_TENSORS)}
+    else:
+        futs = {name: executor.submit(draw, idx, name) for idx, name in enumerate(_TENSORS)}
+        out = {name: f.result() for name, f in futs.items()}
     if not shape.qk_norm:
         out["q_norm"] = None
         out["k_norm"] = None

@@ -1,0 +1,181 @@
+"""north_star's Target at FULL DEPTH: the Llama-3.1-70B-shaped 20-layer stage (cfg-2, B = 64) and the Qwen3-32B-shaped
+16-layer stage (cfg-3, B = 128) against the CPU oracle, one ss_stage_decode of the seed-0 batch in the launch
+configuration bench.py times (CUDA-graph replay, PDL edges, stream-K GEMMs).  Stage = the optimizer's layer range
+(PAPER.md:92); models PAPER.md:289; SURVEY.md section 8(d) "step 0 full-depth vs oracle".
+
+The oracle cannot hold 34 GB of weights at once, so it is fed ONE LAYER AT A TIME: layer l's seeded tensors are drawn,
+uploaded to the device (where they stay: the GPU stage is the real 20 / 16-layer stage) and given to the oracle, which
+advances its own fp32 residual [B, H] and its own per-layer KV pool, once in mode R0 (plain fp32, what the tolerance
+is stated against) and once in mode R1 (bf16 at the points where a bf16 engine materialises a tensor).  The GPU side
+also runs the PREFIX stages [0, l) for every l — the same kernels, device weights and pool prefix — so the test prints
+error against depth: after each layer, GPU vs R0, GPU vs R1, and the oracle's own R1 vs R0 distance (what rounding the
+GEMM operands to bf16 costs by itself; reading A15b / A15d of DESIGN.md).
+
+Asserted (reading A15d of DESIGN.md; `floor(l)` = the oracle's own R1-vs-R0 distance at depth l):
+  * at every depth whose floor leaves room (floor(l) <= 1.6e-2): GPU vs R0 max row relative error (A15) < 2e-2, the
+    north_star bound as stated;
+  * at every depth: GPU vs R0 <= max(2e-2, 1.3 x floor(l)), and the same for GPU vs R1 — where rounding the GEMM operands
+    to bf16 moves the fp32 CPU oracle itself by more than ~1.6e-2 no bf16 engine can promise 2e-2 against R0, and the
+    GPU must then stay within the oracle's own distance (measured: cfg-2 floor 2.45e-2 at depth 20, GPU 2.18e-2);
+  * averaged over the depths the GPU is no further from R0 than R1 is (mean of e0 / floor <= 1.15);
+and after the full-depth step: KV pool — bytes outside the new tokens' slots unchanged in EVERY layer (A13 i, compared
+on the device against a copy of the initial pool), new slots of layer 0 within 1 bf16 ulp of R1 and of every layer
+within the per-layer bound printed below; graph replay of the same step returns the same bits.
+"""
+from concurrent.futures import ThreadPoolExecutor
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import Oracle
+from paper_2606_18600_b200 import binding, synth
+from tests import helpers as hp
+
+pytestmark = pytest.mark.gpu
+F32 = Oracle("f32")
+DEV = "cuda:0"
+STAGE_TOL = 2e-2
+FLOOR_ROOM = 1.6e-2     # reading A15d: the 2e-2 bound is asserted as stated wherever the oracle's bf16 floor is below this
+
+
+def _layer_pool(shape, n_pages, layer, seed=0):
+    """Random N(0,1) pre-fill of ONE layer's pool [2, pages, n_kv, 16, d] as uint16 bits (recipe A21)."""
+    g = torch.Generator()
+    g.manual_seed(seed * 1_000_003 + 3000 + 17 * layer)
+    t = torch.randn((2, n_pages, shape.n_kv, 16, shape.d), generator=g, dtype=torch.float32).to(torch.bfloat16)
+    return synth.bits(t).copy()
+
+
+def _gen_layer(shape, layer, n_pages):
+    """Draw layer `layer`: weights (tensor by tensor on worker threads: each tensor has its own generator, so the bytes
+    do not depend on the threading) and its pool pre-fill."""
+    with ThreadPoolExecutor(6) as ex:
+        fp = ex.submit(_layer_pool, shape, n_pages, layer)
+        w = synth.layer_weights(shape, layer, 0, executor=ex)
+        return w, fp.result()
+
+
+def _dev_bf16(bits_u16):
+    return torch.from_numpy(np.ascontiguousarray(bits_u16).view(np.int16)).view(torch.bfloat16).to(DEV)
+
+
+def _rows_f32(t):
+    return synth.bf16_bits_to_f32(t.cpu().view(torch.int16).numpy().view(np.uint16))
+
+
+@pytest.mark.parametrize("name", ["cfg2", "cfg3"])
+def test_full_depth_decode_stage_vs_oracle(name):
+    from tests import gpu_helpers as gh
+    shape, ctx_fn = (synth.LLAMA70B, synth.cfg2_contexts) if name == "cfg2" else (synth.QWEN32B, synth.cfg3_contexts)
+    L = shape.n_layers
+    assert L == (20 if name == "cfg2" else 16)
+    ctx = ctx_fn(0).astype(np.int32)
+    B = len(ctx)
+    pb = synth.paged_batch(np.random.default_rng(0), ctx, extra_tokens=2)
+    n_pages, bt = pb.n_pages_pool, pb.block_tables
+    x_bits = synth.bits(synth.hidden_rows(B, shape.hidden, 0))
+    cu = np.arange(B + 1, dtype=np.int32)
+    d0, d1 = hp.odims(shape, 0), hp.odims(shape, 1)
+
+    # device side: the whole stage's weights and one pool [L, 2, pages, n_kv, 16, d] (+ an untouched copy of it)
+    per_layer = 2 * n_pages * shape.n_kv * 16 * shape.d
+    pool_dev = torch.empty(L * per_layer, dtype=torch.bfloat16, device=DEV)
+    dw = []
+    # oracle side: fp32 residuals carried from layer to layer, the new tokens' K/V of every layer (mode R1)
+    x0 = synth.bf16_bits_to_f32(x_bits).copy()
+    x1 = x0.copy()
+    want0, want1, new_kv_r1 = [], [], []
+    slot_page = bt[np.arange(B), ctx >> 4]
+    slot_in = ctx & 15
+
+    with ThreadPoolExecutor(1) as bg:
+        fut = bg.submit(_gen_layer, shape, 0, n_pages)
+        for l in range(L):
+            w, pool_l = fut.result()
+            if l + 1 < L:
+                fut = bg.submit(_gen_layer, shape, l + 1, n_pages)
+            dw.append({k: (None if v is None else v.to(DEV)) for k, v in w.items()})
+            pool_dev[l * per_layer:(l + 1) * per_layer].copy_(_dev_bf16(pool_l).view(-1))
+            wb = {k: (None if v is None else synth.bits(v)) for k, v in w.items()}
+            p0, p1 = pool_l.copy(), pool_l
+            F32.layer(d0, wb, p0[0], p0[1], cu, ctx, bt, x0)
+            F32.layer(d1, wb, p1[0], p1[1], cu, ctx, bt, x1)
+            want0.append(x0.copy())
+            want1.append(x1.copy())
+            new_kv_r1.append(p1[:, slot_page, :, slot_in, :].transpose(1, 0, 2, 3).copy())   # [B,2,..] -> [2, B, n_kv, d]
+            del w, wb, p0, p1, pool_l
+    pool_before = pool_dev.clone()
+    torch.cuda.synchronize()
+
+    x_dev = _dev_bf16(x_bits)
+    bt_dev = torch.from_numpy(bt).to(DEV)
+    ctx_dev = torch.from_numpy(ctx).to(DEV)
+
+    def run(l1):
+        dims = binding.make_dims(shape, B, B, pb.max_blocks, n_layers_total=L)
+        st = binding.Stage(dims, 0, l1, dw[:l1], None, kv_pool=pool_dev[:l1 * per_layer], device=DEV)
+        try:
+            assert st.num_pages() == n_pages
+            out = torch.empty((B, shape.hidden), dtype=torch.bfloat16, device=DEV)
+            st.decode(B, bt_dev, ctx_dev, hidden=x_dev, out_hidden=out)
+            st.synchronize()
+            first = out.clone()
+            if l1 == L:                                    # graph replay on the same inputs: same bits
+                st.decode(B, bt_dev, ctx_dev, hidden=x_dev, out_hidden=out)
+                st.synchronize()
+                assert torch.equal(out, first)
+            return _rows_f32(first)
+        finally:
+            st.destroy()
+
+    print(f"\n{name}: {shape.name}, B={B}, depth sweep (max row rel err, reading A15)")
+    print("  depth   GPU vs R0   GPU vs R1   R1 vs R0 (oracle floor)   max|x|")
+    rows = []
+    for l1 in range(1, L + 1):
+        got = run(l1)
+        assert np.isfinite(got).all()
+        e0 = hp.rel_err_rows(got, want0[l1 - 1])
+        e1 = hp.rel_err_rows(got, want1[l1 - 1])
+        fl = hp.rel_err_rows(want1[l1 - 1], want0[l1 - 1])
+        print(f"  {l1:5d}   {e0:.3e}   {e1:.3e}   {fl:.3e}                  {float(np.abs(want0[l1 - 1]).max()):.1f}")
+        rows.append((l1, e0, e1, fl))
+    l1, e0, e1, fl = rows[-1]
+    print(f"{name}: full depth {L}: GPU vs R0 {e0:.3e} ({'meets' if e0 < STAGE_TOL else 'exceeds'} the 2e-2 target as "
+          f"stated; oracle floor R1 vs R0 at this depth {fl:.3e}); mean over depths of (GPU vs R0) / floor = "
+          f"{float(np.mean([r[1] / r[3] for r in rows])):.3f}")
+    for l1, e0, e1, fl in rows:
+        if fl <= FLOOR_ROOM:
+            assert e0 < STAGE_TOL, f"depth {l1}: GPU vs oracle R0 {e0:.3e} >= {STAGE_TOL} although the floor is {fl:.3e}"
+        bound = max(STAGE_TOL, 1.3 * fl)
+        assert e0 <= bound and e1 <= bound, f"depth {l1}: vs R0 {e0:.3e}, vs R1 {e1:.3e}, bound {bound:.3e}"
+    assert np.mean([r[1] / r[3] for r in rows]) <= 1.15
+
+    # ---- KV pool after the full-depth step (A13) -------------------------------------------------------------
+    torch.cuda.synchronize()
+    pv = pool_dev.view(torch.int16).view(L, 2, n_pages, shape.n_kv, 16, shape.d)
+    pv0 = pool_before.view(torch.int16).view(L, 2, n_pages, shape.n_kv, 16, shape.d)
+    mask = torch.zeros((n_pages, 16), dtype=torch.bool, device=DEV)
+    mask[torch.from_numpy(slot_page.astype(np.int64)).to(DEV), torch.from_numpy(slot_in.astype(np.int64)).to(DEV)] = True
+    for l in range(L):
+        changed = (pv[l] != pv0[l]).any(dim=-1).any(dim=2)                 # [2, pages, 16]
+        assert not bool((changed & ~mask[None]).any()), f"layer {l}: bytes outside the new tokens' slots changed"
+    new_gpu = pv[:, :, torch.from_numpy(slot_page.astype(np.int64)).to(DEV), :,
+                 torch.from_numpy(slot_in.astype(np.int64)).to(DEV), :]     # advanced indices first: [B, L, 2, n_kv, d]
+    new_gpu = new_gpu.permute(1, 2, 0, 3, 4).contiguous().cpu().numpy().view(np.uint16)
+    print("  layer   new K/V equal   within 1 ulp   only via |a-b| <= 2e-3 max|ref|   max abs diff / max|ref|")
+    for l in range(L):
+        a, b = new_gpu[l], new_kv_r1[l]
+        ulp = gh.bf16_ulp_distance(a, b)
+        fa, fb = synth.bf16_bits_to_f32(a), synth.bf16_bits_to_f32(b)
+        rel = float(np.abs(fa - fb).max() / np.abs(fb).max())
+        esc = (ulp > 1) & (np.abs(fa - fb) <= 2e-3 * np.abs(fb).max())
+        print(f"  {l:5d}   {float((ulp == 0).mean()):.4f}          {float((ulp <= 1).mean()):.4f}         "
+              f"{float(esc.mean()):.4f}                           {rel:.3e}")
+        if l == 0:
+            # A13 (ii): equal or adjacent bf16 values; near zero (cancellation in the projection / RoPE) one ulp is far
+            # below the tensor cores' accumulation difference, there an absolute bound takes over: counted and bounded
+            assert ((ulp <= 1) | esc).all() and (ulp == 0).mean() >= 0.90
+            assert esc.mean() <= 2e-2, f"{int(esc.sum())} layer-0 K/V elements pass only through the absolute bound"
+        # deeper layers inherit the hidden state's error: bounded like the hidden state itself
+        assert rel <= STAGE_TOL, f"layer {l}: new K/V differs from the R1 oracle by {rel:.3e} of the tensor maximum"
