@@ -37,6 +37,8 @@ def parse():
     ap.add_argument("--layers", type=int, default=0, help="override the stage depth (debug only; marks the line)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-sub", action="store_true",
+                    help="default workload only: skip the cfg-4 prefill and cfg-3 decode sub-records")
     return ap.parse_args()
 
 
@@ -64,17 +66,33 @@ def whole_job_value(units_per_rank, world, ms_max):
     return units_per_rank * world / (ms_max * 1e-3)
 
 
-def ncu_traffic(kernel, workload):
-    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `kernel`, from the committed ncu --set full
-    capture (profiles/r01_traffic.json names its source); None when no capture exists for this workload."""
-    p = os.path.join(ROOT, "profiles", "r01_traffic.json")
+def source_hash():
+    """sha1 over the CUDA sources of the library being timed (what 'the build' means for the ncu captures)."""
+    import hashlib
+    h = hashlib.sha1()
+    d = os.path.join(ROOT, "paper_2606_18600_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh", ".h")):
+            h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()[:12]
+
+
+def ncu_traffic(workload):
+    """dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel (gate/up + SwiGLU GEMM) in
+    this workload, from the committed `ncu --set full` capture (profiles/r02_traffic.json: a profiler cannot run inside
+    the timed program).  Returns (bytes or None, label): the label names the build (source hash) the capture was taken
+    from and says whether it is the build being timed."""
+    p = os.path.join(ROOT, "profiles", "r02_traffic.json")
     try:
-        e = json.load(open(p)).get(kernel)
+        e = json.load(open(p)).get(workload)
     except (OSError, ValueError):
-        return None
-    if not e or e.get("workload") != workload:
-        return None
-    return e["dram_bytes_read"] + e["dram_bytes_write"]
+        return None, "no capture committed"
+    if not e:
+        return None, "no capture committed for this workload"
+    same = e.get("source_hash") == source_hash()
+    return (e["dram_bytes_read"] + e["dram_bytes_write"],
+            f"ncu --set full capture of build {e.get('source_hash')} ({e.get('profile')}); "
+            + ("same sources as the library timed here" if same else "NOT the build timed here: context only"))
 
 
 class ClockSampler:
@@ -205,18 +223,19 @@ def cuda_time_ms(stream, fn, n):
     return e0.elapsed_time(e1)
 
 
-def run_decode(args, shape, ctx_fn, rank, world):
+def run_decode(args, shape, ctx_fn, rank, world, layers=None, K=None, W=None, dominant=True):
     import torch
     from paper_2606_18600_b200 import binding, synth
     dev = torch.device(f"cuda:{int(os.environ.get('LOCAL_RANK', 0))}")
     torch.cuda.set_device(dev)
-    K, W = args.steps, args.warmup
+    K, W = (args.steps if K is None else K), (args.warmup if W is None else W)
     rng = np.random.default_rng(args.seed)
     ctx0 = ctx_fn(args.seed).astype(np.int32)
     B = len(ctx0)
     total_steps = 2 * (K + W) + 8                        # device-timed pass + e2e pass
     pb = synth.paged_batch(rng, ctx0, extra_tokens=total_steps + 1)
-    layers = gpu_weights(shape, dev, args.seed)
+    if layers is None:
+        layers = gpu_weights(shape, dev, args.seed)
     dims = binding.make_dims(shape, max_tokens=B, max_seqs=B, max_blocks=pb.max_blocks,
                              max_pos=int(ctx0.max()) + total_steps + 64)
     st = binding.Stage(dims, 0, shape.n_layers, layers, None, n_pages=pb.n_pages_pool, device=dev)
@@ -283,9 +302,14 @@ def run_decode(args, shape, ctx_fn, rank, world):
         e2e = {"ms_per_step": dt * 1e3 / K, "h2d": h_in[0].numel() * 2 + h_bt.numel() * 4 + B * 4,
                "d2h": h_out.numel() * 2}
 
-    dom = dominant_gemm(st, shape, layers, B, dev)
+    dom = dominant_gemm(st, shape, layers, B, dev) if dominant else None
+    st.synchronize()
+    o32 = out.float()
+    if not bool(torch.isfinite(o32).all()):
+        raise SystemExit("bench.py: the last decode step produced non-finite hidden states")
     res = {"ms": ms, "tokens": B * K, "bytes_per_step": float(byts), "launches": int(launches), "clocks": clocks,
-           "e2e": e2e, "dominant": dom, "B": B, "ctx_sum": int(ctx0.sum()), "pages": int(pb.n_pages_pool)}
+           "e2e": e2e, "dominant": dom, "B": B, "ctx_sum": int(ctx0.sum()), "pages": int(pb.n_pages_pool),
+           "checksum": float(o32.abs().mean()), "K": K, "W": W}
     st.destroy()
     return res
 
@@ -328,19 +352,20 @@ def dominant_gemm(st, shape, layers, T, dev):
             "flops": 4 * T * shape.hidden * shape.ffn}
 
 
-def run_prefill(args, shape, len_fn, rank, world):
+def run_prefill(args, shape, len_fn, rank, world, layers=None, K=None, W=None):
     """cfg4: migration recompute — one ss_stage_prefill over all migrated requests, packed varlen, ctx_before = 0."""
     import torch
     from paper_2606_18600_b200 import binding, synth
     dev = torch.device(f"cuda:{int(os.environ.get('LOCAL_RANK', 0))}")
     torch.cuda.set_device(dev)
-    K, W = args.steps, args.warmup
+    K, W = (args.steps if K is None else K), (args.warmup if W is None else W)
     rng = np.random.default_rng(args.seed)
     lens = len_fn(args.seed).astype(np.int32)
     n = len(lens)
     T = int(lens.sum())
     pb = synth.paged_batch(rng, lens, extra_tokens=1)
-    layers = gpu_weights(shape, dev, args.seed)
+    if layers is None:
+        layers = gpu_weights(shape, dev, args.seed)
     dims = binding.make_dims(shape, max_tokens=T, max_seqs=n, max_blocks=pb.max_blocks, max_pos=int(lens.max()) + 64)
     st = binding.Stage(dims, 0, shape.n_layers, layers, None, n_pages=pb.n_pages_pool, device=dev)
     g = torch.Generator(device=dev)
@@ -390,8 +415,12 @@ def run_prefill(args, shape, len_fn, rank, world):
         dt = time.perf_counter() - t0
         e2e = {"ms_per_step": dt * 1e3 / K, "h2d": h_x.numel() * 2 + h_btp.numel() * 4 + h_cu.numel() * 4,
                "d2h": h_out.numel() * 2}
+    st.synchronize()
+    if not bool(torch.isfinite(out[-4096:].float()).all()):
+        raise SystemExit("bench.py: the prefill produced non-finite hidden states")
     res = {"ms": ms, "tokens": T * K, "flops_per_step": float(prefill_flops(shape, lens)), "launches": int(launches),
-           "clocks": clocks, "e2e": e2e, "T": T, "n_seqs": n, "pages": int(pb.n_pages_pool)}
+           "clocks": clocks, "e2e": e2e, "T": T, "n_seqs": n, "pages": int(pb.n_pages_pool), "K": K, "W": W,
+           "checksum": float(out[-4096:].float().abs().mean())}
     st.destroy()
     return res
 
@@ -721,6 +750,9 @@ def main():
         line = {"impl": "reference", "metric": metric, "value": val, "unit": unit, "n_gpus": 0, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": cfg,
+                # what actually ran: each "step" is a bounded SAMPLE (one decoder layer of the step, timed, x layers)
+                "steps_run": len(ts) - min(args.warmup, 1), "warmup_run": min(args.warmup, 1), "layers_run": 1,
+                "layers_per_step": shape.n_layers, "extrapolated": "ms_per_step = measured layer time x layers",
                 "cpu_baseline": {"value": val, "unit": unit, "cores": cores, "kind": "oracle",
                                  "sample": desc + "; time x layers (extrapolated)"},
                 "e2e": {"value": val, "unit": unit, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
@@ -797,55 +829,112 @@ def main():
                          "finished": res["finished"]}}
         print(json.dumps(line))
         return
-    res = run_decode(args, shape, len_fn, rank, world) if kind == "decode" else \
+    keep_layers = None
+    if kind == "decode" and args.workload == "cfg2" and not args.no_sub:
+        dev = torch.device(f"cuda:{int(os.environ.get('LOCAL_RANK', 0))}")
+        keep_layers = gpu_weights(shape, dev, args.seed)      # cfg-4 (same 70B shapes) re-uses them below
+    res = run_decode(args, shape, len_fn, rank, world, layers=keep_layers) if kind == "decode" else \
         run_prefill(args, shape, len_fn, rank, world)
-    ms = res["ms"]
-    e2e_ms = res["e2e"]["ms_per_step"] if res["e2e"] else None
+    K = args.steps
+    ms, e2e_ms = reduce_times(res, world)
+    line = None
+    if rank == 0:
+        line = {"metric": metric, "unit": unit, "n_gpus": world, "steps": K, "warmup": args.warmup,
+                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+                "config": cfg}
+        line.update(decode_record(res, ms, e2e_ms, world, shape, len_fn, args, pk) if kind == "decode" else
+                    prefill_record(res, ms, e2e_ms, world, shape, len_fn, args, pk))
+        line["build"] = source_hash()
+
+    # ---- the rest of BASELINE.json's metric, in the same line (default workload only): migration-recompute prefill
+    # tokens/s (cfg-4, on the weights already resident) and the second decode configuration (cfg-3) --------------------
+    if keep_layers is not None:
+        sh4, len4, _ = workload_spec("cfg4")
+        r4 = run_prefill(args, sh4, len4, rank, world, layers=keep_layers, K=2, W=1)
+        ms4, e4 = reduce_times(r4, world)
+        if rank == 0:
+            rec = prefill_record(r4, ms4, e4, world, sh4, len4, args, pk)
+            rec.update({"metric": "migration-recompute prefill tokens/s", "unit": unit, "steps": 2, "warmup": 1,
+                        "workload": "configs[3]: migration recompute prefill, 70B shapes, 20 layers, 32 requests "
+                                    "lognormal(med 1200), 40,173 tokens"})
+            line["prefill"] = rec
+        del keep_layers
+        torch.cuda.empty_cache()
+        sh3, len3, _ = workload_spec("cfg3")
+        r3 = run_decode(args, sh3, len3, rank, world, K=max(K, 10), W=max(args.warmup, 3))
+        ms3, e3 = reduce_times(r3, world)
+        if rank == 0:
+            rec = decode_record(r3, ms3, e3, world, sh3, len3, args, pk, workload="cfg3")
+            rec.update({"metric": "stage decode tokens/s", "unit": unit, "steps": r3["K"], "warmup": r3["W"],
+                        "workload": "configs[2]: Qwen3-32B-shaped 16-layer decode stage, B=128, ctx lognormal(med 768)"})
+            line["cfg3"] = rec
     if world > 1:
         import torch.distributed as dist
-        ms, e2e_max = max_over_ranks([ms, e2e_ms or 0.0], "cuda")
-        e2e_ms = e2e_max if e2e_ms is not None else None
         dist.barrier()
         dist.destroy_process_group()
     if rank != 0:
         return
-    K = args.steps
-    tokens_all = res["tokens"] * world
-    value = whole_job_value(res["tokens"], world, ms)
-    line = {"metric": metric, "value": value, "unit": unit, "n_gpus": world, "steps": K, "warmup": args.warmup,
-            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
-            "data": "synthetic", "config": cfg, "clocks": res["clocks"], "gpu_launches": res["launches"]}
-    if res["e2e"]:
-        line["e2e"] = {"value": tokens_all / K / (e2e_ms * 1e-3), "unit": unit,
-                       "h2d_bytes_per_step": int(res["e2e"]["h2d"]), "d2h_bytes_per_step": int(res["e2e"]["d2h"])}
-    if kind == "decode":
-        dom = res["dominant"]
-        ach = dom["bytes"] / (dom["us"] * 1e-6) / 1e9
-        line["roofline"] = {"bound": "hbm", "achieved": ach, "peak": pk["hbm_gbs"], "unit": "GB/s",
-                            "frac": ach / pk["hbm_gbs"], "traffic": ncu_traffic(dom["kernel"], args.workload),
-                            "algorithmic_bytes": dom["bytes"], "kernel": dom["kernel"],
-                            "us_per_launch": dom["us"], "peak_source": pk["source"]}
-        step_gbs = res["bytes_per_step"] / (ms / K * 1e-3) / 1e9
-        line["step_roofline"] = {"bound": "hbm", "algorithmic_GB_per_step": res["bytes_per_step"] / 1e9,
-                                 "achieved": step_gbs, "peak": pk["hbm_gbs"], "unit": "GB/s",
-                                 "frac": step_gbs / pk["hbm_gbs"]}
-        from paper_2606_18600_b200 import estimator
-        line["paper_estimator_ms"] = estimator.decode_step_ms(shape, len_fn(args.seed), pk["bf16_tflops"] * 1e12,
-                                                              pk["hbm_gbs"] * 1e9)
-    else:
-        tf = res["flops_per_step"] / (ms / K * 1e-3) / 1e12
-        line["roofline"] = {"bound": "tensor", "achieved": tf, "peak": pk["bf16_tflops_sustained"], "unit": "TFLOP/s",
-                            "frac": tf / pk["bf16_tflops_sustained"], "traffic": None,
-                            "kernel": "whole prefill step (GEMMs 98.4% of flops)", "peak_source": pk["source"],
-                            "frac_of_burst_peak": tf / pk["bf16_tflops"]}
-        from paper_2606_18600_b200 import estimator
-        line["paper_estimator_ms"] = estimator.prefill_ms(shape, len_fn(args.seed), pk["bf16_tflops"] * 1e12,
-                                                          pk["hbm_gbs"] * 1e9)
     if not args.no_cpu_baseline and world == 1:
         sec, T, cores, desc = oracle_sample(args.workload, args.seed, layers_sample=1)
         line["cpu_baseline"] = {"value": T / sec, "unit": unit, "cores": cores, "kind": "oracle",
                                 "sample": desc + "; time x layers (extrapolated)"}
     print(json.dumps(line))
+
+
+def reduce_times(res, world):
+    """(device-timed ms, e2e ms per step) as the MAX over ranks (replicas: the slowest one is the job's time)."""
+    ms = res["ms"]
+    e2e_ms = res["e2e"]["ms_per_step"] if res["e2e"] else None
+    if world > 1:
+        ms, e2e_max = max_over_ranks([ms, e2e_ms or 0.0], "cuda")
+        e2e_ms = e2e_max if e2e_ms is not None else None
+    return ms, e2e_ms
+
+
+def _common_record(res, ms, e2e_ms, world):
+    K = res["K"]
+    rec = {"value": whole_job_value(res["tokens"], world, ms), "ms_per_step": ms / K, "clocks": res["clocks"],
+           "gpu_launches": res["launches"], "output_checksum_mean_abs": res["checksum"]}
+    if res["e2e"]:
+        rec["e2e"] = {"value": res["tokens"] * world / K / (e2e_ms * 1e-3), "unit": "tokens/s",
+                      "h2d_bytes_per_step": int(res["e2e"]["h2d"]), "d2h_bytes_per_step": int(res["e2e"]["d2h"])}
+    return rec
+
+
+def decode_record(res, ms, e2e_ms, world, shape, len_fn, args, pk, workload=None):
+    from paper_2606_18600_b200 import estimator
+    K = res["K"]
+    rec = _common_record(res, ms, e2e_ms, world)
+    dom = res["dominant"]
+    if dom:
+        ach = dom["bytes"] / (dom["us"] * 1e-6) / 1e9
+        traffic, label = ncu_traffic(workload or args.workload)
+        rec["roofline"] = {"bound": "hbm", "achieved": ach, "peak": pk["hbm_gbs"], "unit": "GB/s",
+                           "frac": ach / pk["hbm_gbs"], "traffic": traffic, "traffic_source": label,
+                           "algorithmic_bytes": dom["bytes"], "kernel": dom["kernel"], "us_per_launch": dom["us"],
+                           "peak_source": pk["source"]}
+    step_gbs = res["bytes_per_step"] / (ms / K * 1e-3) / 1e9
+    rec["step_roofline"] = {"bound": "hbm", "algorithmic_GB_per_step": res["bytes_per_step"] / 1e9,
+                            "achieved": step_gbs, "peak": pk["hbm_gbs"], "unit": "GB/s",
+                            "frac": step_gbs / pk["hbm_gbs"]}
+    rec["paper_estimator_ms"] = estimator.decode_step_ms(shape, len_fn(args.seed), pk["bf16_tflops"] * 1e12,
+                                                         pk["hbm_gbs"] * 1e9)
+    return rec
+
+
+def prefill_record(res, ms, e2e_ms, world, shape, len_fn, args, pk):
+    from paper_2606_18600_b200 import estimator
+    K = res["K"]
+    rec = _common_record(res, ms, e2e_ms, world)
+    tf = res["flops_per_step"] / (ms / K * 1e-3) / 1e12
+    rec["roofline"] = {"bound": "tensor", "achieved": tf, "peak": pk["bf16_tflops_sustained"], "unit": "TFLOP/s",
+                       "frac": tf / pk["bf16_tflops_sustained"], "traffic": None,
+                       "kernel": "whole prefill step (GEMMs 98.4% of flops)", "peak_source": pk["source"],
+                       "peak_kind": "sustained (a >1 s step under the power cap)",
+                       "frac_of_burst_peak": tf / pk["bf16_tflops"]}
+    rec["paper_estimator_ms"] = estimator.prefill_ms(shape, len_fn(args.seed), pk["bf16_tflops"] * 1e12,
+                                                     pk["hbm_gbs"] * 1e9)
+    return rec
 
 
 if __name__ == "__main__":

@@ -36,6 +36,7 @@ pytestmark = pytest.mark.gpu
 F32 = Oracle("f32")
 DEV = "cuda:0"
 STAGE_TOL = 2e-2
+LAYER_TOL = 1e-2
 FLOOR_ROOM = 1.6e-2     # reading A15d: the 2e-2 bound is asserted as stated wherever the oracle's bf16 floor is below this
 
 
@@ -86,6 +87,7 @@ def test_full_depth_decode_stage_vs_oracle(name):
     x0 = synth.bf16_bits_to_f32(x_bits).copy()
     x1 = x0.copy()
     want0, want1, new_kv_r1 = [], [], []
+    tf_in, tf_want = [], []       # per layer (teacher-forced, reading A15): bf16 input bits, R0 answer from that input
     slot_page = bt[np.arange(B), ctx >> 4]
     slot_in = ctx & 15
 
@@ -99,6 +101,13 @@ def test_full_depth_decode_stage_vs_oracle(name):
             pool_dev[l * per_layer:(l + 1) * per_layer].copy_(_dev_bf16(pool_l).view(-1))
             wb = {k: (None if v is None else synth.bits(v)) for k, v in w.items()}
             p0, p1 = pool_l.copy(), pool_l
+            # teacher-forced: the oracle's layer-l input rounded to bf16 (the stage boundary dtype) -> this layer alone
+            xin = synth.bits(torch.from_numpy(x0).to(torch.bfloat16)).copy()
+            xt, pt = synth.bf16_bits_to_f32(xin).copy(), pool_l.copy()
+            F32.layer(d0, wb, pt[0], pt[1], cu, ctx, bt, xt)
+            tf_in.append(xin)
+            tf_want.append(xt)
+            del pt
             F32.layer(d0, wb, p0[0], p0[1], cu, ctx, bt, x0)
             F32.layer(d1, wb, p1[0], p1[1], cu, ctx, bt, x1)
             want0.append(x0.copy())
@@ -112,22 +121,33 @@ def test_full_depth_decode_stage_vs_oracle(name):
     bt_dev = torch.from_numpy(bt).to(DEV)
     ctx_dev = torch.from_numpy(ctx).to(DEV)
 
-    def run(l1):
+    def run(l1, l0=0, x_in=None):
         dims = binding.make_dims(shape, B, B, pb.max_blocks, n_layers_total=L)
-        st = binding.Stage(dims, 0, l1, dw[:l1], None, kv_pool=pool_dev[:l1 * per_layer], device=DEV)
+        st = binding.Stage(dims, l0, l1, dw[l0:l1], None, kv_pool=pool_dev[l0 * per_layer:l1 * per_layer], device=DEV)
         try:
             assert st.num_pages() == n_pages
             out = torch.empty((B, shape.hidden), dtype=torch.bfloat16, device=DEV)
-            st.decode(B, bt_dev, ctx_dev, hidden=x_dev, out_hidden=out)
+            st.decode(B, bt_dev, ctx_dev, hidden=x_dev if x_in is None else x_in, out_hidden=out)
             st.synchronize()
             first = out.clone()
-            if l1 == L:                                    # graph replay on the same inputs: same bits
+            if l1 == L and l0 == 0:                        # graph replay on the same inputs: same bits
                 st.decode(B, bt_dev, ctx_dev, hidden=x_dev, out_hidden=out)
                 st.synchronize()
                 assert torch.equal(out, first)
             return _rows_f32(first)
         finally:
             st.destroy()
+
+    # ---- per layer, teacher-forced, against R0 (north_star: 1e-2 per layer) — every layer of the real stage ------------
+    print(f"\n{name}: per-layer teacher-forced decode, 1-layer stage [l, l+1) from the oracle's bf16 input of layer l")
+    worst_layer = 0.0
+    for l in range(L):
+        got = run(l + 1, l, _dev_bf16(tf_in[l]))
+        e = hp.rel_err_rows(got, tf_want[l])
+        worst_layer = max(worst_layer, e)
+        print(f"  layer {l:2d}: rel err vs R0 {e:.3e}")
+        assert e < LAYER_TOL, f"layer {l}: {e:.3e} >= {LAYER_TOL}"
+    print(f"{name}: worst layer {worst_layer:.3e} < {LAYER_TOL}")
 
     print(f"\n{name}: {shape.name}, B={B}, depth sweep (max row rel err, reading A15)")
     print("  depth   GPU vs R0   GPU vs R1   R1 vs R0 (oracle floor)   max|x|")

@@ -15,6 +15,7 @@ from tests import helpers as hp
 
 pytestmark = pytest.mark.gpu
 F32 = Oracle("f32")
+ESCAPE_FRAC = 2e-2   # at most this fraction of first-layer K/V values may rely on the absolute bound (reading A13 ii)
 
 
 def _sub(shape, L):
@@ -41,13 +42,16 @@ def _check_new_kv(gh, shape, pool_before, pool_oracle_r1, pool_gpu, ctx, bt, lay
     b = synth.bf16_bits_to_f32(pool_oracle_r1[sel]).reshape(L, -1)
     # near zero (cancellation in RoPE / the projections) an absolute bound replaces the ulp bound, as in
     # tests/test_gpu_parity.py::_check_kv
-    ok0 = (ulp[0] <= 1) | (np.abs(a[0] - b[0]) <= 2e-3 * np.abs(b[0]).max())
+    esc0 = (ulp[0] > 1) & (np.abs(a[0] - b[0]) <= 2e-3 * np.abs(b[0]).max())
+    ok0 = (ulp[0] <= 1) | esc0
     eq0 = float((ulp[0] == 0).mean())
-    print(f"new KV, layer 0: equal {eq0:.4f}, outside 1 ulp / 2e-3 abs: {int((~ok0).sum())}; "
+    print(f"new KV, layer 0: equal {eq0:.4f}, <= 1 ulp {float((ulp[0] <= 1).mean()):.4f}, only via the 2e-3 absolute "
+          f"bound {float(esc0.mean()):.4f}, outside both: {int((~ok0).sum())}; "
           f"deeper layers max abs diff {float(np.abs(a - b).max()):.3e} (scale {float(np.abs(b).max()):.2f})")
     # at K = 8192 the tensor cores' fp32 accumulation differs from the CPU loop by ~2e-4 relative, so ~6% of the
-    # bf16 roundings land on the neighbouring value (measured 0.94 equal at cfg-2; 0.97+ at the tiny width)
-    assert ok0.all() and eq0 >= 0.90
+    # bf16 roundings land on the neighbouring value (measured 0.94 equal at cfg-2; 0.97+ at the tiny width); values
+    # near zero differ by more than one of THEIR ulps and pass through the absolute bound: counted, bounded (A13 ii)
+    assert ok0.all() and eq0 >= 0.90 and esc0.mean() <= ESCAPE_FRAC
     assert (np.abs(a - b) <= 1e-2 * np.abs(b).max()).all()
 
 
@@ -129,8 +133,11 @@ def test_full_width_recompute_prefill_and_migration_vs_oracle():
                 b = hp.logical_kv(pool_r1[0, kv], sub_bt[i], int(lens[s]) + 1)
                 ulp = gh.bf16_ulp_distance(a, b)
                 fa, fb = synth.bf16_bits_to_f32(a), synth.bf16_bits_to_f32(b)
-                ok = (ulp <= 1) | (np.abs(fa - fb) <= 2e-3 * np.abs(fb).max())
-                assert ok.all() and (ulp == 0).mean() >= 0.90, (int(s), kv, int((~ok).sum()))
+                esc = (ulp > 1) & (np.abs(fa - fb) <= 2e-3 * np.abs(fb).max())
+                ok = (ulp <= 1) | esc
+                print(f"request {int(s)} {'KV'[kv]}: equal {float((ulp == 0).mean()):.4f}, <= 1 ulp "
+                      f"{float((ulp <= 1).mean()):.4f}, only via the absolute bound {float(esc.mean()):.4f}")
+                assert ok.all() and (ulp == 0).mean() >= 0.90 and esc.mean() <= ESCAPE_FRAC, (int(s), kv, int((~ok).sum()))
         # pages of no sequence keep the sentinel (indexing, A13 i)
         used = np.zeros(pb.n_pages_pool, dtype=bool)
         for s in range(n):
@@ -138,6 +145,56 @@ def test_full_width_recompute_prefill_and_migration_vs_oracle():
         assert (pool_gpu[:, :, ~used] == 0x7FC1).all()
     finally:
         P.close()
+
+
+def test_full_width_migration_recompute_equals_incremental_on_gpu():
+    """The migration invariant (oracle pin P7) GPU against GPU at the paper's width: the two shortest
+    cfg-4 requests, one 70B-shaped layer.  (a) recompute = one ss_stage_prefill over prompt + 3 generated tokens;
+    (b) incremental = prefill of the prompt, then 3 ss_stage_decode steps.  The two must leave the same logical KV
+    (equal or within 2 bf16 ulp; the prefill tiles schedule and the decode stream-K cut sum in different orders) and
+    the same next-token hidden state within the stage tolerance; both match the oracle, for which the two paths are
+    bit-identical."""
+    from tests import gpu_helpers as gh
+    shape = _sub(synth.LLAMA70B, 1)
+    lens_all = synth.cfg4_lengths(0).astype(np.int32)
+    lens = np.sort(lens_all)[:2].astype(np.int32)
+    gen = 3
+    prompt = lens - gen
+    n, T = len(lens), int(lens.sum())
+    pb = synth.paged_batch(np.random.default_rng(5), lens, extra_tokens=2)
+    mk = lambda: gh.Problem(shape, 0, n_pages=pb.n_pages_pool, max_tokens=T, max_seqs=n, max_blocks=pb.max_blocks)
+    P, Q = mk(), mk()
+    try:
+        g = torch.Generator().manual_seed(78)
+        x = synth.bits(synth.randn_bf16((T + n, shape.hidden), 1.0, g))
+        cu = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
+        bt = pb.block_tables
+        P.prefill(lens, bt, x[:T])                                                     # (a)
+        rows = np.concatenate([np.arange(cu[s], cu[s] + prompt[s]) for s in range(n)])
+        Q.prefill(prompt, bt, x[rows])                                                 # (b)
+        for k in range(gen):
+            Q.decode(prompt + k, bt, x[np.array([cu[s] + prompt[s] + k for s in range(n)])])
+        pa, pq = P.pool_bits(), Q.pool_bits()
+        for s in range(n):
+            for kv in range(2):
+                a = hp.logical_kv(pa[0, kv], bt[s], int(lens[s]))
+                b = hp.logical_kv(pq[0, kv], bt[s], int(lens[s]))
+                ulp = gh.bf16_ulp_distance(a, b)
+                fa, fb = synth.bf16_bits_to_f32(a), synth.bf16_bits_to_f32(b)
+                esc = (ulp > 2) & (np.abs(fa - fb) <= 4e-3 * np.abs(fb).max())
+                print(f"request {s} {'KV'[kv]} recompute vs incremental: equal {float((ulp == 0).mean()):.4f}, <= 2 ulp "
+                      f"{float((ulp <= 2).mean()):.4f}, only via the absolute bound {float(esc.mean()):.4f}")
+                assert ((ulp <= 2) | esc).all() and (ulp == 0).mean() >= 0.90 and esc.mean() <= ESCAPE_FRAC
+        ya, yq = P.decode(lens, bt, x[T:]), Q.decode(lens, bt, x[T:])
+        pool = hp.new_pool(shape, pb.n_pages_pool, 1)
+        hp.run_oracle_prefill(F32, shape, P.wb, pool, lens, bt, x[:T])
+        want, _ = hp.run_oracle_decode(F32, shape, P.wb, pool, lens, bt, x[T:])
+        e_ab, e_a, e_b = hp.rel_err_rows(ya, yq), hp.rel_err_rows(ya, want), hp.rel_err_rows(yq, want)
+        print(f"next-token hidden: recompute vs incremental {e_ab:.3e}; vs oracle R0 {e_a:.3e} / {e_b:.3e}")
+        assert e_ab < 2e-2 and e_a < 2e-2 and e_b < 2e-2
+    finally:
+        P.close()
+        Q.close()
 
 
 def test_full_vocab_logits_and_argmax_vs_oracle():

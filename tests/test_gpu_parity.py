@@ -17,6 +17,7 @@ pytestmark = pytest.mark.gpu
 F32 = Oracle("f32")
 STAGE_TOL = 2e-2
 LAYER_TOL = 1e-2
+ESCAPE_FRAC = 5e-3   # at most this fraction of first-layer K/V values may rely on the absolute bound (A13 ii)
 
 
 def _gh():
@@ -139,10 +140,14 @@ def _check_kv(pool_gpu, pool_r1, mask, first_layer_only_ulp=True):
     gh = _gh()
     ulp = gh.bf16_ulp_distance(pool_gpu[0][mask[0]], pool_r1[0][mask[0]])
     a, b = f32b(pool_gpu[0][mask[0]]), f32b(pool_r1[0][mask[0]])
-    # near zero (cancellation in RoPE / projections) an absolute bound replaces the ulp bound
-    ok = (ulp <= 1) | (np.abs(a - b) <= 2e-3 * np.abs(b).max())
+    # near zero (cancellation in RoPE / projections) an absolute bound replaces the ulp bound; the elements that pass
+    # ONLY through it are counted, printed and bounded (so "<= 1 ulp" is what is asserted for all but that fraction)
+    esc = (ulp > 1) & (np.abs(a - b) <= 2e-3 * np.abs(b).max())
+    ok = (ulp <= 1) | esc
+    print(f"first-layer K/V: equal {float((ulp == 0).mean()):.4f}, <= 1 ulp {float((ulp <= 1).mean()):.4f}, "
+          f"only via the absolute bound {float(esc.mean()):.5f} ({int(esc.sum())} of {ulp.size})")
     assert ok.all(), f"first-layer KV differs by more than 1 bf16 ulp in {np.count_nonzero(~ok)} elements"
-    assert (ulp == 0).mean() > 0.97
+    assert (ulp == 0).mean() > 0.97 and esc.mean() <= ESCAPE_FRAC
     for l in range(1, pool_gpu.shape[0]):
         a, b = f32b(pool_gpu[l][mask[l]]).astype(np.float64), f32b(pool_r1[l][mask[l]]).astype(np.float64)
         assert np.abs(a - b).max() <= 1e-2 * np.abs(b).max()
@@ -158,8 +163,10 @@ G16 = synth.ModelShape("tiny-g16-d128", 512, 16, 1, 128, 1024, 2, 1e-6, 1e6, 1, 
                                                 (G12, 0.04, 0), (G16, 0.04, 0)])
 def test_stage_prefill_then_decode_vs_oracle(shape, proj_std, ref):
     """ref = 0: judged against the plain fp32 oracle (R0).  ref = 1: the 'sharp' variant of reading A21 (weights x8,
-    peaked softmax): there the oracle's own R1-vs-R0 distance is 6e-2 (any engine that materialises bf16
-    activations is that far from R0), so the GPU is judged against R1 — see DESIGN.md 'Tolerances'."""
+    peaked softmax), reading A15c: there the oracle's own R1-vs-R0 distance (printed and asserted below as
+    `floor`) is several times 2e-2 — any engine that materialises bf16 activations is that far from R0 — so the 2e-2
+    bound is held against R1, and against R0 the GPU must stay within 1.3 x that floor (the same rule as the
+    full-depth test, reading A15d)."""
     P, lens, pb, x = _problem(shape, proj_std=proj_std)
     try:
         T = int(lens.sum())
@@ -169,12 +176,15 @@ def test_stage_prefill_then_decode_vs_oracle(shape, proj_std, ref):
         want, _, cu = hp.run_oracle_prefill(F32, shape, P.wb, pool0, lens, bt, x[:T])
         pool1 = hp.new_pool(shape, pb.n_pages_pool, P.L)
         want1, _, _ = hp.run_oracle_prefill(F32, shape, P.wb, pool1, lens, bt, x[:T], rounding=1)
-        if ref == 1:
-            want = want1
         got = P.prefill(lens, bt, x[:T])
-        err = hp.rel_err_rows(got, want)
-        print(f"{shape.name} std={proj_std} prefill stage rel err {err:.3e}")
-        assert err < STAGE_TOL
+        err, err1, floor = hp.rel_err_rows(got, want), hp.rel_err_rows(got, want1), hp.rel_err_rows(want1, want)
+        print(f"{shape.name} std={proj_std} prefill stage rel err vs R0 {err:.3e}, vs R1 {err1:.3e}; oracle floor "
+              f"(R1 vs R0) {floor:.3e}")
+        if ref == 1:
+            assert floor > STAGE_TOL, "the sharp case no longer needs reading A15c: judge it against R0"
+            assert err1 < STAGE_TOL and err <= 1.3 * floor
+        else:
+            assert err < STAGE_TOL
         mask = _written_mask(pool0.shape, bt, lens)
         _check_kv(P.pool_bits(), pool1, mask)
         # ---- two decode steps on top (both sides continue from their own pools)
@@ -182,21 +192,28 @@ def test_stage_prefill_then_decode_vs_oracle(shape, proj_std, ref):
             xs = x[T + step * len(lens): T + (step + 1) * len(lens)]
             want_d, _ = hp.run_oracle_decode(F32, shape, P.wb, pool0, lens + step, bt, xs)
             want_d1, _ = hp.run_oracle_decode(F32, shape, P.wb, pool1, lens + step, bt, xs, rounding=1)
-            if ref == 1:
-                want_d = want_d1
             got_d = P.decode(lens + step, bt, xs)
-            err = hp.rel_err_rows(got_d, want_d)
-            print(f"{shape.name} decode step {step} stage rel err {err:.3e}")
-            assert err < STAGE_TOL
+            err, err1, floor = (hp.rel_err_rows(got_d, want_d), hp.rel_err_rows(got_d, want_d1),
+                                hp.rel_err_rows(want_d1, want_d))
+            print(f"{shape.name} decode step {step} stage rel err vs R0 {err:.3e}, vs R1 {err1:.3e}; floor {floor:.3e}")
+            if ref == 1:
+                assert err1 < STAGE_TOL and err <= max(STAGE_TOL, 1.3 * floor)
+            else:
+                assert err < STAGE_TOL
         mask = _written_mask(pool0.shape, bt, lens + 2)
         _check_kv(P.pool_bits(), pool1, mask)
     finally:
         P.close()
 
 
-def test_per_layer_teacher_forced_decode_vs_oracle():
-    """Reading A15 'per layer': a 1-layer stage run from the oracle's bf16-rounded layer input and the oracle's KV."""
-    shape = synth.TINY
+@pytest.mark.parametrize("shape", [synth.TINY, synth.TINY_QWEN, synth.TINY128])
+@pytest.mark.parametrize("phase", ["decode", "prefill"])
+def test_per_layer_teacher_forced_vs_oracle(shape, phase):
+    """Reading A15 'per layer', 1e-2 against the plain fp32 oracle R0: a 1-layer GPU stage holding layer l's weights is
+    run from the oracle's layer-l input (rounded to bf16, the stage-boundary dtype) over the oracle's KV pool of that
+    layer, for every layer, at decode (one new token per sequence on top of a prefilled context) and at prefill (the
+    whole prompt; causal attention + S5 append in qkv_post); Llama-style, Qwen3-style (QK-norm) and d = 128 shapes.
+    The full-width layers of both models are checked the same way in tests/test_gpu_full_depth.py."""
     gh = _gh()
     rng = np.random.default_rng(3)
     lens = synth.cfg1_contexts(3).astype(np.int32)
@@ -205,23 +222,26 @@ def test_per_layer_teacher_forced_decode_vs_oracle():
     T = int(lens.sum())
     x = synth.bits(synth.hidden_rows(T + 8, shape.hidden, 3))
     pool = hp.new_pool(shape, pb.n_pages_pool)
-    _, taps, _ = hp.run_oracle_prefill(F32, shape, wb_all, pool, lens, pb.block_tables, x[:T], taps=True)
+    pool_empty = pool.copy()
+    _, ptaps, cu = hp.run_oracle_prefill(F32, shape, wb_all, pool, lens, pb.block_tables, x[:T], taps=True)
     xs = x[T:T + len(lens)]
-    pool_before = pool.copy()
+    pool_prefilled = pool.copy()
     _, dtaps = hp.run_oracle_decode(F32, shape, wb_all, pool, lens, pb.block_tables, xs, taps=True)
+    dec = phase == "decode"
+    taps, x0, pool_before = (dtaps, xs, pool_prefilled) if dec else (ptaps, x[:T], pool_empty)
+    ctx = lens if dec else np.zeros_like(lens)
+    cu_q = np.arange(len(lens) + 1, dtype=np.int32) if dec else cu
+    sub = synth.ModelShape(shape.name, shape.hidden, shape.n_q, shape.n_kv, shape.d, shape.ffn, 1, shape.eps,
+                           shape.theta, shape.qk_norm, shape.vocab)
     for l in range(shape.n_layers):
-        # oracle input of layer l at the decode step, rounded to bf16 (the stage boundary dtype)
-        x_in = f32b(xs) if l == 0 else dtaps[l - 1]["out"]
+        # oracle input of layer l, rounded to bf16 (the stage boundary dtype), and the oracle's own answer from it
+        x_in = f32b(x0) if l == 0 else taps[l - 1]["out"]
         x_in_bits = synth.bits(torch.from_numpy(np.ascontiguousarray(x_in, dtype=np.float32)).to(torch.bfloat16))
         pool_l = pool_before[l:l + 1].copy()
         want = f32b(x_in_bits).copy()
-        w_l = [wb_all[l]]
-        F32.layer(hp.odims(shape), w_l[0], pool_l[0, 0], pool_l[0, 1], np.arange(len(lens) + 1, dtype=np.int32), lens,
-                  pb.block_tables, want)
+        F32.layer(hp.odims(shape), wb_all[l], pool_l[0, 0], pool_l[0, 1], cu_q, ctx, pb.block_tables, want)
         # GPU: 1-layer stage holding layer l's weights and the oracle's KV for that layer
-        sub = synth.ModelShape(shape.name, shape.hidden, shape.n_q, shape.n_kv, shape.d, shape.ffn, 1, shape.eps,
-                               shape.theta, shape.qk_norm, shape.vocab)
-        P = gh.Problem(sub, 3, n_pages=pb.n_pages_pool, max_tokens=64, max_seqs=16, max_blocks=pb.max_blocks)
+        P = gh.Problem(sub, 3, n_pages=pb.n_pages_pool, max_tokens=T + 64, max_seqs=16, max_blocks=pb.max_blocks)
         try:
             tw = synth.layer_weights(shape, l, 3)
             for k, v in tw.items():
@@ -229,12 +249,74 @@ def test_per_layer_teacher_forced_decode_vs_oracle():
                     P.dw[0][k].copy_(v.to("cuda:0"))
             P.stage.pool_view().copy_(torch.from_numpy(pool_before[l:l + 1].view(np.int16).copy())
                                       .view(torch.bfloat16).to("cuda:0"))
-            got = P.decode(lens, pb.block_tables, x_in_bits)
+            got = P.decode(lens, pb.block_tables, x_in_bits) if dec else P.prefill(lens, pb.block_tables, x_in_bits)
         finally:
             P.close()
         err = hp.rel_err_rows(got, want)
-        print(f"layer {l} teacher-forced decode rel err {err:.3e}")
+        print(f"{shape.name} layer {l} teacher-forced {phase} rel err vs R0 {err:.3e}")
         assert err < LAYER_TOL
+
+
+def test_ss_debug_device_contract_checks(monkeypatch):
+    """SS_DEBUG=1 (include/shuntstage.h, ss_stage_debug_info): a page id outside the pool, a
+    context beyond the listed pages, a position beyond max_pos, a token id outside the vocabulary and a malformed cu_q
+    are caught on the device BEFORE anything is enqueued — the call returns SS_ERR_INVALID_ARG, the violation is
+    reported, the pool keeps every sentinel byte — and a valid call still matches the oracle."""
+    from paper_2606_18600_b200 import binding
+    monkeypatch.setenv("SS_DEBUG", "1")
+    shape = synth.TINY
+    P, lens, pb, x = _problem(shape, seed=5, with_edge=True)
+    try:
+        on, info = P.stage.debug_info()
+        assert on and info == [0, 0, 0, 0]
+        bt = pb.block_tables
+        T, n = int(lens.sum()), len(lens)
+        cu = np.concatenate([[0], np.cumsum(lens)]).astype(np.int32)
+        n_pages = P.stage.num_pages()
+        out = torch.empty((T, shape.hidden), dtype=torch.bfloat16, device="cuda:0")
+        hid = P.bf16(x[:T])
+
+        def prefill(bt_=bt, cu_=cu, ctx_=np.zeros(n, np.int32), ids=None, T_=T):
+            kw = dict(token_ids=P.i32(ids)) if ids is not None else dict(hidden=hid[:T_])
+            rc = P.stage.prefill(n, P.i32(cu_), P.i32(ctx_), P.i32(bt_), T_, out_hidden=out[:T_], check=False, **kw)
+            P.stage.synchronize()
+            return rc, P.stage.debug_info()[1]
+
+        bad = bt.copy(); bad[2, 1] = n_pages                       # first page id past the pool
+        assert prefill(bt_=bad) == (-1, [1, 2, 1, n_pages])
+        bad = bt.copy(); bad[0, 0] = -3
+        assert prefill(bt_=bad) == (-1, [1, 0, 0, -3])
+        far = np.zeros(n, np.int32); far[1] = bt.shape[1] * 16      # ctx + q_len beyond the listed pages
+        rc, info = prefill(ctx_=far)
+        assert rc == -1 and info[0] == 2 and info[1] == 1
+        cu_bad = cu.copy(); cu_bad[2] = cu_bad[1]                   # an empty sequence
+        rc, info = prefill(cu_=cu_bad)
+        assert rc == -1 and info[0] == 5
+        ids = np.arange(T, dtype=np.int32) % shape.vocab; ids[7] = shape.vocab
+        assert prefill(ids=ids) == (-1, [4, -1, 7, shape.vocab])
+        # decode: context that puts the new token beyond max_pos; a bad page id in ss_kv_export
+        ctx_far = lens.copy(); ctx_far[3] = P.dims.max_pos
+        o2 = torch.empty((n, shape.hidden), dtype=torch.bfloat16, device="cuda:0")
+        rc = P.stage.decode(n, P.i32(bt), P.i32(ctx_far), hidden=hid[:n], out_hidden=o2, check=False)
+        assert rc == -1 and P.stage.debug_info()[1][0] in (2, 3) and P.stage.debug_info()[1][1] == 3
+        buf = torch.empty(2 * P.stage.page_bytes // 2, dtype=torch.bfloat16, device="cuda:0")
+        assert P.stage.kv_export(P.i32([1, n_pages + 5]), buf, check=False) == -1
+        assert P.stage.debug_info()[1] == [1, -1, 1, n_pages + 5]
+        # nothing was enqueued by any rejected call: every pool byte still holds the sentinel
+        assert (P.pool_bits() == 0x7FC1).all()
+        # a valid call under SS_DEBUG=1 works and matches the oracle
+        pool0 = hp.new_pool(shape, pb.n_pages_pool, P.L)
+        want, _, _ = hp.run_oracle_prefill(F32, shape, P.wb, pool0, lens, bt, x[:T])
+        got = P.prefill(lens, bt, x[:T])
+        assert hp.rel_err_rows(got, want) < STAGE_TOL
+    finally:
+        P.close()
+    monkeypatch.delenv("SS_DEBUG")
+    Q, _, _, _ = _problem(shape, seed=5)
+    try:
+        assert Q.stage.debug_info()[0] is False
+    finally:
+        Q.close()
 
 
 def test_migration_invariant_on_gpu():
@@ -263,8 +345,11 @@ def test_migration_invariant_on_gpu():
         assert (pa[~mask] == 0x7FC1).all() and (pq[~mask] == 0x7FC1).all()
         ulp = gh.bf16_ulp_distance(pa[mask], pq[mask])
         a, b = f32b(pa[mask]), f32b(pq[mask])
-        assert ((ulp <= 2) | (np.abs(a - b) <= 4e-3 * np.abs(b).max())).all()
-        assert (ulp == 0).mean() > 0.9
+        esc = (ulp > 2) & (np.abs(a - b) <= 4e-3 * np.abs(b).max())
+        print(f"recompute vs incremental K/V: equal {float((ulp == 0).mean()):.4f}, <= 2 ulp "
+              f"{float((ulp <= 2).mean()):.4f}, only via the absolute bound {float(esc.mean()):.5f}")
+        assert ((ulp <= 2) | esc).all()
+        assert (ulp == 0).mean() > 0.9 and esc.mean() <= 2 * ESCAPE_FRAC
         # next decode step from both states
         xs = x[T:T + len(lens)]
         ya = P.decode(lens, bt, xs)
