@@ -72,6 +72,43 @@ cudaError_t launch_input_rmsnorm(const CallArgs *args, const void *embed, const 
   return launch_pdl(input_rmsnorm_kernel, dim3(T), dim3(EW_THREADS), 0, s, args, (const __nv_bfloat16 *)embed, (const __nv_bfloat16 *)ln_w, eps, H, x, (__nv_bfloat16 *)h);
 }
 
+// ---- pieces of an EPI_PARTIAL projection (internal.h GemmPartials): rows [r, r + 4) of row tile `tile`, token column
+// `tok`, added in CTA order.  The loads of up to four pieces are issued together (independent L2 round trips). --------
+__device__ __forceinline__ float4 gemm_partial_sum4(const GemmPartials &gp, int tile, int tok, int r) {
+  const PartialTile pt = gp.tiles[tile];
+  const float *base = gp.slots + (size_t)tok * GEMM_BM + r;
+  auto piece = [&](int q) {
+    const int slot = 2 * (pt.first_cta + q) + (q == 0 ? pt.first_item : 0);
+    return __ldcg(reinterpret_cast<const float4 *>(base + (size_t)slot * gp.slot_floats));
+  };
+  float4 y = piece(0);
+  for (int q = 1; q < pt.count; q += 4) {
+    float4 z[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+      if (q + u < pt.count) z[u] = piece(q + u);
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+      if (q + u < pt.count) {
+        y.x += z[u].x; y.y += z[u].y; y.z += z[u].z; y.w += z[u].w;
+      }
+  }
+  return y;
+}
+
+__device__ __forceinline__ float2 gemm_partial_sum2(const GemmPartials &gp, int tile, int tok, int r) {
+  const PartialTile pt = gp.tiles[tile];
+  const float *base = gp.slots + (size_t)tok * GEMM_BM + r;
+  float2 y = make_float2(0.f, 0.f);
+  for (int q = 0; q < pt.count; ++q) {
+    const int slot = 2 * (pt.first_cta + q) + (q == 0 ? pt.first_item : 0);
+    const float2 z = __ldcg(reinterpret_cast<const float2 *>(base + (size_t)slot * gp.slot_floats));
+    y.x = q == 0 ? z.x : y.x + z.x;
+    y.y = q == 0 ? z.y : y.y + z.y;
+  }
+  return y;
+}
+
 // ---- residual += sum_s part[s]; optional RMSNorm -> h; optional bf16 stage output -----------------------------
 // One CTA of 1024 threads per token row; the whole row lives in registers (IT float4 per thread, H <= IT*4096), all
 // loads are issued before any use, and x is read and written exactly once.
@@ -80,8 +117,8 @@ cudaError_t launch_input_rmsnorm(const CallArgs *args, const void *embed, const 
 template <int IT, int RN_THREADS>
 __global__ void __launch_bounds__(RN_THREADS)
 residual_rmsnorm_kernel(float *__restrict__ x, const float *__restrict__ part, int splits, long long split_stride,
-                        const __nv_bfloat16 *__restrict__ w, float eps, int H, __nv_bfloat16 *__restrict__ h,
-                        const CallArgs *__restrict__ args, int write_out) {
+                        const GemmPartials gp, const __nv_bfloat16 *__restrict__ w, float eps, int H,
+                        __nv_bfloat16 *__restrict__ h, const CallArgs *__restrict__ args, int write_out) {
   pdl_launch_dependents();
   pdl_wait();
   __shared__ float red[32];
@@ -100,6 +137,14 @@ residual_rmsnorm_kernel(float *__restrict__ x, const float *__restrict__ part, i
       if (splits > 0) y[i] = *reinterpret_cast<const float4 *>(pr + j);
     }
   }
+  if (gp.slots) {
+    // the projection left its tiles in pieces (EPI_PARTIAL, internal.h): y = the tile's pieces added in CTA order
+#pragma unroll
+    for (int i = 0; i < IT; ++i) {
+      const int j = (i * RN_THREADS + threadIdx.x) * 4;
+      if (j < H) y[i] = gemm_partial_sum4(gp, j >> 7, t, j & 127);
+    }
+  }
   for (int s = 1; s < splits; ++s) {
 #pragma unroll
     for (int i = 0; i < IT; ++i) {
@@ -116,7 +161,7 @@ residual_rmsnorm_kernel(float *__restrict__ x, const float *__restrict__ part, i
     const int j = (i * RN_THREADS + threadIdx.x) * 4;
     v[i].x += y[i].x; v[i].y += y[i].y; v[i].z += y[i].z; v[i].w += y[i].w;
     if (j < H) {
-      if (splits > 0) *reinterpret_cast<float4 *>(xr + j) = v[i];  // splits == 0: x already holds the sum
+      if (splits > 0 || gp.slots) *reinterpret_cast<float4 *>(xr + j) = v[i];  // otherwise x already holds the sum
       ss += v[i].x * v[i].x + v[i].y * v[i].y + v[i].z * v[i].z + v[i].w * v[i].w;
       if (outp) {
         uint2 o;
@@ -143,13 +188,13 @@ residual_rmsnorm_kernel(float *__restrict__ x, const float *__restrict__ part, i
 }
 
 cudaError_t launch_residual_rmsnorm(float *x, const float *part, int splits, long long split_stride,
-                                    const void *ln_w, float eps, int H, int T, void *h, const CallArgs *args,
-                                    bool write_out_hidden, cudaStream_t s) {
+                                    const GemmPartials &gp, const void *ln_w, float eps, int H, int T, void *h,
+                                    const CallArgs *args, bool write_out_hidden, cudaStream_t s) {
   const __nv_bfloat16 *w = (const __nv_bfloat16 *)ln_w;
   __nv_bfloat16 *hh = (__nv_bfloat16 *)h;
   const int wo = write_out_hidden ? 1 : 0;
   auto go = [&](auto kernel, int threads) {
-    return launch_pdl(kernel, dim3(T), dim3(threads), 0, s, x, part, splits, split_stride, w, eps, H, hh, args, wo);
+    return launch_pdl(kernel, dim3(T), dim3(threads), 0, s, x, part, splits, split_stride, gp, w, eps, H, hh, args, wo);
   };
   if (T >= 512 && H <= 16 * 256 * 4) {  // many rows: 256 threads each
     const int it = (H + 1023) / 1024;
@@ -285,7 +330,23 @@ __global__ void __launch_bounds__(EW_THREADS) qkv_post_kernel(const QkvPostParam
 #pragma unroll
   for (int i = 0; i < V; ++i) lo[i] = hi[i] = 0.f;
   const int ldq = n_heads * d;
-  if (active) {
+  if (active && p.gp.slots) {
+    // the QKV projection left its tiles in pieces (EPI_PARTIAL): this head's d rows lie inside one 128-row tile of its
+    // segment (d divides 128), the low half at row r0 + c, the rotation partners d/2 rows further
+    const int seg = head < p.n_q ? 0 : (head < p.n_q + p.n_kv ? 1 : 2);
+    const int row = (head - (seg == 0 ? 0 : (seg == 1 ? p.n_q : p.n_q + p.n_kv))) * d;
+    const int tile = (seg == 0 ? 0 : (seg == 1 ? p.tile0_k : p.tile0_v)) + (row >> 7);
+    const int r0 = (row & 127) + c;
+    if (V == 4) {
+      const float4 a = gemm_partial_sum4(p.gp, tile, t, r0), b = gemm_partial_sum4(p.gp, tile, t, r0 + half);
+      lo[0] = a.x; lo[1] = a.y; lo[2] = a.z; lo[3] = a.w;
+      hi[0] = b.x; hi[1] = b.y; hi[2] = b.z; hi[3] = b.w;
+    } else {
+      const float2 a = gemm_partial_sum2(p.gp, tile, t, r0), b = gemm_partial_sum2(p.gp, tile, t, r0 + half);
+      lo[0] = a.x; lo[1] = a.y;
+      hi[0] = b.x; hi[1] = b.y;
+    }
+  } else if (active) {
     const float *src = p.qkv_part + (size_t)t * ldq + (size_t)head * d;
     for (int s = 0; s < p.splits; ++s) {
       const float *sp = src + (size_t)s * p.split_stride;

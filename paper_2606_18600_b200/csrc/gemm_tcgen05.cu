@@ -361,7 +361,19 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
         }
       };
 
-      if (!is_first) {
+      if (!DUAL && p.epi == EPI_PARTIAL) {
+        // every piece of a tile (owner's included) goes to its own slot; the consumer kernel adds them (internal.h)
+        float *slot = p.fix_slots + ((size_t)cta * 2 + item) * bn * GEMM_BM;
+        for (int c0 = grp * 32; c0 < bn; c0 += 64) {
+          uint32_t v[32];
+          ld_acc((uint32_t)c0, v);
+#pragma unroll
+          for (int j = 0; j < 32; ++j) slot[(size_t)(c0 + j) * GEMM_BM + r] = __uint_as_float(v[j]);
+        }
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&tempty[buf]);
+      } else if (!is_first) {
         // contributor: dump the raw fp32 accumulator(s) to this CTA's slot, [acc][col][row]
         float *slot = p.fix_slots + (size_t)cta * (DUAL ? 2 : 1) * bn * GEMM_BM;
         for (int c0 = grp * 32; c0 < (int)acc_cols; c0 += 64) {
@@ -613,6 +625,34 @@ void gemm_plan(GemmLaunch &g, int n_sm) {
       const int aligned = (max_grid / nt) * nt;
       if (aligned * 10 >= max_grid * 8) g.grid = aligned;
     }
+  }
+}
+
+bool gemm_partial_ok(const GemmLaunch &g) {
+  const GemmParams &p = g.p;
+  if (g.dual || p.sched != SCHED_STREAMK || p.n_t_tiles != 1) return false;
+  const long long nkb = (p.K + GEMM_BK - 1) / GEMM_BK;
+  const long long U = (long long)p.n_row_tiles * nkb;
+  return (U + g.grid - 1) / g.grid <= nkb;  // a CTA range never spans more than two tiles
+}
+
+void gemm_partial_table(const GemmLaunch &g, PartialTile *out) {
+  const GemmParams &p = g.p;
+  const uint32_t nkb = (uint32_t)((p.K + GEMM_BK - 1) / GEMM_BK), G = (uint32_t)g.grid;
+  const uint32_t U = (uint32_t)p.n_row_tiles * nkb, uq = U / G, ur = U - uq * G;
+  auto rs = [&](uint32_t c) { return c * uq + (c * ur) / G; };  // = WorkIter::range_start
+  uint32_t c = 0;
+  for (int i = 0; i < p.n_row_tiles; ++i) {
+    const uint32_t lo = (uint32_t)i * nkb, hi = lo + nkb;
+    while (rs(c + 1) <= lo) ++c;  // first CTA whose range reaches into tile i
+    PartialTile t;
+    t.first_cta = (int)c;
+    t.first_item = rs(c) < lo ? 1 : 0;  // the CTA started in the previous tile: this tile is its second item
+    uint32_t e = c;
+    while (e + 1 < G && rs(e + 1) < hi) ++e;
+    t.count = (int)(e - c + 1);
+    t.pad = 0;
+    out[i] = t;
   }
 }
 

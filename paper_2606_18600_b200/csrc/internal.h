@@ -26,7 +26,10 @@ constexpr int GEMM_MAX_STAGES = 12;
 enum GemmEpilogue {
   EPI_F32 = 0,          // out_f32[t][col] = acc
   EPI_SWIGLU_BF16 = 1,  // dual: out_bf16[t][col] = silu(acc_gate) * acc_up
-  EPI_RESID_F32 = 2     // out_f32[t][col] += acc   (residual stream updated in place; each element once)
+  EPI_RESID_F32 = 2,    // out_f32[t][col] += acc   (residual stream updated in place; each element once)
+  EPI_PARTIAL = 3       // stream-K, one token tile: every work item dumps its raw fp32 accumulator to slot
+                        // 2 * cta + item of fix_slots ([token column][tile row], bn * 128 floats); the CONSUMER kernel
+                        // (qkv_post, residual_rmsnorm) adds a tile's pieces in CTA order (GemmPartials below)
 };
 enum GemmSchedule { SCHED_STREAMK = 0, SCHED_TILES = 1 };
 
@@ -54,6 +57,19 @@ struct GemmParams {
   int *fix_flags;       // SCHED_STREAMK: gridDim.x flags, zero between launches (consumers reset them)
 };
 
+// What the consumer of an EPI_PARTIAL projection needs to put a tile together again.  Row tile i of the projection
+// was held by the `count` consecutive CTAs starting at `first_cta`; CTA c's piece is slot 2 * c + (c == first_cta ?
+// first_item : 0)  (a CTA range spans at most two tiles: the tail of one, then the head of the next).  The pieces are
+// added in CTA order, which is the order the in-kernel fix-up uses, so both give the same bits.
+struct PartialTile {
+  int32_t first_cta, count, first_item, pad;
+};
+struct GemmPartials {
+  const float *slots;         // null: the projection's result is in its ordinary output buffer
+  const PartialTile *tiles;   // [n_row_tiles] (device)
+  int slot_floats;            // bn * 128
+};
+
 struct GemmLaunch {
   const CUtensorMap *a[3];  // weight maps, box {64, 128}; dual (SwiGLU): a[0] = gate, a[1] = up, n_seg = 1
   const CUtensorMap *b;     // activation map, box {64, bn}
@@ -69,6 +85,10 @@ int make_tmap_bf16_2d(CUtensorMap *out, const void *base, uint64_t rows, uint64_
                       bool weight_like);
 // Fills sched / band / stages / n_*_tiles / grid from the problem shape; fix buffers must be set by the caller.
 void gemm_plan(GemmLaunch &g, int n_sm);
+// true if this planned launch may run with EPI_PARTIAL (stream-K, one token tile, no CTA range spanning > 2 tiles)
+bool gemm_partial_ok(const GemmLaunch &g);
+// host: the PartialTile table of a planned stream-K launch (n_row_tiles entries)
+void gemm_partial_table(const GemmLaunch &g, PartialTile *out);
 cudaError_t gemm_launch(const GemmLaunch &g);
 cudaError_t gemm_init();  // sets max dynamic smem attributes once
 cudaError_t gemm_set_debug_buffer(unsigned long long *host_mapped);  // see gemm_tcgen05.cu wait_expired()
@@ -77,7 +97,7 @@ int gemm_pick_stages(int bn, bool dual);
 size_t gemm_smem_bytes(int bn, bool dual, int stages);
 constexpr int GEMM_MAX_GRID = 256;                       // upper bound on persistent CTAs (sizes the fix buffers)
 constexpr size_t GEMM_FIX_FLAG_BYTES = 1024;             // GEMM_MAX_GRID ints
-constexpr size_t GEMM_FIX_SLOT_BYTES = 2 * 256 * 128 * 4;  // worst case: dual, bn = 256
+constexpr size_t GEMM_FIX_SLOT_BYTES = 2 * 256 * 128 * 4;  // worst case: dual, bn = 256 (or two plain items of a CTA)
 inline size_t gemm_fix_bytes() { return GEMM_FIX_FLAG_BYTES + GEMM_MAX_GRID * GEMM_FIX_SLOT_BYTES; }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -100,9 +120,10 @@ cudaError_t launch_input_rmsnorm(const CallArgs *args, const void *embed, const 
                                  int T, float *x, void *h, cudaStream_t s);
 // x[t,:] += sum_{s<splits} part[s][t,:]; then (w != null) h = bf16(rmsnorm(x) * w); (out_from_args) the bf16 of
 // x goes to args->out_hidden when that is non-null.
+// gp.slots != null: additionally x[t,:] += the pieces of an EPI_PARTIAL projection (added in CTA order first).
 cudaError_t launch_residual_rmsnorm(float *x, const float *part, int splits, long long split_stride,
-                                    const void *ln_w, float eps, int H, int T, void *h, const CallArgs *args,
-                                    bool write_out_hidden, cudaStream_t s);
+                                    const GemmPartials &gp, const void *ln_w, float eps, int H, int T, void *h,
+                                    const CallArgs *args, bool write_out_hidden, cudaStream_t s);
 // gather the last row of each sequence: hl[s,:] = bf16(rmsnorm(x[last(s),:]) * wf)
 cudaError_t launch_final_norm_rows(const float *x, const CallArgs *args, bool decode, const void *wf, float eps,
                                    int H, int n_seqs, void *hl, cudaStream_t s);
@@ -112,6 +133,8 @@ cudaError_t launch_logits_argmax(const float *logits, int V, int n_rows, float *
                                  const CallArgs *args, cudaStream_t s);
 
 struct QkvPostParams {
+  GemmPartials gp;         // slots != null: the QKV projection's tiles are in pieces (EPI_PARTIAL) instead of qkv_part
+  int tile0_k, tile0_v;    // first row tile of the k and v segments (q starts at tile 0)
   const float *qkv_part;   // [splits][T][Hq+2Hkv]
   int splits;
   long long split_stride;
@@ -172,14 +195,16 @@ struct PrefillPlan {
 // seq0: the first seq0 sequences get no query tiles (mixed batches: their attention runs in the decode kernel)
 cudaError_t launch_prefill_plan(const CallArgs *args, int n_seqs, int seq0, PrefillPlan plan, cudaStream_t s);
 struct PrefillAttnParams {
-  const void *q;             // bf16 [T,Hq]
-  const void *kpool, *vpool;
+  const CUtensorMap *q_map;  // q bf16 [max_tokens, Hq] as a 2-D tensor, box {64 columns, 128 rows}
+  const CUtensorMap *kv_map; // this layer's pool, as in DecodeAttnParams
+  int n_pages;
   int n_seqs, T, n_q, n_kv, d;
   PrefillPlan plan;
   void *out;                 // bf16 [T,Hq]
   const CallArgs *args;
-  int max_tiles;             // upper bound on query tiles = ceil(T/64) + n_seqs
+  int max_tiles;             // upper bound on query tiles = ceil(T / prefill_attn_tile_rows()) + n_seqs
 };
+int prefill_attn_tile_rows();
 cudaError_t launch_prefill_attn(const PrefillAttnParams &p, cudaStream_t s);
 cudaError_t prefill_attn_init();
 

@@ -44,12 +44,13 @@ static int cuda_fail(cudaError_t e, const char *where) {
     if (e__ != cudaSuccess) return cuda_fail(e__, #call); \
   } while (0)
 
+constexpr int PTAB_STRIDE = 512;    // row tiles per table: (16384 + 2 * 16384) / 128 = 384 at most, see dims_ok
 constexpr int MAX_WORKERS = 4096;  // upper bound on decode-attention worker warps (sizes the partial buffers)
 
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Carve {  // byte offsets into the workspace
-  size_t args, err, rope, x, h, qkv_part, q, kv_new, attn_out, fix, a, part_o, part_ml, cum_pages, meta, tp_part, am_part, tok_seq,
+  size_t args, err, ptab, rope, x, h, qkv_part, q, kv_new, attn_out, fix, a, part_o, part_ml, cum_pages, meta, tp_part, am_part, tok_seq,
       tok_pos, tile_cum, tile_order, hl, logits, total;
 };
 
@@ -64,6 +65,7 @@ static bool dims_ok(const ss_model_dims *d, int l0, int l1, int *why) {
   if (d->page_size != 16) return false;
   if (d->n_q_heads % d->n_kv_heads != 0 || d->n_q_heads / d->n_kv_heads > 16) return false;
   if (d->hidden % 8 != 0 || d->ffn % 8 != 0 || d->hidden > 16384) return false;
+  if ((long long)d->n_q_heads * d->head_dim > 16384) return false;
   return true;
 }
 
@@ -81,6 +83,8 @@ static Carve carve(const ss_model_dims *d) {
   };
   c.args = take(sizeof(CallArgs));
   c.err = take(16);  // SS_DEBUG device error word {code, sequence, index, value}
+  // EPI_PARTIAL tile tables of the QKV, O and down projections (internal.h PartialTile), PTAB_STRIDE entries each
+  c.ptab = take(3 * PTAB_STRIDE * sizeof(PartialTile));
   c.rope = take((size_t)d->max_pos * (d->head_dim / 2) * 2 * sizeof(float));
   c.x = take(Tm * H * 4);
   c.h = take(Tm * H * 2);
@@ -182,7 +186,9 @@ struct ss_stage {
   int n_workers;
   std::vector<LayerMaps> maps;
   CUtensorMap lm_map;
+  CUtensorMap q_map;   // q [Tm, Hq] bf16, box {64, 128}: the prefill attention's query tiles
   CUtensorMap b_h[9], b_attn[9], b_a[9], b_hl[9];  // activation maps for bn = 16 and 32, 64, ..., 256 (index bn / 32)
+  bool ptab_ok[3];  // the QKV / O / down projection may leave its tiles in pieces at decode-sized calls
   ss_pool pages;
   int64_t launches;
   std::map<int, Graph> graphs;  // key = batch*2 + tail
@@ -347,6 +353,7 @@ int ss_stage_create(ss_stage **out, const ss_model_dims *dims, int l0, int l1, c
     rc |= make_tmap_bf16_2d(&m.kv, st->kpool(l), (uint64_t)2 * st->num_pages * dims->n_kv_heads * 16,
                             (uint64_t)dims->head_dim, 16, true);
   }
+  rc |= make_tmap_bf16_2d(&st->q_map, st->ws + c.q, Tm, Hq, 128, false);
   if (rc == 0 && edge && edge->lm_head)
     rc |= make_tmap_bf16_2d(&st->lm_map, edge->lm_head, (uint64_t)dims->vocab, H, GEMM_BM, true);
   const int bns[9] = {16, 32, 64, 96, 128, 160, 192, 224, 256};
@@ -359,6 +366,26 @@ int ss_stage_create(ss_stage **out, const ss_model_dims *dims, int l0, int l1, c
   if (rc != 0) {
     g_cuda_err = "cuTensorMapEncodeTiled failed (code " + std::to_string(rc) + ")";
     return fail(SS_ERR_CUDA);
+  }
+
+  {  // EPI_PARTIAL tile tables: the stream-K cut of a one-token-tile launch depends on the shape only, not on T
+    std::vector<PartialTile> tab(3 * PTAB_STRIDE);
+    const int rows[3][3] = {{(int)Hq, (int)Hkv, (int)Hkv}, {(int)H, 0, 0}, {(int)H, 0, 0}};
+    const int nseg[3] = {3, 1, 1}, Ks[3] = {(int)H, (int)Hq, (int)F};
+    for (int i = 0; i < 3; ++i) {
+      GemmLaunch g;
+      memset(&g, 0, sizeof(g));
+      g.p.n_seg = nseg[i];
+      for (int j = 0; j < 3; ++j) g.p.seg_rows[j] = rows[i][j];
+      g.p.T = 1;
+      g.p.K = Ks[i];
+      gemm_plan(g, st->n_sm);
+      st->ptab_ok[i] = gemm_partial_ok(g) && g.p.n_row_tiles <= PTAB_STRIDE;
+      if (st->ptab_ok[i]) gemm_partial_table(g, tab.data() + (size_t)i * PTAB_STRIDE);
+    }
+    e = cudaMemcpyAsync(st->ws + c.ptab, tab.data(), tab.size() * sizeof(PartialTile), cudaMemcpyHostToDevice, st->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st->stream);
+    if (e != cudaSuccess) return fail(cuda_fail(e, "partial tables upload"));
   }
 
   st->pages.init(st->num_pages);
@@ -510,9 +537,11 @@ int ss_kv_import(ss_stage *st, int n, const int32_t *page_ids_dev, const void *b
 namespace ss {
 
 // one projection through the persistent tcgen05 GEMM
+// `piece` (0 QKV, 1 O, 2 down; -1 none): if the planned launch allows it, the projection leaves its tiles in pieces
+// (EPI_PARTIAL) and *gp tells the consumer kernel where; otherwise gp->slots = null and `epi` is used as given.
 static cudaError_t run_gemm(const ss_stage *st, const CUtensorMap *const a[3], int n_seg, const int rows[3],
                             bool dual, const CUtensorMap bmaps[5], int T, int K, int epi, float *out_f32,
-                            void *out_bf16, int ld_out) {
+                            void *out_bf16, int ld_out, int piece = -1, GemmPartials *gp = nullptr) {
   GemmLaunch g;
   memset(&g, 0, sizeof(g));
   GemmParams &p = g.p;
@@ -533,6 +562,15 @@ static cudaError_t run_gemm(const ss_stage *st, const CUtensorMap *const a[3], i
   g.stream = st->stream;
   gemm_plan(g, st->n_sm);
   g.b = &bmaps[p.bn / 32];
+  if (gp) {
+    gp->slots = nullptr;
+    if (piece >= 0 && st->ptab_ok[piece] && gemm_partial_ok(g)) {
+      p.epi = EPI_PARTIAL;
+      gp->slots = p.fix_slots;
+      gp->tiles = st->at<PartialTile>(st->c.ptab) + (size_t)piece * PTAB_STRIDE;
+      gp->slot_floats = p.bn * GEMM_BM;
+    }
+  }
   return gemm_launch(g);
 }
 
@@ -572,13 +610,18 @@ static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T,
   for (int l = 0; l < st->L; ++l) {
     const ss_layer_weights &w = st->lw[l];
     const LayerMaps &m = st->maps[l];
-    {  // S2: QKV projection -> fp32 [T][Hq+2Hkv]
+    GemmPartials gp_qkv, gp_o, gp_d;
+    const GemmPartials gp_none{nullptr, nullptr, 0};
+    {  // S2: QKV projection -> fp32 [T][Hq+2Hkv] (or pieces, added by qkv_post)
       const CUtensorMap *a[3] = {&m.wq, &m.wk, &m.wv};
       const int rows[3] = {Hq, Hkv, Hkv};
-      CKE(run_gemm(st, a, 3, rows, false, st->b_h, T, H, EPI_F32, qkv_part, nullptr, Nqkv));
+      CKE(run_gemm(st, a, 3, rows, false, st->b_h, T, H, EPI_F32, qkv_part, nullptr, Nqkv, 0, &gp_qkv));
     }
     QkvPostParams qp;
     memset(&qp, 0, sizeof(qp));
+    qp.gp = gp_qkv;
+    qp.tile0_k = (Hq + GEMM_BM - 1) / GEMM_BM;
+    qp.tile0_v = qp.tile0_k + (Hkv + GEMM_BM - 1) / GEMM_BM;
     qp.qkv_part = qkv_part;
     qp.splits = 1;
     qp.split_stride = 0;
@@ -619,25 +662,26 @@ static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T,
     if (!decode && n_dec < n_seqs) {  // S6b
       PrefillAttnParams ap;
       memset(&ap, 0, sizeof(ap));
-      ap.q = st->at<void>(c.q);
-      ap.kpool = st->kpool(l); ap.vpool = st->vpool(l);
+      ap.q_map = &st->q_map;
+      ap.kv_map = &st->maps[l].kv;
+      ap.n_pages = st->num_pages;
       ap.n_seqs = n_seqs; ap.T = T; ap.n_q = d.n_q_heads; ap.n_kv = d.n_kv_heads; ap.d = dh;
       ap.plan = pplan;
       ap.out = st->at<void>(c.attn_out);
       ap.args = args;
-      ap.max_tiles = (T - n_dec + 63) / 64 + (n_seqs - n_dec);
+      ap.max_tiles = (T - n_dec + prefill_attn_tile_rows() - 1) / prefill_attn_tile_rows() + (n_seqs - n_dec);
       CKE(launch_prefill_attn(ap, s));
     }
     {  // S7: output projection, then S8: x1 = x + o Wo^T ; h2 = rmsnorm(x1; ln2)
       const CUtensorMap *a[3] = {&m.wo, nullptr, nullptr};
       const int rows[3] = {H, 0, 0};
       if (!tp) {
-        CKE(run_gemm(st, a, 1, rows, false, st->b_attn, T, Hq, EPI_RESID_F32, x, nullptr, H));
-        CKE(launch_residual_rmsnorm(x, nullptr, 0, 0, w.ln2, d.rms_eps, H, T, h, args, false, s));
+        CKE(run_gemm(st, a, 1, rows, false, st->b_attn, T, Hq, EPI_RESID_F32, x, nullptr, H, 1, &gp_o));
+        CKE(launch_residual_rmsnorm(x, nullptr, 0, 0, gp_o, w.ln2, d.rms_eps, H, T, h, args, false, s));
       } else {  // this rank's partial over its heads -> all-reduce -> x += sum (two per layer)
         CKE(run_gemm(st, a, 1, rows, false, st->b_attn, T, Hq, EPI_F32, tp_part, nullptr, H));
         if (st->allreduce(tp_part, (size_t)T * H, st->allreduce_user, (void *)s) != 0) return cudaErrorLaunchFailure;
-        CKE(launch_residual_rmsnorm(x, tp_part, 1, 0, w.ln2, d.rms_eps, H, T, h, args, false, s));
+        CKE(launch_residual_rmsnorm(x, tp_part, 1, 0, gp_none, w.ln2, d.rms_eps, H, T, h, args, false, s));
       }
     }
     {  // S9: gate/up + SwiGLU fused -> a bf16 [T,F]
@@ -651,12 +695,12 @@ static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T,
       const bool last = (l == st->L - 1);
       const void *next_ln = last ? nullptr : st->lw[l + 1].ln1;
       if (!tp) {
-        CKE(run_gemm(st, a, 1, rows, false, st->b_a, T, F, EPI_RESID_F32, x, nullptr, H));
-        CKE(launch_residual_rmsnorm(x, nullptr, 0, 0, next_ln, d.rms_eps, H, T, h, args, last, s));
+        CKE(run_gemm(st, a, 1, rows, false, st->b_a, T, F, EPI_RESID_F32, x, nullptr, H, 2, &gp_d));
+        CKE(launch_residual_rmsnorm(x, nullptr, 0, 0, gp_d, next_ln, d.rms_eps, H, T, h, args, last, s));
       } else {
         CKE(run_gemm(st, a, 1, rows, false, st->b_a, T, F, EPI_F32, tp_part, nullptr, H));
         if (st->allreduce(tp_part, (size_t)T * H, st->allreduce_user, (void *)s) != 0) return cudaErrorLaunchFailure;
-        CKE(launch_residual_rmsnorm(x, tp_part, 1, 0, next_ln, d.rms_eps, H, T, h, args, last, s));
+        CKE(launch_residual_rmsnorm(x, tp_part, 1, 0, gp_none, next_ln, d.rms_eps, H, T, h, args, last, s));
       }
     }
   }
