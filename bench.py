@@ -37,6 +37,8 @@ def parse():
     ap.add_argument("--layers", type=int, default=0, help="override the stage depth (debug only; marks the line)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--batch-invariant", action="store_true",
+                    help="run the stage in ss_stage_set_batch_invariant mode (measures what exact migration costs)")
     ap.add_argument("--no-sub", action="store_true",
                     help="default workload only: skip the cfg-4 prefill and cfg-3 decode sub-records")
     return ap.parse_args()
@@ -239,6 +241,7 @@ def run_decode(args, shape, ctx_fn, rank, world, layers=None, K=None, W=None, do
     dims = binding.make_dims(shape, max_tokens=B, max_seqs=B, max_blocks=pb.max_blocks,
                              max_pos=int(ctx0.max()) + total_steps + 64)
     st = binding.Stage(dims, 0, shape.n_layers, layers, None, n_pages=pb.n_pages_pool, device=dev)
+    st.set_batch_invariant(args.batch_invariant)
     g = torch.Generator(device=dev)
     g.manual_seed(args.seed + 99)
     _fill_randn(st.kv_pool.view(-1), g)                  # random KV pre-fill N(0,1) (A21)
@@ -368,6 +371,7 @@ def run_prefill(args, shape, len_fn, rank, world, layers=None, K=None, W=None):
         layers = gpu_weights(shape, dev, args.seed)
     dims = binding.make_dims(shape, max_tokens=T, max_seqs=n, max_blocks=pb.max_blocks, max_pos=int(lens.max()) + 64)
     st = binding.Stage(dims, 0, shape.n_layers, layers, None, n_pages=pb.n_pages_pool, device=dev)
+    st.set_batch_invariant(args.batch_invariant)
     g = torch.Generator(device=dev)
     g.manual_seed(args.seed + 99)
     x = torch.randn((T, shape.hidden), generator=g, device=dev, dtype=torch.float32).to(torch.bfloat16)
@@ -733,6 +737,8 @@ def main():
            "l2_policy": "inputs larger than L2 (weights 34 GB / KV streamed once per step)"}
     if args.layers:
         cfg["debug_layers_override"] = args.layers
+    if args.batch_invariant:
+        cfg["mode"] = "batch-invariant (ss_stage_set_batch_invariant: bit-exact migration; not the headline mode)"
 
     # ---------------- reference arm: the CPU oracle, rank 0 only ----------------
     if args.impl == "reference":

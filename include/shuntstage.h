@@ -192,6 +192,19 @@ int ss_stage_decode(ss_stage *st, int batch,
 /* Number of kernels the stage launched (directly or inside replayed graphs) since creation. */
 int64_t ss_stage_launch_count(const ss_stage *st);
 
+/* Batch-invariant mode (the paper's migration is OUTPUT-PRESERVING: recomputing prompt + generated
+ * tokens must reconstruct the KV cache the incremental decode built).  In the default mode the GPU reproduces that only
+ * up to the summation order of its kernels (a stream-K cut, an attention split and a reduction tree that depend on how
+ * many rows a call has: KV equal or within 2 bf16 ulp).  With on != 0 every reduction of a token row is done in an order
+ * that depends on that row alone — projections: every output tile's whole K by one CTA, k-blocks in order, one
+ * accumulator; RMSNorm: one reduction tree; attention: each (row, kv head) walked from page 0 to its last page by one
+ * warp of the decode kernel, prefill tokens included, no split and no merge — so ss_stage_prefill over prompt + generated
+ * tokens leaves KV pages and next-token hidden states BIT-IDENTICAL to prefill of the prompt followed by ss_stage_decode
+ * steps, whatever the batch composition or chunking (tests/test_gpu_parity.py).  It is an opt-in exactness mode: the
+ * projections lose stream-K's load balance and prefill attention re-reads the keys per token (cost in DESIGN.md).
+ * Switching synchronises the stream and drops the captured decode graphs. */
+int ss_stage_set_batch_invariant(ss_stage *st, int on);
+
 /* Tensor parallelism inside a stage.  A rank of a D_TP-way stage is an
  * ordinary ss_stage created with that rank's SHARD: dims.n_q_heads, n_kv_heads and ffn divided by D_TP (hidden
  * unchanged), wq/wk/wv and w_gate/w_up = the rank's rows, wo = the rank's columns [H, Hq/D_TP] and w_down = [H, F/D_TP]

@@ -24,7 +24,7 @@ EXPORTS = ["ss_stage_workspace_bytes", "ss_kv_page_bytes", "ss_stage_create", "s
            "ss_stage_decode",
            "ss_stage_launch_count", "ss_op_gemm_scratch_bytes", "ss_op_gemm_bf16", "ss_op_gemm_swiglu_bf16", "ss_strerror",
            "ss_last_cuda_error", "ss_version", "ss_debug_buffer", "ss_pool_create", "ss_pool_destroy",
-           "ss_pool_num_pages", "ss_pool_num_free", "ss_pool_alloc", "ss_pool_free", "ss_kv_export", "ss_kv_import", "ss_stage_set_allreduce",
+           "ss_pool_num_pages", "ss_pool_num_free", "ss_pool_alloc", "ss_pool_free", "ss_kv_export", "ss_kv_import", "ss_stage_set_allreduce", "ss_stage_set_batch_invariant",
            "ss_stage_debug_tap", "ss_stage_debug_info", "ss_store_alloc", "ss_store_free", "ss_store_upload", "ss_store_export", "ss_store_attach", "ss_store_detach"]
 
 
@@ -97,6 +97,7 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     lib.ss_stage_debug_info.argtypes = [C.c_void_p, C.POINTER(C.c_int32)]
     lib.ss_stage_debug_tap.argtypes = [C.c_void_p, C.c_char_p, C.POINTER(C.c_void_p), C.POINTER(C.c_size_t)]
     lib.ss_stage_set_allreduce.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.ss_stage_set_batch_invariant.argtypes = [C.c_void_p, C.c_int]
     lib.ss_kv_export.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_size_t]
     lib.ss_kv_import.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_size_t]
     lib.ss_pool_create.argtypes = [C.POINTER(C.c_void_p), C.c_int]
@@ -240,6 +241,11 @@ class Stage:
         if check and rc != SS_OK:
             raise ShuntStageError(rc, "ss_stage_decode")
         return rc
+
+    def set_batch_invariant(self, on: bool = True):
+        rc = self.lib.ss_stage_set_batch_invariant(self.h, 1 if on else 0)
+        if rc != SS_OK:
+            raise ShuntStageError(rc, "ss_stage_set_batch_invariant")
 
     def set_allreduce(self, fn):
         """fn(partial: float32 torch view of the workspace, stream_ptr: int) -> None: enqueue an in-place sum across

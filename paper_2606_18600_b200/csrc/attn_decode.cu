@@ -100,21 +100,36 @@ decode_attn_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodeAttnP
   }
   __syncwarp();
 
-  const int total = p.plan.meta[0], quota = p.plan.meta[1];
-  const int g0 = w * quota;
-  const int g1 = min(g0 + quota, total);
-  if (g0 >= g1) return;
   const int n_kv = p.n_kv, G = p.n_q / p.n_kv;
   const int32_t *cum = p.plan.cum_pages;
   const CallArgs *args = p.args;
-  const int32_t *bt = args->block_tables;
   const int max_blocks = args->max_blocks;
-  const __nv_bfloat16 *kpool = (const __nv_bfloat16 *)p.kpool;
-  const __nv_bfloat16 *vpool = (const __nv_bfloat16 *)p.vpool;
+  // batch-invariant mode: this warp owns ONE (row, kv head) pair, all its pages, and writes the row's result itself
+  const bool per_pair = p.per_pair != 0;
+  int g0, g1, pp_ctx = 0;
+  const int32_t *bt = args->block_tables;
+  if (per_pair) {
+    if (w >= p.n_rows * n_kv) return;
+    const int row = w / n_kv;
+    pp_ctx = p.row_pos ? p.row_pos[row] : args->ctx[row];
+    bt += (size_t)(p.row_seq ? p.row_seq[row] : row) * max_blocks;  // the row's block-table row
+    g0 = 0;
+    g1 = (pp_ctx + 16) >> 4;
+  } else {
+    const int total = p.plan.meta[0], quota = p.plan.meta[1];
+    g0 = w * quota;
+    g1 = min(g0 + quota, total);
+    if (g0 >= g1) return;
+  }
 
   // locate g0: largest b with cum[b]*n_kv <= g0
   Cursor lc;
-  {
+  if (per_pair) {
+    lc.b = w / n_kv;
+    lc.h = w - lc.b * n_kv;
+    lc.pg = 0;
+    lc.pages_b = g1;
+  } else {
     int lo = 0, hi = p.batch;  // invariant: cum[lo]*n_kv <= g0 < cum[hi]*n_kv
     while (hi - lo > 1) {
       const int mid = (lo + hi) >> 1;
@@ -144,7 +159,7 @@ decode_attn_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodeAttnP
   const int v_row0 = p.n_pages * n_kv * 16;
   auto issue_load = [&](const Cursor &c, int slot) {
     if (lane == 0) {
-      const int page = bt[(size_t)c.b * max_blocks + c.pg];
+      const int page = bt[(per_pair ? (size_t)0 : (size_t)c.b * max_blocks) + c.pg];
       const int row = (page * n_kv + c.h) * 16;
       uint8_t *kd = ring + (size_t)slot * 2 * PAGE_BYTES;
       fence_proxy_async();  // the slot's previous contents were read through the generic proxy (ldmatrix)
@@ -181,7 +196,7 @@ decode_attn_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodeAttnP
     }
     mbar_wait(&bars[i % DA_STAGES], (uint32_t)(i / DA_STAGES) & 1u);
 
-    const int ctx = args->ctx[cc.b];
+    const int ctx = per_pair ? pp_ctx : args->ctx[cc.b];
     if (!seg_open) {
       // new (b,h) segment: query fragments of the G heads of kv head h (rows >= G are zero)
       const __nv_bfloat16 *qb = (const __nv_bfloat16 *)p.q + (size_t)cc.b * p.n_q * D + (size_t)cc.h * G * D;
@@ -215,7 +230,7 @@ decode_attn_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodeAttnP
       // fused KV append (step S5): slot ctx & 15 of the sequence's last page <- bf16 k', v' of the new token
       n_valid = (ctx & 15) + 1;
       const int r = ctx & 15;
-      const int page = bt[(size_t)cc.b * max_blocks + cc.pg];
+      const int page = bt[(per_pair ? (size_t)0 : (size_t)cc.b * max_blocks) + cc.pg];
       const uint8_t *src = (const uint8_t *)p.kv_new + ((size_t)cc.b * 2 * n_kv * D + (size_t)cc.h * D) * 2;
       const size_t goff = (((size_t)page * n_kv + cc.h) * 16 + r) * ROW_BYTES;
       for (int idx = lane; idx < (p.append ? 2 * CHUNKS : 0); idx += 32) {
@@ -314,7 +329,25 @@ decode_attn_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodeAttnP
 
     // ---- segment end?  (next item belongs to another (b,h), or this was the warp's last item)
     const bool seg_end = (i == n - 1) || (cc.pg + 1 == cc.pages_b);
-    if (seg_end) {
+    if (seg_end && per_pair) {
+      // the pair's only segment: out = O / l, exactly what decode_merge computes for one segment (weight 2^0 = 1)
+      __nv_bfloat16 *ob = (__nv_bfloat16 *)p.out + (size_t)cc.b * p.n_q * D + (size_t)cc.h * G * D;
+      if (qrow < G) {
+        const float inv = 1.0f / l_run[0];
+#pragma unroll
+        for (int t = 0; t < NT; ++t)
+          *reinterpret_cast<uint32_t *>(ob + (size_t)qrow * D + t * 8 + qcol) = pack_bf16x2(o[t][0] * inv, o[t][1] * inv);
+      }
+      if constexpr (HI) {
+        if (qrow + 8 < G) {
+          const float inv = 1.0f / l_run[1];
+#pragma unroll
+          for (int t = 0; t < NT; ++t)
+            *reinterpret_cast<uint32_t *>(ob + (size_t)(qrow + 8) * D + t * 8 + qcol) = pack_bf16x2(o[t][2] * inv, o[t][3] * inv);
+        }
+      }
+      seg_open = false;
+    } else if (seg_end) {
       const int slot = w + cc.b * n_kv + cc.h;
       float *po = p.part_o + (size_t)slot * 16 * D;
       float *pml = p.part_ml + (size_t)slot * 32;
@@ -403,7 +436,7 @@ cudaError_t attn_init() {
 }
 
 cudaError_t launch_decode_attn(const DecodeAttnParams &p, cudaStream_t s) {
-  const int ctas = p.n_workers / DA_WARPS;
+  const int ctas = p.per_pair ? (p.n_rows * p.n_kv + DA_WARPS - 1) / DA_WARPS : p.n_workers / DA_WARPS;
   const bool hi = p.n_q / p.n_kv > 8;
   const dim3 g(ctas), b(DA_WARPS * 32);
   if (p.d == 128)

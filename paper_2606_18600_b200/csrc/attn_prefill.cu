@@ -5,20 +5,22 @@
 // qkv_post before this kernel runs), which is what makes prefill == incremental decode.
 //
 // Both products are dense contractions, so they run on the tcgen05 tensor cores with the accumulators in tensor memory:
-//   S = Q K^T   UMMA M = 128 query rows x N = 128 keys, K = d; Q and K tiles in smem (TMA, SWIZZLE_128B, K-major)
-//   O += P V    UMMA M = 128 x N = d, K = 128 keys; P (bf16) is read from TENSOR MEMORY, where the softmax warps wrote it
+//   S = Q K^T   UMMA M = 128 query rows x N = 64 keys, K = d; Q and K tiles in smem (TMA, SWIZZLE_128B, K-major)
+//   O += P V    UMMA M = 128 x N = d, K = 64 keys; P (bf16) is read from TENSOR MEMORY, where the softmax warps wrote it
 //               over the S tile it came from; V tile in smem as TMA wrote it ([key][d]: the MN-major B operand)
-// CTA = one 128-row query tile of one (sequence, q head); 8 warps, one role each:
-//   warp 0  TMA producer: the Q tile once, then per key tile 8 pages of K and of V (16 tokens x d, one 2-D box per 64
-//           columns; the layer's pool is one 2-D tensor), 3-stage ring
-//   warp 1  issues the S MMAs (one lane) into a DOUBLE-buffered S so that S_{j+1} is computed while tile j is in softmax
-//   warp 2  issues the P.V MMAs (one lane); a separate issuing thread because one tcgen05.mma occupies its issuer
-//           ~128 cycles whatever its shape
-//   warps 4-7  softmax: thread = query row = TMEM lane, so row max / row sum need no shuffle; tcgen05.ld of the S row,
-//           exp2 in fp32, P -> bf16 -> tcgen05.st; the running maximum is only moved when it grows by more than 2^8
-//           (then, rarely, the O accumulator is rescaled in place), else P simply is up to 2^8 larger — the final
-//           O / l is unchanged
-// The 8 q heads of a GQA group are adjacent in blockIdx.x so their K/V re-reads hit L2.
+// CTA = the same 128 query positions of TWO q heads of one GQA group ("tile A", "tile B": they attend the same keys, so
+// one K/V ring serves both and every K/V byte fetched from L2 feeds 256 query rows); 12 warps, one role each:
+//   warp 0      TMA producer: both Q tiles once, then per key tile 4 pages of K and of V (16 tokens x d, one 2-D box per
+//               64 columns; the layer's pool is one 2-D tensor) into a 5-stage ring
+//   warps 1, 2  issue the S MMAs of tile A / tile B (one lane each) into DOUBLE-buffered S tiles, so S_{j+1} is computed
+//               while tile j is in softmax
+//   warp 3      issues the P.V MMAs of both tiles (separate issuing threads because one tcgen05.mma occupies its issuer
+//               ~128 cycles whatever its shape)
+//   warps 4-7 / 8-11  softmax of tile A / B: thread = query row = TMEM lane, so row max / row sum need no shuffle;
+//               tcgen05.ld of the S row, exp2 in fp32, P -> bf16 -> tcgen05.st; the running maximum is only moved when it
+//               grows by more than 2^8 (then, rarely, the O accumulator is rescaled in place), else P simply is up to
+//               2^8 larger — the final O / l is unchanged
+// TMEM (512 columns): S_A0 S_A1 S_B0 S_B1 (64 each), O_A, O_B (d each).
 #include <cuda.h>
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
@@ -28,14 +30,14 @@
 
 namespace ss {
 
-constexpr int TA_BM = 128;      // query rows per CTA = UMMA M = TMEM lanes
-constexpr int TA_BN = 128;      // keys per tile
-constexpr int TA_STAGES = 3;    // K/V ring depth
-constexpr int TA_THREADS = 256;
+constexpr int TA_BM = 128;      // query rows per tile = UMMA M = TMEM lanes
+constexpr int TA_BN = 64;       // keys per ring stage (4 pages)
+constexpr int TA_STAGES = 5;    // K/V ring depth: 320 keys in flight per CTA
+constexpr int TA_THREADS = 384;
 constexpr int TA_PAGES = TA_BN / 16;
 constexpr float TA_LAZY = 8.0f; // the running maximum (log2 units) is moved only when exceeded by more than this
 
-// ---- plan: token -> (sequence, position) and the prefix sum of query tiles --------------------------------------
+// ---- plan: token -> (sequence, position), the prefix sum of query tiles and one descriptor per launch slot ---------
 __global__ void prefill_plan_kernel(const CallArgs *__restrict__ args, int n_seqs, int seq0, PrefillPlan plan) {
   pdl_launch_dependents();
   pdl_wait();
@@ -55,14 +57,18 @@ __global__ void prefill_plan_kernel(const CallArgs *__restrict__ args, int n_seq
     // blockIdx order, and a causal batch in natural order would start its most expensive tiles last
     const int n = min(n_tiles_s, plan.max_tiles);
     int32_t *key = plan.tile_order + plan.max_tiles;
-    for (int i = threadIdx.x; i < n; i += blockDim.x) {
-      int lo = 0, hi = n_seqs;
+    auto seq_of = [&](int i) {
+      int lo = 0, hi = n_seqs;  // tile_cum[lo] <= i < tile_cum[hi]
       while (hi - lo > 1) {
         const int mid = (lo + hi) >> 1;
         if (plan.tile_cum[mid] <= i) lo = mid; else hi = mid;
       }
-      const int q_len = args->cu_q[lo + 1] - args->cu_q[lo];
-      key[i] = args->ctx[lo] + min(q_len, (i - plan.tile_cum[lo] + 1) * TA_BM);
+      return lo;
+    };
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+      const int s = seq_of(i);
+      const int q_len = args->cu_q[s + 1] - args->cu_q[s];
+      key[i] = args->ctx[s] + min(q_len, (i - plan.tile_cum[s] + 1) * TA_BM);
     }
     __syncthreads();
     for (int i = threadIdx.x; i < n; i += blockDim.x) {  // rank sort (stable): n is a few hundred, once per call
@@ -72,7 +78,19 @@ __global__ void prefill_plan_kernel(const CallArgs *__restrict__ args, int n_seq
         const int kj = key[j];
         rank += (kj > k || (kj == k && j < i)) ? 1 : 0;
       }
-      plan.tile_order[rank] = i;
+      plan.tile_order[i] = rank;   // launch slot of tile i
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+      const int s = seq_of(i);
+      const int q_begin = args->cu_q[s], q_len = args->cu_q[s + 1] - q_begin;
+      const int i0 = (i - plan.tile_cum[s]) * TA_BM;
+      int4 d;
+      d.x = q_begin + i0;              // first packed row of the tile
+      d.y = min(TA_BM, q_len - i0);    // its rows
+      d.z = args->ctx[s] + i0;         // global position of its first query
+      d.w = s;
+      reinterpret_cast<int4 *>(plan.tile_desc)[plan.tile_order[i]] = d;
     }
   }
   for (int s = blockIdx.x; s < n_seqs; s += gridDim.x) {
@@ -86,7 +104,7 @@ __global__ void prefill_plan_kernel(const CallArgs *__restrict__ args, int n_seq
 
 cudaError_t launch_prefill_plan(const CallArgs *args, int n_seqs, int seq0, PrefillPlan plan, cudaStream_t s) {
   int blocks = n_seqs < 1 ? 1 : (n_seqs > 1024 ? 1024 : n_seqs);
-  return launch_pdl(prefill_plan_kernel, dim3(blocks), dim3(256), 0, s, args, n_seqs, seq0, plan);
+  return launch_pdl(prefill_plan_kernel, dim3(blocks), dim3(1024), 0, s, args, n_seqs, seq0, plan);
 }
 int prefill_attn_tile_rows() { return TA_BM; }
 
@@ -95,21 +113,25 @@ __global__ void __launch_bounds__(TA_THREADS, 1)
 prefill_attn_kernel(const __grid_constant__ CUtensorMap q_map, const __grid_constant__ CUtensorMap kv_map,
                     const PrefillAttnParams p) {
   constexpr int NH = D / 64;                     // 64-column halves of a row (one 128-byte swizzle row each)
-  constexpr uint32_t HALF_BYTES = TA_BM * 128;   // [128 rows][64 bf16]
+  constexpr uint32_t QHALF_BYTES = TA_BM * 128;  // Q: [128 rows][64 bf16] per half
+  constexpr uint32_t QTILE_BYTES = NH * QHALF_BYTES;
+  constexpr uint32_t HALF_BYTES = TA_BN * 128;   // K, V: [TA_BN keys][64 bf16] per half
   constexpr uint32_t TILE_BYTES = NH * HALF_BYTES;
-  constexpr uint32_t S_COLS = TA_BN;             // fp32 S tile; P (bf16) lives in its first 64 columns
-  constexpr uint32_t O_COL = 2 * S_COLS;
+  constexpr uint32_t S_COLS = TA_BN;             // fp32 S tile; P (bf16) lives in its first TA_BN / 2 columns
+  constexpr uint32_t O_COL = 4 * S_COLS;         // S_A0 S_A1 S_B0 S_B1 | O_A O_B
   constexpr uint32_t TMEM_COLS = 512;
+  static_assert(O_COL + 2 * D <= TMEM_COLS, "TMEM budget");
   extern __shared__ uint8_t smem_raw[];
   uint8_t *base = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-  uint8_t *q_s = base;
-  uint8_t *k_s = q_s + TILE_BYTES;                       // [TA_STAGES][TILE_BYTES]
+  uint8_t *q_s = base;                                   // [2 tiles][QTILE_BYTES]
+  uint8_t *k_s = q_s + 2 * QTILE_BYTES;                  // [TA_STAGES][TILE_BYTES]
   uint8_t *v_s = k_s + (size_t)TA_STAGES * TILE_BYTES;   // [TA_STAGES][TILE_BYTES]
   uint64_t *bars = (uint64_t *)(v_s + (size_t)TA_STAGES * TILE_BYTES);
   uint64_t *q_full = bars;
   uint64_t *k_full = bars + 1, *v_full = k_full + TA_STAGES, *kv_empty = v_full + TA_STAGES;
-  uint64_t *s_full = kv_empty + TA_STAGES, *p_full = s_full + 2, *pv_done = p_full + 2;
-  uint32_t *tmem_slot = (uint32_t *)(pv_done + 2);
+  uint64_t *s_full = kv_empty + TA_STAGES;  // [tile][buffer]
+  uint64_t *p_full = s_full + 4, *pv_done = p_full + 4;
+  uint32_t *tmem_slot = (uint32_t *)(pv_done + 4);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   pdl_launch_dependents();
@@ -120,11 +142,11 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap q_map, const __grid_cons
     for (int i = 0; i < TA_STAGES; ++i) {
       mbar_init(&k_full[i], 1);
       mbar_init(&v_full[i], 1);
-      mbar_init(&kv_empty[i], 2);  // the S issuer's and the P.V issuer's commits
+      mbar_init(&kv_empty[i], 3);  // the two S issuers' and the P.V issuer's commits
     }
-    for (int i = 0; i < 2; ++i) {
+    for (int i = 0; i < 4; ++i) {
       mbar_init(&s_full[i], 1);
-      mbar_init(&p_full[i], 128);  // every softmax thread
+      mbar_init(&p_full[i], 128);  // every softmax thread of the tile
       mbar_init(&pv_done[i], 1);
     }
     mbar_fence_init();
@@ -136,38 +158,31 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap q_map, const __grid_cons
   const uint32_t tmem_base = *tmem_slot;
   pdl_wait();  // q, the pools and the plan are written by earlier kernels of this call
 
-  // ---- which tile
-  const int head = blockIdx.x;
-  const int32_t *tile_cum = p.plan.tile_cum;
-  const bool live = (int)blockIdx.y < tile_cum[p.n_seqs];
-  int n_kt = 0, s = 0, q_begin = 0, i0 = 0, rows = 0, p0 = 0, kv_len = 0, hk = 0;
-  const CallArgs *args = p.args;
+  // ---- which tile pair: blockIdx.x = (kv head, pair of its q heads), blockIdx.y = launch slot of the query tile
+  const int G = p.n_q / p.n_kv, pairs = (G + 1) >> 1;
+  const int hk = blockIdx.x / pairs, pi = blockIdx.x - hk * pairs;
+  const int head_a = hk * G + 2 * pi;
+  const bool has_b = 2 * pi + 1 < G;   // an odd group leaves its last head alone
+  const bool live = (int)blockIdx.y < p.plan.tile_cum[p.n_seqs];
+  int row0 = 0, rows = 0, p0 = 0, s = 0;
   if (live) {
-    const int slot = p.plan.tile_order[blockIdx.y];
-    int lo = 0, hi = p.n_seqs;  // tile_cum[lo] <= slot < tile_cum[hi]
-    while (hi - lo > 1) {
-      const int mid = (lo + hi) >> 1;
-      if (tile_cum[mid] <= slot) lo = mid; else hi = mid;
-    }
-    s = lo;
-    q_begin = args->cu_q[s];
-    const int q_len = args->cu_q[s + 1] - q_begin;
-    i0 = (slot - tile_cum[s]) * TA_BM;
-    rows = min(TA_BM, q_len - i0);
-    p0 = args->ctx[s] + i0;      // global position of the tile's first query
-    kv_len = p0 + rows;          // keys 0..kv_len-1 are needed by this tile
-    n_kt = (kv_len + TA_BN - 1) / TA_BN;
-    hk = head / (p.n_q / p.n_kv);
+    const int4 d = reinterpret_cast<const int4 *>(p.plan.tile_desc)[blockIdx.y];
+    row0 = d.x; rows = d.y; p0 = d.z; s = d.w;
   }
+  const int kv_len = p0 + rows;                       // keys 0..kv_len-1 are needed by this tile
+  const int n_kt = (kv_len + TA_BN - 1) / TA_BN;
   const int n_pages_seq = (kv_len + 15) >> 4;
+  const CallArgs *args = p.args;
 
   if (warp == 0) {
     if (lane == 0 && live) {
       // ---------------- TMA producer ----------------
-      const uint64_t pol_q = l2_policy_evict_first(), pol_kv = l2_policy_evict_last();  // K/V: re-read by the group's heads
-      mbar_expect_tx(q_full, TILE_BYTES);
+      const uint64_t pol_q = l2_policy_evict_first(), pol_kv = l2_policy_evict_last();  // K/V: re-read by other tiles
+      mbar_expect_tx(q_full, (has_b ? 2u : 1u) * QTILE_BYTES);
+      for (int t = 0; t < (has_b ? 2 : 1); ++t)
 #pragma unroll
-      for (int h = 0; h < NH; ++h) tma_load_2d(q_s + h * HALF_BYTES, &q_map, q_full, head * D + h * 64, q_begin + i0, pol_q);
+        for (int h = 0; h < NH; ++h)
+          tma_load_2d(q_s + t * QTILE_BYTES + h * QHALF_BYTES, &q_map, q_full, (head_a + t) * D + h * 64, row0, pol_q);
       const int32_t *bt = args->block_tables + (size_t)s * args->max_blocks;
       const int v_row0 = p.n_pages * p.n_kv * 16;
       for (int j = 0; j < n_kt; ++j) {
@@ -197,61 +212,70 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap q_map, const __grid_cons
           }
       }
     }
-  } else if (warp == 1) {
+  } else if (warp == 1 || warp == 2) {
     if (lane == 0 && live) {
-      // ---------------- S = Q K^T issuer ----------------
+      // ---------------- S = Q K^T issuer of tile t ----------------
+      const int t = warp - 1;
+      const bool on = t == 0 || has_b;
       const uint32_t idesc = umma_idesc_bf16(TA_BM, TA_BN);
-      mbar_wait(q_full, 0);
+      if (on) mbar_wait(q_full, 0);
       for (int j = 0; j < n_kt; ++j) {
         const int st = j % TA_STAGES, b = j & 1;
-        if (j >= 2) mbar_wait(&pv_done[b], ((uint32_t)((j - 2) >> 1)) & 1u);  // P_{j-2} (in this S buffer) was consumed
+        if (on && j >= 2) mbar_wait(&pv_done[t * 2 + b], ((uint32_t)((j - 2) >> 1)) & 1u);  // P_{j-2} (in this S buffer) consumed
         mbar_wait(&k_full[st], ((uint32_t)(j / TA_STAGES)) & 1u);
-        tc_fence_after();
-        const uint32_t qa = smem_u32(q_s), ka = smem_u32(k_s + (size_t)st * TILE_BYTES);
+        if (on) {
+          tc_fence_after();
+          const uint32_t qa = smem_u32(q_s + t * QTILE_BYTES), ka = smem_u32(k_s + (size_t)st * TILE_BYTES);
+          const uint32_t acc = tmem_base + (uint32_t)(t * 2 + b) * S_COLS;
 #pragma unroll
-        for (int ks = 0; ks < D / 16; ++ks) {
-          const uint32_t off = (uint32_t)(ks >> 2) * HALF_BYTES + (uint32_t)(ks & 3) * 32u;
-          umma_bf16(tmem_base + (uint32_t)b * S_COLS, umma_desc_k_sw128(qa + off), umma_desc_k_sw128(ka + off), idesc,
-                    ks > 0 ? 1u : 0u);
+          for (int ks = 0; ks < D / 16; ++ks) {
+            const uint32_t in_row = (uint32_t)(ks & 3) * 32u;
+            umma_bf16(acc, umma_desc_k_sw128(qa + (uint32_t)(ks >> 2) * QHALF_BYTES + in_row),
+                      umma_desc_k_sw128(ka + (uint32_t)(ks >> 2) * HALF_BYTES + in_row), idesc, ks > 0 ? 1u : 0u);
+          }
+          umma_commit(&s_full[t * 2 + b]);
         }
-        umma_commit(&s_full[b]);
-        umma_commit(&kv_empty[st]);
+        umma_commit(&kv_empty[st]);  // (an absent tile B releases the stage as soon as it has landed)
       }
     }
-  } else if (warp == 2) {
+  } else if (warp == 3) {
     if (lane == 0 && live) {
-      // ---------------- O += P V issuer ----------------
+      // ---------------- O += P V issuer (both tiles) ----------------
       const uint32_t idesc = umma_idesc_bf16_b_mn(TA_BM, D);
       for (int j = 0; j < n_kt; ++j) {
         const int st = j % TA_STAGES, b = j & 1;
-        mbar_wait(&p_full[b], ((uint32_t)(j >> 1)) & 1u);
-        mbar_wait(&v_full[st], ((uint32_t)(j / TA_STAGES)) & 1u);
-        tc_fence_after();
         const uint32_t va = smem_u32(v_s + (size_t)st * TILE_BYTES);
         const int n_pg = min(TA_PAGES, n_pages_seq - j * TA_PAGES);  // one k-step = one page of 16 keys
-        for (int ks = 0; ks < n_pg; ++ks)
-          umma_bf16_ts(tmem_base + O_COL, tmem_base + (uint32_t)b * S_COLS + (uint32_t)ks * 8u,
-                       umma_desc_mn_sw128(va + (uint32_t)ks * 2048u, HALF_BYTES, 1024u), idesc, (j > 0 || ks > 0) ? 1u : 0u);
+        for (int t = 0; t < (has_b ? 2 : 1); ++t) {
+          mbar_wait(&p_full[t * 2 + b], ((uint32_t)(j >> 1)) & 1u);
+          if (t == 0) mbar_wait(&v_full[st], ((uint32_t)(j / TA_STAGES)) & 1u);
+          tc_fence_after();
+          for (int ks = 0; ks < n_pg; ++ks)
+            umma_bf16_ts(tmem_base + O_COL + (uint32_t)t * D, tmem_base + (uint32_t)(t * 2 + b) * S_COLS + (uint32_t)ks * 8u,
+                         umma_desc_mn_sw128(va + (uint32_t)ks * 2048u, HALF_BYTES, 1024u), idesc, (j > 0 || ks > 0) ? 1u : 0u);
+          umma_commit(&pv_done[t * 2 + b]);
+        }
         umma_commit(&kv_empty[st]);
-        umma_commit(&pv_done[b]);
       }
     }
-  } else if (warp >= 4 && live) {
-    // ---------------- softmax: thread = query row ----------------
+  } else if (live && (warp < 8 || has_b)) {
+    // ---------------- softmax of tile t: thread = query row ----------------
+    const int t = warp >= 8 ? 1 : 0;
     const int quad = warp & 3;
     const int r = quad * 32 + lane;
     const uint32_t lane_base = tmem_base + ((uint32_t)(quad * 32) << 16);
+    const uint32_t o_addr = lane_base + O_COL + (uint32_t)t * D;
     const float sl2 = 1.4426950408889634f / sqrtf((float)D);  // log2(e) / sqrt(d)
     const int qpos = p0 + r;
     float m_used = -INFINITY, l_run = 0.f;  // m_used in log2 units (score * sl2)
     for (int j = 0; j < n_kt; ++j) {
       const int b = j & 1, st = j % TA_STAGES;
-      mbar_wait(&s_full[b], ((uint32_t)(j >> 1)) & 1u);
+      const uint32_t s_addr = lane_base + (uint32_t)(t * 2 + b) * S_COLS;
+      mbar_wait(&s_full[t * 2 + b], ((uint32_t)(j >> 1)) & 1u);
       tc_fence_after();
       uint32_t v[TA_BN];
 #pragma unroll
-      for (int c = 0; c < TA_BN / 32; ++c)
-        tmem_ld_32x32(lane_base + (uint32_t)b * S_COLS + (uint32_t)c * 32u, *reinterpret_cast<uint32_t(*)[32]>(&v[c * 32]));
+      for (int c = 0; c < TA_BN / 32; ++c) tmem_ld_32x32(s_addr + (uint32_t)c * 32u, *reinterpret_cast<uint32_t(*)[32]>(&v[c * 32]));
       tmem_ld_wait();
       const int jbase = j * TA_BN;
       if (jbase + TA_BN - 1 > p0) {  // the tile reaches past the first query's position: causal mask
@@ -259,10 +283,10 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap q_map, const __grid_cons
         for (int c = 0; c < TA_BN; ++c)
           if (jbase + c > qpos) v[c] = 0xff800000u;  // -inf
       }
-      float mx = -INFINITY;
+      float mx4[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};  // four independent chains
 #pragma unroll
-      for (int c = 0; c < TA_BN; ++c) mx = fmaxf(mx, __uint_as_float(v[c]));
-      mx *= sl2;
+      for (int c = 0; c < TA_BN; ++c) mx4[c & 3] = fmaxf(mx4[c & 3], __uint_as_float(v[c]));
+      const float mx = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3])) * sl2;
       // lazy maximum: move it only when the tile's maximum exceeds it by more than TA_LAZY (P then stays <= 2^TA_LAZY)
       const bool move = mx > m_used + TA_LAZY;   // also true on the first tile (m_used = -inf; key 0 is visible to all)
       float alpha = 1.0f;
@@ -273,35 +297,34 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap q_map, const __grid_cons
       }
       if (j > 0 && __any_sync(0xffffffffu, move)) {
         // rescale the O accumulator in place (rare): P.V of tile j-1 must have completed first
-        mbar_wait(&pv_done[(j - 1) & 1], ((uint32_t)((j - 1) >> 1)) & 1u);
+        mbar_wait(&pv_done[t * 2 + ((j - 1) & 1)], ((uint32_t)((j - 1) >> 1)) & 1u);
         tc_fence_after();
 #pragma unroll
         for (int c = 0; c < D / 32; ++c) {
           uint32_t o[32];
-          tmem_ld_32x32(lane_base + O_COL + (uint32_t)c * 32u, o);
+          tmem_ld_32x32(o_addr + (uint32_t)c * 32u, o);
           tmem_ld_wait();
 #pragma unroll
           for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
-          tmem_st_32x32(lane_base + O_COL + (uint32_t)c * 32u, o);
+          tmem_st_32x32(o_addr + (uint32_t)c * 32u, o);
         }
       }
-      float rs = 0.f;
+      float rs4[4] = {0.f, 0.f, 0.f, 0.f};
       uint32_t pk[TA_BN / 2];
       const float neg_m = -m_used;
 #pragma unroll
       for (int c = 0; c < TA_BN; c += 2) {
         const float e0 = fast_exp2(fmaf(__uint_as_float(v[c]), sl2, neg_m));
         const float e1 = fast_exp2(fmaf(__uint_as_float(v[c + 1]), sl2, neg_m));
-        rs += e0 + e1;
+        rs4[(c >> 1) & 3] += e0 + e1;
         pk[c >> 1] = pack_bf16x2(e0, e1);
       }
-      l_run += rs;
-#pragma unroll
-      for (int c = 0; c < TA_BN / 64; ++c)
-        tmem_st_32x32(lane_base + (uint32_t)b * S_COLS + (uint32_t)c * 32u, *reinterpret_cast<uint32_t(*)[32]>(&pk[c * 32]));
-      if (j == n_kt - 1 && (kv_len & 15) != 0) {
+      l_run += (rs4[0] + rs4[1]) + (rs4[2] + rs4[3]);
+      tmem_st_32x32(s_addr, pk);
+      if (t == 0 && j == n_kt - 1 && (kv_len & 15) != 0) {
         // the sequence's last page holds slots past its end with whatever the pool held: zero those V rows so that
-        // 0 * garbage (possibly NaN) cannot reach the output (their P is exactly 0: the causal mask covers them)
+        // 0 * garbage (possibly NaN) cannot reach the output (their P is exactly 0: the causal mask covers them).
+        // Done by tile A's warps before they publish P_A; the P.V issuer takes tile A first.
         mbar_wait(&v_full[st], ((uint32_t)(j / TA_STAGES)) & 1u);
         const int k0 = kv_len - jbase, k1 = (n_pages_seq - j * TA_PAGES) * 16;  // rows [k0, k1) of the tile
         uint8_t *vd = v_s + (size_t)st * TILE_BYTES;
@@ -313,17 +336,17 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap q_map, const __grid_cons
       }
       tmem_st_wait();
       tc_fence_before();
-      mbar_arrive(&p_full[b]);
+      mbar_arrive(&p_full[t * 2 + b]);
     }
     // ---- normalise and store
-    mbar_wait(&pv_done[(n_kt - 1) & 1], ((uint32_t)((n_kt - 1) >> 1)) & 1u);
+    mbar_wait(&pv_done[t * 2 + ((n_kt - 1) & 1)], ((uint32_t)((n_kt - 1) >> 1)) & 1u);
     tc_fence_after();
     const float inv = 1.0f / l_run;
-    __nv_bfloat16 *og = (__nv_bfloat16 *)p.out + ((size_t)(q_begin + i0 + r) * p.n_q + head) * D;
+    __nv_bfloat16 *og = (__nv_bfloat16 *)p.out + ((size_t)(row0 + r) * p.n_q + head_a + t) * D;
 #pragma unroll
     for (int c = 0; c < D / 32; ++c) {
       uint32_t o[32];
-      tmem_ld_32x32(lane_base + O_COL + (uint32_t)c * 32u, o);
+      tmem_ld_32x32(o_addr + (uint32_t)c * 32u, o);
       tmem_ld_wait();
       if (r < rows) {
 #pragma unroll
@@ -347,7 +370,7 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap q_map, const __grid_cons
 }
 
 static size_t prefill_smem(int d) {
-  return 1024 + (size_t)(1 + 2 * TA_STAGES) * (d / 64) * TA_BM * 128 + 8 * (1 + 3 * TA_STAGES + 6) + 16;
+  return 1024 + (size_t)(d / 64) * (2 * TA_BM + 2 * TA_STAGES * TA_BN) * 128 + 8 * (1 + 3 * TA_STAGES + 12) + 16;
 }
 
 cudaError_t prefill_attn_init() {  // per device: called from ss_stage_create
@@ -359,7 +382,8 @@ cudaError_t prefill_attn_init() {  // per device: called from ss_stage_create
 }
 
 cudaError_t launch_prefill_attn(const PrefillAttnParams &p, cudaStream_t s) {
-  dim3 grid(p.n_q, p.max_tiles);
+  const int G = p.n_q / p.n_kv;
+  dim3 grid(p.n_kv * ((G + 1) / 2), p.max_tiles);
   if (p.d == 128)
     return launch_pdl(prefill_attn_kernel<128>, dim3(grid), dim3(TA_THREADS), prefill_smem(128), s, *p.q_map, *p.kv_map, p);
   return launch_pdl(prefill_attn_kernel<64>, dim3(grid), dim3(TA_THREADS), prefill_smem(64), s, *p.q_map, *p.kv_map, p);

@@ -189,14 +189,14 @@ residual_rmsnorm_kernel(float *__restrict__ x, const float *__restrict__ part, i
 
 cudaError_t launch_residual_rmsnorm(float *x, const float *part, int splits, long long split_stride,
                                     const GemmPartials &gp, const void *ln_w, float eps, int H, int T, void *h,
-                                    const CallArgs *args, bool write_out_hidden, cudaStream_t s) {
+                                    const CallArgs *args, bool write_out_hidden, cudaStream_t s, bool fixed_shape) {
   const __nv_bfloat16 *w = (const __nv_bfloat16 *)ln_w;
   __nv_bfloat16 *hh = (__nv_bfloat16 *)h;
   const int wo = write_out_hidden ? 1 : 0;
   auto go = [&](auto kernel, int threads) {
     return launch_pdl(kernel, dim3(T), dim3(threads), 0, s, x, part, splits, split_stride, gp, w, eps, H, hh, args, wo);
   };
-  if (T >= 512 && H <= 16 * 256 * 4) {  // many rows: 256 threads each
+  if (!fixed_shape && T >= 512 && H <= 16 * 256 * 4) {  // many rows: 256 threads each
     const int it = (H + 1023) / 1024;
     if (it <= 2) return go(residual_rmsnorm_kernel<2, 256>, 256);
     if (it <= 4) return go(residual_rmsnorm_kernel<4, 256>, 256);

@@ -589,6 +589,7 @@ void gemm_plan(GemmLaunch &g, int n_sm) {
   p.sched = (n_tiles >= 4LL * max_grid || full_waves) ? SCHED_TILES : SCHED_STREAMK;
   if (p.n_t_tiles == 1) p.sched = SCHED_STREAMK;  // HBM-bound whatever the tile count (lm_head: 1,002-1,187 tiles = 6.8-8.02 waves)
   p.sched = tune("SS_GEMM_SCHED", p.sched);
+  if (g.invariant) p.sched = SCHED_TILES;  // every tile's whole K by one CTA, k-blocks in order
   if (n_tiles * nkb >= (1LL << 31)) p.sched = SCHED_TILES;  // the stream-K unit cursor is 32-bit
   p.band = tune("SS_GEMM_BAND", g.dual ? 8 : 16);
   if (p.band > p.n_row_tiles) p.band = p.n_row_tiles;
@@ -604,6 +605,7 @@ void gemm_plan(GemmLaunch &g, int n_sm) {
     // 119 -> 113 us, O 51.5 -> 45.5 us, T = 128 gate/up 155.6 -> 153.9 us with one issuer).  Tensor-bound: one issuer
     // (the tensor pipe waits on L2 there, not on the issuing thread).
     p.issuers = (hbm_bound && 4 * acc_cols <= 512) ? 2 : 1;
+    if (g.invariant) p.issuers = 1;  // one accumulator: no sum of two interleaved k-block sets
     const int forced_iss = tune("SS_GEMM_ISSUERS", 0);
     if (forced_iss == 1 || (forced_iss == 2 && 2 * acc_cols <= 512)) p.issuers = forced_iss;
     p.single_buf = tune("SS_GEMM_SINGLE_BUF", 0);

@@ -74,6 +74,7 @@ struct GemmLaunch {
   const CUtensorMap *a[3];  // weight maps, box {64, 128}; dual (SwiGLU): a[0] = gate, a[1] = up, n_seg = 1
   const CUtensorMap *b;     // activation map, box {64, bn}
   bool dual;
+  bool invariant;           // batch-invariant mode: whole-K tiles, one issuer (the K order of an element never depends on T)
   bool no_pdl;              // weights may have been written by the preceding kernel (op-level entry points)
   int grid;                 // persistent CTAs
   GemmParams p;
@@ -121,9 +122,11 @@ cudaError_t launch_input_rmsnorm(const CallArgs *args, const void *embed, const 
 // x[t,:] += sum_{s<splits} part[s][t,:]; then (w != null) h = bf16(rmsnorm(x) * w); (out_from_args) the bf16 of
 // x goes to args->out_hidden when that is non-null.
 // gp.slots != null: additionally x[t,:] += the pieces of an EPI_PARTIAL projection (added in CTA order first).
+// fixed_shape: always the 1024-threads-per-row variant (batch-invariant mode: the reduction tree of a row must not
+// depend on how many rows the call has)
 cudaError_t launch_residual_rmsnorm(float *x, const float *part, int splits, long long split_stride,
                                     const GemmPartials &gp, const void *ln_w, float eps, int H, int T, void *h,
-                                    const CallArgs *args, bool write_out_hidden, cudaStream_t s);
+                                    const CallArgs *args, bool write_out_hidden, cudaStream_t s, bool fixed_shape = false);
 // gather the last row of each sequence: hl[s,:] = bf16(rmsnorm(x[last(s),:]) * wf)
 cudaError_t launch_final_norm_rows(const float *x, const CallArgs *args, bool decode, const void *wf, float eps,
                                    int H, int n_seqs, void *hl, cudaStream_t s);
@@ -178,6 +181,13 @@ struct DecodeAttnParams {
   int n_workers;             // worker warps in the grid
   int append;                // 1: write kv_new into the last page (decode step); 0: the token is already in the pool
   int warps_per_cta;
+  // batch-invariant mode (ss_stage_set_batch_invariant): worker w = one (row, kv head) pair, walked from page 0 to the
+  // last by ONE warp, result normalised and written by that warp (no split, no merge kernel): the summation order of a
+  // row depends on its own context only.  row_seq / row_pos (prefill rows: the plan's tok_seq / tok_pos) replace
+  // args->ctx and the row's own block-table row; null for a decode step.
+  int per_pair;
+  int n_rows;
+  const int32_t *row_seq, *row_pos;
 };
 cudaError_t launch_decode_attn(const DecodeAttnParams &p, cudaStream_t s);
 cudaError_t launch_decode_merge(const DecodeAttnParams &p, cudaStream_t s);
@@ -188,8 +198,9 @@ int decode_attn_default_ctas_per_sm();
 struct PrefillPlan {
   int32_t *tok_seq;          // [max_tokens]
   int32_t *tok_pos;          // [max_tokens]
-  int32_t *tile_cum;         // [max_seqs+1] prefix sum of 64-row query tiles per sequence
-  int32_t *tile_order;       // [2 * max_tiles]: launch slot -> tile, heaviest (most keys) first; second half = sort keys
+  int32_t *tile_cum;         // [max_seqs+1] prefix sum of 128-row query tiles per sequence
+  int32_t *tile_order;       // [2 * max_tiles]: tile -> launch slot, heaviest (most keys) first; second half = sort keys
+  int32_t *tile_desc;        // [max_tiles][4]: per launch slot {first packed row, rows, first position, sequence}
   int max_tiles;             // capacity: max_tokens / 64 + max_seqs + 1
 };
 // seq0: the first seq0 sequences get no query tiles (mixed batches: their attention runs in the decode kernel)

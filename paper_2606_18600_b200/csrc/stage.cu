@@ -51,7 +51,7 @@ static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Carve {  // byte offsets into the workspace
   size_t args, err, ptab, rope, x, h, qkv_part, q, kv_new, attn_out, fix, a, part_o, part_ml, cum_pages, meta, tp_part, am_part, tok_seq,
-      tok_pos, tile_cum, tile_order, hl, logits, total;
+      tok_pos, tile_cum, tile_order, tile_desc, hl, logits, total;
 };
 
 static bool dims_ok(const ss_model_dims *d, int l0, int l1, int *why) {
@@ -104,6 +104,7 @@ static Carve carve(const ss_model_dims *d) {
   c.tok_pos = take(Tm * 4);
   c.tile_cum = take(((size_t)d->max_seqs + 1) * 4);
   c.tile_order = take(2 * (Tm / 64 + (size_t)d->max_seqs + 1) * 4);
+  c.tile_desc = take(4 * (Tm / 64 + (size_t)d->max_seqs + 1) * 4);
   c.hl = take((size_t)d->max_seqs * H * 2);
   c.logits = take(d->vocab > 0 ? (size_t)d->max_seqs * d->vocab * 4 : 0);
   c.total = o;
@@ -193,6 +194,7 @@ struct ss_stage {
   int64_t launches;
   std::map<int, Graph> graphs;  // key = batch*2 + tail
   bool use_graph;
+  bool invariant;      // ss_stage_set_batch_invariant
   ss_allreduce_fn allreduce;  // non-null: tensor-parallel shard (ss_stage_set_allreduce)
   void *allreduce_user;
   CallArgs *h_args;    // pinned host staging for the argument block (+ 4 ints behind it: the SS_DEBUG error word)
@@ -282,6 +284,7 @@ int ss_stage_create(ss_stage **out, const ss_model_dims *dims, int l0, int l1, c
   st->stream = (cudaStream_t)cuda_stream;
   st->launches = 0;
   st->use_graph = (cuda_stream != nullptr) && env_int("SS_NO_GRAPH", 0) == 0;
+  st->invariant = false;
   st->h_args = nullptr;
   st->args_ev = nullptr;
   st->debug = env_int("SS_DEBUG", 0) != 0;
@@ -495,6 +498,19 @@ int ss_stage_debug_tap(const ss_stage *st, const char *name, void **dev_ptr_out,
   return SS_ERR_INVALID_ARG;
 }
 
+int ss_stage_set_batch_invariant(ss_stage *st, int on) {
+  if (!st) return SS_ERR_INVALID_ARG;
+  if (st->invariant != (on != 0)) {  // the captured decode graphs hold the other mode's kernels
+    cudaError_t e = cudaStreamSynchronize(st->stream);
+    if (e != cudaSuccess) return cuda_fail(e, "ss_stage_set_batch_invariant");
+    for (auto &g : st->graphs)
+      if (g.second.exec) cudaGraphExecDestroy(g.second.exec);
+    st->graphs.clear();
+    st->invariant = on != 0;
+  }
+  return SS_OK;
+}
+
 int ss_stage_set_allreduce(ss_stage *st, ss_allreduce_fn fn, void *user) {
   if (!st) return SS_ERR_INVALID_ARG;
   st->allreduce = fn;
@@ -559,6 +575,7 @@ static cudaError_t run_gemm(const ss_stage *st, const CUtensorMap *const a[3], i
   p.fix_flags = st->at<int>(st->c.fix);
   p.fix_slots = (float *)(st->ws + st->c.fix + GEMM_FIX_FLAG_BYTES);
   g.dual = dual;
+  g.invariant = st->invariant;
   g.stream = st->stream;
   gemm_plan(g, st->n_sm);
   g.b = &bmaps[p.bn / 32];
@@ -598,7 +615,8 @@ static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T,
   float *tp_part = st->at<float>(c.tp_part);
   DecodePlan dplan{st->at<int32_t>(c.cum_pages), st->at<int32_t>(c.meta)};
   PrefillPlan pplan{st->at<int32_t>(c.tok_seq), st->at<int32_t>(c.tok_pos), st->at<int32_t>(c.tile_cum),
-                    st->at<int32_t>(c.tile_order), (int)(d.max_tokens / 64 + d.max_seqs + 1)};
+                    st->at<int32_t>(c.tile_order), st->at<int32_t>(c.tile_desc),
+                    (int)(d.max_tokens / 64 + d.max_seqs + 1)};
   if (decode)
     CKE(launch_decode_plan(args, n_seqs, d.n_kv_heads, st->n_workers, dplan, s));
   else {
@@ -639,7 +657,9 @@ static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T,
     qp.decode = decode ? 1 : 0;
     CKE(launch_qkv_post(qp, s));  // S3, S4 (+S5 in prefill)
 
-    if (decode || n_dec > 0) {  // S5 + S6a (mixed call: the decode rows' K/V were appended by qkv_post already)
+    if (st->invariant) {
+      // batch-invariant mode: every row (decode rows and prefill tokens alike) is one (row, kv head) walk of the decode
+      // kernel from page 0 to its last page by one warp — the same arithmetic in the same order whatever the call
       DecodeAttnParams ap;
       memset(&ap, 0, sizeof(ap));
       ap.q = st->at<void>(c.q);
@@ -647,41 +667,62 @@ static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T,
       ap.kpool = st->kpool(l); ap.vpool = st->vpool(l);
       ap.kv_map = &st->maps[l].kv;
       ap.n_pages = st->num_pages;
-      ap.batch = decode ? n_seqs : n_dec; ap.n_q = d.n_q_heads; ap.n_kv = d.n_kv_heads; ap.d = dh;
+      ap.batch = 0; ap.n_q = d.n_q_heads; ap.n_kv = d.n_kv_heads; ap.d = dh;
       ap.plan = dplan;
-      ap.part_o = st->at<float>(c.part_o);
-      ap.part_ml = st->at<float>(c.part_ml);
       ap.out = st->at<void>(c.attn_out);
       ap.args = args;
-      ap.n_workers = st->n_workers;
       ap.warps_per_cta = decode_attn_warps_per_cta();
-      ap.append = decode ? 1 : 0;
+      ap.per_pair = 1;
+      ap.n_rows = T;
+      ap.append = decode ? 1 : 0;  // prefill: qkv_post has appended every token already
+      ap.row_seq = decode ? nullptr : pplan.tok_seq;
+      ap.row_pos = decode ? nullptr : pplan.tok_pos;
       CKE(launch_decode_attn(ap, s));
-      CKE(launch_decode_merge(ap, s));
-    }
-    if (!decode && n_dec < n_seqs) {  // S6b
-      PrefillAttnParams ap;
-      memset(&ap, 0, sizeof(ap));
-      ap.q_map = &st->q_map;
-      ap.kv_map = &st->maps[l].kv;
-      ap.n_pages = st->num_pages;
-      ap.n_seqs = n_seqs; ap.T = T; ap.n_q = d.n_q_heads; ap.n_kv = d.n_kv_heads; ap.d = dh;
-      ap.plan = pplan;
-      ap.out = st->at<void>(c.attn_out);
-      ap.args = args;
-      ap.max_tiles = (T - n_dec + prefill_attn_tile_rows() - 1) / prefill_attn_tile_rows() + (n_seqs - n_dec);
-      CKE(launch_prefill_attn(ap, s));
+    } else {
+      if (decode || n_dec > 0) {  // S5 + S6a (mixed call: the decode rows' K/V were appended by qkv_post already)
+        DecodeAttnParams ap;
+        memset(&ap, 0, sizeof(ap));
+        ap.q = st->at<void>(c.q);
+        ap.kv_new = st->at<void>(c.kv_new);
+        ap.kpool = st->kpool(l); ap.vpool = st->vpool(l);
+        ap.kv_map = &st->maps[l].kv;
+        ap.n_pages = st->num_pages;
+        ap.batch = decode ? n_seqs : n_dec; ap.n_q = d.n_q_heads; ap.n_kv = d.n_kv_heads; ap.d = dh;
+        ap.plan = dplan;
+        ap.part_o = st->at<float>(c.part_o);
+        ap.part_ml = st->at<float>(c.part_ml);
+        ap.out = st->at<void>(c.attn_out);
+        ap.args = args;
+        ap.n_workers = st->n_workers;
+        ap.warps_per_cta = decode_attn_warps_per_cta();
+        ap.append = decode ? 1 : 0;
+        CKE(launch_decode_attn(ap, s));
+        CKE(launch_decode_merge(ap, s));
+      }
+      if (!decode && n_dec < n_seqs) {  // S6b
+        PrefillAttnParams ap;
+        memset(&ap, 0, sizeof(ap));
+        ap.q_map = &st->q_map;
+        ap.kv_map = &st->maps[l].kv;
+        ap.n_pages = st->num_pages;
+        ap.n_seqs = n_seqs; ap.T = T; ap.n_q = d.n_q_heads; ap.n_kv = d.n_kv_heads; ap.d = dh;
+        ap.plan = pplan;
+        ap.out = st->at<void>(c.attn_out);
+        ap.args = args;
+        ap.max_tiles = (T - n_dec + prefill_attn_tile_rows() - 1) / prefill_attn_tile_rows() + (n_seqs - n_dec);
+        CKE(launch_prefill_attn(ap, s));
+      }
     }
     {  // S7: output projection, then S8: x1 = x + o Wo^T ; h2 = rmsnorm(x1; ln2)
       const CUtensorMap *a[3] = {&m.wo, nullptr, nullptr};
       const int rows[3] = {H, 0, 0};
       if (!tp) {
         CKE(run_gemm(st, a, 1, rows, false, st->b_attn, T, Hq, EPI_RESID_F32, x, nullptr, H, 1, &gp_o));
-        CKE(launch_residual_rmsnorm(x, nullptr, 0, 0, gp_o, w.ln2, d.rms_eps, H, T, h, args, false, s));
+        CKE(launch_residual_rmsnorm(x, nullptr, 0, 0, gp_o, w.ln2, d.rms_eps, H, T, h, args, false, s, st->invariant));
       } else {  // this rank's partial over its heads -> all-reduce -> x += sum (two per layer)
         CKE(run_gemm(st, a, 1, rows, false, st->b_attn, T, Hq, EPI_F32, tp_part, nullptr, H));
         if (st->allreduce(tp_part, (size_t)T * H, st->allreduce_user, (void *)s) != 0) return cudaErrorLaunchFailure;
-        CKE(launch_residual_rmsnorm(x, tp_part, 1, 0, gp_none, w.ln2, d.rms_eps, H, T, h, args, false, s));
+        CKE(launch_residual_rmsnorm(x, tp_part, 1, 0, gp_none, w.ln2, d.rms_eps, H, T, h, args, false, s, st->invariant));
       }
     }
     {  // S9: gate/up + SwiGLU fused -> a bf16 [T,F]
@@ -696,11 +737,11 @@ static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T,
       const void *next_ln = last ? nullptr : st->lw[l + 1].ln1;
       if (!tp) {
         CKE(run_gemm(st, a, 1, rows, false, st->b_a, T, F, EPI_RESID_F32, x, nullptr, H, 2, &gp_d));
-        CKE(launch_residual_rmsnorm(x, nullptr, 0, 0, gp_d, next_ln, d.rms_eps, H, T, h, args, last, s));
+        CKE(launch_residual_rmsnorm(x, nullptr, 0, 0, gp_d, next_ln, d.rms_eps, H, T, h, args, last, s, st->invariant));
       } else {
         CKE(run_gemm(st, a, 1, rows, false, st->b_a, T, F, EPI_F32, tp_part, nullptr, H));
         if (st->allreduce(tp_part, (size_t)T * H, st->allreduce_user, (void *)s) != 0) return cudaErrorLaunchFailure;
-        CKE(launch_residual_rmsnorm(x, tp_part, 1, 0, gp_none, next_ln, d.rms_eps, H, T, h, args, last, s));
+        CKE(launch_residual_rmsnorm(x, tp_part, 1, 0, gp_none, next_ln, d.rms_eps, H, T, h, args, last, s, st->invariant));
       }
     }
   }

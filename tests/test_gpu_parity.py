@@ -365,6 +365,72 @@ def test_migration_invariant_on_gpu():
         Q.close()
 
 
+@pytest.mark.parametrize("shape", [synth.TINY, synth.TINY_QWEN, synth.TINY128])
+def test_migration_is_bit_exact_in_batch_invariant_mode(shape):
+    """ss_stage_set_batch_invariant (include/shuntstage.h; SURVEY 8(f) "later": batch-invariant summation).  The paper's
+    migration is output-PRESERVING: in this mode the GPU meets that bit for bit — recompute (one
+    prefill over prompt + generated tokens), a chunked recompute with another batch composition, and incremental decode
+    (prefill of the prompt + decode steps) leave IDENTICAL KV pages, and the next decode step from each state returns
+    identical hidden-state bits; all of it still matches the oracle within the stage tolerance."""
+    P, lens, pb, x = _problem(shape, seed=1)
+    Q, _, _, _ = _problem(shape, seed=1)
+    R, _, _, _ = _problem(shape, seed=1)
+    try:
+        for S in (P, Q, R):
+            S.stage.set_batch_invariant(True)
+        bt = pb.block_tables
+        n, T = len(lens), int(lens.sum())
+        cu = np.concatenate([[0], np.cumsum(lens)]).astype(np.int32)
+        gen = 3
+        prompt = lens - gen
+        # (a) recompute: one prefill over everything
+        P.prefill(lens, bt, x[:T])
+        # (b) incremental: prompt, then one decode step per generated token
+        rows = np.concatenate([np.arange(cu[s], cu[s] + prompt[s]) for s in range(n)])
+        Q.prefill(prompt, bt, x[rows])
+        for g in range(gen):
+            Q.decode(prompt + g, bt, x[np.array([cu[s] + prompt[s] + g for s in range(n)])])
+        # (c) chunked recompute in another batch composition: sequences 0-1 first, then 2-3, each in two chunks
+        for grp in (np.arange(0, n // 2), np.arange(n // 2, n)):
+            half = lens[grp] // 2
+            r1 = np.concatenate([np.arange(cu[s], cu[s] + lens[s] // 2) for s in grp])
+            r2 = np.concatenate([np.arange(cu[s] + lens[s] // 2, cu[s + 1]) for s in grp])
+            R.prefill(half, bt[grp], x[r1])
+            R.prefill(lens[grp], bt[grp], x[r2], ctx_before=half)
+        pa, pq, pr = P.pool_bits(), Q.pool_bits(), R.pool_bits()
+        assert np.array_equal(pa, pq), f"recompute vs incremental: {int((pa != pq).sum())} KV elements differ"
+        assert np.array_equal(pa, pr), f"recompute vs chunked recompute: {int((pa != pr).sum())} KV elements differ"
+        mask = _written_mask(pa.shape, bt, lens)
+        assert (pa[~mask] == 0x7FC1).all() and (pa[mask] != 0x7FC1).all()
+        xs = x[T:T + n]
+        ya, yq, yr = P.decode(lens, bt, xs), Q.decode(lens, bt, xs), R.decode(lens, bt, xs)
+        assert np.array_equal(ya, yq) and np.array_equal(ya, yr)
+        # a decode step of a sub-batch returns the same bits for its rows (batch composition)
+        sub = np.array([2, 0])
+        P2, _, _, _ = _problem(shape, seed=1)
+        try:
+            P2.stage.set_batch_invariant(True)
+            P2.prefill(lens, bt, x[:T])
+            ys = P2.decode(lens[sub], bt[sub], xs[sub])
+            assert np.array_equal(ys, ya[sub])
+        finally:
+            P2.close()
+        pool0 = hp.new_pool(shape, pb.n_pages_pool, P.L)
+        hp.run_oracle_prefill(F32, shape, P.wb, pool0, lens, bt, x[:T])
+        want, _ = hp.run_oracle_decode(F32, shape, P.wb, pool0, lens, bt, xs)
+        err = hp.rel_err_rows(ya, want)
+        print(f"{shape.name}: batch-invariant mode, next-token hidden vs oracle R0 {err:.3e}")
+        assert err < STAGE_TOL
+        # back in the default mode the stage still works (graphs re-captured)
+        P.stage.set_batch_invariant(False)
+        yd = P.decode(lens + 1, bt, xs)
+        assert np.isfinite(yd).all()
+    finally:
+        P.close()
+        Q.close()
+        R.close()
+
+
 def test_chunked_prefill_and_mixed_batch_on_gpu():
     """Prior context (ctx_before > 0) and q_len = 1 rows in a prefill call (mixed iteration, reading A19)."""
     shape = synth.TINY_QWEN
