@@ -496,6 +496,230 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
 }
 
 // ---------------------------------------------------------------------------------------------------------------
+// The tensor-bound (prefill) shapes on CTA PAIRS: a cluster of two CTAs on the two SMs of a TPC computes one
+// 256-weight-row x 256-token tile with tcgen05.mma.cta_group::2.  Each CTA loads ITS 128 weight rows (A) and HALF of
+// the token tile (B: 128 tokens); the pair's tensor cores read the other half from the peer's shared memory, so a
+// stage is 32 KB per CTA instead of 48 KB (a 128 x 256 single-CTA tile re-reads the whole activation tile per 128
+// weight rows) and the L2 -> SM traffic per flop drops by a third — what held the plain projections at 83-85% of the
+// cuBLAS-sustained rate while the dual gate/up tile (two weight tiles per activation tile) ran at 94%.
+// Roles per CTA: warp 0 TMA producer (both CTAs; all bytes are counted on the LEADER's full barrier), warp 1 MMA issuer
+// (leader only; its commits arrive on both CTAs' barriers), warps 2-5 and 7-10 epilogue (each CTA its own 128 rows).
+// Whole tiles only (SCHED_TILES), band-rasterised like the single-CTA kernel.
+// ---------------------------------------------------------------------------------------------------------------
+constexpr int PAIR_BN = 256;                       // tokens per pair tile
+constexpr int PAIR_BHALF_BYTES = (PAIR_BN / 2) * 128;  // this CTA's half of the activation tile, per stage
+
+size_t gemm_pair_smem_bytes(bool dual, int stages) {
+  const size_t stage = (size_t)A_TILE_BYTES * (dual ? 2 : 1) + PAIR_BHALF_BYTES;
+  return 1024 + stage * stages + 8 * (2 * stages + 4) + 16;
+}
+
+template <bool DUAL>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEMM_THREADS, 1)
+gemm_pair_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUtensorMap ta1,
+                 const __grid_constant__ CUtensorMap ta2, const __grid_constant__ CUtensorMap tb, const GemmParams p) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t *base = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  constexpr uint32_t a_bytes = A_TILE_BYTES * (DUAL ? 2 : 1);
+  constexpr uint32_t stage_bytes = a_bytes + PAIR_BHALF_BYTES;
+  const int stages = p.stages;
+  uint64_t *full = (uint64_t *)(base + (size_t)stages * stage_bytes);  // used in the leader CTA only
+  uint64_t *empty = full + stages;   // per CTA: the slot may be refilled (the leader's commit arrives on both)
+  uint64_t *tfull = empty + stages;  // [2] per CTA: accumulator complete
+  uint64_t *tempty = tfull + 2;      // [2] leader only: both CTAs' epilogues have drained the accumulator
+  uint32_t *tmem_slot = (uint32_t *)(tempty + 2);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = cluster_ctarank();
+  const int cluster = blockIdx.x >> 1, n_clusters = gridDim.x >> 1;
+  constexpr uint32_t acc_cols = PAIR_BN * (DUAL ? 2u : 1u);
+  constexpr int nbuf = DUAL ? 1 : 2;
+  constexpr uint32_t tmem_cols = 512;
+
+  pdl_launch_dependents();
+  if (warp == 0 && lane == 0) {
+    tma_prefetch_desc(&ta0);
+    if (DUAL || p.n_seg > 1) tma_prefetch_desc(&ta1);
+    if (p.n_seg > 2) tma_prefetch_desc(&ta2);
+    tma_prefetch_desc(&tb);
+    for (int i = 0; i < stages; ++i) {
+      mbar_init(&full[i], 1);
+      mbar_init(&empty[i], 1);
+    }
+    for (int i = 0; i < 2; ++i) {
+      mbar_init(&tfull[i], 1);
+      mbar_init(&tempty[i], 2 * EPI_WARPS);  // one arrival per epilogue warp of either CTA
+    }
+    mbar_fence_init();
+  }
+  if (warp == 1) tmem_alloc_pair(tmem_slot, tmem_cols);
+  tc_fence_before();
+  __syncthreads();
+  cluster_sync_all();  // the peer's barriers exist before anything signals them
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+
+  // pair items: (row PAIR, token tile); this CTA's row tile is 2 * pair + rank
+  GemmParams pp = p;
+  pp.n_row_tiles = (p.n_row_tiles + 1) >> 1;
+  pp.sched = SCHED_TILES;
+
+  if (warp == 0) {
+    if (lane == 0) {
+      // ---------------- TMA producer (both CTAs) ----------------
+      const uint64_t pol = l2_policy_evict_last();
+      pdl_wait();
+      WorkIter it(pp, cluster, n_clusters);
+      WorkItem w;
+      int s = 0;
+      uint32_t ph = 0;
+      while (it.next(w)) {
+        const int row_tile = 2 * w.row_tile + (int)rank;
+        int seg = 0;
+#pragma unroll
+        for (int i = 1; i < 3; ++i)
+          if (i < p.n_seg && row_tile >= p.seg_tile0[i]) seg = i;
+        // a row tile past the end (odd tile count) loads rows past its tensor: TMA fills zeros and counts the bytes
+        const int row0 = row_tile < p.n_row_tiles ? (row_tile - p.seg_tile0[seg]) * GEMM_BM : (1 << 28);
+        const int t0 = w.t_tile * PAIR_BN + (int)rank * (PAIR_BN / 2);
+        const CUtensorMap *ta = DUAL ? &ta0 : (seg == 0 ? &ta0 : (seg == 1 ? &ta1 : &ta2));
+        for (int kb = w.kb0; kb < w.kb1; ++kb) {
+          mbar_wait_site(&empty[s], ph ^ 1u, 1, (uint32_t)s);
+          uint8_t *st = base + (size_t)s * stage_bytes;
+          if (rank == 0) mbar_expect_tx(&full[s], 2 * stage_bytes);  // both CTAs' loads land on the leader's barrier
+          tma_load_2d_pair(st, ta, &full[s], kb * GEMM_BK, row0, pol);
+          if (DUAL) tma_load_2d_pair(st + A_TILE_BYTES, &ta1, &full[s], kb * GEMM_BK, row0, pol);
+          tma_load_2d_pair(st + a_bytes, &tb, &full[s], kb * GEMM_BK, t0, pol);
+          if (++s == stages) {
+            s = 0;
+            ph ^= 1u;
+          }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    if (lane == 0 && rank == 0) {
+      // ---------------- MMA issuer (leader CTA, for the pair) ----------------
+      const uint32_t idesc = umma_idesc_bf16(2 * GEMM_BM, PAIR_BN);
+      WorkIter it(pp, cluster, n_clusters);
+      WorkItem w;
+      uint32_t item = 0;
+      int ms = 0;
+      uint32_t mph = 0;
+      while (it.next(w)) {
+        const uint32_t buf = item % nbuf, tph = (item / nbuf) & 1u;
+        mbar_wait_site(&tempty[buf], tph ^ 1u, 2, item);  // both epilogues have drained this accumulator
+        tc_fence_after();
+        const uint32_t acc_addr = tmem_base + buf * acc_cols;
+        bool first = true;
+        for (int kb = w.kb0; kb < w.kb1; ++kb) {
+          mbar_wait_site(&full[ms], mph, 4, (uint32_t)kb);
+          tc_fence_after();
+          const uint32_t st = smem_u32(base + (size_t)ms * stage_bytes);
+          const uint64_t da = umma_desc_k_sw128(st);
+          const uint64_t da1 = umma_desc_k_sw128(st + A_TILE_BYTES);
+          const uint64_t db = umma_desc_k_sw128(st + a_bytes);
+#pragma unroll
+          for (int k = 0; k < GEMM_BK / 16; ++k) {
+            const uint32_t acc = (!first || k > 0) ? 1u : 0u;
+            umma_bf16_pair(acc_addr, da + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc, acc);
+            if (DUAL) umma_bf16_pair(acc_addr + PAIR_BN, da1 + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc, acc);
+          }
+          first = false;
+          umma_commit_pair(&empty[ms]);  // frees the slot in BOTH CTAs when these MMAs have read it
+          if (++ms == stages) {
+            ms = 0;
+            mph ^= 1u;
+          }
+        }
+        umma_commit_pair(&tfull[buf]);
+        ++item;
+      }
+    }
+  } else if ((warp >= 2 && warp < 6) || (warp >= 7 && warp < 11)) {
+    // ---------------- epilogue: this CTA's 128 rows x 256 tokens, TMEM -> registers -> global ----------------
+    pdl_wait();
+    const int quad = warp & 3;
+    const int r = quad * 32 + lane;
+    const int grp = warp >= 7 ? 1 : 0;
+    WorkIter it(pp, cluster, n_clusters);
+    WorkItem w;
+    uint32_t item = 0;
+    while (it.next(w)) {
+      const uint32_t buf = item % nbuf, tph = (item / nbuf) & 1u;
+      const int row_tile = 2 * w.row_tile + (int)rank;
+      int seg = 0;
+#pragma unroll
+      for (int i = 1; i < 3; ++i)
+        if (i < p.n_seg && row_tile >= p.seg_tile0[i]) seg = i;
+      const int row_in_seg = (row_tile - p.seg_tile0[seg]) * GEMM_BM + r;
+      const bool row_ok = row_tile < p.n_row_tiles && row_in_seg < p.seg_rows[seg];
+      const int col = p.seg_col[seg] + row_in_seg;
+      const int t0 = w.t_tile * PAIR_BN;
+      mbar_wait_site(&tfull[buf], tph, 6, item);
+      tc_fence_after();
+      const uint32_t tq = tmem_base + buf * acc_cols + ((uint32_t)(quad * 32) << 16);
+      for (int c0 = grp * 32; c0 < PAIR_BN; c0 += 64) {
+        if (t0 + c0 >= p.T) break;  // (uniform per warp) nothing but padding from here on
+        uint32_t v[32], u[32];
+        float xv[32];
+        if (!DUAL && p.epi == EPI_RESID_F32 && row_ok) {
+          const float *o = p.out_f32 + col;
+#pragma unroll
+          for (int j = 0; j < 32; ++j) {
+            const int t = t0 + c0 + j;
+            xv[j] = (t < p.T) ? __ldcg(o + (size_t)t * p.ld_out) : 0.f;
+          }
+        }
+        tmem_ld_32x32(tq + (uint32_t)c0, v);
+        if (DUAL) tmem_ld_32x32(tq + (uint32_t)(PAIR_BN + c0), u);
+        tmem_ld_wait();
+        if (DUAL) {
+          __nv_bfloat16 *o = (__nv_bfloat16 *)p.out_bf16;
+          const bool odd = (lane & 1) != 0;
+#pragma unroll
+          for (int j = 0; j < 32; j += 2) {
+            const float g0 = __uint_as_float(v[j]), g1 = __uint_as_float(v[j + 1]);
+            const float a0 = __fdividef(g0, 1.0f + __expf(-g0)) * __uint_as_float(u[j]);
+            const float a1 = __fdividef(g1, 1.0f + __expf(-g1)) * __uint_as_float(u[j + 1]);
+            const float got = __shfl_xor_sync(0xffffffffu, odd ? a0 : a1, 1);
+            const int t = t0 + c0 + j + (odd ? 1 : 0);
+            const uint32_t pk = odd ? pack_bf16x2(got, a1) : pack_bf16x2(a0, got);
+            if (row_ok && t < p.T) *reinterpret_cast<uint32_t *>(o + (size_t)t * p.ld_out + (col & ~1)) = pk;
+          }
+        } else if (row_ok) {
+          float *o = p.out_f32 + col;
+          if (p.epi == EPI_RESID_F32) {
+#pragma unroll
+            for (int j = 0; j < 32; ++j) {
+              const int t = t0 + c0 + j;
+              if (t < p.T) o[(size_t)t * p.ld_out] = xv[j] + __uint_as_float(v[j]);
+            }
+          } else {
+#pragma unroll
+            for (int j = 0; j < 32; ++j) {
+              const int t = t0 + c0 + j;
+              if (t < p.T) o[(size_t)t * p.ld_out] = __uint_as_float(v[j]);
+            }
+          }
+        }
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive_leader(&tempty[buf]);
+      ++item;
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  cluster_sync_all();  // neither CTA leaves (or frees its TMEM) while the pair may still touch it
+  if (warp == 1) {
+    tc_fence_after();
+    tmem_dealloc_pair(tmem_base, tmem_cols);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------------------------
 typedef CUresult (*PFN_encodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
@@ -610,6 +834,23 @@ void gemm_plan(GemmLaunch &g, int n_sm) {
     if (forced_iss == 1 || (forced_iss == 2 && 2 * acc_cols <= 512)) p.issuers = forced_iss;
     p.single_buf = tune("SS_GEMM_SINGLE_BUF", 0);
   }
+  // tensor-bound shapes (several token tiles, whole-tile schedule): CTA pairs on 256 x 256 tiles (gemm_pair_kernel)
+  const int pair_mode = tune("SS_GEMM_PAIR", 1);  // tuning builds: 0 never, 1 always, 2 plain only, 3 plain with K <= 8192
+  g.pair = pair_mode != 0 && !g.invariant && p.sched == SCHED_TILES && p.T > 2 * PAIR_BN && n_sm >= 2 &&
+           (pair_mode < 2 || !g.dual) && (pair_mode < 3 || p.K <= 8192);
+  if (g.pair) {
+    p.bn = PAIR_BN;
+    p.n_t_tiles = (p.T + PAIR_BN - 1) / PAIR_BN;
+    p.issuers = 1;
+    p.stages = GEMM_MAX_STAGES;
+    while (p.stages > 2 && gemm_pair_smem_bytes(g.dual, p.stages) > 227 * 1024) --p.stages;
+    const long long pair_tiles = (long long)((p.n_row_tiles + 1) / 2) * p.n_t_tiles;
+    const long long clusters = pair_tiles < max_grid / 2 ? pair_tiles : max_grid / 2;
+    p.band = tune("SS_GEMM_BAND", g.dual ? 4 : 8);  // in row PAIRS
+    if (p.band > (p.n_row_tiles + 1) / 2) p.band = (p.n_row_tiles + 1) / 2;
+    g.grid = (int)(2 * clusters);
+    return;
+  }
   const long long work = p.sched == SCHED_STREAMK ? n_tiles * nkb : n_tiles;
   g.grid = (int)(work < max_grid ? work : max_grid);
   {
@@ -665,7 +906,11 @@ cudaError_t gemm_set_debug_buffer(unsigned long long *host_mapped) {
 cudaError_t gemm_init() {
   cudaError_t e = cudaFuncSetAttribute(gemm_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
   if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(gemm_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+  e = cudaFuncSetAttribute(gemm_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(gemm_pair_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(gemm_pair_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
 }
 
 cudaError_t gemm_launch(const GemmLaunch &g) {
@@ -673,6 +918,12 @@ cudaError_t gemm_launch(const GemmLaunch &g) {
   size_t smem = gemm_smem_bytes(p.bn, g.dual, p.stages);
   const CUtensorMap *a1 = g.a[1] ? g.a[1] : g.a[0];
   const CUtensorMap *a2 = g.a[2] ? g.a[2] : g.a[0];
+  if (g.pair) {
+    smem = gemm_pair_smem_bytes(g.dual, p.stages);
+    if (g.dual)
+      return launch_pdl_if(!g.no_pdl, gemm_pair_kernel<true>, dim3(g.grid), dim3(GEMM_THREADS), smem, g.stream, *g.a[0], *a1, *a2, *g.b, p);
+    return launch_pdl_if(!g.no_pdl, gemm_pair_kernel<false>, dim3(g.grid), dim3(GEMM_THREADS), smem, g.stream, *g.a[0], *a1, *a2, *g.b, p);
+  }
   if (g.dual)
     return launch_pdl_if(!g.no_pdl, gemm_kernel<true>, dim3(g.grid), dim3(GEMM_THREADS), smem, g.stream, *g.a[0], *a1, *a2, *g.b, p);
   return launch_pdl_if(!g.no_pdl, gemm_kernel<false>, dim3(g.grid), dim3(GEMM_THREADS), smem, g.stream, *g.a[0], *a1, *a2, *g.b, p);

@@ -74,6 +74,7 @@ struct GemmLaunch {
   const CUtensorMap *a[3];  // weight maps, box {64, 128}; dual (SwiGLU): a[0] = gate, a[1] = up, n_seg = 1
   const CUtensorMap *b;     // activation map, box {64, bn}
   bool dual;
+  bool pair;                // set by gemm_plan: run on CTA pairs (gemm_pair_kernel; b must be the 128-row activation map)
   bool invariant;           // batch-invariant mode: whole-K tiles, one issuer (the K order of an element never depends on T)
   bool no_pdl;              // weights may have been written by the preceding kernel (op-level entry points)
   int grid;                 // persistent CTAs

@@ -578,7 +578,7 @@ static cudaError_t run_gemm(const ss_stage *st, const CUtensorMap *const a[3], i
   g.invariant = st->invariant;
   g.stream = st->stream;
   gemm_plan(g, st->n_sm);
-  g.b = &bmaps[p.bn / 32];
+  g.b = &bmaps[(g.pair ? 128 : p.bn) / 32];  // a CTA pair loads the token tile in two 128-row halves
   if (gp) {
     gp->slots = nullptr;
     if (piece >= 0 && st->ptab_ok[piece] && gemm_partial_ok(g)) {
@@ -931,7 +931,7 @@ static int op_gemm(const void *x_dev, const void *w0, const void *w1, float *c_f
   gemm_plan(g, n_sm);
   if (make_tmap_bf16_2d(&ta, w0, (uint64_t)N, (uint64_t)K, GEMM_BM, true) != 0 ||
       (dual && make_tmap_bf16_2d(&tu, w1, (uint64_t)N, (uint64_t)K, GEMM_BM, true) != 0) ||
-      make_tmap_bf16_2d(&tb, x_dev, (uint64_t)T, (uint64_t)K, (uint32_t)p.bn, false) != 0) {
+      make_tmap_bf16_2d(&tb, x_dev, (uint64_t)T, (uint64_t)K, (uint32_t)(g.pair ? 128 : p.bn), false) != 0) {
     g_cuda_err = "cuTensorMapEncodeTiled failed";
     return SS_ERR_CUDA;
   }

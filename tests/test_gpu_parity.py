@@ -39,6 +39,8 @@ def f32b(b):
     # every token-tile width: 96, 160, 192, 224 columns, and two ragged tiles of 160 / 224
     (65, 700, 1024), (96, 512, 8192), (129, 1300, 2048), (160, 256, 4096), (190, 4000, 512), (224, 640, 1024),
     (300, 900, 1536), (420, 520, 768),
+    # the CTA-pair kernel (cta_group::2, 256 x 256 pair tiles): odd row-tile count, ragged T / N, long K
+    (1100, 9000, 1024), (2049, 4224, 2048), (513, 38000, 512), (3000, 8192, 4096),
 ])
 def test_op_gemm_vs_oracle(T, N, K):
     """Covers both schedules: stream-K with in-kernel fix-up (few tiles; one tile cut across up to 148 CTAs at
@@ -93,7 +95,8 @@ def test_op_gemm_full_grid_long_k_is_stable(dual, T, N, K):
 
 @pytest.mark.parametrize("T,F,K", [(64, 256, 256), (4, 688, 256), (130, 1376, 512), (300, 200, 1000), (16, 128, 64),
                                    (64, 384, 8192), (128, 3000, 1024), (700, 20000, 128), (96, 1000, 2048),
-                                   (150, 640, 4096), (192, 384, 1024), (200, 2000, 512), (310, 300, 1024)])
+                                   (150, 640, 4096), (192, 384, 1024), (200, 2000, 512), (310, 300, 1024),
+                                   (1300, 12000, 768), (2100, 9100, 2048)])   # CTA-pair kernel
 def test_op_gemm_swiglu_vs_oracle(T, F, K):
     from paper_2606_18600_b200 import binding
     g = torch.Generator().manual_seed(T + F + K)
