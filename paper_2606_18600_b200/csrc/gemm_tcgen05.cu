@@ -503,11 +503,13 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
 // weight rows) and the L2 -> SM traffic per flop drops by a third — what held the plain projections at 83-85% of the
 // cuBLAS-sustained rate while the dual gate/up tile (two weight tiles per activation tile) ran at 94%.
 // Roles per CTA: warp 0 TMA producer (both CTAs; all bytes are counted on the LEADER's full barrier), warp 1 MMA issuer
-// (leader only; its commits arrive on both CTAs' barriers), warps 2-5 and 7-10 epilogue (each CTA its own 128 rows).
+// (leader only; its commits arrive on both CTAs' barriers), warps 4-19 epilogue (each CTA its own 128 rows).
 // Whole tiles only (SCHED_TILES), band-rasterised like the single-CTA kernel.
 // ---------------------------------------------------------------------------------------------------------------
 constexpr int PAIR_BN = 256;                       // tokens per pair tile
 constexpr int PAIR_BHALF_BYTES = (PAIR_BN / 2) * 128;  // this CTA's half of the activation tile, per stage
+constexpr int PAIR_EPI_WARPS = 16;
+constexpr int PAIR_THREADS = 32 * (4 + PAIR_EPI_WARPS);  // warp 0 producer, 1 MMA issuer, 2-3 idle, 4-19 epilogue
 
 size_t gemm_pair_smem_bytes(bool dual, int stages) {
   const size_t stage = (size_t)A_TILE_BYTES * (dual ? 2 : 1) + PAIR_BHALF_BYTES;
@@ -515,7 +517,7 @@ size_t gemm_pair_smem_bytes(bool dual, int stages) {
 }
 
 template <bool DUAL>
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEMM_THREADS, 1)
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PAIR_THREADS, 1)
 gemm_pair_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUtensorMap ta1,
                  const __grid_constant__ CUtensorMap ta2, const __grid_constant__ CUtensorMap tb, const GemmParams p) {
   extern __shared__ uint8_t smem_raw[];
@@ -548,7 +550,7 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant_
     }
     for (int i = 0; i < 2; ++i) {
       mbar_init(&tfull[i], 1);
-      mbar_init(&tempty[i], 2 * EPI_WARPS);  // one arrival per epilogue warp of either CTA
+      mbar_init(&tempty[i], 2 * PAIR_EPI_WARPS);  // one arrival per epilogue warp of either CTA
     }
     mbar_fence_init();
   }
@@ -636,12 +638,14 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant_
         ++item;
       }
     }
-  } else if ((warp >= 2 && warp < 6) || (warp >= 7 && warp < 11)) {
+  } else if (warp >= 4) {
     // ---------------- epilogue: this CTA's 128 rows x 256 tokens, TMEM -> registers -> global ----------------
+    // 16 warps, four per TMEM lane quadrant, 16-column chunks: the dual tile leaves no second TMEM buffer, so its
+    // epilogue is exposed once per item and is spread as wide as the register file allows (640 threads x 96 registers)
     pdl_wait();
     const int quad = warp & 3;
     const int r = quad * 32 + lane;
-    const int grp = warp >= 7 ? 1 : 0;
+    const int grp = (warp - 4) >> 2;  // 0..3
     WorkIter it(pp, cluster, n_clusters);
     WorkItem w;
     uint32_t item = 0;
@@ -659,26 +663,26 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant_
       mbar_wait_site(&tfull[buf], tph, 6, item);
       tc_fence_after();
       const uint32_t tq = tmem_base + buf * acc_cols + ((uint32_t)(quad * 32) << 16);
-      for (int c0 = grp * 32; c0 < PAIR_BN; c0 += 64) {
+      for (int c0 = grp * 16; c0 < PAIR_BN; c0 += 64) {
         if (t0 + c0 >= p.T) break;  // (uniform per warp) nothing but padding from here on
-        uint32_t v[32], u[32];
-        float xv[32];
+        uint32_t v[16], u[16];
+        float xv[16];
         if (!DUAL && p.epi == EPI_RESID_F32 && row_ok) {
           const float *o = p.out_f32 + col;
 #pragma unroll
-          for (int j = 0; j < 32; ++j) {
+          for (int j = 0; j < 16; ++j) {
             const int t = t0 + c0 + j;
             xv[j] = (t < p.T) ? __ldcg(o + (size_t)t * p.ld_out) : 0.f;
           }
         }
-        tmem_ld_32x32(tq + (uint32_t)c0, v);
-        if (DUAL) tmem_ld_32x32(tq + (uint32_t)(PAIR_BN + c0), u);
+        tmem_ld_32x16(tq + (uint32_t)c0, v);
+        if (DUAL) tmem_ld_32x16(tq + (uint32_t)(PAIR_BN + c0), u);
         tmem_ld_wait();
         if (DUAL) {
           __nv_bfloat16 *o = (__nv_bfloat16 *)p.out_bf16;
           const bool odd = (lane & 1) != 0;
 #pragma unroll
-          for (int j = 0; j < 32; j += 2) {
+          for (int j = 0; j < 16; j += 2) {
             const float g0 = __uint_as_float(v[j]), g1 = __uint_as_float(v[j + 1]);
             const float a0 = __fdividef(g0, 1.0f + __expf(-g0)) * __uint_as_float(u[j]);
             const float a1 = __fdividef(g1, 1.0f + __expf(-g1)) * __uint_as_float(u[j + 1]);
@@ -691,13 +695,13 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant_
           float *o = p.out_f32 + col;
           if (p.epi == EPI_RESID_F32) {
 #pragma unroll
-            for (int j = 0; j < 32; ++j) {
+            for (int j = 0; j < 16; ++j) {
               const int t = t0 + c0 + j;
               if (t < p.T) o[(size_t)t * p.ld_out] = xv[j] + __uint_as_float(v[j]);
             }
           } else {
 #pragma unroll
-            for (int j = 0; j < 32; ++j) {
+            for (int j = 0; j < 16; ++j) {
               const int t = t0 + c0 + j;
               if (t < p.T) o[(size_t)t * p.ld_out] = __uint_as_float(v[j]);
             }
@@ -921,8 +925,8 @@ cudaError_t gemm_launch(const GemmLaunch &g) {
   if (g.pair) {
     smem = gemm_pair_smem_bytes(g.dual, p.stages);
     if (g.dual)
-      return launch_pdl_if(!g.no_pdl, gemm_pair_kernel<true>, dim3(g.grid), dim3(GEMM_THREADS), smem, g.stream, *g.a[0], *a1, *a2, *g.b, p);
-    return launch_pdl_if(!g.no_pdl, gemm_pair_kernel<false>, dim3(g.grid), dim3(GEMM_THREADS), smem, g.stream, *g.a[0], *a1, *a2, *g.b, p);
+      return launch_pdl_if(!g.no_pdl, gemm_pair_kernel<true>, dim3(g.grid), dim3(PAIR_THREADS), smem, g.stream, *g.a[0], *a1, *a2, *g.b, p);
+    return launch_pdl_if(!g.no_pdl, gemm_pair_kernel<false>, dim3(g.grid), dim3(PAIR_THREADS), smem, g.stream, *g.a[0], *a1, *a2, *g.b, p);
   }
   if (g.dual)
     return launch_pdl_if(!g.no_pdl, gemm_kernel<true>, dim3(g.grid), dim3(GEMM_THREADS), smem, g.stream, *g.a[0], *a1, *a2, *g.b, p);
