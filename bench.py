@@ -32,13 +32,16 @@ def parse():
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "cfg5", "migrate", "pipeline", "estimator", "gemm", "tiny"])
+    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "cfg5", "migrate", "pipeline", "estimator", "gemm", "tp_emul", "tiny"])
     ap.add_argument("--seed", type=int, default=0)
     ap.add_argument("--layers", type=int, default=0, help="override the stage depth (debug only; marks the line)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--batch-invariant", action="store_true",
                     help="run the stage in ss_stage_set_batch_invariant mode (measures what exact migration costs)")
+    ap.add_argument("--tp", action="store_true",
+                    help="cfg2/cfg3 decode as ONE stage sharded over the N ranks (tensor parallelism, fused all-reduce over "
+                         "peer memory, DESIGN.md 8d) instead of N replicas; scaling = strong")
     ap.add_argument("--no-sub", action="store_true",
                     help="default workload only: skip the cfg-4 prefill and cfg-3 decode sub-records")
     return ap.parse_args()
@@ -169,6 +172,8 @@ def workload_spec(name, layers_override=0):
         shape, ctx, kind = synth.LLAMA70B, None, "estimator"
     elif name == "gemm":
         shape, ctx, kind = synth.LLAMA70B, synth.cfg4_lengths, "gemm"
+    elif name == "tp_emul":
+        shape, ctx, kind = synth.LLAMA70B, synth.cfg2_contexts, "tp_emul"
     else:
         shape, ctx, kind = synth.TINY, synth.cfg1_contexts, "decode"
     L = layers_override or shape.n_layers
@@ -238,12 +243,18 @@ def run_decode(args, shape, ctx_fn, rank, world, layers=None, K=None, W=None, do
     B = len(ctx0)
     total_steps = 2 * (K + W) + 8                        # device-timed pass + e2e pass
     pb = synth.paged_batch(rng, ctx0, extra_tokens=total_steps + 1)
+    full_shape = shape
+    if args.tp:
+        from paper_2606_18600_b200 import tp as tpmod
+        shape = tpmod.shard_shape(shape, world)          # this rank's shard (random-init: drawn at the shard's shape)
+        layers = None
     if layers is None:
-        layers = gpu_weights(shape, dev, args.seed)
+        layers = gpu_weights(shape, dev, args.seed + (1000 * rank if args.tp else 0))
     dims = binding.make_dims(shape, max_tokens=B, max_seqs=B, max_blocks=pb.max_blocks,
                              max_pos=int(ctx0.max()) + total_steps + 64)
     st = binding.Stage(dims, 0, shape.n_layers, layers, None, n_pages=pb.n_pages_pool, device=dev)
     st.set_batch_invariant(args.batch_invariant)
+    tp_state = tp_fused_setup(st, rank, world) if args.tp else None
     g = torch.Generator(device=dev)
     g.manual_seed(args.seed + 99)
     _fill_randn(st.kv_pool.view(-1), g)                  # random KV pre-fill N(0,1) (A21)
@@ -276,7 +287,7 @@ def run_decode(args, shape, ctx_fn, rank, world, layers=None, K=None, W=None, do
     launches = st.launch_count() - n0
     clocks = sampler.stop()
     # algorithmic bytes averaged over the timed steps (contexts grow by one token per step)
-    byts = np.mean([decode_bytes_per_step(shape, ctx0 + first_step + i) for i in range(K)])
+    byts = np.mean([decode_bytes_per_step(full_shape, ctx0 + first_step + i) for i in range(K)])
 
     # ---- e2e: the same step through the C-ABI with HOST buffers (pinned), H2D of inputs + D2H of the result inside
     e2e = None
@@ -314,9 +325,53 @@ def run_decode(args, shape, ctx_fn, rank, world, layers=None, K=None, W=None, do
         raise SystemExit("bench.py: the last decode step produced non-finite hidden states")
     res = {"ms": ms, "tokens": B * K, "bytes_per_step": float(byts), "launches": int(launches), "clocks": clocks,
            "e2e": e2e, "dominant": dom, "B": B, "ctx_sum": int(ctx0.sum()), "pages": int(pb.n_pages_pool),
-           "checksum": float(o32.abs().mean()), "K": K, "W": W}
+           "checksum": float(o32.abs().mean()), "K": K, "W": W, "graphs": st.graph_count()}
     st.destroy()
+    if tp_state is not None:
+        tp_fused_teardown(tp_state, world)
     return res
+
+
+def tp_fused_setup(st, rank, world):
+    """Exchange buffers of the fused tensor-parallel all-reduce: one whole allocation per rank (ss_store_alloc), its
+    CUDA IPC handle all-gathered over torch.distributed, the peers' buffers attached (ss_store_attach)."""
+    import ctypes as C
+    import torch.distributed as dist
+    from paper_2606_18600_b200 import binding
+    lib = binding.load_library()
+    nbytes = lib.ss_tp_xchg_bytes(world)
+    mine = C.c_void_p()
+    if lib.ss_store_alloc(C.byref(mine), nbytes) != 0:
+        raise SystemExit("ss_store_alloc failed: " + lib.ss_last_cuda_error().decode())
+    handle = (C.c_ubyte * 64)()
+    lib.ss_store_export(mine, handle)
+    handles = [None] * world
+    if world > 1:
+        dist.all_gather_object(handles, bytes(handle))
+    ptrs, attached = [None] * world, []
+    for r in range(world):
+        if r == rank:
+            ptrs[r] = mine.value
+        else:
+            p = C.c_void_p()
+            if lib.ss_store_attach((C.c_ubyte * 64).from_buffer_copy(handles[r]), C.byref(p)) != 0:
+                raise SystemExit("ss_store_attach failed: " + lib.ss_last_cuda_error().decode())
+            ptrs[r] = p.value
+            attached.append(p)
+    st.set_tp_fused(rank, world, ptrs)
+    if world > 1:
+        dist.barrier()                      # every rank's counters are zero before anybody's first step
+    return lib, mine, attached
+
+
+def tp_fused_teardown(state, world):
+    lib, mine, attached = state
+    for p in attached:
+        lib.ss_store_detach(p)
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()                      # every peer has detached
+    lib.ss_store_free(mine)
 
 
 def _fill_randn(pool, g):
@@ -669,6 +724,75 @@ def run_gemm_sustained(args, shape, len_fn, seconds=4.0):
     return rows
 
 
+def run_tp_emulated(args, shape, ctx_fn, size=2):
+    """What the fused tensor-parallel all-reduce costs in kernels and waits, measured where only one GPU exists: the
+    cfg-2 stage cut into `size` shards (tp.shard_shape), every shard a stage of THIS process on its own stream of the
+    ONE device, exchange buffers = plain device memory (so the "peer" stores and counters are local: no NVLink time in
+    this number).  The two ranks' steps run concurrently as far as the SMs allow, so the step time is about the sum
+    of the shards' work: compare with the un-sharded stage on the same box (the default workload)."""
+    import torch
+    from paper_2606_18600_b200 import binding, synth, tp as tpmod
+    dev = torch.device("cuda:0")
+    torch.cuda.set_device(dev)
+    K, W = args.steps, args.warmup
+    ctx0 = ctx_fn(args.seed).astype(np.int32)
+    B = len(ctx0)
+    total = K + W + 4
+    pb = synth.paged_batch(np.random.default_rng(args.seed), ctx0, extra_tokens=total + 1)
+    sshape = tpmod.shard_shape(shape, size)
+    lib = binding.load_library()
+    xchg = [torch.empty(lib.ss_tp_xchg_bytes(size), dtype=torch.uint8, device=dev) for _ in range(size)]
+    stages = []
+    g = torch.Generator(device=dev)
+    g.manual_seed(args.seed + 99)
+    for r in range(size):
+        layers = gpu_weights(sshape, dev, args.seed + 1000 * r)
+        dims = binding.make_dims(sshape, max_tokens=B, max_seqs=B, max_blocks=pb.max_blocks,
+                                 max_pos=int(ctx0.max()) + total + 64)
+        st = binding.Stage(dims, 0, sshape.n_layers, layers, None, n_pages=pb.n_pages_pool, device=dev)
+        _fill_randn(st.kv_pool.view(-1), g)
+        stages.append(st)
+    for r, st in enumerate(stages):
+        st.set_tp_fused(r, size, [b.data_ptr() for b in xchg])
+    x = torch.randn((B, shape.hidden), generator=g, device=dev, dtype=torch.float32).to(torch.bfloat16)
+    bt = torch.from_numpy(pb.block_tables).to(dev)
+    ctxs = torch.from_numpy(ctx0[None, :] + np.arange(total, dtype=np.int32)[:, None]).to(dev).contiguous()
+    outs = [torch.empty((B, shape.hidden), dtype=torch.bfloat16, device=dev) for _ in range(size)]
+    torch.cuda.synchronize(dev)
+    no = [0]
+
+    def step():
+        for r, st in enumerate(stages):
+            st.decode(B, bt, ctxs[no[0]], hidden=x, out_hidden=outs[r])
+        no[0] += 1
+
+    for _ in range(W):
+        step()
+    torch.cuda.synchronize(dev)
+    sampler = ClockSampler(0)
+    sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in stages]
+    n0 = sum(st.launch_count() for st in stages)
+    for (e0, _), st in zip(ev, stages):
+        e0.record(st.stream)
+    for _ in range(K):
+        step()
+    for (_, e1), st in zip(ev, stages):
+        e1.record(st.stream)
+    torch.cuda.synchronize(dev)
+    ms = max(e0.elapsed_time(e1) for e0, e1 in ev)
+    clocks = sampler.stop()
+    launches = sum(st.launch_count() for st in stages) - n0
+    same = all(torch.equal(outs[r], outs[0]) for r in range(size))
+    graphs = [st.graph_count() for st in stages]
+    for st in stages:
+        st.destroy()
+    byts = decode_bytes_per_step(shape, ctx0 + W + K // 2)
+    return {"ms_per_step": ms / K, "tokens_per_s": B * K / (ms * 1e-3), "launches": int(launches), "clocks": clocks,
+            "ranks_bit_identical": bool(same), "decode_graphs_per_rank": graphs, "bytes_per_step": float(byts), "B": B,
+            "size": size}
+
+
 def run_online(args, shape, rank, world):
     """cfg5: online mixed batches (96 decode rows + <= 4 prefill chunks of <= 512 tokens per ss_stage_prefill call)
     driven by paper_2606_18600_b200/online.py over a page pool at ~85% occupancy; K timed iterations."""
@@ -776,6 +900,7 @@ def main():
                         "pipeline": "80-layer 70B-shaped model in 4 stages (even / uneven), per-stage decode latency",
                         "estimator": "estimator accuracy (Fig. 8 protocol), 70B shapes",
                         "gemm": "prefill projections alone, 70B layer shapes, T = 40,173",
+                        "tp_emul": "cfg-2 stage sharded D_TP = 2, both ranks on ONE GPU (fused all-reduce exercised, no NVLink)",
                         "tiny": "configs[0]: tiny Llama-style stage"}[args.workload],
            "layers": shape.n_layers, "hidden": shape.hidden, "ffn": shape.ffn, "heads": f"{shape.n_q}/{shape.n_kv}",
            "page_size": 16, "seed": args.seed, "parallelism": f"replicas x{world}",
@@ -826,6 +951,21 @@ def main():
                           "config": {"workload": "70B-shaped 20-layer stage, one request, contexts 1K-64K",
                                      "link": "modelled: NVLink 5, 900 GB/s per direction (single-GPU box)"},
                           "rows": rows}))
+        return
+    if kind == "tp_emul":
+        if rank != 0:
+            return
+        r = run_tp_emulated(args, shape, len_fn)
+        gbs = r["bytes_per_step"] / (r["ms_per_step"] * 1e-3) / 1e9
+        print(json.dumps({"metric": "stage decode tokens/s, stage sharded D_TP = 2 with both ranks on one GPU (fused "
+                                    "all-reduce path exercised end to end; no NVLink in this number)",
+                          "value": r["tokens_per_s"], "unit": "tokens/s", "n_gpus": 1, "steps": args.steps,
+                          "warmup": args.warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True,
+                          "dtype": "bf16", "data": "synthetic", "gpu_launches": r["launches"], "clocks": r["clocks"],
+                          "ranks_bit_identical": r["ranks_bit_identical"], "decode_graphs_per_rank": r["decode_graphs_per_rank"],
+                          "step_roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm_gbs"], "unit": "GB/s",
+                                            "frac": gbs / pk["hbm_gbs"]},
+                          "config": dict(cfg, parallelism="tp2 emulated on one GPU")}))
         return
     if kind == "gemm":
         if rank != 0:
@@ -894,18 +1034,25 @@ def main():
         print(json.dumps(line))
         return
     keep_layers = None
-    if kind == "decode" and args.workload == "cfg2" and not args.no_sub:
+    if kind == "decode" and args.workload == "cfg2" and not args.no_sub and not args.tp:
         dev = torch.device(f"cuda:{int(os.environ.get('LOCAL_RANK', 0))}")
         keep_layers = gpu_weights(shape, dev, args.seed)      # cfg-4 (same 70B shapes) re-uses them below
+    if args.tp and (kind != "decode" or world > 8):
+        raise SystemExit("--tp applies to the decode workloads (cfg2, cfg3, tiny) on at most 8 ranks")
     res = run_decode(args, shape, len_fn, rank, world, layers=keep_layers) if kind == "decode" else \
         run_prefill(args, shape, len_fn, rank, world)
+    if args.tp:
+        res["tp"] = True
     K = args.steps
     ms, e2e_ms = reduce_times(res, world)
     line = None
     if rank == 0:
         line = {"metric": metric, "unit": unit, "n_gpus": world, "steps": K, "warmup": args.warmup,
-                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-                "config": cfg}
+                "higher_is_better": True, "scaling": "strong" if args.tp else "weak", "vs_baseline": None,
+                "dtype": "bf16", "data": "synthetic", "config": cfg}
+        if args.tp:
+            cfg["parallelism"] = f"tp{world} (one stage sharded over {world} ranks, fused all-reduce over peer memory)"
+            line["decode_graphs"] = res.get("graphs")
         line.update(decode_record(res, ms, e2e_ms, world, shape, len_fn, args, pk) if kind == "decode" else
                     prefill_record(res, ms, e2e_ms, world, shape, len_fn, args, pk))
         line["build"] = source_hash()
@@ -957,6 +1104,8 @@ def reduce_times(res, world):
 
 def _common_record(res, ms, e2e_ms, world):
     K = res["K"]
+    if res.get("tp"):
+        world = 1            # tensor parallelism: the N ranks process ONE batch together
     rec = {"value": whole_job_value(res["tokens"], world, ms), "ms_per_step": ms / K, "clocks": res["clocks"],
            "gpu_launches": res["launches"], "output_checksum_mean_abs": res["checksum"]}
     if res["e2e"]:
@@ -978,9 +1127,10 @@ def decode_record(res, ms, e2e_ms, world, shape, len_fn, args, pk, workload=None
                            "algorithmic_bytes": dom["bytes"], "kernel": dom["kernel"], "us_per_launch": dom["us"],
                            "peak_source": pk["source"]}
     step_gbs = res["bytes_per_step"] / (ms / K * 1e-3) / 1e9
+    n_hbm = world if res.get("tp") else 1      # a tensor-parallel stage streams its bytes from all N ranks' HBM
     rec["step_roofline"] = {"bound": "hbm", "algorithmic_GB_per_step": res["bytes_per_step"] / 1e9,
-                            "achieved": step_gbs, "peak": pk["hbm_gbs"], "unit": "GB/s",
-                            "frac": step_gbs / pk["hbm_gbs"]}
+                            "achieved": step_gbs, "peak": pk["hbm_gbs"] * n_hbm, "unit": "GB/s",
+                            "frac": step_gbs / (pk["hbm_gbs"] * n_hbm)}
     rec["paper_estimator_ms"] = estimator.decode_step_ms(shape, len_fn(args.seed), pk["bf16_tflops"] * 1e12,
                                                          pk["hbm_gbs"] * 1e9)
     return rec

@@ -218,6 +218,26 @@ int ss_stage_set_batch_invariant(ss_stage *st, int on);
 typedef int (*ss_allreduce_fn)(float *partial_dev, size_t count, void *user, void *cuda_stream);
 int ss_stage_set_allreduce(ss_stage *st, ss_allreduce_fn fn, void *user);
 
+/* The same all-reduce FUSED into the projections (Eq. 3), for decode-sized calls
+ * (tokens <= 128), with no collective library call and no host callback, so the decode step stays one CUDA graph:
+ *   gather  — the O / down projection's epilogue warps store every stream-K piece of their accumulator into the
+ *             exchange buffer of EVERY rank (plain stores to peer-mapped memory: over NVLink for the other ranks), then
+ *             each CTA raises, with system scope, one arrival counter per rank;
+ *   wait    — each rank's STREAM waits until all ranks' counters in its own buffer have reached the grid size
+ *             (cuStreamWaitValue32) and re-arms them; no kernel ever spins on another rank;
+ *   reduce  — the consumer kernel that runs next anyway (residual add + RMSNorm) adds the pieces of all ranks in
+ *             (rank, CTA) order: every rank gets the same bits, and each value crosses the link exactly once per peer.
+ * Every rank allocates one exchange buffer of ss_tp_xchg_bytes(tp_size) bytes (device, 256-byte aligned; across
+ * processes a whole allocation made by ss_store_alloc, handed over with ss_store_export / ss_store_attach; with peer
+ * access enabled) and passes the device addresses of ALL ranks' buffers, indexed by rank, as xchg_dev (HOST array of
+ * tp_size pointers; xchg_dev[rank] is its own).  The call zeroes this rank's counters: no rank may start its first step
+ * before every rank has returned from it.  Two buffers alternate inside (O, down), which is enough because a rank cannot
+ * run more than one all-reduce point ahead of another.  Calls with more than 128 tokens (prefill) use the callback of
+ * ss_stage_set_allreduce, which a shard with tp_size > 1 must also register.  size = 0 switches the mode off.
+ * SS_ERR_INVALID_ARG (rank / size / null or misaligned pointers), SS_ERR_UNSUPPORTED (no stream memory operations). */
+size_t ss_tp_xchg_bytes(int tp_size);
+int ss_stage_set_tp_fused(ss_stage *st, int rank, int size, void *const *xchg_dev);
+
 /* Migration by KV transfer (the alternative to recomputation the paper measures; SURVEY
  * 8(f) NEXT-4).  ss_kv_export gathers the n pages `page_ids_dev[0..n)` (DEVICE int32) of every layer of the stage into
  * the caller's contiguous DEVICE buffer, laid out [layer][K/V][i][h_kv][16][d] bf16 (n * ss_kv_page_bytes() bytes) —
@@ -227,6 +247,10 @@ int ss_stage_set_allreduce(ss_stage *st, ss_allreduce_fn fn, void *user);
  * SS_ERR_CAPACITY (buffer too small).  Page ids out of range are undefined behaviour. */
 int ss_kv_export(ss_stage *st, int n, const int32_t *page_ids_dev, void *buf_dev, size_t buf_bytes);
 int ss_kv_import(ss_stage *st, int n, const int32_t *page_ids_dev, const void *buf_dev, size_t buf_bytes);
+
+/* Number of decode CUDA graphs the stage has captured so far (0 while SS_NO_GRAPH=1 or while an all-reduce CALLBACK is
+ * in use; the fused tensor-parallel mode keeps its graphs). */
+int64_t ss_stage_graph_count(const ss_stage *st);
 
 /* Device-side contract checks: block tables, context lengths, cu_q and token ids live in
  * device memory, so the host cannot validate them, and in a normal run a violation is undefined behaviour (a page id

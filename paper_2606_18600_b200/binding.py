@@ -24,8 +24,8 @@ EXPORTS = ["ss_stage_workspace_bytes", "ss_kv_page_bytes", "ss_stage_create", "s
            "ss_stage_decode",
            "ss_stage_launch_count", "ss_op_gemm_scratch_bytes", "ss_op_gemm_bf16", "ss_op_gemm_swiglu_bf16", "ss_strerror",
            "ss_last_cuda_error", "ss_version", "ss_debug_buffer", "ss_pool_create", "ss_pool_destroy",
-           "ss_pool_num_pages", "ss_pool_num_free", "ss_pool_alloc", "ss_pool_free", "ss_kv_export", "ss_kv_import", "ss_stage_set_allreduce", "ss_stage_set_batch_invariant",
-           "ss_stage_debug_tap", "ss_stage_debug_info", "ss_store_alloc", "ss_store_free", "ss_store_upload", "ss_store_export", "ss_store_attach", "ss_store_detach"]
+           "ss_pool_num_pages", "ss_pool_num_free", "ss_pool_alloc", "ss_pool_free", "ss_kv_export", "ss_kv_import", "ss_stage_set_allreduce", "ss_stage_set_batch_invariant", "ss_tp_xchg_bytes", "ss_stage_set_tp_fused",
+           "ss_stage_debug_tap", "ss_stage_debug_info", "ss_stage_graph_count", "ss_store_alloc", "ss_store_free", "ss_store_upload", "ss_store_export", "ss_store_attach", "ss_store_detach"]
 
 
 ALLREDUCE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p)
@@ -95,9 +95,14 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     lib.ss_stage_launch_count.argtypes = [C.c_void_p]
     lib.ss_debug_buffer.argtypes = [C.c_void_p]
     lib.ss_stage_debug_info.argtypes = [C.c_void_p, C.POINTER(C.c_int32)]
+    lib.ss_stage_graph_count.restype = C.c_int64
+    lib.ss_stage_graph_count.argtypes = [C.c_void_p]
     lib.ss_stage_debug_tap.argtypes = [C.c_void_p, C.c_char_p, C.POINTER(C.c_void_p), C.POINTER(C.c_size_t)]
     lib.ss_stage_set_allreduce.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
     lib.ss_stage_set_batch_invariant.argtypes = [C.c_void_p, C.c_int]
+    lib.ss_tp_xchg_bytes.restype = C.c_size_t
+    lib.ss_tp_xchg_bytes.argtypes = [C.c_int]
+    lib.ss_stage_set_tp_fused.argtypes = [C.c_void_p, C.c_int, C.c_int, C.POINTER(C.c_void_p)]
     lib.ss_kv_export.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_size_t]
     lib.ss_kv_import.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_size_t]
     lib.ss_pool_create.argtypes = [C.POINTER(C.c_void_p), C.c_int]
@@ -247,6 +252,13 @@ class Stage:
         if rc != SS_OK:
             raise ShuntStageError(rc, "ss_stage_set_batch_invariant")
 
+    def set_tp_fused(self, rank: int, size: int, xchg_ptrs):
+        """ss_stage_set_tp_fused: xchg_ptrs = device addresses (ints) of every rank's exchange buffer, indexed by rank."""
+        arr = (C.c_void_p * max(size, 1))(*[int(p) for p in xchg_ptrs]) if size else None
+        rc = self.lib.ss_stage_set_tp_fused(self.h, rank, size, arr)
+        if rc != SS_OK:
+            raise ShuntStageError(rc, "ss_stage_set_tp_fused")
+
     def set_allreduce(self, fn):
         """fn(partial: float32 torch view of the workspace, stream_ptr: int) -> None: enqueue an in-place sum across
         the tensor-parallel ranks on that stream (see paper_2606_18600_b200/tp.py).  None clears it."""
@@ -301,6 +313,9 @@ class Stage:
         cap = max(d.max_tokens, d.max_seqs)
         dt = torch.float32 if name in ("x", "qkv") else torch.bfloat16
         return self.workspace[off:off + n.value].view(dt).view(cap, -1)[:rows]
+
+    def graph_count(self) -> int:
+        return int(self.lib.ss_stage_graph_count(self.h))
 
     def launch_count(self) -> int:
         return int(self.lib.ss_stage_launch_count(self.h))

@@ -77,19 +77,22 @@ cudaError_t launch_input_rmsnorm(const CallArgs *args, const void *embed, const 
 __device__ __forceinline__ float4 gemm_partial_sum4(const GemmPartials &gp, int tile, int tok, int r) {
   const PartialTile pt = gp.tiles[tile];
   const float *base = gp.slots + (size_t)tok * GEMM_BM + r;
+  // piece q of source rank q / count (one rank unless the fused tensor-parallel all-reduce is on), rank-major, CTA order
+  const int n = pt.count * gp.n_src;
   auto piece = [&](int q) {
-    const int slot = 2 * (pt.first_cta + q) + (q == 0 ? pt.first_item : 0);
-    return __ldcg(reinterpret_cast<const float4 *>(base + (size_t)slot * gp.slot_floats));
+    const int src = q / pt.count, c = q - src * pt.count;
+    const int slot = 2 * (pt.first_cta + c) + (c == 0 ? pt.first_item : 0);
+    return __ldcg(reinterpret_cast<const float4 *>(base + (size_t)src * gp.src_stride + (size_t)slot * gp.slot_floats));
   };
   float4 y = piece(0);
-  for (int q = 1; q < pt.count; q += 4) {
+  for (int q = 1; q < n; q += 4) {
     float4 z[4];
 #pragma unroll
     for (int u = 0; u < 4; ++u)
-      if (q + u < pt.count) z[u] = piece(q + u);
+      if (q + u < n) z[u] = piece(q + u);
 #pragma unroll
     for (int u = 0; u < 4; ++u)
-      if (q + u < pt.count) {
+      if (q + u < n) {
         y.x += z[u].x; y.y += z[u].y; y.z += z[u].z; y.w += z[u].w;
       }
   }
@@ -189,12 +192,12 @@ residual_rmsnorm_kernel(float *__restrict__ x, const float *__restrict__ part, i
 
 cudaError_t launch_residual_rmsnorm(float *x, const float *part, int splits, long long split_stride,
                                     const GemmPartials &gp, const void *ln_w, float eps, int H, int T, void *h,
-                                    const CallArgs *args, bool write_out_hidden, cudaStream_t s, bool fixed_shape) {
+                                    const CallArgs *args, bool write_out_hidden, cudaStream_t s, bool fixed_shape, bool pdl) {
   const __nv_bfloat16 *w = (const __nv_bfloat16 *)ln_w;
   __nv_bfloat16 *hh = (__nv_bfloat16 *)h;
   const int wo = write_out_hidden ? 1 : 0;
   auto go = [&](auto kernel, int threads) {
-    return launch_pdl(kernel, dim3(T), dim3(threads), 0, s, x, part, splits, split_stride, gp, w, eps, H, hh, args, wo);
+    return launch_pdl_if(pdl, kernel, dim3(T), dim3(threads), 0, s, x, part, splits, split_stride, gp, w, eps, H, hh, args, wo);
   };
   if (!fixed_shape && T >= 512 && H <= 16 * 256 * 4) {  // many rows: 256 threads each
     const int it = (H + 1023) / 1024;

@@ -363,12 +363,23 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
 
       if (!DUAL && p.epi == EPI_PARTIAL) {
         // every piece of a tile (owner's included) goes to its own slot; the consumer kernel adds them (internal.h)
-        float *slot = p.fix_slots + ((size_t)cta * 2 + item) * bn * GEMM_BM;
+        const size_t slot_off = ((size_t)cta * 2 + item) * bn * GEMM_BM;
+        float *slot = p.fix_slots + slot_off;
         for (int c0 = grp * 32; c0 < bn; c0 += 64) {
           uint32_t v[32];
           ld_acc((uint32_t)c0, v);
+          if (p.tp_size > 0) {
+            // fused tensor-parallel all-reduce, gather half: the piece goes into the exchange buffer of EVERY rank
+            // (plain stores; for the other ranks they travel over NVLink to peer-mapped memory)
+            for (int d = 0; d < p.tp_size; ++d) {
+              float *ds = p.tp_slots[d] + slot_off;
 #pragma unroll
-          for (int j = 0; j < 32; ++j) slot[(size_t)(c0 + j) * GEMM_BM + r] = __uint_as_float(v[j]);
+              for (int j = 0; j < 32; ++j) ds[(size_t)(c0 + j) * GEMM_BM + r] = __uint_as_float(v[j]);
+            }
+          } else {
+#pragma unroll
+            for (int j = 0; j < 32; ++j) slot[(size_t)(c0 + j) * GEMM_BM + r] = __uint_as_float(v[j]);
+          }
         }
         tc_fence_before();
         __syncwarp();
@@ -484,6 +495,14 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
       }
       if (et == 0) trace(p, 6 + 4 * (int)item);
       ++item;
+    }
+    if (!DUAL && p.epi == EPI_PARTIAL && p.tp_size > 0) {
+      // publish: every epilogue thread's stores -> barrier -> one system-scope fence -> one arrival per rank
+      epi_bar();
+      if (et == 0) {
+        __threadfence_system();
+        for (int d = 0; d < p.tp_size; ++d) atomicAdd_system(p.tp_flags[d], 1u);
+      }
     }
   }
   tc_fence_before();

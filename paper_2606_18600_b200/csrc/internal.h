@@ -22,6 +22,7 @@ namespace ss {
 constexpr int GEMM_BM = 128;  // weight rows per tile
 constexpr int GEMM_BK = 64;   // K elements per stage (= one 128-byte swizzle row of bf16)
 constexpr int GEMM_MAX_STAGES = 12;
+constexpr int SS_TP_MAX = 8;   // tensor-parallel degree of the fused all-reduce (ss_stage_set_tp_fused)
 
 enum GemmEpilogue {
   EPI_F32 = 0,          // out_f32[t][col] = acc
@@ -52,6 +53,9 @@ struct GemmParams {
   int ld_out;           // leading dimension (elements) of the output
   float *out_f32;
   void *out_bf16;
+  int tp_size;          // > 0 (EPI_PARTIAL only): every piece is stored into the exchange buffer of EVERY rank
+  float *tp_slots[SS_TP_MAX];     // rank d's region for pieces coming from THIS rank (peer-mapped for d != this rank)
+  unsigned *tp_flags[SS_TP_MAX];  // rank d's arrival counter for this rank's pieces: += 1 per CTA, system scope
   float *fix_slots;     // SCHED_STREAMK: gridDim.x partial-accumulator slots of (dual ? 2 : 1) * bn * 128 floats
   unsigned long long *trace;  // profiling builds (-DSS_GEMM_TRACE): [grid][64] globaltimer stamps, else null
   int *fix_flags;       // SCHED_STREAMK: gridDim.x flags, zero between launches (consumers reset them)
@@ -68,7 +72,18 @@ struct GemmPartials {
   const float *slots;         // null: the projection's result is in its ordinary output buffer
   const PartialTile *tiles;   // [n_row_tiles] (device)
   int slot_floats;            // bn * 128
+  int n_src;                  // 1, or the tensor-parallel degree: the pieces of EVERY rank are added, rank-major
+  long long src_stride;       // floats between two ranks' slot regions
 };
+
+// Fused tensor-parallel all-reduce (ss_stage_set_tp_fused): exchange buffer layout, identical on every rank:
+//   [buffer 0 = O projection | buffer 1 = down projection][source rank][TP_SLOTS slots of TP_SLOT_FLOATS floats],
+//   then one 128-byte flag line per (buffer, source rank).
+constexpr int TP_SLOTS = 320;                    // 2 items x up to 160 CTAs
+constexpr int TP_SLOT_FLOATS = 128 * GEMM_BM;    // token tiles up to 128 columns
+inline size_t tp_region_floats() { return (size_t)TP_SLOTS * TP_SLOT_FLOATS; }
+inline size_t tp_flags_offset(int size) { return 2 * (size_t)size * tp_region_floats() * sizeof(float); }
+inline size_t tp_xchg_bytes(int size) { return tp_flags_offset(size) + 2 * (size_t)size * 128; }
 
 struct GemmLaunch {
   const CUtensorMap *a[3];  // weight maps, box {64, 128}; dual (SwiGLU): a[0] = gate, a[1] = up, n_seg = 1
@@ -127,7 +142,8 @@ cudaError_t launch_input_rmsnorm(const CallArgs *args, const void *embed, const 
 // depend on how many rows the call has)
 cudaError_t launch_residual_rmsnorm(float *x, const float *part, int splits, long long split_stride,
                                     const GemmPartials &gp, const void *ln_w, float eps, int H, int T, void *h,
-                                    const CallArgs *args, bool write_out_hidden, cudaStream_t s, bool fixed_shape = false);
+                                    const CallArgs *args, bool write_out_hidden, cudaStream_t s, bool fixed_shape = false,
+                                    bool pdl = true);
 // gather the last row of each sequence: hl[s,:] = bf16(rmsnorm(x[last(s),:]) * wf)
 cudaError_t launch_final_norm_rows(const float *x, const CallArgs *args, bool decode, const void *wf, float eps,
                                    int H, int n_seqs, void *hl, cudaStream_t s);

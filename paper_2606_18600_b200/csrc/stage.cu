@@ -49,6 +49,25 @@ constexpr int MAX_WORKERS = 4096;  // upper bound on decode-attention worker war
 
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
+// stream-ordered wait / write on a 32-bit word in device memory (driver API, resolved at run time): the cross-rank
+// synchronisation of the fused tensor-parallel all-reduce is done by the STREAM, never by a spinning kernel
+typedef CUresult (*PFN_streamValue32)(CUstream, CUdeviceptr, cuuint32_t, unsigned int);
+static PFN_streamValue32 g_wait32 = nullptr, g_write32 = nullptr;
+static bool load_stream_memops() {
+  if (g_wait32 && g_write32) return true;
+  void *fw = nullptr, *fr = nullptr;
+  cudaDriverEntryPointQueryResult q1, q2;
+  if (cudaGetDriverEntryPoint("cuStreamWaitValue32", &fw, cudaEnableDefault, &q1) != cudaSuccess || !fw ||
+      q1 != cudaDriverEntryPointSuccess)
+    return false;
+  if (cudaGetDriverEntryPoint("cuStreamWriteValue32", &fr, cudaEnableDefault, &q2) != cudaSuccess || !fr ||
+      q2 != cudaDriverEntryPointSuccess)
+    return false;
+  g_wait32 = (PFN_streamValue32)fw;
+  g_write32 = (PFN_streamValue32)fr;
+  return true;
+}
+
 struct Carve {  // byte offsets into the workspace
   size_t args, err, ptab, rope, x, h, qkv_part, q, kv_new, attn_out, fix, a, part_o, part_ml, cum_pages, meta, tp_part, am_part, tok_seq,
       tok_pos, tile_cum, tile_order, tile_desc, hl, logits, total;
@@ -195,8 +214,11 @@ struct ss_stage {
   std::map<int, Graph> graphs;  // key = batch*2 + tail
   bool use_graph;
   bool invariant;      // ss_stage_set_batch_invariant
+  int64_t graph_captures;  // decode graphs captured so far (ss_stage_graph_count)
   ss_allreduce_fn allreduce;  // non-null: tensor-parallel shard (ss_stage_set_allreduce)
   void *allreduce_user;
+  int tp_rank, tp_size;       // ss_stage_set_tp_fused: > 0 ranks, this stage's rank
+  uint8_t *tp_xchg[SS_TP_MAX];  // every rank's exchange buffer (own and peer-mapped), internal.h layout
   CallArgs *h_args;    // pinned host staging for the argument block (+ 4 ints behind it: the SS_DEBUG error word)
   cudaEvent_t args_ev; // the last H2D copy out of h_args (the host must not overwrite the block before it has run)
   bool debug;          // SS_DEBUG=1 at create: every call validates its device-side arguments first
@@ -285,12 +307,16 @@ int ss_stage_create(ss_stage **out, const ss_model_dims *dims, int l0, int l1, c
   st->launches = 0;
   st->use_graph = (cuda_stream != nullptr) && env_int("SS_NO_GRAPH", 0) == 0;
   st->invariant = false;
+  st->graph_captures = 0;
   st->h_args = nullptr;
   st->args_ev = nullptr;
   st->debug = env_int("SS_DEBUG", 0) != 0;
   memset(st->dbg_info, 0, sizeof(st->dbg_info));
   st->allreduce = nullptr;
   st->allreduce_user = nullptr;
+  st->tp_rank = 0;
+  st->tp_size = 0;
+  memset(st->tp_xchg, 0, sizeof(st->tp_xchg));
 
   auto fail = [&](int code) {
     if (st->h_args) cudaFreeHost(st->h_args);
@@ -474,6 +500,8 @@ int ss_store_detach(void *dev_ptr) {
 
 int64_t ss_stage_launch_count(const ss_stage *st) { return st ? st->launches : 0; }
 
+int64_t ss_stage_graph_count(const ss_stage *st) { return st ? st->graph_captures : 0; }
+
 int ss_stage_debug_info(const ss_stage *st, int32_t out[4]) {
   if (!st || !out) return SS_ERR_INVALID_ARG;
   memcpy(out, st->dbg_info, 16);
@@ -508,6 +536,37 @@ int ss_stage_set_batch_invariant(ss_stage *st, int on) {
     st->graphs.clear();
     st->invariant = on != 0;
   }
+  return SS_OK;
+}
+
+size_t ss_tp_xchg_bytes(int tp_size) {
+  return (tp_size >= 1 && tp_size <= SS_TP_MAX) ? tp_xchg_bytes(tp_size) : 0;
+}
+
+int ss_stage_set_tp_fused(ss_stage *st, int rank, int size, void *const *xchg_dev) {
+  if (!st) return SS_ERR_INVALID_ARG;
+  if (size == 0) {  // off
+    st->tp_size = 0;
+  } else {
+    if (size < 1 || size > SS_TP_MAX || rank < 0 || rank >= size || !xchg_dev) return SS_ERR_INVALID_ARG;
+    for (int i = 0; i < size; ++i)
+      if (!xchg_dev[i] || ((uintptr_t)xchg_dev[i] & 255)) return SS_ERR_INVALID_ARG;
+    if (!load_stream_memops()) {
+      g_cuda_err = "cuStreamWaitValue32 / cuStreamWriteValue32 not available";
+      return SS_ERR_UNSUPPORTED;
+    }
+    st->tp_rank = rank;
+    st->tp_size = size;
+    for (int i = 0; i < size; ++i) st->tp_xchg[i] = (uint8_t *)xchg_dev[i];
+    // this rank's arrival counters start at zero (the caller must not start any rank's first call before every rank
+    // has returned from this function: the counters are written by the peers' first projection)
+    CK(cudaMemsetAsync(st->tp_xchg[rank] + tp_flags_offset(size), 0, 2 * (size_t)size * 128, st->stream));
+    CK(cudaStreamSynchronize(st->stream));
+  }
+  CK(cudaStreamSynchronize(st->stream));
+  for (auto &g : st->graphs)
+    if (g.second.exec) cudaGraphExecDestroy(g.second.exec);
+  st->graphs.clear();
   return SS_OK;
 }
 
@@ -553,6 +612,11 @@ int ss_kv_import(ss_stage *st, int n, const int32_t *page_ids_dev, const void *b
 namespace ss {
 
 // one projection through the persistent tcgen05 GEMM
+// the fused tensor-parallel all-reduce applies to a decode-sized projection whose pieces fit the exchange slots
+static bool tp_fused_ok(const ss_stage *st, int T, int grid) {
+  return st->tp_size > 0 && T <= 128 && 2 * grid <= TP_SLOTS;
+}
+
 // `piece` (0 QKV, 1 O, 2 down; -1 none): if the planned launch allows it, the projection leaves its tiles in pieces
 // (EPI_PARTIAL) and *gp tells the consumer kernel where; otherwise gp->slots = null and `epi` is used as given.
 static cudaError_t run_gemm(const ss_stage *st, const CUtensorMap *const a[3], int n_seg, const int rows[3],
@@ -581,11 +645,36 @@ static cudaError_t run_gemm(const ss_stage *st, const CUtensorMap *const a[3], i
   g.b = &bmaps[(g.pair ? 128 : p.bn) / 32];  // a CTA pair loads the token tile in two 128-row halves
   if (gp) {
     gp->slots = nullptr;
+    gp->n_src = 1;
+    gp->src_stride = 0;
     if (piece >= 0 && st->ptab_ok[piece] && gemm_partial_ok(g)) {
       p.epi = EPI_PARTIAL;
       gp->slots = p.fix_slots;
       gp->tiles = st->at<PartialTile>(st->c.ptab) + (size_t)piece * PTAB_STRIDE;
       gp->slot_floats = p.bn * GEMM_BM;
+      if (piece >= 1 && tp_fused_ok(st, T, g.grid)) {
+        // fused all-reduce (Eq. 3): the pieces go to every rank's exchange buffer (O: buffer 0, down:
+        // buffer 1; a rank is never more than one all-reduce point ahead of another), the consumer adds all ranks'
+        const int buf = piece - 1, size = st->tp_size;
+        p.tp_size = size;
+        for (int d = 0; d < size; ++d) {
+          p.tp_slots[d] = (float *)st->tp_xchg[d] + ((size_t)buf * size + st->tp_rank) * tp_region_floats();
+          p.tp_flags[d] = (unsigned *)(st->tp_xchg[d] + tp_flags_offset(size) + ((size_t)buf * size + st->tp_rank) * 128);
+        }
+        gp->slots = (const float *)st->tp_xchg[st->tp_rank] + (size_t)buf * size * tp_region_floats();
+        gp->n_src = size;
+        gp->src_stride = (long long)tp_region_floats();
+        cudaError_t e = gemm_launch(g);
+        if (e != cudaSuccess) return e;
+        // wait (stream-ordered) until every rank's CTAs have arrived on this rank's counters, then re-arm them
+        for (int q = 0; q < size; ++q) {
+          const CUdeviceptr flag = (CUdeviceptr)(st->tp_xchg[st->tp_rank] + tp_flags_offset(size) + ((size_t)buf * size + q) * 128);
+          if (g_wait32((CUstream)st->stream, flag, (cuuint32_t)g.grid, CU_STREAM_WAIT_VALUE_GEQ) != CUDA_SUCCESS ||
+              g_write32((CUstream)st->stream, flag, 0u, CU_STREAM_WRITE_VALUE_DEFAULT) != CUDA_SUCCESS)
+            return cudaErrorUnknown;
+        }
+        return cudaSuccess;
+      }
     }
   }
   return gemm_launch(g);
@@ -611,7 +700,10 @@ static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T,
   float *qkv_part = st->at<float>(c.qkv_part);
   cudaStream_t s = st->stream;
 
-  const bool tp = st->allreduce != nullptr;
+  // tensor-parallel shard: the fused exchange for decode-sized calls, else the caller's all-reduce callback
+  const bool fused = st->tp_size > 0 && T <= 128 && st->ptab_ok[1] && st->ptab_ok[2] && 2 * st->n_sm <= TP_SLOTS;
+  const bool tp = !fused && (st->allreduce != nullptr || st->tp_size > 1);
+  if (tp && !st->allreduce) return cudaErrorNotSupported;  // a TP shard's large calls need ss_stage_set_allreduce
   float *tp_part = st->at<float>(c.tp_part);
   DecodePlan dplan{st->at<int32_t>(c.cum_pages), st->at<int32_t>(c.meta)};
   PrefillPlan pplan{st->at<int32_t>(c.tok_seq), st->at<int32_t>(c.tok_pos), st->at<int32_t>(c.tile_cum),
@@ -629,7 +721,7 @@ static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T,
     const ss_layer_weights &w = st->lw[l];
     const LayerMaps &m = st->maps[l];
     GemmPartials gp_qkv, gp_o, gp_d;
-    const GemmPartials gp_none{nullptr, nullptr, 0};
+    const GemmPartials gp_none{nullptr, nullptr, 0, 1, 0};
     {  // S2: QKV projection -> fp32 [T][Hq+2Hkv] (or pieces, added by qkv_post)
       const CUtensorMap *a[3] = {&m.wq, &m.wk, &m.wv};
       const int rows[3] = {Hq, Hkv, Hkv};
@@ -718,7 +810,7 @@ static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T,
       const int rows[3] = {H, 0, 0};
       if (!tp) {
         CKE(run_gemm(st, a, 1, rows, false, st->b_attn, T, Hq, EPI_RESID_F32, x, nullptr, H, 1, &gp_o));
-        CKE(launch_residual_rmsnorm(x, nullptr, 0, 0, gp_o, w.ln2, d.rms_eps, H, T, h, args, false, s, st->invariant));
+        CKE(launch_residual_rmsnorm(x, nullptr, 0, 0, gp_o, w.ln2, d.rms_eps, H, T, h, args, false, s, st->invariant, gp_o.n_src == 1));
       } else {  // this rank's partial over its heads -> all-reduce -> x += sum (two per layer)
         CKE(run_gemm(st, a, 1, rows, false, st->b_attn, T, Hq, EPI_F32, tp_part, nullptr, H));
         if (st->allreduce(tp_part, (size_t)T * H, st->allreduce_user, (void *)s) != 0) return cudaErrorLaunchFailure;
@@ -737,7 +829,7 @@ static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T,
       const void *next_ln = last ? nullptr : st->lw[l + 1].ln1;
       if (!tp) {
         CKE(run_gemm(st, a, 1, rows, false, st->b_a, T, F, EPI_RESID_F32, x, nullptr, H, 2, &gp_d));
-        CKE(launch_residual_rmsnorm(x, nullptr, 0, 0, gp_d, next_ln, d.rms_eps, H, T, h, args, last, s, st->invariant));
+        CKE(launch_residual_rmsnorm(x, nullptr, 0, 0, gp_d, next_ln, d.rms_eps, H, T, h, args, last, s, st->invariant, gp_d.n_src == 1));
       } else {
         CKE(run_gemm(st, a, 1, rows, false, st->b_a, T, F, EPI_F32, tp_part, nullptr, H));
         if (st->allreduce(tp_part, (size_t)T * H, st->allreduce_user, (void *)s) != 0) return cudaErrorLaunchFailure;
@@ -847,7 +939,9 @@ int ss_stage_decode(ss_stage *st, int batch, const void *hidden_bf16, const int3
   if ((rc = upload_args(st, a)) != SS_OK) return rc;
   if ((rc = debug_check(st, true, 0)) != SS_OK) return rc;
   const bool tail = out_logits || out_argmax;
-  if (!st->use_graph || st->allreduce) {  // a tensor-parallel shard calls back into the caller: never captured
+  const bool tp_callback = (st->allreduce || st->tp_size > 1) &&
+                           !(st->tp_size > 0 && batch <= 128 && st->ptab_ok[1] && st->ptab_ok[2] && 2 * st->n_sm <= TP_SLOTS);
+  if (!st->use_graph || tp_callback) {  // the all-reduce CALLBACK calls back into the caller: never captured
     const int64_t before = g_launches;
     cudaError_t e = enqueue_forward(st, true, batch, batch, tail);
     st->launches += g_launches - before;
@@ -868,6 +962,7 @@ int ss_stage_decode(ss_stage *st, int batch, const void *hidden_bf16, const int3
       if (graph) cudaGraphDestroy(graph);
       return cuda_fail(e != cudaSuccess ? e : e2, "decode graph capture");
     }
+    st->graph_captures += 1;
     Graph gr;
     e = cudaGraphInstantiate(&gr.exec, graph, 0);
     cudaGraphDestroy(graph);

@@ -434,6 +434,47 @@ def test_migration_is_bit_exact_in_batch_invariant_mode(shape):
         R.close()
 
 
+# odd groups and no grouping at all: the prefill attention pairs the q heads of a GQA group per CTA, an odd group leaves
+# its last head alone, MHA (G = 1) leaves every head alone
+G3 = synth.ModelShape("tiny-g3", 192, 3, 1, 64, 384, 2, 1e-5, 5e5, 0, 512)
+MHA = synth.ModelShape("tiny-mha-d128", 256, 2, 2, 128, 512, 2, 1e-6, 1e6, 1, 512)
+
+
+@pytest.mark.parametrize("shape,lens,first", [
+    (G3, [300, 1, 129, 64], [0, 0, 0, 0]),                       # odd group; 1-row tile; a tile boundary at 128 / 64
+    (MHA, [257, 128, 65], [0, 0, 0]),                            # MHA, d = 128, a 1-row last tile (257 = 2 x 128 + 1)
+    (synth.TINY128, [700, 33], [517, 20]),                       # chunk on top of a long prior context, unaligned start
+    (synth.TINY, [2100, 2049], [2000, 0]),                       # > 2,048 keys: 33 ring stages per tile, ring wrap-around
+])
+def test_prefill_attention_edge_shapes_vs_oracle(shape, lens, first):
+    """Edge cases of the tcgen05 prefill attention (two heads per CTA, 128-row query tiles, 64-key stages, lazy maximum,
+    dead rows of the last page zeroed): whole 2-layer stage vs the oracle, KV pages strict."""
+    lens, first = np.array(lens, dtype=np.int32), np.array(first, dtype=np.int32)
+    P, lens, pb, x = _problem(shape, seed=9, lens=lens, extra=4)
+    try:
+        bt = pb.block_tables
+        n = len(lens)
+        cu_full = np.concatenate([[0], np.cumsum(lens)]).astype(np.int32)
+        pool0 = hp.new_pool(shape, pb.n_pages_pool, P.L)
+        if first.any():   # prior context first (sequences with first == 0 take no part in that call)
+            keep = first > 0
+            rows1 = np.concatenate([np.arange(cu_full[s], cu_full[s] + first[s]) for s in range(n) if keep[s]])
+            w1, _, _ = hp.run_oracle_prefill(F32, shape, P.wb, pool0, first[keep], bt[keep], x[rows1])
+            g1 = P.prefill(first[keep], bt[keep], x[rows1])
+            assert hp.rel_err_rows(g1, w1) < STAGE_TOL
+        rows2 = np.concatenate([np.arange(cu_full[s] + first[s], cu_full[s + 1]) for s in range(n)])
+        w2, _, _ = hp.run_oracle_prefill(F32, shape, P.wb, pool0, lens, bt, x[rows2], ctx_before=first)
+        g2 = P.prefill(lens, bt, x[rows2], ctx_before=first)
+        err = hp.rel_err_rows(g2, w2)
+        print(f"{shape.name} lens {lens.tolist()} after {first.tolist()}: prefill rel err vs R0 {err:.3e}")
+        assert np.isfinite(g2).all() and err < STAGE_TOL
+        mask = _written_mask(pool0.shape, bt, lens)
+        pg = P.pool_bits()
+        assert (pg[~mask] == 0x7FC1).all() and (pg[mask] != 0x7FC1).all()
+    finally:
+        P.close()
+
+
 def test_chunked_prefill_and_mixed_batch_on_gpu():
     """Prior context (ctx_before > 0) and q_len = 1 rows in a prefill call (mixed iteration, reading A19)."""
     shape = synth.TINY_QWEN

@@ -52,3 +52,13 @@ def test_create_rejects_bad_arguments_before_touching_cuda():
     arr = (binding.ss_layer_weights * 2)()
     assert lib.ss_stage_create(C.byref(h), C.byref(d), 0, 2, arr, None, 1024, 1 << 20, 1024, 1 << 20, None) == -2
     assert lib.ss_kv_num_pages(None) == -1 and lib.ss_kv_alloc(None, 1, None) == -1
+
+
+def test_tp_exchange_buffer_size_is_host_only_arithmetic():
+    """ss_tp_xchg_bytes (fused tensor-parallel all-reduce): 2 buffers x D_TP source regions of 320 slots of 128 x 128 fp32,
+    plus one 128-byte counter line per (buffer, source); 0 for a degree outside 1..8."""
+    lib = binding.load_library()
+    for size in range(1, 9):
+        assert lib.ss_tp_xchg_bytes(size) == 2 * size * 320 * 128 * 128 * 4 + 2 * size * 128
+    assert lib.ss_tp_xchg_bytes(0) == 0 and lib.ss_tp_xchg_bytes(9) == 0 and lib.ss_tp_xchg_bytes(-1) == 0
+    assert lib.ss_stage_set_tp_fused(None, 0, 1, None) == -1 and lib.ss_stage_set_batch_invariant(None, 1) == -1
