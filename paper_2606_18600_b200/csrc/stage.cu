@@ -616,6 +616,11 @@ namespace ss {
 static bool tp_fused_ok(const ss_stage *st, int T, int grid) {
   return st->tp_size > 0 && T <= 128 && 2 * grid <= TP_SLOTS;
 }
+// ... and a call uses it only if BOTH its O and down projections will (the batch-invariant mode runs whole tiles, which
+// leave no pieces: it falls back to the all-reduce callback)
+static bool tp_fused_eligible(const ss_stage *st, int T) {
+  return st->tp_size > 0 && T <= 128 && !st->invariant && st->ptab_ok[1] && st->ptab_ok[2] && 2 * st->n_sm <= TP_SLOTS;
+}
 
 // `piece` (0 QKV, 1 O, 2 down; -1 none): if the planned launch allows it, the projection leaves its tiles in pieces
 // (EPI_PARTIAL) and *gp tells the consumer kernel where; otherwise gp->slots = null and `epi` is used as given.
@@ -701,7 +706,7 @@ static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T,
   cudaStream_t s = st->stream;
 
   // tensor-parallel shard: the fused exchange for decode-sized calls, else the caller's all-reduce callback
-  const bool fused = st->tp_size > 0 && T <= 128 && st->ptab_ok[1] && st->ptab_ok[2] && 2 * st->n_sm <= TP_SLOTS;
+  const bool fused = tp_fused_eligible(st, T);
   const bool tp = !fused && (st->allreduce != nullptr || st->tp_size > 1);
   if (tp && !st->allreduce) return cudaErrorNotSupported;  // a TP shard's large calls need ss_stage_set_allreduce
   float *tp_part = st->at<float>(c.tp_part);
@@ -939,8 +944,7 @@ int ss_stage_decode(ss_stage *st, int batch, const void *hidden_bf16, const int3
   if ((rc = upload_args(st, a)) != SS_OK) return rc;
   if ((rc = debug_check(st, true, 0)) != SS_OK) return rc;
   const bool tail = out_logits || out_argmax;
-  const bool tp_callback = (st->allreduce || st->tp_size > 1) &&
-                           !(st->tp_size > 0 && batch <= 128 && st->ptab_ok[1] && st->ptab_ok[2] && 2 * st->n_sm <= TP_SLOTS);
+  const bool tp_callback = (st->allreduce || st->tp_size > 1) && !tp_fused_eligible(st, batch);
   if (!st->use_graph || tp_callback) {  // the all-reduce CALLBACK calls back into the caller: never captured
     const int64_t before = g_launches;
     cudaError_t e = enqueue_forward(st, true, batch, batch, tail);
