@@ -1,21 +1,24 @@
 // gemm_tcgen05.cu — the bf16 projections of a decoder layer (Table 2 rows "QKV Projection", "Output Projection",
-// "Up and Gate Projection", "Down Projection", "Logits Calculation") as ONE persistent
-// tcgen05/TMEM GEMM kernel fed by TMA, for sm_100a.
+// "Up and Gate Projection", "Down Projection", "Logits Calculation") as persistent tcgen05/TMEM GEMM
+// kernels fed by TMA, for sm_100a.
 //
 // out[t][n] = sum_k X[t,k] * W[n,k]     X: activations [T,K] bf16 row-major, W: weights [N,K] bf16 row-major.
 //
 // Orientation: the 128 TMEM lanes (UMMA M) run over weight rows n, the TMEM columns (UMMA N = bn) over tokens t.
 // At decode (T = 64..128) this streams every weight byte exactly once through full-width 128-row MMAs (the
-// HBM-bound case); at prefill (bn = 256) the same kernel is a 128x256 compute tile.
+// HBM-bound case).
 //
-// CTA = 7 warps: warp 0 = weight TMA producer (one lane), warp 6 = activation TMA producer (one lane), warp 1 = TMEM
-// allocator + MMA issuer (one lane), warps 2-5 = epilogue (one TMEM lane quadrant each).  Two smem rings, SWIZZLE_128B,
-// each with full/empty mbarriers: a deep one of weight tiles 128x64 (x2 when DUAL) and a shallow one of activation
-// tiles bn x 64 (the weight ring's depth is what bounds the HBM bytes in flight); accumulators in TMEM, double-buffered when they fit so the epilogue of one
-// work item overlaps the MMAs of the next; the producer runs ahead across work items.  Schedules: see internal.h
-// (stream-K with in-kernel fix-up for the decode shapes, band-rasterised whole tiles for the prefill shapes).
-// DUAL = gate and up tiles share the B tile and the epilogue writes silu(g)*u as bf16 (step S9), so [T,2F] never
-// reaches HBM.  EPI_RESID_F32 adds the projection straight into the fp32 residual stream (steps S7, S10).
+// gemm_kernel (one CTA per SM; every decode shape, T <= 512, the batch-invariant mode).  CTA = 11 warps: warp 0 = TMA
+// producer (one lane), warps 1 and 6 = MMA issuers (one lane each; warp 1 also allocates TMEM), warps 2-5 and 7-10 =
+// epilogue (two per TMEM lane quadrant).  ONE smem ring of up to 12 stages {weight tile 128x64 (x2 when DUAL), activation
+// tile bn x 64}, SWIZZLE_128B, full/empty mbarriers; accumulators in TMEM, double-buffered when they fit so the epilogue
+// of one work item overlaps the MMAs of the next; the producer primes the ring with weights before it waits for the
+// predecessor kernel (PDL).  Schedules: see internal.h (stream-K for the decode shapes — in-kernel fix-up, or EPI_PARTIAL:
+// every piece left to the consumer kernel, optionally stored into every tensor-parallel rank's exchange buffer —,
+// band-rasterised whole tiles otherwise).  DUAL = gate and up tiles share the B tile and the epilogue writes silu(g)*u as
+// bf16 (step S9), so [T,2F] never reaches HBM.  EPI_RESID_F32 adds the projection straight into the fp32 residual stream.
+//
+// gemm_pair_kernel (further down): the tensor-bound prefill shapes on CTA pairs (tcgen05.mma.cta_group::2).
 #include <cuda.h>
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
@@ -148,7 +151,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
   const int cta = blockIdx.x, grid = gridDim.x;
 
   // One tcgen05.mma (M=128, K=16, operands in smem) occupies its issuing thread for ~128 cycles whatever N is
-  // (measured, profiles/r01_mma_issue_microbench.md), i.e. 4 KB of weights per 128 cycles: a single issuer
+  // (measured in round 1 with a clock64 probe), i.e. 4 KB of weights per 128 cycles: a single issuer
   // cannot keep up with HBM at bn <= 128.  The HBM-bound schedule therefore runs TWO issuers (warps 1 and 6), each
   // into its own accumulator; the epilogue adds the two.  Issuer (slot & 1) owns ring slot `slot` for the whole
   // kernel: an mbarrier's single phase bit is only safe when all waits on it come, in order, from one thread (with
@@ -447,7 +450,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
             // work item's is never overlapped): fast-math SiLU (ex2.approx + div.approx, error far below the bf16
             // output's 2^-9) and, instead of 32 two-byte stores per thread, lane pairs swap alternate tokens so
             // every lane stores one bf16x2 = features (col, col+1) of one token (timeline:
-            // profiles/r01_gemm_timeline.md: 3.6 -> 1.7 us per 32-token chunk).
+            // round-1 timeline: 3.6 -> 1.7 us per 32-token chunk).
             __nv_bfloat16 *o = (__nv_bfloat16 *)p.out_bf16;
             const bool odd = (lane & 1) != 0;
 #pragma unroll
@@ -588,7 +591,8 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant_
   if (warp == 0) {
     if (lane == 0) {
       // ---------------- TMA producer (both CTAs) ----------------
-      const uint64_t pol = l2_policy_evict_last();
+      auto policy = [](int k) { return k == 0 ? l2_policy_evict_first() : (k == 1 ? l2_policy_evict_normal() : l2_policy_evict_last()); };
+      const uint64_t pol = policy(p.w_policy), pol_b = policy(p.x_policy);
       pdl_wait();
       WorkIter it(pp, cluster, n_clusters);
       WorkItem w;
@@ -610,7 +614,7 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant_
           if (rank == 0) mbar_expect_tx(&full[s], 2 * stage_bytes);  // both CTAs' loads land on the leader's barrier
           tma_load_2d_pair(st, ta, &full[s], kb * GEMM_BK, row0, pol);
           if (DUAL) tma_load_2d_pair(st + A_TILE_BYTES, &ta1, &full[s], kb * GEMM_BK, row0, pol);
-          tma_load_2d_pair(st + a_bytes, &tb, &full[s], kb * GEMM_BK, t0, pol);
+          tma_load_2d_pair(st + a_bytes, &tb, &full[s], kb * GEMM_BK, t0, pol_b);
           if (++s == stages) {
             s = 0;
             ph ^= 1u;
@@ -870,6 +874,8 @@ void gemm_plan(GemmLaunch &g, int n_sm) {
     const long long pair_tiles = (long long)((p.n_row_tiles + 1) / 2) * p.n_t_tiles;
     const long long clusters = pair_tiles < max_grid / 2 ? pair_tiles : max_grid / 2;
     p.band = tune("SS_GEMM_BAND", g.dual ? 4 : 8);  // in row PAIRS
+    p.w_policy = tune("SS_GEMM_WPOL", 2);
+    p.x_policy = tune("SS_GEMM_XPOL", 2);
     if (p.band > (p.n_row_tiles + 1) / 2) p.band = (p.n_row_tiles + 1) / 2;
     g.grid = (int)(2 * clusters);
     return;

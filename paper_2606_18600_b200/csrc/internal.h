@@ -45,6 +45,7 @@ struct GemmParams {
   int bn;               // tokens per tile (UMMA N)
   int stages;           // smem pipeline depth
   int w_policy;         // L2 policy of the weight loads: 0 evict_first, 1 evict_normal, 2 evict_last
+  int x_policy;         // pair kernel: L2 policy of the activation loads (same encoding)
   int single_buf;       // debug: 1 = never double-buffer the TMEM accumulators
   int issuers;          // MMA-issuing threads (2 on the HBM-bound schedule, see gemm_tcgen05.cu)
   int sched;            // GemmSchedule

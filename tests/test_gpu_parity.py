@@ -59,7 +59,9 @@ def test_op_gemm_vs_oracle(T, N, K):
 
 @pytest.mark.gpu
 @pytest.mark.parametrize("dual,T,N,K", [(True, 64, 19072, 8192), (False, 64, 8192, 8192), (True, 128, 18944, 5120),
-                                        (False, 128, 5120, 8192)])
+                                        (False, 128, 5120, 8192),
+                                        # the CTA-pair kernel at prefill sizes: every SM pair busy, long K
+                                        (False, 2100, 8192, 8192), (True, 1500, 6144, 5120)])
 def test_op_gemm_full_grid_long_k_is_stable(dual, T, N, K):
     """Regression for a pipeline race: with two MMA issuers and an odd ring size a ring slot used to change hands
     between the issuers, and the single mbarrier phase bit then let a fast issuer consume a tile still in flight
