@@ -117,7 +117,7 @@ __device__ __forceinline__ float2 gemm_partial_sum2(const GemmPartials &gp, int 
 // loads are issued before any use, and x is read and written exactly once.
 // Few rows (decode): 1024 threads per row for latency.  Many rows (prefill): 256 threads per row, so 8 rows are in
 // flight per SM and the block reduction is two warps deep instead of 32.
-template <int IT, int RN_THREADS>
+template <int IT, int RN_THREADS, bool PARTS>  // PARTS = false: nothing to add to x (no partial sums, no stream-K pieces)
 __global__ void __launch_bounds__(RN_THREADS)
 residual_rmsnorm_kernel(float *__restrict__ x, const float *__restrict__ part, int splits, long long split_stride,
                         const GemmPartials gp, const __nv_bfloat16 *__restrict__ w, float eps, int H,
@@ -130,41 +130,50 @@ residual_rmsnorm_kernel(float *__restrict__ x, const float *__restrict__ part, i
   const float *pr = part + (size_t)t * H;
   __nv_bfloat16 *outp = nullptr;
   if (write_out && args->out_hidden) outp = (__nv_bfloat16 *)args->out_hidden + (size_t)t * H;
-  float4 v[IT], y[IT];
+  float4 v[IT];
 #pragma unroll
   for (int i = 0; i < IT; ++i) {
     const int j = (i * RN_THREADS + threadIdx.x) * 4;
-    v[i] = y[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (j < H) {
-      v[i] = *reinterpret_cast<const float4 *>(xr + j);
-      if (splits > 0) y[i] = *reinterpret_cast<const float4 *>(pr + j);
-    }
+    v[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (j < H) v[i] = *reinterpret_cast<const float4 *>(xr + j);
   }
-  if (gp.slots) {
-    // the projection left its tiles in pieces (EPI_PARTIAL, internal.h): y = the tile's pieces added in CTA order
+  if constexpr (PARTS) {
+    float4 y[IT];
 #pragma unroll
     for (int i = 0; i < IT; ++i) {
       const int j = (i * RN_THREADS + threadIdx.x) * 4;
-      if (j < H) y[i] = gemm_partial_sum4(gp, j >> 7, t, j & 127);
+      y[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (j < H && splits > 0) y[i] = *reinterpret_cast<const float4 *>(pr + j);
     }
-  }
-  for (int s = 1; s < splits; ++s) {
+    if (gp.slots) {
+      // the projection left its tiles in pieces (EPI_PARTIAL, internal.h): y = the tile's pieces added in CTA order
 #pragma unroll
-    for (int i = 0; i < IT; ++i) {
-      const int j = (i * RN_THREADS + threadIdx.x) * 4;
-      if (j < H) {
-        const float4 q = *reinterpret_cast<const float4 *>(pr + (size_t)s * split_stride + j);
-        y[i].x += q.x; y[i].y += q.y; y[i].z += q.z; y[i].w += q.w;
+      for (int i = 0; i < IT; ++i) {
+        const int j = (i * RN_THREADS + threadIdx.x) * 4;
+        if (j < H) y[i] = gemm_partial_sum4(gp, j >> 7, t, j & 127);
       }
+    }
+    for (int s = 1; s < splits; ++s) {
+#pragma unroll
+      for (int i = 0; i < IT; ++i) {
+        const int j = (i * RN_THREADS + threadIdx.x) * 4;
+        if (j < H) {
+          const float4 q = *reinterpret_cast<const float4 *>(pr + (size_t)s * split_stride + j);
+          y[i].x += q.x; y[i].y += q.y; y[i].z += q.z; y[i].w += q.w;
+        }
+      }
+    }
+#pragma unroll
+    for (int i = 0; i < IT; ++i) {
+      v[i].x += y[i].x; v[i].y += y[i].y; v[i].z += y[i].z; v[i].w += y[i].w;
     }
   }
   float ss = 0.f;
 #pragma unroll
   for (int i = 0; i < IT; ++i) {
     const int j = (i * RN_THREADS + threadIdx.x) * 4;
-    v[i].x += y[i].x; v[i].y += y[i].y; v[i].z += y[i].z; v[i].w += y[i].w;
     if (j < H) {
-      if (splits > 0 || gp.slots) *reinterpret_cast<float4 *>(xr + j) = v[i];  // otherwise x already holds the sum
+      if (PARTS) *reinterpret_cast<float4 *>(xr + j) = v[i];  // otherwise x already holds the sum
       ss += v[i].x * v[i].x + v[i].y * v[i].y + v[i].z * v[i].z + v[i].w * v[i].w;
       if (outp) {
         uint2 o;
@@ -196,20 +205,23 @@ cudaError_t launch_residual_rmsnorm(float *x, const float *part, int splits, lon
   const __nv_bfloat16 *w = (const __nv_bfloat16 *)ln_w;
   __nv_bfloat16 *hh = (__nv_bfloat16 *)h;
   const int wo = write_out_hidden ? 1 : 0;
+  const bool parts = splits > 0 || gp.slots != nullptr;
   auto go = [&](auto kernel, int threads) {
     return launch_pdl_if(pdl, kernel, dim3(T), dim3(threads), 0, s, x, part, splits, split_stride, gp, w, eps, H, hh, args, wo);
   };
+#define SS_RN(IT, TH) (parts ? go(residual_rmsnorm_kernel<IT, TH, true>, TH) : go(residual_rmsnorm_kernel<IT, TH, false>, TH))
   if (!fixed_shape && T >= 512 && H <= 16 * 256 * 4) {  // many rows: 256 threads each
     const int it = (H + 1023) / 1024;
-    if (it <= 2) return go(residual_rmsnorm_kernel<2, 256>, 256);
-    if (it <= 4) return go(residual_rmsnorm_kernel<4, 256>, 256);
-    if (it <= 8) return go(residual_rmsnorm_kernel<8, 256>, 256);
-    return go(residual_rmsnorm_kernel<16, 256>, 256);
+    if (it <= 2) return SS_RN(2, 256);
+    if (it <= 4) return SS_RN(4, 256);
+    if (it <= 8) return SS_RN(8, 256);
+    return SS_RN(16, 256);
   }
   const int it = (H + 4095) / 4096;
-  if (it <= 1) return go(residual_rmsnorm_kernel<1, 1024>, 1024);
-  if (it <= 2) return go(residual_rmsnorm_kernel<2, 1024>, 1024);
-  if (it <= 4) return go(residual_rmsnorm_kernel<4, 1024>, 1024);
+  if (it <= 1) return SS_RN(1, 1024);
+  if (it <= 2) return SS_RN(2, 1024);
+  if (it <= 4) return SS_RN(4, 1024);
+#undef SS_RN
   return cudaErrorInvalidValue;  // hidden > 16384 is rejected at create
 }
 
