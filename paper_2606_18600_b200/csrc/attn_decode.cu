@@ -158,7 +158,7 @@ decode_attn_kernel(const __grid_constant__ CUtensorMap kv_map, const DecodeAttnP
   const uint64_t pol = l2_policy_evict_first();  // every K/V byte is read once per step
   const int v_row0 = p.n_pages * n_kv * 16;
   auto issue_load = [&](const Cursor &c, int slot) {
-    if (lane == 0) {
+    if (elect_one()) {  // (not `lane == 0`: only under elect does nvcc issue UTMALDG straight from uniform registers)
       const int page = bt[(per_pair ? (size_t)0 : (size_t)c.b * max_blocks) + c.pg];
       const int row = (page * n_kv + c.h) * 16;
       uint8_t *kd = ring + (size_t)slot * 2 * PAGE_BYTES;

@@ -10,12 +10,14 @@
 //               over the S tile it came from; V tile in smem as TMA wrote it ([key][d]: the MN-major B operand)
 // CTA = the same 128 query positions of TWO q heads of one GQA group ("tile A", "tile B": they attend the same keys, so
 // one K/V ring serves both and every K/V byte fetched from L2 feeds 256 query rows); 12 warps, one role each:
-//   warp 0      TMA producer: both Q tiles once, then per key tile 4 pages of K and of V (16 tokens x d, one 2-D box per
-//               64 columns; the layer's pool is one 2-D tensor) into a 5-stage ring
-//   warps 1, 2  issue the S MMAs of tile A / tile B (one lane each) into DOUBLE-buffered S tiles, so S_{j+1} is computed
-//               while tile j is in softmax
-//   warp 3      issues the P.V MMAs of both tiles (separate issuing threads because one tcgen05.mma occupies its issuer
-//               ~128 cycles whatever its shape)
+//   warps 0, 3  TMA producers of K and of V: both Q tiles once (warp 0), then per key tile 4 pages (16 tokens x d, one 2-D
+//               box per 64 columns; the layer's pool is one 2-D tensor) into a 5-stage ring.  Two threads because one
+//               cp.async.bulk.tensor occupies its issuer ~100 cycles (clock64 stamps: 16 boxes per stage = 1,650 cycles)
+//   warps 1, 2  issue ALL MMAs of tile A / tile B (one lane each): S_j into DOUBLE-buffered S tiles, then P.V of stage
+//               j - 1, so S_j is computed while tile j - 1 is in softmax.  One thread per tile because one tcgen05.mma
+//               occupies its issuer 75-150 cycles whatever its shape (a single P.V thread for both tiles was busy
+//               ~2,000 cycles per stage); the MMAs of one thread execute in issue order, so S_j cannot overtake the
+//               P.V_{j-2} that still reads the P stored over that S buffer
 //   warps 4-7 / 8-11  softmax of tile A / B: thread = query row = TMEM lane, so row max / row sum need no shuffle;
 //               tcgen05.ld of the S row, exp2 in fp32, P -> bf16 -> tcgen05.st; the running maximum is only moved when it
 //               grows by more than 2^8 (then, rarely, the O accumulator is rescaled in place), else P simply is up to
@@ -142,7 +144,7 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap q_map, const __grid_cons
     for (int i = 0; i < TA_STAGES; ++i) {
       mbar_init(&k_full[i], 1);
       mbar_init(&v_full[i], 1);
-      mbar_init(&kv_empty[i], 3);  // the two S issuers' and the P.V issuer's commits
+      mbar_init(&kv_empty[i], 2);  // one commit per tile's MMA-issuing thread, after its P.V of the stage
     }
     for (int i = 0; i < 4; ++i) {
       mbar_init(&s_full[i], 1);
@@ -174,91 +176,87 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap q_map, const __grid_cons
   const int n_pages_seq = (kv_len + 15) >> 4;
   const CallArgs *args = p.args;
 
-  if (warp == 0) {
-    if (lane == 0 && live) {
-      // ---------------- TMA producer ----------------
+  if (warp == 0 || warp == 3) {
+    if (live) {
+      // ---------------- TMA producers: warp 0 = Q and K, warp 3 = V ----------------
+      const bool is_k = warp == 0;
       const uint64_t pol_q = l2_policy_evict_first(), pol_kv = l2_policy_evict_last();  // K/V: re-read by other tiles
-      mbar_expect_tx(q_full, (has_b ? 2u : 1u) * QTILE_BYTES);
-      for (int t = 0; t < (has_b ? 2 : 1); ++t)
+      if (is_k && elect_one()) {
+        mbar_expect_tx(q_full, (has_b ? 2u : 1u) * QTILE_BYTES);
+        for (int t = 0; t < (has_b ? 2 : 1); ++t)
 #pragma unroll
-        for (int h = 0; h < NH; ++h)
-          tma_load_2d(q_s + t * QTILE_BYTES + h * QHALF_BYTES, &q_map, q_full, (head_a + t) * D + h * 64, row0, pol_q);
+          for (int h = 0; h < NH; ++h)
+            tma_load_2d(q_s + t * QTILE_BYTES + h * QHALF_BYTES, &q_map, q_full, (head_a + t) * D + h * 64, row0, pol_q);
+      }
       const int32_t *bt = args->block_tables + (size_t)s * args->max_blocks;
-      const int v_row0 = p.n_pages * p.n_kv * 16;
+      const int row_off = is_k ? 0 : p.n_pages * p.n_kv * 16;   // the V rows follow the K rows in the layer's tensor
+      uint8_t *ring = is_k ? k_s : v_s;
+      uint64_t *full = is_k ? k_full : v_full;
       for (int j = 0; j < n_kt; ++j) {
         const int st = j % TA_STAGES;
-        mbar_wait(&kv_empty[st], (((uint32_t)(j / TA_STAGES)) & 1u) ^ 1u);
         const int n_pg = min(TA_PAGES, n_pages_seq - j * TA_PAGES);  // pages past the sequence's end are never touched
-        uint8_t *kd = k_s + (size_t)st * TILE_BYTES, *vd = v_s + (size_t)st * TILE_BYTES;
-        mbar_expect_tx(&k_full[st], (uint32_t)n_pg * NH * 2048u);
-        mbar_expect_tx(&v_full[st], (uint32_t)n_pg * NH * 2048u);
         int rowv[TA_PAGES];
 #pragma unroll
         for (int pg = 0; pg < TA_PAGES; ++pg)
-          rowv[pg] = pg < n_pg ? (bt[j * TA_PAGES + pg] * p.n_kv + hk) * 16 : 0;
+          rowv[pg] = pg < n_pg ? (bt[j * TA_PAGES + pg] * p.n_kv + hk) * 16 + row_off : 0;
+        mbar_wait(&kv_empty[st], (((uint32_t)(j / TA_STAGES)) & 1u) ^ 1u);
+        uint8_t *dst = ring + (size_t)st * TILE_BYTES;
+        if (elect_one()) {
+          mbar_expect_tx(&full[st], (uint32_t)n_pg * NH * 2048u);
 #pragma unroll
-        for (int pg = 0; pg < TA_PAGES; ++pg)
-          if (pg < n_pg) {
+          for (int pg = 0; pg < TA_PAGES; ++pg)
+            if (pg < n_pg) {
 #pragma unroll
-            for (int h = 0; h < NH; ++h)
-              tma_load_2d(kd + h * HALF_BYTES + pg * 2048, &kv_map, &k_full[st], h * 64, rowv[pg], pol_kv);
-          }
-#pragma unroll
-        for (int pg = 0; pg < TA_PAGES; ++pg)
-          if (pg < n_pg) {
-#pragma unroll
-            for (int h = 0; h < NH; ++h)
-              tma_load_2d(vd + h * HALF_BYTES + pg * 2048, &kv_map, &v_full[st], h * 64, v_row0 + rowv[pg], pol_kv);
-          }
+              for (int h = 0; h < NH; ++h)
+                tma_load_2d(dst + h * HALF_BYTES + pg * 2048, &kv_map, &full[st], h * 64, rowv[pg], pol_kv);
+            }
+        }
+        __syncwarp();
       }
     }
   } else if (warp == 1 || warp == 2) {
-    if (lane == 0 && live) {
-      // ---------------- S = Q K^T issuer of tile t ----------------
+    if (live) {
+      // ---------------- MMA issuer of tile t: S_j, then P.V_{j-1} ----------------
       const int t = warp - 1;
       const bool on = t == 0 || has_b;
-      const uint32_t idesc = umma_idesc_bf16(TA_BM, TA_BN);
+      const uint32_t idesc_s = umma_idesc_bf16(TA_BM, TA_BN), idesc_pv = umma_idesc_bf16_b_mn(TA_BM, D);
       if (on) mbar_wait(q_full, 0);
-      for (int j = 0; j < n_kt; ++j) {
-        const int st = j % TA_STAGES, b = j & 1;
-        if (on && j >= 2) mbar_wait(&pv_done[t * 2 + b], ((uint32_t)((j - 2) >> 1)) & 1u);  // P_{j-2} (in this S buffer) consumed
-        mbar_wait(&k_full[st], ((uint32_t)(j / TA_STAGES)) & 1u);
-        if (on) {
-          tc_fence_after();
-          const uint32_t qa = smem_u32(q_s + t * QTILE_BYTES), ka = smem_u32(k_s + (size_t)st * TILE_BYTES);
-          const uint32_t acc = tmem_base + (uint32_t)(t * 2 + b) * S_COLS;
+      for (int j = 0; j <= n_kt; ++j) {
+        if (j < n_kt) {
+          const int st = j % TA_STAGES, b = j & 1;
+          mbar_wait(&k_full[st], ((uint32_t)(j / TA_STAGES)) & 1u);
+          if (on && elect_one()) {
+            // (S buffer b still holds P_{j-2}: P.V_{j-2} was issued by this thread before, and executes before this)
+            tc_fence_after();
+            const uint32_t qa = smem_u32(q_s + t * QTILE_BYTES), ka = smem_u32(k_s + (size_t)st * TILE_BYTES);
+            const uint32_t acc = tmem_base + (uint32_t)(t * 2 + b) * S_COLS;
 #pragma unroll
-          for (int ks = 0; ks < D / 16; ++ks) {
-            const uint32_t in_row = (uint32_t)(ks & 3) * 32u;
-            umma_bf16(acc, umma_desc_k_sw128(qa + (uint32_t)(ks >> 2) * QHALF_BYTES + in_row),
-                      umma_desc_k_sw128(ka + (uint32_t)(ks >> 2) * HALF_BYTES + in_row), idesc, ks > 0 ? 1u : 0u);
+            for (int ks = 0; ks < D / 16; ++ks) {
+              const uint32_t in_row = (uint32_t)(ks & 3) * 32u;
+              umma_bf16(acc, umma_desc_k_sw128(qa + (uint32_t)(ks >> 2) * QHALF_BYTES + in_row),
+                        umma_desc_k_sw128(ka + (uint32_t)(ks >> 2) * HALF_BYTES + in_row), idesc_s, ks > 0 ? 1u : 0u);
+            }
+            umma_commit(&s_full[t * 2 + b]);
           }
-          umma_commit(&s_full[t * 2 + b]);
         }
-        umma_commit(&kv_empty[st]);  // (an absent tile B releases the stage as soon as it has landed)
+        if (j >= 1) {
+          const int i = j - 1, st = i % TA_STAGES, b = i & 1;
+          const int n_pg = min(TA_PAGES, n_pages_seq - i * TA_PAGES);  // one k-step = one page of 16 keys
+          if (on) mbar_wait(&p_full[t * 2 + b], ((uint32_t)(i >> 1)) & 1u);
+          mbar_wait(&v_full[st], ((uint32_t)(i / TA_STAGES)) & 1u);
+          if (on && elect_one()) {
+            tc_fence_after();
+            const uint32_t va = smem_u32(v_s + (size_t)st * TILE_BYTES);
+            for (int ks = 0; ks < n_pg; ++ks)
+              umma_bf16_ts(tmem_base + O_COL + (uint32_t)t * D, tmem_base + (uint32_t)(t * 2 + b) * S_COLS + (uint32_t)ks * 8u,
+                           umma_desc_mn_sw128(va + (uint32_t)ks * 2048u, HALF_BYTES, 1024u), idesc_pv, (i > 0 || ks > 0) ? 1u : 0u);
+            umma_commit(&pv_done[t * 2 + b]);
+          }
+          if (elect_one()) umma_commit(&kv_empty[st]);  // this thread's S_i and P.V_i have read the stage (an absent tile B: at once)
+        }
       }
     }
-  } else if (warp == 3) {
-    if (lane == 0 && live) {
-      // ---------------- O += P V issuer (both tiles) ----------------
-      const uint32_t idesc = umma_idesc_bf16_b_mn(TA_BM, D);
-      for (int j = 0; j < n_kt; ++j) {
-        const int st = j % TA_STAGES, b = j & 1;
-        const uint32_t va = smem_u32(v_s + (size_t)st * TILE_BYTES);
-        const int n_pg = min(TA_PAGES, n_pages_seq - j * TA_PAGES);  // one k-step = one page of 16 keys
-        for (int t = 0; t < (has_b ? 2 : 1); ++t) {
-          mbar_wait(&p_full[t * 2 + b], ((uint32_t)(j >> 1)) & 1u);
-          if (t == 0) mbar_wait(&v_full[st], ((uint32_t)(j / TA_STAGES)) & 1u);
-          tc_fence_after();
-          for (int ks = 0; ks < n_pg; ++ks)
-            umma_bf16_ts(tmem_base + O_COL + (uint32_t)t * D, tmem_base + (uint32_t)(t * 2 + b) * S_COLS + (uint32_t)ks * 8u,
-                         umma_desc_mn_sw128(va + (uint32_t)ks * 2048u, HALF_BYTES, 1024u), idesc, (j > 0 || ks > 0) ? 1u : 0u);
-          umma_commit(&pv_done[t * 2 + b]);
-        }
-        umma_commit(&kv_empty[st]);
-      }
-    }
-  } else if (live && (warp < 8 || has_b)) {
+  } else if (warp >= 4 && live && (warp < 8 || has_b)) {
     // ---------------- softmax of tile t: thread = query row ----------------
     const int t = warp >= 8 ? 1 : 0;
     const int quad = warp & 3;
@@ -321,10 +319,10 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap q_map, const __grid_cons
       }
       l_run += (rs4[0] + rs4[1]) + (rs4[2] + rs4[3]);
       tmem_st_32x32(s_addr, pk);
-      if (t == 0 && j == n_kt - 1 && (kv_len & 15) != 0) {
+      if (j == n_kt - 1 && (kv_len & 15) != 0) {
         // the sequence's last page holds slots past its end with whatever the pool held: zero those V rows so that
         // 0 * garbage (possibly NaN) cannot reach the output (their P is exactly 0: the causal mask covers them).
-        // Done by tile A's warps before they publish P_A; the P.V issuer takes tile A first.
+        // Done by BOTH tiles' warps (the same zeros), each before it publishes its own P to its own issuer.
         mbar_wait(&v_full[st], ((uint32_t)(j / TA_STAGES)) & 1u);
         const int k0 = kv_len - jbase, k1 = (n_pages_seq - j * TA_PAGES) * 16;  // rows [k0, k1) of the tile
         uint8_t *vd = v_s + (size_t)st * TILE_BYTES;

@@ -188,8 +188,12 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
   const uint32_t tmem_base = *tmem_slot;
   if (threadIdx.x == 0) trace(p, 7);
 
+  // The single-thread roles run their loops on the WHOLE warp (uniform control flow: every lane waits on the barriers
+  // and walks the same items) and issue under elect_one(): under `if (lane == 0)` nvcc cannot keep the TMA / MMA operands
+  // in uniform registers and wraps every UTMALDG / UTCHMMA in an ELECT + 5 x R2UR.BROADCAST + BRA.U.ANY loop, which is
+  // what made one issue cost ~100-130 cycles whatever its shape.
   if (warp == 0) {
-    if (lane == 0) {
+    {
       // ---------------- TMA producer ----------------
       // Weights are never written by the stage, so the first `stages` weight tiles are requested BEFORE waiting for
       // the predecessor kernel (PDL): the ring is full of weights by the time the activations exist.
@@ -219,19 +223,23 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
           if (!waited && n == stages) {  // ring primed with weights: now the activations of those k-blocks
             pdl_wait();
             waited = true;
-            for (int i = 0; i < stages; ++i)
-              tma_load_2d(base + (size_t)i * stage_bytes + a_bytes, &tb, &full[i], pend_kb[i] * GEMM_BK, pend_t0[i],
-                          pol_x);
+            if (elect_one())
+              for (int i = 0; i < stages; ++i)
+                tma_load_2d(base + (size_t)i * stage_bytes + a_bytes, &tb, &full[i], pend_kb[i] * GEMM_BK, pend_t0[i],
+                            pol_x);
+            __syncwarp();
           }
           mbar_wait_site(&empty[s], ph ^ 1u, 1, (uint32_t)s);
           uint8_t *st = base + (size_t)s * stage_bytes;
-          mbar_expect_tx(&full[s], stage_bytes);
-          tma_load_2d(st, ta, &full[s], kb * GEMM_BK, row0, pol_w);
-          if (n == 0) trace(p, 8);
-          if (DUAL) tma_load_2d(st + A_TILE_BYTES, &ta1, &full[s], kb * GEMM_BK, row0, pol_w);
-          if (waited) {
-            tma_load_2d(st + a_bytes, &tb, &full[s], kb * GEMM_BK, t0, pol_x);
-          } else {
+          if (elect_one()) {
+            mbar_expect_tx(&full[s], stage_bytes);
+            tma_load_2d(st, ta, &full[s], kb * GEMM_BK, row0, pol_w);
+            if (n == 0) trace(p, 8);
+            if (DUAL) tma_load_2d(st + A_TILE_BYTES, &ta1, &full[s], kb * GEMM_BK, row0, pol_w);
+            if (waited) tma_load_2d(st + a_bytes, &tb, &full[s], kb * GEMM_BK, t0, pol_x);
+          }
+          __syncwarp();
+          if (!waited) {
             pend_kb[n] = kb;
             pend_t0[n] = t0;
             ++n;
@@ -244,13 +252,14 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
       }
       if (!waited) {  // fewer k-blocks than stages
         pdl_wait();
-        for (int i = 0; i < n; ++i)
-          tma_load_2d(base + (size_t)i * stage_bytes + a_bytes, &tb, &full[i], pend_kb[i] * GEMM_BK, pend_t0[i], pol_x);
+        if (elect_one())
+          for (int i = 0; i < n; ++i)
+            tma_load_2d(base + (size_t)i * stage_bytes + a_bytes, &tb, &full[i], pend_kb[i] * GEMM_BK, pend_t0[i], pol_x);
       }
     }
   } else if (warp == 1 || warp == 6) {
     const int me = warp == 1 ? 0 : 1;
-    if (lane == 0 && me < n_iss) {
+    if (me < n_iss) {
       // ---------------- MMA issuer `me` ----------------
       // the k-blocks in ring slots s = me (mod n_iss), into this issuer's own accumulator
       const uint32_t idesc = umma_idesc_bf16(GEMM_BM, (uint32_t)bn);
@@ -277,23 +286,29 @@ gemm_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant__ CUt
           }
           if (((uint32_t)s & iss_mask) != my_slots) continue;  // a slot always belongs to the same issuer
           mbar_wait_site(&full[s], ph, 4 + me, n);
-          if (n == 0) trace(p, 2);
+          if (n == 0 && lane == 0) trace(p, 2);
           tc_fence_after();
           const uint32_t st = smem_u32(base + (size_t)s * stage_bytes);
           const uint64_t da = umma_desc_k_sw128(st);
           const uint64_t da1 = umma_desc_k_sw128(st + A_TILE_BYTES);
           const uint64_t db = umma_desc_k_sw128(st + a_bytes);
+          if (elect_one()) {
 #pragma unroll
-          for (int k = 0; k < GEMM_BK / 16; ++k) {
-            const uint32_t acc = (!first || k > 0) ? 1u : 0u;
-            umma_bf16(acc_addr, da + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc, acc);
-            if (DUAL) umma_bf16(acc_addr + (uint32_t)bn, da1 + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc, acc);
+            for (int k = 0; k < GEMM_BK / 16; ++k) {
+              const uint32_t acc = (!first || k > 0) ? 1u : 0u;
+              umma_bf16(acc_addr, da + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc, acc);
+              if (DUAL) umma_bf16(acc_addr + (uint32_t)bn, da1 + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc, acc);
+            }
+            umma_commit(&empty[s]);  // frees the smem slot when these MMAs have read it
           }
+          __syncwarp();
           first = false;
-          umma_commit(&empty[s]);  // frees the smem slot when these MMAs have read it
         }
-        umma_commit(&tfull[buf]);  // arrives at once if this issuer had no k-block in the item
-        if (me == 0) trace(p, 3 + 4 * (int)item);
+        if (elect_one()) {
+          umma_commit(&tfull[buf]);  // arrives at once if this issuer had no k-block in the item
+          if (me == 0) trace(p, 3 + 4 * (int)item);
+        }
+        __syncwarp();
         ++item;
       }
     }
@@ -589,8 +604,8 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant_
   pp.sched = SCHED_TILES;
 
   if (warp == 0) {
-    if (lane == 0) {
-      // ---------------- TMA producer (both CTAs) ----------------
+    {
+      // ---------------- TMA producer (both CTAs; whole warp, issue under elect_one: see gemm_kernel) ----------------
       auto policy = [](int k) { return k == 0 ? l2_policy_evict_first() : (k == 1 ? l2_policy_evict_normal() : l2_policy_evict_last()); };
       const uint64_t pol = policy(p.w_policy), pol_b = policy(p.x_policy);
       pdl_wait();
@@ -611,10 +626,13 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant_
         for (int kb = w.kb0; kb < w.kb1; ++kb) {
           mbar_wait_site(&empty[s], ph ^ 1u, 1, (uint32_t)s);
           uint8_t *st = base + (size_t)s * stage_bytes;
-          if (rank == 0) mbar_expect_tx(&full[s], 2 * stage_bytes);  // both CTAs' loads land on the leader's barrier
-          tma_load_2d_pair(st, ta, &full[s], kb * GEMM_BK, row0, pol);
-          if (DUAL) tma_load_2d_pair(st + A_TILE_BYTES, &ta1, &full[s], kb * GEMM_BK, row0, pol);
-          tma_load_2d_pair(st + a_bytes, &tb, &full[s], kb * GEMM_BK, t0, pol_b);
+          if (elect_one()) {
+            if (rank == 0) mbar_expect_tx(&full[s], 2 * stage_bytes);  // both CTAs' loads land on the leader's barrier
+            tma_load_2d_pair(st, ta, &full[s], kb * GEMM_BK, row0, pol);
+            if (DUAL) tma_load_2d_pair(st + A_TILE_BYTES, &ta1, &full[s], kb * GEMM_BK, row0, pol);
+            tma_load_2d_pair(st + a_bytes, &tb, &full[s], kb * GEMM_BK, t0, pol_b);
+          }
+          __syncwarp();
           if (++s == stages) {
             s = 0;
             ph ^= 1u;
@@ -623,7 +641,7 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant_
       }
     }
   } else if (warp == 1) {
-    if (lane == 0 && rank == 0) {
+    if (rank == 0) {
       // ---------------- MMA issuer (leader CTA, for the pair) ----------------
       const uint32_t idesc = umma_idesc_bf16(2 * GEMM_BM, PAIR_BN);
       WorkIter it(pp, cluster, n_clusters);
@@ -644,20 +662,24 @@ gemm_pair_kernel(const __grid_constant__ CUtensorMap ta0, const __grid_constant_
           const uint64_t da = umma_desc_k_sw128(st);
           const uint64_t da1 = umma_desc_k_sw128(st + A_TILE_BYTES);
           const uint64_t db = umma_desc_k_sw128(st + a_bytes);
+          if (elect_one()) {
 #pragma unroll
-          for (int k = 0; k < GEMM_BK / 16; ++k) {
-            const uint32_t acc = (!first || k > 0) ? 1u : 0u;
-            umma_bf16_pair(acc_addr, da + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc, acc);
-            if (DUAL) umma_bf16_pair(acc_addr + PAIR_BN, da1 + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc, acc);
+            for (int k = 0; k < GEMM_BK / 16; ++k) {
+              const uint32_t acc = (!first || k > 0) ? 1u : 0u;
+              umma_bf16_pair(acc_addr, da + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc, acc);
+              if (DUAL) umma_bf16_pair(acc_addr + PAIR_BN, da1 + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc, acc);
+            }
+            umma_commit_pair(&empty[ms]);  // frees the slot in BOTH CTAs when these MMAs have read it
           }
+          __syncwarp();
           first = false;
-          umma_commit_pair(&empty[ms]);  // frees the slot in BOTH CTAs when these MMAs have read it
           if (++ms == stages) {
             ms = 0;
             mph ^= 1u;
           }
         }
-        umma_commit_pair(&tfull[buf]);
+        if (elect_one()) umma_commit_pair(&tfull[buf]);
+        __syncwarp();
         ++item;
       }
     }
