@@ -129,11 +129,12 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap q_map, const __grid_cons
   uint8_t *k_s = q_s + 2 * QTILE_BYTES;                  // [TA_STAGES][TILE_BYTES]
   uint8_t *v_s = k_s + (size_t)TA_STAGES * TILE_BYTES;   // [TA_STAGES][TILE_BYTES]
   uint64_t *bars = (uint64_t *)(v_s + (size_t)TA_STAGES * TILE_BYTES);
-  uint64_t *q_full = bars;
-  uint64_t *k_full = bars + 1, *v_full = k_full + TA_STAGES, *kv_empty = v_full + TA_STAGES;
+  uint64_t *q_full = bars, *q_empty = bars + 1;
+  uint64_t *k_full = bars + 2, *v_full = k_full + TA_STAGES, *kv_empty = v_full + TA_STAGES;
   uint64_t *s_full = kv_empty + TA_STAGES;  // [tile][buffer]
   uint64_t *p_full = s_full + 4, *pv_done = p_full + 4;
-  uint32_t *tmem_slot = (uint32_t *)(pv_done + 4);
+  uint64_t *o_free = pv_done + 4;           // [tile]
+  uint32_t *tmem_slot = (uint32_t *)(o_free + 2);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   pdl_launch_dependents();
@@ -141,6 +142,7 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap q_map, const __grid_cons
     tma_prefetch_desc(&q_map);
     tma_prefetch_desc(&kv_map);
     mbar_init(q_full, 1);
+    mbar_init(q_empty, 2);         // one commit per issuing thread, after its last S of the item
     for (int i = 0; i < TA_STAGES; ++i) {
       mbar_init(&k_full[i], 1);
       mbar_init(&v_full[i], 1);
@@ -151,6 +153,8 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap q_map, const __grid_cons
       mbar_init(&p_full[i], 128);  // every softmax thread of the tile
       mbar_init(&pv_done[i], 1);
     }
+    mbar_init(&o_free[0], 128);    // every softmax thread has read its O row out of tensor memory
+    mbar_init(&o_free[1], 128);
     mbar_fence_init();
   }
   if (warp == 1) tmem_alloc_dyn(tmem_slot, TMEM_COLS);
@@ -160,46 +164,64 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap q_map, const __grid_cons
   const uint32_t tmem_base = *tmem_slot;
   pdl_wait();  // q, the pools and the plan are written by earlier kernels of this call
 
-  // ---- which tile pair: blockIdx.x = (kv head, pair of its q heads), blockIdx.y = launch slot of the query tile
-  const int G = p.n_q / p.n_kv, pairs = (G + 1) >> 1;
-  const int hk = blockIdx.x / pairs, pi = blockIdx.x - hk * pairs;
-  const int head_a = hk * G + 2 * pi;
-  const bool has_b = 2 * pi + 1 < G;   // an odd group leaves its last head alone
-  const bool live = (int)blockIdx.y < p.plan.tile_cum[p.n_seqs];
-  int row0 = 0, rows = 0, p0 = 0, s = 0;
-  if (live) {
-    const int4 d = reinterpret_cast<const int4 *>(p.plan.tile_desc)[blockIdx.y];
-    row0 = d.x; rows = d.y; p0 = d.z; s = d.w;
-  }
-  const int kv_len = p0 + rows;                       // keys 0..kv_len-1 are needed by this tile
-  const int n_kt = (kv_len + TA_BN - 1) / TA_BN;
-  const int n_pages_seq = (kv_len + 15) >> 4;
+  // ---- work items: (launch slot y of a query tile, heaviest first; x = (kv head, pair of its q heads)), dealt to the
+  // persistent CTAs in snake order (round r runs left to right, r + 1 right to left) so that the sums stay level.
+  // Every role walks the same list; all ring / buffer phases run on counters that continue across items:
+  //   g    key stages so far (K/V ring slot g % TA_STAGES)       gt  the same for tile t alone (S buffer gt & 1)
+  const int G = p.n_q / p.n_kv, pairs = (G + 1) >> 1, n_x = p.n_kv * pairs;
+  const int n_items = min(p.plan.tile_cum[p.n_seqs], p.max_tiles) * n_x;
   const CallArgs *args = p.args;
+  struct Item {
+    int row0, rows, p0, s, hk, head_a, n_kt, n_pages_seq, kv_len;
+    bool has_b;
+  };
+  auto get_item = [&](int k, Item &w) -> bool {
+    const int idx = k * (int)gridDim.x + ((k & 1) ? (int)gridDim.x - 1 - (int)blockIdx.x : (int)blockIdx.x);
+    if (idx >= n_items) return false;
+    const int y = idx / n_x, x = idx - y * n_x;
+    const int4 d = reinterpret_cast<const int4 *>(p.plan.tile_desc)[y];
+    w.row0 = d.x; w.rows = d.y; w.p0 = d.z; w.s = d.w;
+    w.hk = x / pairs;
+    const int pi = x - w.hk * pairs;
+    w.head_a = w.hk * G + 2 * pi;
+    w.has_b = 2 * pi + 1 < G;            // an odd group leaves its last head alone
+    w.kv_len = w.p0 + w.rows;            // keys 0..kv_len-1 are needed by this tile
+    w.n_kt = (w.kv_len + TA_BN - 1) / TA_BN;
+    w.n_pages_seq = (w.kv_len + 15) >> 4;
+    return true;
+  };
+  Item w;
 
+  // (whole-warp roles, issue under elect_one(): see gemm_tcgen05.cu)
   if (warp == 0 || warp == 3) {
-    if (live) {
-      // ---------------- TMA producers: warp 0 = Q and K, warp 3 = V ----------------
-      const bool is_k = warp == 0;
-      const uint64_t pol_q = l2_policy_evict_first(), pol_kv = l2_policy_evict_last();  // K/V: re-read by other tiles
-      if (is_k && elect_one()) {
-        mbar_expect_tx(q_full, (has_b ? 2u : 1u) * QTILE_BYTES);
-        for (int t = 0; t < (has_b ? 2 : 1); ++t)
+    // ---------------- TMA producers: warp 0 = Q and K, warp 3 = V ----------------
+    const bool is_k = warp == 0;
+    const uint64_t pol_q = l2_policy_evict_first(), pol_kv = l2_policy_evict_last();  // K/V: re-read by other tiles
+    const int row_off = is_k ? 0 : p.n_pages * p.n_kv * 16;   // the V rows follow the K rows in the layer's tensor
+    uint8_t *ring = is_k ? k_s : v_s;
+    uint64_t *full = is_k ? k_full : v_full;
+    uint32_t g = 0;
+    for (int k = 0; get_item(k, w); ++k) {
+      if (is_k) {
+        if (k > 0) mbar_wait(q_empty, (uint32_t)(k - 1) & 1u);  // the previous item's S MMAs have read its Q tiles
+        if (elect_one()) {
+          mbar_expect_tx(q_full, (w.has_b ? 2u : 1u) * QTILE_BYTES);
+          for (int t = 0; t < (w.has_b ? 2 : 1); ++t)
 #pragma unroll
-          for (int h = 0; h < NH; ++h)
-            tma_load_2d(q_s + t * QTILE_BYTES + h * QHALF_BYTES, &q_map, q_full, (head_a + t) * D + h * 64, row0, pol_q);
+            for (int h = 0; h < NH; ++h)
+              tma_load_2d(q_s + t * QTILE_BYTES + h * QHALF_BYTES, &q_map, q_full, (w.head_a + t) * D + h * 64, w.row0, pol_q);
+        }
+        __syncwarp();
       }
-      const int32_t *bt = args->block_tables + (size_t)s * args->max_blocks;
-      const int row_off = is_k ? 0 : p.n_pages * p.n_kv * 16;   // the V rows follow the K rows in the layer's tensor
-      uint8_t *ring = is_k ? k_s : v_s;
-      uint64_t *full = is_k ? k_full : v_full;
-      for (int j = 0; j < n_kt; ++j) {
-        const int st = j % TA_STAGES;
-        const int n_pg = min(TA_PAGES, n_pages_seq - j * TA_PAGES);  // pages past the sequence's end are never touched
+      const int32_t *bt = args->block_tables + (size_t)w.s * args->max_blocks;
+      for (int j = 0; j < w.n_kt; ++j, ++g) {
+        const int st = (int)(g % TA_STAGES);
+        const int n_pg = min(TA_PAGES, w.n_pages_seq - j * TA_PAGES);  // pages past the sequence's end are never touched
         int rowv[TA_PAGES];
 #pragma unroll
         for (int pg = 0; pg < TA_PAGES; ++pg)
-          rowv[pg] = pg < n_pg ? (bt[j * TA_PAGES + pg] * p.n_kv + hk) * 16 + row_off : 0;
-        mbar_wait(&kv_empty[st], (((uint32_t)(j / TA_STAGES)) & 1u) ^ 1u);
+          rowv[pg] = pg < n_pg ? (bt[j * TA_PAGES + pg] * p.n_kv + w.hk) * 16 + row_off : 0;
+        mbar_wait(&kv_empty[st], ((g / TA_STAGES) & 1u) ^ 1u);
         uint8_t *dst = ring + (size_t)st * TILE_BYTES;
         if (elect_one()) {
           mbar_expect_tx(&full[st], (uint32_t)n_pg * NH * 2048u);
@@ -215,18 +237,45 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap q_map, const __grid_cons
       }
     }
   } else if (warp == 1 || warp == 2) {
-    if (live) {
-      // ---------------- MMA issuer of tile t: S_j, then P.V_{j-1} ----------------
-      const int t = warp - 1;
-      const bool on = t == 0 || has_b;
-      const uint32_t idesc_s = umma_idesc_bf16(TA_BM, TA_BN), idesc_pv = umma_idesc_bf16_b_mn(TA_BM, D);
-      if (on) mbar_wait(q_full, 0);
-      for (int j = 0; j <= n_kt; ++j) {
-        if (j < n_kt) {
-          const int st = j % TA_STAGES, b = j & 1;
-          mbar_wait(&k_full[st], ((uint32_t)(j / TA_STAGES)) & 1u);
-          if (on && elect_one()) {
-            // (S buffer b still holds P_{j-2}: P.V_{j-2} was issued by this thread before, and executes before this)
+    // ---------------- MMA issuer of tile t: S of stage g, then P.V of stage g - 1 ----------------
+    const int t = warp - 1;
+    const uint32_t idesc_s = umma_idesc_bf16(TA_BM, TA_BN), idesc_pv = umma_idesc_bf16_b_mn(TA_BM, D);
+    uint32_t g = 0, gt = 0, it_t = 0;
+    // the P.V that is still owed: of the previous stage (possibly the previous item's last)
+    bool pend = false, pend_on = false, pend_first = false;
+    int pend_st = 0, pend_npg = 0;
+    uint32_t pend_b = 0, pend_pp = 0, pend_vp = 0, pend_op = 0;
+    auto flush_pv = [&]() {
+      if (!pend) return;
+      if (pend_on) {
+        mbar_wait(&p_full[t * 2 + pend_b], pend_pp);
+        if (pend_first && it_t > 0) mbar_wait(&o_free[t], pend_op);  // the previous item's O has been read out
+      }
+      mbar_wait(&v_full[pend_st], pend_vp);
+      if (pend_on && elect_one()) {
+        tc_fence_after();
+        const uint32_t va = smem_u32(v_s + (size_t)pend_st * TILE_BYTES);
+        for (int ks = 0; ks < pend_npg; ++ks)  // one k-step = one page of 16 keys
+          umma_bf16_ts(tmem_base + O_COL + (uint32_t)t * D, tmem_base + (uint32_t)(t * 2 + pend_b) * S_COLS + (uint32_t)ks * 8u,
+                       umma_desc_mn_sw128(va + (uint32_t)ks * 2048u, HALF_BYTES, 1024u), idesc_pv,
+                       (!pend_first || ks > 0) ? 1u : 0u);
+        umma_commit(&pv_done[t * 2 + pend_b]);
+      }
+      if (elect_one()) umma_commit(&kv_empty[pend_st]);  // this thread's S and P.V of the stage have read it (absent tile B: at once)
+      __syncwarp();
+      pend = false;
+    };
+    for (int k = 0; get_item(k, w); ++k) {
+      const bool on = t == 0 || w.has_b;
+      flush_pv();  // the previous item's last P.V goes first: this item's Q may still be in flight
+      if (on) mbar_wait(q_full, (uint32_t)k & 1u);
+      for (int j = 0; j < w.n_kt; ++j) {
+        const int st = (int)(g % TA_STAGES);
+        const uint32_t b = gt & 1u;
+        mbar_wait(&k_full[st], (g / TA_STAGES) & 1u);
+        if (elect_one()) {
+          if (on) {
+            // (S buffer b still holds P of stage gt - 2: that P.V was issued by this thread before, and executes before this)
             tc_fence_after();
             const uint32_t qa = smem_u32(q_s + t * QTILE_BYTES), ka = smem_u32(k_s + (size_t)st * TILE_BYTES);
             const uint32_t acc = tmem_base + (uint32_t)(t * 2 + b) * S_COLS;
@@ -238,25 +287,20 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap q_map, const __grid_cons
             }
             umma_commit(&s_full[t * 2 + b]);
           }
+          if (j == w.n_kt - 1) umma_commit(q_empty);  // the item's Q tiles may be overwritten once these S MMAs are done
         }
-        if (j >= 1) {
-          const int i = j - 1, st = i % TA_STAGES, b = i & 1;
-          const int n_pg = min(TA_PAGES, n_pages_seq - i * TA_PAGES);  // one k-step = one page of 16 keys
-          if (on) mbar_wait(&p_full[t * 2 + b], ((uint32_t)(i >> 1)) & 1u);
-          mbar_wait(&v_full[st], ((uint32_t)(i / TA_STAGES)) & 1u);
-          if (on && elect_one()) {
-            tc_fence_after();
-            const uint32_t va = smem_u32(v_s + (size_t)st * TILE_BYTES);
-            for (int ks = 0; ks < n_pg; ++ks)
-              umma_bf16_ts(tmem_base + O_COL + (uint32_t)t * D, tmem_base + (uint32_t)(t * 2 + b) * S_COLS + (uint32_t)ks * 8u,
-                           umma_desc_mn_sw128(va + (uint32_t)ks * 2048u, HALF_BYTES, 1024u), idesc_pv, (i > 0 || ks > 0) ? 1u : 0u);
-            umma_commit(&pv_done[t * 2 + b]);
-          }
-          if (elect_one()) umma_commit(&kv_empty[st]);  // this thread's S_i and P.V_i have read the stage (an absent tile B: at once)
-        }
+        __syncwarp();
+        if (j >= 1) flush_pv();
+        pend = true; pend_on = on; pend_first = j == 0; pend_st = st; pend_b = b;
+        pend_npg = min(TA_PAGES, w.n_pages_seq - j * TA_PAGES);
+        pend_pp = (gt >> 1) & 1u; pend_vp = (g / TA_STAGES) & 1u; pend_op = (it_t - 1u) & 1u;
+        ++g;
+        if (on) ++gt;
       }
+      if (on) ++it_t;
     }
-  } else if (warp >= 4 && live && (warp < 8 || has_b)) {
+    flush_pv();
+  } else if (warp >= 4) {
     // ---------------- softmax of tile t: thread = query row ----------------
     const int t = warp >= 8 ? 1 : 0;
     const int quad = warp & 3;
@@ -264,97 +308,109 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap q_map, const __grid_cons
     const uint32_t lane_base = tmem_base + ((uint32_t)(quad * 32) << 16);
     const uint32_t o_addr = lane_base + O_COL + (uint32_t)t * D;
     const float sl2 = 1.4426950408889634f / sqrtf((float)D);  // log2(e) / sqrt(d)
-    const int qpos = p0 + r;
-    float m_used = -INFINITY, l_run = 0.f;  // m_used in log2 units (score * sl2)
-    for (int j = 0; j < n_kt; ++j) {
-      const int b = j & 1, st = j % TA_STAGES;
-      const uint32_t s_addr = lane_base + (uint32_t)(t * 2 + b) * S_COLS;
-      mbar_wait(&s_full[t * 2 + b], ((uint32_t)(j >> 1)) & 1u);
-      tc_fence_after();
-      uint32_t v[TA_BN];
-#pragma unroll
-      for (int c = 0; c < TA_BN / 32; ++c) tmem_ld_32x32(s_addr + (uint32_t)c * 32u, *reinterpret_cast<uint32_t(*)[32]>(&v[c * 32]));
-      tmem_ld_wait();
-      const int jbase = j * TA_BN;
-      if (jbase + TA_BN - 1 > p0) {  // the tile reaches past the first query's position: causal mask
-#pragma unroll
-        for (int c = 0; c < TA_BN; ++c)
-          if (jbase + c > qpos) v[c] = 0xff800000u;  // -inf
+    uint32_t g = 0, gt = 0;
+    for (int k = 0; get_item(k, w); ++k) {
+      if (t == 1 && !w.has_b) {
+        g += (uint32_t)w.n_kt;
+        continue;
       }
-      float mx4[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};  // four independent chains
-#pragma unroll
-      for (int c = 0; c < TA_BN; ++c) mx4[c & 3] = fmaxf(mx4[c & 3], __uint_as_float(v[c]));
-      const float mx = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3])) * sl2;
-      // lazy maximum: move it only when the tile's maximum exceeds it by more than TA_LAZY (P then stays <= 2^TA_LAZY)
-      const bool move = mx > m_used + TA_LAZY;   // also true on the first tile (m_used = -inf; key 0 is visible to all)
-      float alpha = 1.0f;
-      if (move) {
-        alpha = fast_exp2(m_used - mx);  // 0 on the first tile
-        m_used = mx;
-        l_run *= alpha;
-      }
-      if (j > 0 && __any_sync(0xffffffffu, move)) {
-        // rescale the O accumulator in place (rare): P.V of tile j-1 must have completed first
-        mbar_wait(&pv_done[t * 2 + ((j - 1) & 1)], ((uint32_t)((j - 1) >> 1)) & 1u);
+      const int qpos = w.p0 + r, n_kt = w.n_kt;
+      float m_used = -INFINITY, l_run = 0.f;  // m_used in log2 units (score * sl2)
+      for (int j = 0; j < n_kt; ++j, ++g, ++gt) {
+        const uint32_t b = gt & 1u;
+        const int st = (int)(g % TA_STAGES);
+        const uint32_t s_addr = lane_base + (uint32_t)(t * 2 + b) * S_COLS;
+        mbar_wait(&s_full[t * 2 + b], (gt >> 1) & 1u);
         tc_fence_after();
+        uint32_t v[TA_BN];
 #pragma unroll
-        for (int c = 0; c < D / 32; ++c) {
-          uint32_t o[32];
-          tmem_ld_32x32(o_addr + (uint32_t)c * 32u, o);
-          tmem_ld_wait();
+        for (int c = 0; c < TA_BN / 32; ++c) tmem_ld_32x32(s_addr + (uint32_t)c * 32u, *reinterpret_cast<uint32_t(*)[32]>(&v[c * 32]));
+        tmem_ld_wait();
+        const int jbase = j * TA_BN;
+        if (jbase + TA_BN - 1 > w.p0) {  // the tile reaches past the first query's position: causal mask
 #pragma unroll
-          for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
-          tmem_st_32x32(o_addr + (uint32_t)c * 32u, o);
+          for (int c = 0; c < TA_BN; ++c)
+            if (jbase + c > qpos) v[c] = 0xff800000u;  // -inf
         }
-      }
-      float rs4[4] = {0.f, 0.f, 0.f, 0.f};
-      uint32_t pk[TA_BN / 2];
-      const float neg_m = -m_used;
+        float mx4[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};  // four independent chains
 #pragma unroll
-      for (int c = 0; c < TA_BN; c += 2) {
-        const float e0 = fast_exp2(fmaf(__uint_as_float(v[c]), sl2, neg_m));
-        const float e1 = fast_exp2(fmaf(__uint_as_float(v[c + 1]), sl2, neg_m));
-        rs4[(c >> 1) & 3] += e0 + e1;
-        pk[c >> 1] = pack_bf16x2(e0, e1);
-      }
-      l_run += (rs4[0] + rs4[1]) + (rs4[2] + rs4[3]);
-      tmem_st_32x32(s_addr, pk);
-      if (j == n_kt - 1 && (kv_len & 15) != 0) {
-        // the sequence's last page holds slots past its end with whatever the pool held: zero those V rows so that
-        // 0 * garbage (possibly NaN) cannot reach the output (their P is exactly 0: the causal mask covers them).
-        // Done by BOTH tiles' warps (the same zeros), each before it publishes its own P to its own issuer.
-        mbar_wait(&v_full[st], ((uint32_t)(j / TA_STAGES)) & 1u);
-        const int k0 = kv_len - jbase, k1 = (n_pages_seq - j * TA_PAGES) * 16;  // rows [k0, k1) of the tile
-        uint8_t *vd = v_s + (size_t)st * TILE_BYTES;
-        for (int idx = r; idx < (k1 - k0) * NH * 8; idx += 128) {
-          const int row = k0 + idx / (NH * 8), rem = idx % (NH * 8);
-          *reinterpret_cast<uint4 *>(vd + (rem >> 3) * HALF_BYTES + row * 128 + (rem & 7) * 16) = make_uint4(0u, 0u, 0u, 0u);
+        for (int c = 0; c < TA_BN; ++c) mx4[c & 3] = fmaxf(mx4[c & 3], __uint_as_float(v[c]));
+        const float mx = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3])) * sl2;
+        // lazy maximum: move it only when the tile's maximum exceeds it by more than TA_LAZY (P then stays <= 2^TA_LAZY)
+        const bool move = mx > m_used + TA_LAZY;   // also true on the first tile (m_used = -inf; key 0 is visible to all)
+        float alpha = 1.0f;
+        if (move) {
+          alpha = fast_exp2(m_used - mx);  // 0 on the first tile
+          m_used = mx;
+          l_run *= alpha;
         }
-        fence_proxy_async();
+        if (j > 0 && __any_sync(0xffffffffu, move)) {
+          // rescale the O accumulator in place (rare): P.V of the previous stage must have completed first
+          mbar_wait(&pv_done[t * 2 + ((gt - 1u) & 1u)], ((gt - 1u) >> 1) & 1u);
+          tc_fence_after();
+#pragma unroll
+          for (int c = 0; c < D / 32; ++c) {
+            uint32_t o[32];
+            tmem_ld_32x32(o_addr + (uint32_t)c * 32u, o);
+            tmem_ld_wait();
+#pragma unroll
+            for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
+            tmem_st_32x32(o_addr + (uint32_t)c * 32u, o);
+          }
+        }
+        float rs4[4] = {0.f, 0.f, 0.f, 0.f};
+        uint32_t pk[TA_BN / 2];
+        const float neg_m = -m_used;
+#pragma unroll
+        for (int c = 0; c < TA_BN; c += 2) {
+          const float e0 = fast_exp2(fmaf(__uint_as_float(v[c]), sl2, neg_m));
+          const float e1 = fast_exp2(fmaf(__uint_as_float(v[c + 1]), sl2, neg_m));
+          rs4[(c >> 1) & 3] += e0 + e1;
+          pk[c >> 1] = pack_bf16x2(e0, e1);
+        }
+        l_run += (rs4[0] + rs4[1]) + (rs4[2] + rs4[3]);
+        tmem_st_32x32(s_addr, pk);
+        if (j == n_kt - 1 && (w.kv_len & 15) != 0) {
+          // the sequence's last page holds slots past its end with whatever the pool held: zero those V rows so that
+          // 0 * garbage (possibly NaN) cannot reach the output (their P is exactly 0: the causal mask covers them).
+          // Done by BOTH tiles' warps (the same zeros), each before it publishes its own P to its own issuer.
+          mbar_wait(&v_full[st], (g / TA_STAGES) & 1u);
+          const int k0 = w.kv_len - jbase, k1 = (w.n_pages_seq - j * TA_PAGES) * 16;  // rows [k0, k1) of the tile
+          uint8_t *vd = v_s + (size_t)st * TILE_BYTES;
+          for (int idx = r; idx < (k1 - k0) * NH * 8; idx += 128) {
+            const int row = k0 + idx / (NH * 8), rem = idx % (NH * 8);
+            *reinterpret_cast<uint4 *>(vd + (rem >> 3) * HALF_BYTES + row * 128 + (rem & 7) * 16) = make_uint4(0u, 0u, 0u, 0u);
+          }
+          fence_proxy_async();
+        }
+        tmem_st_wait();
+        tc_fence_before();
+        mbar_arrive(&p_full[t * 2 + b]);
       }
-      tmem_st_wait();
-      tc_fence_before();
-      mbar_arrive(&p_full[t * 2 + b]);
-    }
-    // ---- normalise and store
-    mbar_wait(&pv_done[t * 2 + ((n_kt - 1) & 1)], ((uint32_t)((n_kt - 1) >> 1)) & 1u);
-    tc_fence_after();
-    const float inv = 1.0f / l_run;
-    __nv_bfloat16 *og = (__nv_bfloat16 *)p.out + ((size_t)(row0 + r) * p.n_q + head_a + t) * D;
+      // ---- normalise and store; the O accumulator is handed back (o_free) as soon as this row has left tensor memory
+      mbar_wait(&pv_done[t * 2 + ((gt - 1u) & 1u)], ((gt - 1u) >> 1) & 1u);
+      tc_fence_after();
+      const float inv = 1.0f / l_run;
+      __nv_bfloat16 *og = (__nv_bfloat16 *)p.out + ((size_t)(w.row0 + r) * p.n_q + w.head_a + t) * D;
 #pragma unroll
-    for (int c = 0; c < D / 32; ++c) {
-      uint32_t o[32];
-      tmem_ld_32x32(o_addr + (uint32_t)c * 32u, o);
-      tmem_ld_wait();
-      if (r < rows) {
+      for (int c = 0; c < D / 32; ++c) {
+        uint32_t o[32];
+        tmem_ld_32x32(o_addr + (uint32_t)c * 32u, o);
+        tmem_ld_wait();
+        if (c == D / 32 - 1) {
+          tc_fence_before();
+          mbar_arrive(&o_free[t]);
+        }
+        if (r < w.rows) {
 #pragma unroll
-        for (int i = 0; i < 32; i += 8) {
-          uint4 w;
-          w.x = pack_bf16x2(__uint_as_float(o[i]) * inv, __uint_as_float(o[i + 1]) * inv);
-          w.y = pack_bf16x2(__uint_as_float(o[i + 2]) * inv, __uint_as_float(o[i + 3]) * inv);
-          w.z = pack_bf16x2(__uint_as_float(o[i + 4]) * inv, __uint_as_float(o[i + 5]) * inv);
-          w.w = pack_bf16x2(__uint_as_float(o[i + 6]) * inv, __uint_as_float(o[i + 7]) * inv);
-          *reinterpret_cast<uint4 *>(og + c * 32 + i) = w;
+          for (int i = 0; i < 32; i += 8) {
+            uint4 q4;
+            q4.x = pack_bf16x2(__uint_as_float(o[i]) * inv, __uint_as_float(o[i + 1]) * inv);
+            q4.y = pack_bf16x2(__uint_as_float(o[i + 2]) * inv, __uint_as_float(o[i + 3]) * inv);
+            q4.z = pack_bf16x2(__uint_as_float(o[i + 4]) * inv, __uint_as_float(o[i + 5]) * inv);
+            q4.w = pack_bf16x2(__uint_as_float(o[i + 6]) * inv, __uint_as_float(o[i + 7]) * inv);
+            *reinterpret_cast<uint4 *>(og + c * 32 + i) = q4;
+          }
         }
       }
     }
@@ -368,7 +424,7 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap q_map, const __grid_cons
 }
 
 static size_t prefill_smem(int d) {
-  return 1024 + (size_t)(d / 64) * (2 * TA_BM + 2 * TA_STAGES * TA_BN) * 128 + 8 * (1 + 3 * TA_STAGES + 12) + 16;
+  return 1024 + (size_t)(d / 64) * (2 * TA_BM + 2 * TA_STAGES * TA_BN) * 128 + 8 * (2 + 3 * TA_STAGES + 12 + 2) + 16;
 }
 
 cudaError_t prefill_attn_init() {  // per device: called from ss_stage_create
@@ -381,7 +437,8 @@ cudaError_t prefill_attn_init() {  // per device: called from ss_stage_create
 
 cudaError_t launch_prefill_attn(const PrefillAttnParams &p, cudaStream_t s) {
   const int G = p.n_q / p.n_kv;
-  dim3 grid(p.n_kv * ((G + 1) / 2), p.max_tiles);
+  const long long items = (long long)p.n_kv * ((G + 1) / 2) * p.max_tiles;  // upper bound; the live count is on the device
+  dim3 grid((unsigned)(items < p.n_sm ? items : p.n_sm));                   // persistent: one CTA per SM
   if (p.d == 128)
     return launch_pdl(prefill_attn_kernel<128>, dim3(grid), dim3(TA_THREADS), prefill_smem(128), s, *p.q_map, *p.kv_map, p);
   return launch_pdl(prefill_attn_kernel<64>, dim3(grid), dim3(TA_THREADS), prefill_smem(64), s, *p.q_map, *p.kv_map, p);

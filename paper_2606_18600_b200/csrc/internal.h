@@ -232,6 +232,7 @@ struct PrefillAttnParams {
   void *out;                 // bf16 [T,Hq]
   const CallArgs *args;
   int max_tiles;             // upper bound on query tiles = ceil(T / prefill_attn_tile_rows()) + n_seqs
+  int n_sm;                  // SMs of the device: the kernel is persistent, one CTA per SM
 };
 int prefill_attn_tile_rows();
 cudaError_t launch_prefill_attn(const PrefillAttnParams &p, cudaStream_t s);

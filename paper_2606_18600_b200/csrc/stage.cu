@@ -807,6 +807,7 @@ static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T,
         ap.out = st->at<void>(c.attn_out);
         ap.args = args;
         ap.max_tiles = (T - n_dec + prefill_attn_tile_rows() - 1) / prefill_attn_tile_rows() + (n_seqs - n_dec);
+        ap.n_sm = st->n_sm;
         CKE(launch_prefill_attn(ap, s));
       }
     }
