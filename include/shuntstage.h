@@ -293,6 +293,24 @@ int ss_op_gemm_bf16(const void *x_dev, const void *w_dev, float *c_dev, int T, i
 int ss_op_gemm_swiglu_bf16(const void *x_dev, const void *wg_dev, const void *wu_dev, void *a_dev,
                            int T, int F, int K, void *scratch_dev, size_t scratch_bytes, void *cuda_stream);
 
+/* The same GEMM for callers that may NOT allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): C[T, N] (fp32, row-major, ld = N) = X[T, K] (bf16) * W[N, K]^T (bf16), as
+ * ss_op_gemm_bf16 (same kernel, same launch plan, bit-identical result), but the stream-K fix-up scratch is a fixed
+ * __device__ array inside the library instead of a caller buffer.  The call allocates nothing: no cudaMalloc / cudaFree
+ * and no allocating library routine; on the stream it enqueues one 1 KiB memset node (the fix-up flags) and the kernel.
+ *   Limit: T <= SS_OP_GEMM_STATIC_MAX_T (decode batches); any N, K with K % 8 == 0; x_dev / w_dev 16-byte aligned.
+ *   Cost: SS_OP_GEMM_STATIC_SCRATCH_BYTES of device memory on EVERY GPU that loads the library, held until exit.
+ *   Sharing: every call on a device uses the same array.  Calls that overlap on the GPU (two streams, two host
+ *   threads, a captured graph replayed while another call is in flight) RACE on it and give wrong sums or trip the
+ *   kernel's bounded waits; serialise them on one stream or with events.  Nothing else is kept between calls.
+ * Errors: SS_ERR_INVALID_ARG (null pointer, non-positive size), SS_ERR_UNSUPPORTED (K % 8, alignment),
+ * SS_ERR_CAPACITY (T > SS_OP_GEMM_STATIC_MAX_T: refused, never clipped; ss_last_cuda_error says so), SS_ERR_CUDA.
+ * The device address of the array is looked up once per device on the first call made with that device current
+ * (cudaGetSymbolAddress; not an allocation): make one call outside graph capture first. */
+#define SS_OP_GEMM_STATIC_MAX_T 128
+#define SS_OP_GEMM_STATIC_SCRATCH_BYTES (1024 + 256 * 128 * 128 * 4) /* flags + 256 CTAs x (128 x 128 fp32) = 16 MiB + 1 KiB */
+int ss_op_gemm_bf16_static(const void *x_dev, const void *w_dev, float *c_dev, int T, int N, int K, void *cuda_stream);
+
 /* Shared Tensor Store attach (Section 5.2 "Concurrent initialization", Figure 7).  The paper keeps
  * the weight tensors and the KV-cache space in a separate per-node process and shares them with the inference engine
  * "in a zero-copy manner through CUDA IPC handles", so that a replacement engine can be initialised beside the serving

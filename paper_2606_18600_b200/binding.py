@@ -22,7 +22,7 @@ ERRORS = {0: "SS_OK", -1: "SS_ERR_INVALID_ARG", -2: "SS_ERR_UNSUPPORTED", -3: "S
 EXPORTS = ["ss_stage_workspace_bytes", "ss_kv_page_bytes", "ss_stage_create", "ss_stage_destroy",
            "ss_kv_num_pages", "ss_kv_num_free", "ss_kv_alloc", "ss_kv_free", "ss_stage_prefill", "ss_stage_mixed",
            "ss_stage_decode",
-           "ss_stage_launch_count", "ss_op_gemm_scratch_bytes", "ss_op_gemm_bf16", "ss_op_gemm_swiglu_bf16", "ss_strerror",
+           "ss_stage_launch_count", "ss_op_gemm_scratch_bytes", "ss_op_gemm_bf16", "ss_op_gemm_swiglu_bf16", "ss_op_gemm_bf16_static", "ss_strerror",
            "ss_last_cuda_error", "ss_version", "ss_debug_buffer", "ss_pool_create", "ss_pool_destroy",
            "ss_pool_num_pages", "ss_pool_num_free", "ss_pool_alloc", "ss_pool_free", "ss_kv_export", "ss_kv_import", "ss_stage_set_allreduce", "ss_stage_set_batch_invariant", "ss_tp_xchg_bytes", "ss_stage_set_tp_fused",
            "ss_stage_debug_tap", "ss_stage_debug_info", "ss_stage_graph_count", "ss_store_alloc", "ss_store_free", "ss_store_upload", "ss_store_export", "ss_store_attach", "ss_store_detach"]
@@ -122,6 +122,7 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
                                     C.c_size_t, C.c_void_p]
     lib.ss_op_gemm_swiglu_bf16.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int,
                                            C.c_int, C.c_void_p, C.c_size_t, C.c_void_p]
+    lib.ss_op_gemm_bf16_static.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p]
     lib.ss_strerror.restype = C.c_char_p
     lib.ss_strerror.argtypes = [C.c_int]
     lib.ss_last_cuda_error.restype = C.c_char_p
@@ -367,6 +368,23 @@ def op_gemm_bf16(x: torch.Tensor, w: torch.Tensor, stream=None) -> torch.Tensor:
     if rc != SS_OK:
         raise ShuntStageError(rc, "ss_op_gemm_bf16")
     return c
+
+
+OP_GEMM_STATIC_MAX_T = 128  # SS_OP_GEMM_STATIC_MAX_T
+
+
+def op_gemm_bf16_static(x: torch.Tensor, w: torch.Tensor, out: torch.Tensor, stream=None) -> torch.Tensor:
+    """ss_op_gemm_bf16_static: out[T,N] fp32 = x[T,K] bf16 @ w[N,K]^T bf16 with the library's own static scratch.  The
+    caller passes the output too, so that nothing at all is allocated by the call (T <= OP_GEMM_STATIC_MAX_T)."""
+    lib = load_library()
+    T, K = x.shape
+    N = w.shape[0]
+    assert out.shape == (T, N) and out.dtype == torch.float32
+    st = _op_stream(stream)
+    rc = lib.ss_op_gemm_bf16_static(_ptr(x), _ptr(w), _ptr(out), T, N, K, st.cuda_stream)
+    if rc != SS_OK:
+        raise ShuntStageError(rc, "ss_op_gemm_bf16_static")
+    return out
 
 
 def op_gemm_swiglu_bf16(x: torch.Tensor, wg: torch.Tensor, wu: torch.Tensor, stream=None) -> torch.Tensor:

@@ -8,7 +8,7 @@ from pathlib import Path
 HERE = Path(__file__).resolve().parent
 CSRC = HERE / "csrc"
 LIB = HERE / "libshuntstage.so"
-SOURCES = ["gemm_tcgen05.cu", "attn_decode.cu", "attn_prefill.cu", "elementwise.cu", "stage.cu"]
+SOURCES = ["gemm_tcgen05.cu", "attn_decode.cu", "attn_prefill.cu", "elementwise.cu", "stage.cu", "op_static.cu"]
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC",
          "--use_fast_math=false"]
 

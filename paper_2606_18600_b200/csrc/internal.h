@@ -108,6 +108,9 @@ bool gemm_partial_ok(const GemmLaunch &g);
 // host: the PartialTile table of a planned stream-K launch (n_row_tiles entries)
 void gemm_partial_table(const GemmLaunch &g, PartialTile *out);
 cudaError_t gemm_launch(const GemmLaunch &g);
+// stage.cu: record the text that ss_last_cuda_error returns (thread-local) and hand back the code to return
+int note_cuda_error(cudaError_t e, const char *where);  // -> SS_ERR_CUDA
+int note_error(int code, const char *text);             // -> code
 cudaError_t gemm_init();  // sets max dynamic smem attributes once
 cudaError_t gemm_set_debug_buffer(unsigned long long *host_mapped);  // see gemm_tcgen05.cu wait_expired()
 int gemm_pick_bn(int T);  // 32 for T <= 32, else the narrowest multiple of 32 covering T in ceil(T / 256) token tiles

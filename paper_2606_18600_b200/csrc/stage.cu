@@ -38,6 +38,12 @@ static int cuda_fail(cudaError_t e, const char *where) {
   cudaGetLastError();  // reported through the return code: do not leave a non-sticky error for the caller's next CUDA call
   return SS_ERR_CUDA;
 }
+// for the other translation units of the library (op_static.cu): record the text ss_last_cuda_error returns
+int note_cuda_error(cudaError_t e, const char *where) { return cuda_fail(e, where); }
+int note_error(int code, const char *text) {
+  g_cuda_err = text;
+  return code;
+}
 #define CK(call)                                          \
   do {                                                    \
     cudaError_t e__ = (call);                             \
