@@ -477,6 +477,42 @@ def test_prefill_attention_edge_shapes_vs_oracle(shape, lens, first):
         P.close()
 
 
+@pytest.mark.gpu
+@pytest.mark.parametrize("shape,n_seqs,long_len", [
+    (G3, 230, 700),          # odd group, d = 64: the items of a CTA alternate between two heads and a lone head
+    (MHA, 200, 600),         # MHA, d = 128: tile B is absent in every item
+    (synth.TINY128, 400, 1500),   # G = 8, d = 128: 4 head pairs per tile, ~2,000 items
+])
+def test_prefill_attention_persistent_ctas_take_several_items_vs_oracle(shape, n_seqs, long_len):
+    """The prefill attention is persistent: one CTA per SM walks the heaviest-first list of (query tile, head pair) items
+    in snake order, and its barrier phases, ring slots and S / O buffers carry on from one item to the next.  The other
+    attention cases have fewer items than SMs; here every CTA takes several, of very different weights (a few long
+    sequences among many of 1-130 tokens, so 1-row tiles, 1-stage items and ring wrap-arounds meet in one CTA), with and
+    without the second head of the pair.  Whole 2-layer stage vs the oracle, KV pages strict."""
+    rng = np.random.default_rng(n_seqs)
+    lens = rng.integers(1, 131, size=n_seqs).astype(np.int32)
+    lens[rng.choice(n_seqs, size=5, replace=False)] = [long_len, long_len - 63, 257, 129, 128]
+    P, lens, pb, x = _problem(shape, seed=13, lens=lens, extra=4)
+    try:
+        bt = pb.block_tables
+        pairs = (shape.n_q // shape.n_kv + 1) // 2
+        n_items = int(((lens + 127) // 128).sum()) * shape.n_kv * pairs
+        assert n_items > 2 * 148, n_items        # several items per CTA on a 148-SM part
+        pool0 = hp.new_pool(shape, pb.n_pages_pool, P.L)
+        want, _, _ = hp.run_oracle_prefill(F32, shape, P.wb, pool0, lens, bt, x[:int(lens.sum())])
+        got = P.prefill(lens, bt, x[:int(lens.sum())])
+        err = hp.rel_err_rows(got, want)
+        print(f"{shape.name}: {n_seqs} sequences, {int(lens.sum())} tokens, {n_items} attention items: rel err vs R0 {err:.3e}")
+        assert np.isfinite(got).all() and err < STAGE_TOL
+        mask = _written_mask(pool0.shape, bt, lens)
+        pg = P.pool_bits()
+        assert (pg[~mask] == 0x7FC1).all() and (pg[mask] != 0x7FC1).all()
+        again = P.prefill(lens, bt, x[:int(lens.sum())])   # same call again: same bits (no state left behind in the CTAs' walk)
+        assert np.array_equal(again, got)
+    finally:
+        P.close()
+
+
 def test_chunked_prefill_and_mixed_batch_on_gpu():
     """Prior context (ctx_before > 0) and q_len = 1 rows in a prefill call (mixed iteration, reading A19)."""
     shape = synth.TINY_QWEN
