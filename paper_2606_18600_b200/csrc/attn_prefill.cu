@@ -10,7 +10,7 @@
 //               over the S tile it came from; V tile in smem as TMA wrote it ([key][d]: the MN-major B operand)
 // CTA = the same 128 query positions of TWO q heads of one GQA group ("tile A", "tile B": they attend the same keys, so
 // one K/V ring serves both and every K/V byte fetched from L2 feeds 256 query rows); 12 warps, one role each:
-//   warps 0, 3  TMA producers of K and of V: both Q tiles once (warp 0), then per key tile 4 pages (16 tokens x d, one 2-D
+//   warps 0, 3  TMA producers of K and of V: both Q tiles per item (warp 0), then per key tile 4 pages (16 tokens x d, one 2-D
 //               box per 64 columns; the layer's pool is one 2-D tensor) into a 5-stage ring.  Two threads because one
 //               cp.async.bulk.tensor occupies its issuer ~100 cycles (clock64 stamps: 16 boxes per stage = 1,650 cycles)
 //   warps 1, 2  issue ALL MMAs of tile A / tile B (one lane each): S_j into DOUBLE-buffered S tiles, then P.V of stage
@@ -20,8 +20,8 @@
 //               P.V_{j-2} that still reads the P stored over that S buffer
 //   warps 4-7 / 8-11  softmax of tile A / B: thread = query row = TMEM lane, so row max / row sum need no shuffle;
 //               tcgen05.ld of the S row, exp2 in fp32, P -> bf16 -> tcgen05.st; the running maximum is only moved when it
-//               grows by more than 2^8 (then, rarely, the O accumulator is rescaled in place), else P simply is up to
-//               2^8 larger — the final O / l is unchanged
+//               grows by more than 2^16 (then, rarely, the O accumulator is rescaled in place), else P simply is up to
+//               2^16 larger — the final O / l is unchanged (at 2^8 the maximum still moved in 13% of the stages)
 // TMEM (512 columns): S_A0 S_A1 S_B0 S_B1 (64 each), O_A, O_B (d each).
 #include <cuda.h>
 #include <cuda_bf16.h>
@@ -37,7 +37,7 @@ constexpr int TA_BN = 64;       // keys per ring stage (4 pages)
 constexpr int TA_STAGES = 5;    // K/V ring depth: 320 keys in flight per CTA
 constexpr int TA_THREADS = 384;
 constexpr int TA_PAGES = TA_BN / 16;
-constexpr float TA_LAZY = 8.0f; // the running maximum (log2 units) is moved only when exceeded by more than this
+constexpr float TA_LAZY = 16.0f; // the running maximum (log2 units) is moved only when exceeded by more than this
 
 // ---- plan: token -> (sequence, position), the prefix sum of query tiles and one descriptor per launch slot ---------
 __global__ void prefill_plan_kernel(const CallArgs *__restrict__ args, int n_seqs, int seq0, PrefillPlan plan) {
@@ -150,11 +150,11 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap q_map, const __grid_cons
     }
     for (int i = 0; i < 4; ++i) {
       mbar_init(&s_full[i], 1);
-      mbar_init(&p_full[i], 128);  // every softmax thread of the tile
+      mbar_init(&p_full[i], 4);    // one arrival per softmax warp of the tile (32 arrivals of a warp on one barrier serialise)
       mbar_init(&pv_done[i], 1);
     }
-    mbar_init(&o_free[0], 128);    // every softmax thread has read its O row out of tensor memory
-    mbar_init(&o_free[1], 128);
+    mbar_init(&o_free[0], 4);      // per softmax warp: every thread has read its O row out of tensor memory
+    mbar_init(&o_free[1], 4);
     mbar_fence_init();
   }
   if (warp == 1) tmem_alloc_dyn(tmem_slot, TMEM_COLS);
@@ -214,13 +214,21 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap q_map, const __grid_cons
         __syncwarp();
       }
       const int32_t *bt = args->block_tables + (size_t)w.s * args->max_blocks;
+      // page ids: lane l holds the id of page 32 * blk + l of the sequence, fetched one block of 32 pages (8 stages)
+      // ahead, so that no global-load latency sits in the per-stage loop (it was ~half of this warp's time per stage)
+      int ids_next = lane < w.n_pages_seq ? bt[lane] : 0, ids = 0;
       for (int j = 0; j < w.n_kt; ++j, ++g) {
+        if ((j & 7) == 0) {
+          ids = ids_next;
+          const int nx = (j + 8) * TA_PAGES + lane;
+          ids_next = nx < w.n_pages_seq ? bt[nx] : 0;
+        }
         const int st = (int)(g % TA_STAGES);
         const int n_pg = min(TA_PAGES, w.n_pages_seq - j * TA_PAGES);  // pages past the sequence's end are never touched
         int rowv[TA_PAGES];
 #pragma unroll
         for (int pg = 0; pg < TA_PAGES; ++pg)
-          rowv[pg] = pg < n_pg ? (bt[j * TA_PAGES + pg] * p.n_kv + w.hk) * 16 + row_off : 0;
+          rowv[pg] = (__shfl_sync(0xffffffffu, ids, (j & 7) * TA_PAGES + pg) * p.n_kv + w.hk) * 16 + row_off;
         mbar_wait(&kv_empty[st], ((g / TA_STAGES) & 1u) ^ 1u);
         uint8_t *dst = ring + (size_t)st * TILE_BYTES;
         if (elect_one()) {
@@ -385,7 +393,8 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap q_map, const __grid_cons
         }
         tmem_st_wait();
         tc_fence_before();
-        mbar_arrive(&p_full[t * 2 + b]);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&p_full[t * 2 + b]);
       }
       // ---- normalise and store; the O accumulator is handed back (o_free) as soon as this row has left tensor memory
       mbar_wait(&pv_done[t * 2 + ((gt - 1u) & 1u)], ((gt - 1u) >> 1) & 1u);
@@ -399,7 +408,8 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap q_map, const __grid_cons
         tmem_ld_wait();
         if (c == D / 32 - 1) {
           tc_fence_before();
-          mbar_arrive(&o_free[t]);
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&o_free[t]);
         }
         if (r < w.rows) {
 #pragma unroll
