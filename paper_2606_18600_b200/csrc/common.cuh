@@ -335,7 +335,7 @@ __device__ __forceinline__ void mma_bf16_16816(float (&d)[4], const uint32_t (&a
 // The same MMA when only rows 0-7 of the 16-row A tile are live (a[1] = a[3] = 0, C rows 8-15 = 0): the results
 // of rows 8-15 go to two scratch registers, so the caller keeps 2 accumulator registers per tile instead of 4.
 __device__ __forceinline__ void mma_bf16_16816_lo(float (&d)[2], uint32_t a0, uint32_t a2, uint32_t b0, uint32_t b1) {
-  float j2, j3;
+  [[maybe_unused]] float j2, j3;  // rows 8-15: discarded
   asm volatile(
       "mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%10,%10};"
       : "+f"(d[0]), "+f"(d[1]), "=f"(j2), "=f"(j3)

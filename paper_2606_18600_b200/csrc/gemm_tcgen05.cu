@@ -31,7 +31,6 @@
 namespace ss {
 
 constexpr int A_TILE_BYTES = GEMM_BM * GEMM_BK * 2;  // 16 KB
-constexpr int EPI_THREADS = 128;
 constexpr int GEMM_THREADS = 352;  // warp 0: TMA producer, 1: MMA issuer 0, 6: MMA issuer 1, 2-5 and 7-10: epilogue
 constexpr int EPI_WARPS = 8;       // two warps per TMEM lane quadrant, taking alternate 32-column chunks
 
