@@ -56,3 +56,31 @@ def test_static_scratch_gemm_rejects_sizes_beyond_its_maximum():
     assert b"SS_OP_GEMM_STATIC_MAX_T" in binding.load_library().ss_last_cuda_error()
     torch.cuda.synchronize()
     assert float(out.abs().max()) == 0.0  # refused, not clipped: nothing was launched
+
+
+@pytest.mark.gpu
+def test_static_scratch_gemm_can_be_captured_in_a_cuda_graph():
+    """The use the entry point exists for: after one set-up call outside the capture, two calls are recorded into a CUDA
+    graph (a memset node and a kernel node each, nothing allocated) and the replay gives the existing path's bits."""
+    from paper_2606_18600_b200 import binding
+    (x1, w1), (x2, w2) = _operands(64, 8192, 8192, 21), _operands(128, 5120, 8192, 22)
+    o1 = torch.zeros((64, 8192), dtype=torch.float32, device="cuda")
+    o2 = torch.zeros((128, 5120), dtype=torch.float32, device="cuda")
+    xs, ws = _operands(8, 128, 64, 1)
+    binding.op_gemm_bf16_static(xs, ws, torch.empty((8, 128), dtype=torch.float32, device="cuda"))  # set-up call
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        graph.capture_begin()
+        binding.op_gemm_bf16_static(x1, w1, o1, stream=side)
+        binding.op_gemm_bf16_static(x2, w2, o2, stream=side)
+        graph.capture_end()
+    torch.cuda.synchronize()
+    assert float(o1.abs().max()) == 0.0 and float(o2.abs().max()) == 0.0  # captured, not run
+    for _ in range(2):
+        o1.fill_(float("nan"))
+        o2.fill_(float("nan"))
+        graph.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(o1, binding.op_gemm_bf16(x1, w1)) and torch.equal(o2, binding.op_gemm_bf16(x2, w2))
