@@ -832,7 +832,8 @@ def run_online(args, shape, rank, world):
     occ = drv.stats["occupancy"][W:]
     res = {"ms": ms, "decode_tokens": drv.stats["decode_tokens"] - d0, "prefill_tokens": drv.stats["prefill_tokens"] - p0,
            "launches": st.launch_count() - n0, "clocks": clocks, "occupancy": [min(occ), float(np.mean(occ)), max(occ)],
-           "dropped": drv.stats["dropped"], "finished": drv.stats["finished"], "pages": n_pages}
+           "dropped": drv.stats["dropped"], "preempted": drv.stats["preempted"], "finished": drv.stats["finished"],
+           "pages": n_pages}
     st.destroy()
     return res
 
@@ -1029,7 +1030,7 @@ def main():
                 "gpu_launches": int(res["launches"]),
                 "decode_tokens_per_s": res["decode_tokens"] * world / (ms * 1e-3),
                 "prefill_tokens_per_s": res["prefill_tokens"] * world / (ms * 1e-3),
-                "pool": {"pages": res["pages"], "occupancy_min_mean_max": res["occupancy"], "dropped": res["dropped"],
+                "pool": {"pages": res["pages"], "occupancy_min_mean_max": res["occupancy"], "dropped": res["dropped"], "preempted": res["preempted"],
                          "finished": res["finished"]}}
         print(json.dumps(line))
         return

@@ -11,7 +11,9 @@ numpy.random.default_rng(seed): decode slots start with ctx ~ LN(1024) in [16, 8
 prune), consumed <= 512 tokens per iteration; a finished prompt enters a ready FIFO (pages kept) and
 its slot takes a new request; a decode slot whose remaining output hits 0 frees its pages and takes the FIFO head
 (or, if the FIFO is empty, a fresh already-prefilled context); FIFO entries are dropped (pages freed) while the
-occupancy exceeds 0.85.
+occupancy exceeds 0.85.  A decode row always gets the page its next token needs: if the pool is out of pages, FIFO entries
+and then prompts in mid-prefill are preempted (pages freed, the prompt starts over), and a prefill chunk is only admitted
+while one free page per decode row remains.
 """
 from __future__ import annotations
 
@@ -57,7 +59,10 @@ class OnlineDriver:
         self.decode = [self._fresh_decode() for _ in range(N_DECODE)]
         self.prefill = [self._fresh_prefill() for _ in range(N_PREFILL)]
         self.fifo: deque = deque()
-        self.stats = {"decode_tokens": 0, "prefill_tokens": 0, "dropped": 0, "finished": 0, "occupancy": []}
+        self.stats = {"decode_tokens": 0, "prefill_tokens": 0, "dropped": 0, "preempted": 0, "evicted": 0, "finished": 0, "occupancy": []}
+        self.h_bt = None  # staging buffers: made by the first step() (plan() / _advance() are host-only and testable without a GPU)
+
+    def _staging(self):
         S = N_DECODE + N_PREFILL
         # pinned host staging + device copies of the per-call integer inputs
         self.h_bt = torch.zeros((S, self.max_blocks), dtype=torch.int32).pin_memory()
@@ -102,7 +107,9 @@ class OnlineDriver:
         ctx, rem = self._draw_decode(self.rng)
         r = Req(ctx=ctx, remaining=rem)
         while not self._alloc(r, ctx + 1):      # pool too full for this draw: halve it (keeps the run going)
-            ctx = max(16, ctx // 2)
+            if ctx == 0:
+                raise RuntimeError("page pool exhausted: not one free page for a new request")
+            ctx = ctx // 2 if ctx > 16 else 0
             r.ctx = ctx
         return r
 
@@ -115,18 +122,47 @@ class OnlineDriver:
     # ---- one iteration: build the batch, call the stage, advance the state ----
     def plan(self):
         """Rows of this iteration: (request, q_len) for the 96 decode slots then the active prefill slots."""
+        # Decode rows first: a running request gets the page its next token needs.  When the pool cannot give it, pages are
+        # taken back in the order a continuous-batching scheduler preempts: prefilled requests still waiting in the FIFO
+        # (newest first), then prompts in the middle of their prefill (they start over: recomputation), and last the
+        # running request that holds the most pages (evicted; its slot takes a fresh, shorter request) — the decode set
+        # alone outgrows a pool sized at 85% of the INITIAL contexts once every request has aged a few hundred tokens.
+        for i in range(N_DECODE):
+            if self.decode[i].remaining < 0:                   # evicted in this pass: refilled below
+                continue
+            while not self._alloc(self.decode[i], self.decode[i].ctx + 1):
+                if self.fifo:
+                    self._free(self.fifo.pop())
+                    self.stats["dropped"] += 1
+                    continue
+                victim = max((p for p in self.prefill if p.pages), key=lambda p: len(p.pages), default=None)
+                if victim is not None:
+                    self._free(victim)
+                    victim.ctx = 0
+                    self.stats["preempted"] += 1
+                    continue
+                j = max((k for k in range(N_DECODE) if k != i and len(self.decode[k].pages) > 1),
+                        key=lambda k: len(self.decode[k].pages), default=None)
+                assert j is not None, "page pool smaller than one page per decode row"
+                self._free(self.decode[j])
+                self.stats["evicted"] += 1
+                self.decode[j] = Req(remaining=-1)             # placeholder
+        for k in range(N_DECODE):                              # evicted slots take a fresh request that fits
+            if self.decode[k].remaining < 0:
+                self.decode[k] = self._fresh_decode()
         rows = [(r, 1) for r in self.decode]
+        # Prefill chunks only out of what is left beyond one page per decode row (the next iteration's worst case)
         for r in self.prefill:
             q = min(CHUNK, r.prompt - r.ctx)
-            if q > 0 and self._alloc(r, r.ctx + q):
+            need = (r.ctx + q + PAGE - 1) // PAGE - len(r.pages)
+            if q > 0 and self.stage.num_free() - need >= N_DECODE and self._alloc(r, r.ctx + q):
                 rows.append((r, q))
-        for r, _ in rows[:N_DECODE]:
-            ok = self._alloc(r, r.ctx + 1)
-            assert ok, "page pool exhausted for a decode row (the 85% rule should prevent this)"
         return rows
 
     def step(self, hidden_bank: torch.Tensor, out: torch.Tensor) -> Iteration:
         """hidden_bank: bf16 [>= T, H] device rows to feed (synthetic stage input); out: bf16 [>= T, H]."""
+        if self.h_bt is None:
+            self._staging()
         rows = self.plan()
         n = len(rows)
         q = np.array([ql for _, ql in rows], dtype=np.int32)
