@@ -753,6 +753,42 @@ def test_decode_graph_replay_is_deterministic_and_pointer_safe():
         P.close()
 
 
+def test_stage_create_destroy_cycles_leak_nothing_on_the_device():
+    """A serving process re-creates stages (the paper's reconfiguration after a spot interruption): each
+    cycle builds a stage, runs a prefill and two decode steps (which captures and replays a CUDA graph) and destroys it.
+    The stage allocates no device memory of its own, so after the first cycles the device's free memory must not move
+    and every cycle must give the same bits."""
+    import gc
+    shape = synth.TINY_QWEN
+
+    def cycle():
+        P, lens, pb, x = _problem(shape, seed=4, lens=[40, 17, 70, 3])
+        try:
+            T = int(lens.sum())
+            P.prefill(lens, pb.block_tables, x[:T])
+            y = P.decode(lens, pb.block_tables, x[T:T + len(lens)])
+            y = P.decode(lens + 1, pb.block_tables, x[T:T + len(lens)])
+            return y.copy()
+        finally:
+            P.close()
+
+    first = cycle()
+    for _ in range(2):
+        cycle()
+    gc.collect()
+    torch.cuda.synchronize()
+    torch.cuda.empty_cache()
+    free0 = torch.cuda.mem_get_info()[0]
+    for _ in range(25):
+        assert np.array_equal(cycle(), first)
+    gc.collect()
+    torch.cuda.synchronize()
+    torch.cuda.empty_cache()
+    free1 = torch.cuda.mem_get_info()[0]
+    print(f"free device memory before / after 25 cycles: {free0} / {free1}")
+    assert free0 - free1 <= 2 << 20   # nothing accumulates (2 MiB of slack for the driver's own pools)
+
+
 def test_edge_cases_and_error_codes():
     shape = synth.TINY
     gh = _gh()
