@@ -753,6 +753,44 @@ def test_decode_graph_replay_is_deterministic_and_pointer_safe():
         P.close()
 
 
+@pytest.mark.parametrize("shape", [synth.TINY128, synth.TINY_QWEN])
+def test_decode_batch_size_sweep_vs_oracle(shape):
+    """Decode batches across every size boundary of the path: the GEMM's token-tile width (32 ... 256 columns, then
+    several token tiles), the stream-K pieces left to the consumer kernels or not, the variants of the residual + RMSNorm
+    and qkv_post kernels, one CUDA graph per batch size, the decode attention's page split over few or many rows.  One
+    stage holds 300 sequences; a prefix of B of them takes one decode step (the others' pages must not change)."""
+    n = 300
+    rng = np.random.default_rng(21)
+    lens = rng.integers(1, 90, size=n).astype(np.int32)
+    lens[[0, 7, 130]] = [300, 1, 16]
+    P, lens, pb, _ = _problem(shape, seed=6, lens=lens, extra=4)
+    try:
+        T = int(lens.sum())
+        x = synth.bits(synth.hidden_rows(T + n, shape.hidden, 6))
+        bt = pb.block_tables
+        pool = hp.new_pool(shape, pb.n_pages_pool, P.L)
+        hp.run_oracle_prefill(F32, shape, P.wb, pool, lens, bt, x[:T])
+        P.prefill(lens, bt, x[:T])
+        snap_gpu = P.stage.pool_view().clone()
+        worst = 0.0
+        for B in (1, 2, 3, 5, 17, 32, 33, 64, 65, 100, 128, 129, 200, 256, 257, 300):
+            P.stage.pool_view().copy_(snap_gpu)          # every batch starts from the prefilled pool
+            torch.cuda.synchronize()
+            pool_b = pool.copy()
+            xs = x[T:T + B]
+            want, _ = hp.run_oracle_decode(F32, shape, P.wb, pool_b, lens[:B], bt[:B], xs)
+            got = P.decode(lens[:B], bt[:B], xs)
+            err = hp.rel_err_rows(got, want)
+            worst = max(worst, err)
+            assert np.isfinite(got).all() and err < STAGE_TOL, (B, err)
+            mask = _written_mask(pool.shape, bt[:B], lens[:B] + 1) | _written_mask(pool.shape, bt, lens)
+            pg = P.pool_bits()
+            assert (pg[~mask] == 0x7FC1).all() and (pg[mask] != 0x7FC1).all(), B
+        print(f"{shape.name}: decode batches 1..300, worst stage rel err vs R0 {worst:.3e}")
+    finally:
+        P.close()
+
+
 def test_stage_create_destroy_cycles_leak_nothing_on_the_device():
     """A serving process re-creates stages (the paper's reconfiguration after a spot interruption): each
     cycle builds a stage, runs a prefill and two decode steps (which captures and replays a CUDA graph) and destroys it.
