@@ -85,6 +85,40 @@ def test_full_width_decode_step_vs_oracle(name):
         P.close()
 
 
+@pytest.mark.parametrize("name,b_max,batches", [("cfg3", 256, (1, 5, 32, 33, 96, 129, 224, 256)),
+                                                ("cfg2", 160, (1, 3, 17, 48, 65, 128, 160))])
+def test_full_width_decode_batch_sizes_vs_oracle(name, b_max, batches):
+    """The decode plans change with the batch size (GEMM token-tile width 32 ... 256, stream-K grids, consumer-side
+    reduction, attention page split); bench.py times only B = 64 / 128.  Rows are independent of the batch they sit in
+    (oracle pin P9), so the oracle runs once on b_max rows and every prefix B of them, decoded by the GPU from the same
+    pool, is held to the stage tolerance; graph replay of the same batch gives the same bits."""
+    from tests import gpu_helpers as gh
+    full = synth.LLAMA70B if name == "cfg2" else synth.QWEN32B
+    shape = _sub(full, 2)
+    rng = np.random.default_rng(5)
+    ctx = synth.lognormal_lengths(rng, b_max, 400, 16, 2048).astype(np.int32)
+    pb = synth.paged_batch(rng, ctx, extra_tokens=2)
+    P = gh.Problem(shape, 0, n_pages=pb.n_pages_pool, max_tokens=b_max, max_seqs=b_max, max_blocks=pb.max_blocks,
+                   pool_fill="random")
+    try:
+        x = synth.bits(synth.hidden_rows(b_max, shape.hidden, 5))
+        pool_before = P.pool_cpu.copy()
+        want, _ = hp.run_oracle_decode(F32, shape, P.wb, pool_before.copy(), ctx, pb.block_tables, x)
+        snap = P.stage.pool_view().clone()
+        for B in batches:
+            P.stage.pool_view().copy_(snap)
+            torch.cuda.synchronize()
+            got = P.decode(ctx[:B], pb.block_tables[:B], x[:B])
+            P.stage.pool_view().copy_(snap)
+            torch.cuda.synchronize()
+            assert np.array_equal(got, P.decode(ctx[:B], pb.block_tables[:B], x[:B]))
+            err = hp.rel_err_rows(got, want[:B])
+            print(f"{name} width, 2 layers, B={B}: max row rel err vs R0 {err:.3e}")
+            assert np.isfinite(got).all() and err < 2e-2, (B, err)
+    finally:
+        P.close()
+
+
 def test_full_width_recompute_prefill_and_migration_vs_oracle():
     """cfg-4: one ss_stage_prefill over all 32 migrated requests (40,173 tokens, packed varlen), then one decode
     step; the oracle follows the two shortest requests through the same two calls."""
