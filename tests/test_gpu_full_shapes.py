@@ -181,6 +181,52 @@ def test_full_width_recompute_prefill_and_migration_vs_oracle():
         P.close()
 
 
+@pytest.mark.parametrize("T_target", [120, 300, 512, 513, 777, 1100, 2144, 5000])
+def test_full_width_prefill_token_counts_vs_oracle(T_target):
+    """The prefill plans change with the token count: one token tile up to 256, single-CTA tiles / stream-K up to 512,
+    CTA pairs above (256-token tiles with a ragged last one), few or many attention items.  bench.py times 40,173 tokens
+    only.  A packed batch of T_target tokens (two short sequences and fillers of mixed lengths) at the cfg-2 layer
+    shapes; the oracle follows the two short sequences (sequences are independent, pin P9)."""
+    from tests import gpu_helpers as gh
+    shape = _sub(synth.LLAMA70B, 1)
+    rng = np.random.default_rng(T_target)
+    lens = [23, 40]
+    while sum(lens) < T_target:
+        lens.append(int(min(rng.integers(1, 700), T_target - sum(lens))))
+    lens = np.array(lens, dtype=np.int32)
+    order = rng.permutation(len(lens))
+    lens = lens[order]
+    n, T = len(lens), int(lens.sum())
+    assert T == T_target
+    pb = synth.paged_batch(rng, lens, extra_tokens=2)
+    P = gh.Problem(shape, 0, n_pages=pb.n_pages_pool, max_tokens=T, max_seqs=max(n, 16), max_blocks=pb.max_blocks)
+    try:
+        g = torch.Generator().manual_seed(T_target)
+        x = synth.bits(synth.randn_bf16((T, shape.hidden), 1.0, g))
+        cu = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
+        got = P.prefill(lens, pb.block_tables, x)
+        assert np.isfinite(got).all()
+        assert np.array_equal(got, P.prefill(lens, pb.block_tables, x))   # same call again: same bits
+        pick = np.argsort(lens, kind="stable")[:2]
+        rows = np.concatenate([np.arange(cu[s], cu[s + 1]) for s in pick])
+        pool = hp.new_pool(shape, pb.n_pages_pool, 1)
+        want, _, _ = hp.run_oracle_prefill(F32, shape, P.wb, pool, lens[pick], pb.block_tables[pick], x[rows])
+        pool_r1 = hp.new_pool(shape, pb.n_pages_pool, 1)
+        want1, _, _ = hp.run_oracle_prefill(F32, shape, P.wb, pool_r1, lens[pick], pb.block_tables[pick], x[rows], rounding=1)
+        err, err1, floor = (hp.rel_err_rows(got[rows], want), hp.rel_err_rows(got[rows], want1),
+                            hp.rel_err_rows(want1, want))
+        print(f"T={T} ({n} sequences): {len(rows)} oracle-checked rows: vs R0 {err:.3e}, vs R1 {err1:.3e}, floor {floor:.3e}")
+        # per-layer bound against R1 (reading A15b), stage bound against R0, and within 1.3 x the oracle's own floor
+        # (the factor of reading A15d) where that floor exceeds the per-layer bound
+        assert err1 < 1e-2 and err < 2e-2 and err <= 1.3 * max(floor, 1e-2)
+        used = np.zeros(pb.n_pages_pool, dtype=bool)
+        for s in range(n):
+            used[pb.block_tables[s, : (int(lens[s]) + 15) // 16]] = True
+        assert (P.pool_bits()[:, :, ~used] == 0x7FC1).all()
+    finally:
+        P.close()
+
+
 def test_full_width_migration_recompute_equals_incremental_on_gpu():
     """The migration invariant (oracle pin P7) GPU against GPU at the paper's width: the two shortest
     cfg-4 requests, one 70B-shaped layer.  (a) recompute = one ss_stage_prefill over prompt + 3 generated tokens;
