@@ -447,6 +447,8 @@ MHA = synth.ModelShape("tiny-mha-d128", 256, 2, 2, 128, 512, 2, 1e-6, 1e6, 1, 51
     (MHA, [257, 128, 65], [0, 0, 0]),                            # MHA, d = 128, a 1-row last tile (257 = 2 x 128 + 1)
     (synth.TINY128, [700, 33], [517, 20]),                       # chunk on top of a long prior context, unaligned start
     (synth.TINY, [2100, 2049], [2000, 0]),                       # > 2,048 keys: 33 ring stages per tile, ring wrap-around
+    (synth.TINY, [9001, 40], [0, 0]),                            # one long sequence: items of 1 ... 141 stages, 71 query tiles
+    (synth.TINY128, [8200, 300], [7900, 290]),                   # short chunks on top of ~8K tokens of prior context
 ])
 def test_prefill_attention_edge_shapes_vs_oracle(shape, lens, first):
     """Edge cases of the tcgen05 prefill attention (two heads per CTA, 128-row query tiles, 64-key stages, lazy maximum,
