@@ -31,8 +31,11 @@
  *   SS_DEBUG=1    every call first runs the device-side contract checks described at ss_stage_debug_info and waits
  *                 for their verdict (one stream synchronisation per call);
  *   SS_NO_GRAPH=1 ss_stage_decode enqueues its kernels directly instead of replaying a captured CUDA graph;
- *   SS_NO_PDL=1   kernels are launched without programmatic dependent launch (plain stream order).
- * The last two change scheduling only, never results (tests compare them bit for bit).
+ *   SS_NO_PDL=1   kernels are launched without programmatic dependent launch (plain stream order);
+ *   SS_ATTN_LAZY=n (0..64, default 16) the prefill attention moves a row's running maximum only when a key tile exceeds
+ *                 it by more than 2^n, and then rescales its accumulator in place; n changes rounding only (O / l is the
+ *                 same quotient).  A test aid: with 0 every growth of the maximum takes the rescale path.
+ * SS_NO_GRAPH and SS_NO_PDL change scheduling only, never results (tests compare them bit for bit).
  *
  * Readings of points the paper leaves open are listed in DESIGN.md ("Readings"), numbered A1..A22 after
  * SURVEY.md §8(c).

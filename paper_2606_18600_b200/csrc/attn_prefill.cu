@@ -37,7 +37,7 @@ constexpr int TA_BN = 64;       // keys per ring stage (4 pages)
 constexpr int TA_STAGES = 5;    // K/V ring depth: 320 keys in flight per CTA
 constexpr int TA_THREADS = 384;
 constexpr int TA_PAGES = TA_BN / 16;
-constexpr float TA_LAZY = 16.0f; // the running maximum (log2 units) is moved only when exceeded by more than this
+// (the running maximum, in log2 units, is moved only when exceeded by more than PrefillAttnParams::lazy = 16)
 
 // ---- plan: token -> (sequence, position), the prefix sum of query tiles and one descriptor per launch slot ---------
 __global__ void prefill_plan_kernel(const CallArgs *__restrict__ args, int n_seqs, int seq0, PrefillPlan plan) {
@@ -344,8 +344,8 @@ prefill_attn_kernel(const __grid_constant__ CUtensorMap q_map, const __grid_cons
 #pragma unroll
         for (int c = 0; c < TA_BN; ++c) mx4[c & 3] = fmaxf(mx4[c & 3], __uint_as_float(v[c]));
         const float mx = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3])) * sl2;
-        // lazy maximum: move it only when the tile's maximum exceeds it by more than TA_LAZY (P then stays <= 2^TA_LAZY)
-        const bool move = mx > m_used + TA_LAZY;   // also true on the first tile (m_used = -inf; key 0 is visible to all)
+        // lazy maximum: move it only when the tile's maximum exceeds it by more than p.lazy (P then stays <= 2^lazy)
+        const bool move = mx > m_used + p.lazy;    // also true on the first tile (m_used = -inf; key 0 is visible to all)
         float alpha = 1.0f;
         if (move) {
           alpha = fast_exp2(m_used - mx);  // 0 on the first tile

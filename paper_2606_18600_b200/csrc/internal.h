@@ -236,6 +236,7 @@ struct PrefillAttnParams {
   const CallArgs *args;
   int max_tiles;             // upper bound on query tiles = ceil(T / prefill_attn_tile_rows()) + n_seqs
   int n_sm;                  // SMs of the device: the kernel is persistent, one CTA per SM
+  float lazy;                // log2 threshold of the lazy running maximum (16; SS_ATTN_LAZY overrides: a test aid)
 };
 int prefill_attn_tile_rows();
 cudaError_t launch_prefill_attn(const PrefillAttnParams &p, cudaStream_t s);

@@ -228,6 +228,7 @@ struct ss_stage {
   CallArgs *h_args;    // pinned host staging for the argument block (+ 4 ints behind it: the SS_DEBUG error word)
   cudaEvent_t args_ev; // the last H2D copy out of h_args (the host must not overwrite the block before it has run)
   bool debug;          // SS_DEBUG=1 at create: every call validates its device-side arguments first
+  float attn_lazy;     // prefill attention: log2 threshold of the lazy running maximum (SS_ATTN_LAZY, default 16)
   int32_t dbg_info[4]; // last violation {code, sequence, index, value}
   int32_t *h_err() const { return (int32_t *)(h_args + 1); }
 
@@ -317,6 +318,10 @@ int ss_stage_create(ss_stage **out, const ss_model_dims *dims, int l0, int l1, c
   st->h_args = nullptr;
   st->args_ev = nullptr;
   st->debug = env_int("SS_DEBUG", 0) != 0;
+  {
+    const int lz = env_int("SS_ATTN_LAZY", 16);
+    st->attn_lazy = (float)(lz < 0 ? 0 : (lz > 64 ? 64 : lz));
+  }
   memset(st->dbg_info, 0, sizeof(st->dbg_info));
   st->allreduce = nullptr;
   st->allreduce_user = nullptr;
@@ -814,6 +819,7 @@ static cudaError_t enqueue_forward(ss_stage *st, bool decode, int n_seqs, int T,
         ap.args = args;
         ap.max_tiles = (T - n_dec + prefill_attn_tile_rows() - 1) / prefill_attn_tile_rows() + (n_seqs - n_dec);
         ap.n_sm = st->n_sm;
+        ap.lazy = st->attn_lazy;
         CKE(launch_prefill_attn(ap, s));
       }
     }

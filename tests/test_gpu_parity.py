@@ -515,6 +515,45 @@ def test_prefill_attention_persistent_ctas_take_several_items_vs_oracle(shape, n
         P.close()
 
 
+@pytest.mark.parametrize("shape,lens,first", [
+    (synth.TINY128, [1500, 333, 64], [0, 0, 0]),
+    (synth.TINY, [700, 2100], [300, 2000]),
+    (G3, [400, 129], [0, 100]),
+])
+def test_prefill_attention_rescale_path_vs_oracle_and_default(monkeypatch, shape, lens, first):
+    """The prefill attention rescales its O accumulator in tensor memory only when a key tile exceeds a row's running
+    maximum by more than 2^16 — rare on these inputs.  SS_ATTN_LAZY=0 makes every growth of the maximum take that path
+    (tcgen05.ld / scale / tcgen05.st of O after waiting for the previous P.V): the result must still match the oracle, and
+    the default build's result up to rounding (O / l is the same quotient)."""
+    gh = _gh()
+    lens, first = np.array(lens, dtype=np.int32), np.array(first, dtype=np.int32)
+    P, lens, pb, x = _problem(shape, seed=17, lens=lens, extra=4)
+    monkeypatch.setenv("SS_ATTN_LAZY", "0")
+    Q = gh.Problem(shape, 17, n_pages=pb.n_pages_pool, max_tokens=int(lens.sum()) + 64, max_seqs=16, max_blocks=pb.max_blocks)
+    monkeypatch.delenv("SS_ATTN_LAZY")
+    try:
+        bt, n = pb.block_tables, len(lens)
+        cu_full = np.concatenate([[0], np.cumsum(lens)]).astype(np.int32)
+        pool0 = hp.new_pool(shape, pb.n_pages_pool, P.L)
+        if first.any():
+            keep = first > 0
+            rows1 = np.concatenate([np.arange(cu_full[s], cu_full[s] + first[s]) for s in range(n) if keep[s]])
+            hp.run_oracle_prefill(F32, shape, P.wb, pool0, first[keep], bt[keep], x[rows1])
+            P.prefill(first[keep], bt[keep], x[rows1])
+            Q.prefill(first[keep], bt[keep], x[rows1])
+        rows2 = np.concatenate([np.arange(cu_full[s] + first[s], cu_full[s + 1]) for s in range(n)])
+        want, _, _ = hp.run_oracle_prefill(F32, shape, P.wb, pool0, lens, bt, x[rows2], ctx_before=first)
+        a = P.prefill(lens, bt, x[rows2], ctx_before=first)
+        b = Q.prefill(lens, bt, x[rows2], ctx_before=first)
+        ea, eb, d = hp.rel_err_rows(a, want), hp.rel_err_rows(b, want), hp.rel_err_rows(b, a)
+        print(f"{shape.name} lens {lens.tolist()}: default vs R0 {ea:.3e}, always-rescale vs R0 {eb:.3e}, between them {d:.3e}")
+        assert np.isfinite(b).all() and ea < STAGE_TOL and eb < STAGE_TOL and d < 1e-2   # (bf16 outputs: single-step flips)
+        assert not np.array_equal(a, b), "SS_ATTN_LAZY=0 changed nothing: the rescale path was not taken"
+    finally:
+        P.close()
+        Q.close()
+
+
 def test_chunked_prefill_and_mixed_batch_on_gpu():
     """Prior context (ctx_before > 0) and q_len = 1 rows in a prefill call (mixed iteration, reading A19)."""
     shape = synth.TINY_QWEN
