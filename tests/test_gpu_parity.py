@@ -717,6 +717,87 @@ def test_migration_by_kv_transfer_is_bit_exact():
         B.close()
 
 
+@pytest.mark.parametrize("invariant", [False, True])
+def test_generation_then_migration_recompute_gives_the_same_tokens(invariant):
+    """BASELINE.json configs[3] end to end, on the tiny model run as ONE stage with its embedding and lm_head: requests
+    generate greedily (token ids in, argmax out, fed back) for k steps; the request is then 'migrated': a fresh stage
+    instance recomputes prompt + generated tokens in one prefill and continues.  Output-preserving
+    means the tokens after the migration equal the ones the original instance goes on to produce.  In batch-invariant
+    mode that must hold for every row, bit for bit in the logits; in the default mode for every row whose top-2 logit margin
+    exceeds the recompute-vs-incremental logit difference (reading A14), which is printed."""
+    shape = synth.TINY_QWEN
+    k_before, k_after = 6, 4
+    P, lens, pb, _ = _problem(shape, seed=9, with_edge=True, extra=k_before + k_after + 2)
+    Q, _, _, _ = _problem(shape, seed=9, with_edge=True, extra=k_before + k_after + 2)
+    try:
+        for st in (P.stage, Q.stage):
+            st.set_batch_invariant(invariant)
+        n, bt = len(lens), pb.block_tables
+        rng = np.random.default_rng(9)
+        prompt = rng.integers(0, shape.vocab, int(lens.sum())).astype(np.int32)
+        cu = np.concatenate([[0], np.cumsum(lens)]).astype(np.int32)
+        dev = "cuda:0"
+
+        def prefill(stage, ids, cu_q):
+            lg = torch.empty((n, shape.vocab), dtype=torch.float32, device=dev)
+            am = torch.empty((n,), dtype=torch.int32, device=dev)
+            stage.prefill(n, P.i32(cu_q), P.i32(np.zeros(n)), P.i32(bt), int(cu_q[-1]), token_ids=P.i32(ids), out_logits=lg,
+                          out_argmax=am)
+            stage.synchronize()
+            return lg.cpu().numpy(), am.cpu().numpy()
+
+        def decode(stage, ctx, ids):
+            lg = torch.empty((n, shape.vocab), dtype=torch.float32, device=dev)
+            am = torch.empty((n,), dtype=torch.int32, device=dev)
+            stage.decode(n, P.i32(bt), P.i32(ctx), token_ids=P.i32(ids), out_logits=lg, out_argmax=am)
+            stage.synchronize()
+            return lg.cpu().numpy(), am.cpu().numpy()
+
+        # ---- the original instance: prompt, then k_before + k_after greedy steps
+        _, tok = prefill(P.stage, prompt, cu)
+        gen, logit_log = [tok], []
+        for step in range(k_before + k_after):
+            lg, tok = decode(P.stage, lens + step, gen[-1])
+            gen.append(tok)
+            logit_log.append(lg)
+        gen = np.stack(gen, axis=1)                                  # [n, 1 + k_before + k_after]
+        # ---- migration after k_before generated tokens have been CONSUMED: recompute prompt + gen[:, :k_before] ...
+        lens2 = lens + k_before
+        cu2 = np.concatenate([[0], np.cumsum(lens2)]).astype(np.int32)
+        ids2 = np.concatenate([np.concatenate([prompt[cu[s]:cu[s + 1]], gen[s, :k_before]]) for s in range(n)]).astype(np.int32)
+        lg_m, tok_m = prefill(Q.stage, ids2, cu2)
+        # ... whose last-row logits are those of incremental step k_before - 1 (input gen[:, k_before - 1])
+        ref = logit_log[k_before - 1]
+        diff = float(np.abs(lg_m - ref).max())
+        top2 = np.sort(ref, axis=1)[:, -2:]
+        safe = (top2[:, 1] - top2[:, 0]) > 4 * diff
+        print(f"invariant={invariant}: recompute vs incremental logits max abs diff {diff:.3e} (scale {float(np.abs(ref).max()):.2f}); "
+              f"rows over margin {int(safe.sum())}/{n}")
+        if invariant:
+            assert np.array_equal(lg_m, ref) and np.array_equal(tok_m, gen[:, k_before])
+        else:
+            assert hp.rel_err_rows(lg_m, ref) < STAGE_TOL and np.array_equal(tok_m[safe], gen[safe, k_before])
+        # ---- and the migrated instance continues with the same tokens
+        follow = safe if not invariant else np.ones(n, dtype=bool)
+        tok = gen[:, k_before].copy()                # feed the original's token (rows off the margin may differ by a near-tie)
+        for step in range(k_before, k_before + k_after):
+            lg, tok_n = decode(Q.stage, lens + step, tok)
+            ref = logit_log[step]
+            if invariant:
+                assert np.array_equal(lg, ref), step
+            else:
+                d = float(np.abs(lg - ref).max())
+                t2 = np.sort(ref, axis=1)[:, -2:]
+                follow = follow & ((t2[:, 1] - t2[:, 0]) > 4 * d)
+                assert hp.rel_err_rows(lg, ref) < STAGE_TOL
+            assert np.array_equal(tok_n[follow], gen[follow, step + 1]), step
+            tok = gen[:, step + 1]
+        assert follow.sum() >= n // 2
+    finally:
+        P.close()
+        Q.close()
+
+
 def test_token_ids_logits_and_argmax():
     """S0 embedding gather and S11 logits/argmax (Table 2 'Logits Calculation'; reading A14)."""
     shape = synth.TINY
